@@ -1,0 +1,8 @@
+"""bege -- B200-native FFT matched filtering over chirp-template banks (arXiv:1708.01609 hot path).
+
+`paper_1708_01609_b200.bege` is the thin Python binding over the C-ABI library
+(`include/bege.h`, built from `csrc/`); `paper_1708_01609_b200.synth` holds the seeded
+synthetic inputs.  Importing this package does not load the CUDA library; the first
+use of the binding does, and fails loudly if it is missing.
+"""
+__all__ = ["bege", "synth"]

@@ -1,0 +1,341 @@
+"""Pins of the fp64 CPU oracle against things other than itself (CPU only, `-m "not gpu"`).
+
+Each test names the passage of PAPER.md (or the DESIGN.md reading) it fixes and is chosen so
+that a plausible mistake in oracle/bege_oracle.c -- a dropped term, a wrong sign or index, a
+transposed operand, a missing conjugate or normalisation -- fails at least one of them.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from oracle import bege_oracle as bo
+from paper_1708_01609_b200 import synth
+
+FS, N, BAND, TAU = synth.FS, synth.N_SEG, synth.BAND, synth.TAU
+GOLD = os.path.join(os.path.dirname(__file__), "golden", "paper_numbers.txt")
+
+
+def _gold():
+    out = {}
+    with open(GOLD) as fh:
+        for line in fh:
+            if line.startswith("#") or not line.strip():
+                continue
+            name, val, tol, _cite = [p.strip() for p in line.split("|", 3)]
+            out[name] = (float(val), float(tol))
+    return out
+
+
+# ------------------------------------------------------------------ FFT (eq.8)
+@pytest.mark.parametrize("n", [1, 2, 4, 8, 64, 256, 1024])
+@pytest.mark.parametrize("sign", [-1, 1])
+def test_fft_equals_textbook_dft_matrix(n, sign):
+    rng = np.random.default_rng(n + 7)
+    a = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    k = np.arange(n)
+    F = np.exp(sign * 2j * np.pi * np.outer(k, k) / n)      # the O(N^2) definition
+    ref = F @ a
+    got = bo.fft(a, sign)
+    assert np.max(np.abs(got - ref)) <= 1e-11 * max(1.0, np.linalg.norm(a))
+
+
+def test_fft_matches_library_routine_at_full_size():
+    rng = np.random.default_rng(11)
+    a = rng.standard_normal(N) + 1j * rng.standard_normal(N)
+    assert np.linalg.norm(bo.fft(a, -1) - np.fft.fft(a)) <= 1e-13 * np.linalg.norm(a) * math.sqrt(N)
+    assert np.linalg.norm(bo.fft(a, +1) - np.fft.ifft(a) * N) <= 1e-13 * np.linalg.norm(a) * math.sqrt(N)
+
+
+def test_fft_roundtrip_and_parseval():
+    rng = np.random.default_rng(12)
+    a = rng.standard_normal(N) + 1j * rng.standard_normal(N)
+    A = bo.fft(a, -1)
+    back = bo.fft(A, +1) / N
+    assert np.max(np.abs(back - a)) < 1e-12
+    # PAPER.md:98 Parseval: sum |x|^2 = N^-1 sum |X|^2
+    assert abs(np.sum(np.abs(a) ** 2) - np.sum(np.abs(A) ** 2) / N) < 1e-12 * N
+
+
+def test_fft_rejects_non_power_of_two():
+    with pytest.raises(ValueError):
+        bo.fft(np.zeros(12, dtype=complex), -1)
+
+
+def test_fft_delta_and_tone():
+    # a unit impulse at n0 transforms to exp(-2 pi i k n0/N): fixes the sign of the exponent
+    n, n0 = 256, 3
+    a = np.zeros(n, dtype=complex)
+    a[n0] = 1.0
+    assert np.allclose(bo.fft(a, -1), np.exp(-2j * np.pi * np.arange(n) * n0 / n), atol=1e-13)
+    # a tone exp(+2 pi i k0 n/N) has its forward transform at bin +k0
+    k0 = 5
+    A = bo.fft(np.exp(2j * np.pi * k0 * np.arange(n) / n), -1)
+    assert abs(A[k0] - n) < 1e-10 and np.sum(np.abs(A)) - abs(A[k0]) < 1e-9
+
+
+# ------------------------------------------------------- band mask
+def test_band_mask_bins():
+    X = bo.band_mask(np.ones(N, dtype=complex), FS, *BAND)
+    keep = np.flatnonzero(X.real)
+    # 350 Hz = bin 5600, 2000 Hz = bin 32000 at df = 1/16 Hz, inclusive; mirrored at N-k
+    expect = np.concatenate([np.arange(5600, 32001), np.arange(N - 32000, N - 5600 + 1)])
+    assert np.array_equal(keep, expect)
+    assert keep.size == 52802 and X[0] == 0 and X[N // 2] == 0
+
+
+def test_segment_spectrum_is_fft_then_mask():
+    x = synth.white_noise(5, 4096)
+    X = bo.segment_spectrum(x, FS, *BAND)
+    f = np.abs(np.fft.fftfreq(4096, 1 / FS))
+    ref = np.fft.fft(x) * ((f >= BAND[0]) & (f <= BAND[1]))
+    assert np.linalg.norm(X - ref) < 1e-10 * np.linalg.norm(ref)
+
+
+# ---------------------------------------------------- template (BASELINE cfg0)
+def test_template_norm_window_padding():
+    h = bo.template(1000.0, 50.0, TAU, FS, N)
+    L = 4096
+    assert abs(np.linalg.norm(h) - 1.0) < 1e-14
+    assert np.all(h[L:] == 0) and h[0] == 0 and abs(h[L - 1]) < 1e-15   # symmetric Hann: zero at both ends
+    # closed form: sum_n hann^2 = 3 (L-1)/8  =>  envelope = hann/sqrt(3 (L-1)/8); L even, so the largest
+    # sample sits half a step off the window centre: hann(2047) = 1/2 - 1/2 cos(2 pi 2047/4095)
+    env = np.abs(h[:L])
+    w_max = 0.5 - 0.5 * math.cos(2 * math.pi * 2047 / 4095)
+    assert abs(env.max() - w_max / math.sqrt(3 * (L - 1) / 8)) < 1e-15
+    assert np.allclose(env, env[::-1], atol=1e-15)                      # symmetric window
+
+
+def test_template_instantaneous_frequency():
+    # d(phase)/dt / 2 pi = f0 + fdot t: fixes the 1/2 in front of fdot and the sign of i
+    f0, fd = 700.0, -120.0
+    h = bo.template(f0, fd, TAU, FS, N)[1:4095]
+    dphi = np.angle(h[1:] * np.conj(h[:-1]))
+    t_mid = (np.arange(1, 4094) + 0.5) / FS
+    finst = dphi * FS / (2 * np.pi)
+    assert np.max(np.abs(finst - (f0 + fd * t_mid))) < 1e-6
+
+
+def test_template_spectrum_of_pure_tone():
+    # fdot = 0, bin-centred f0: the spectrum is the Hann kernel centred on bin f0*N/fs, positive frequency
+    f0 = 1000.0
+    H = bo.fft(bo.template(f0, 0.0, TAU, FS, N), -1)
+    assert int(np.argmax(np.abs(H))) == int(f0 * N / FS)
+    # Hann main lobe is +-2 Hz for a 1 s window, side lobes fall at 18 dB/octave: all but <1e-6 of
+    # the energy lies within +-8 Hz of f0, and none of it at negative frequencies
+    k0, w = int(f0 * N / FS), 128
+    tot = np.sum(np.abs(H) ** 2)
+    assert abs(tot - N) < 1e-8 * N                        # unit-norm h, unnormalised DFT (Parseval)
+    assert np.sum(np.abs(H[k0 - w:k0 + w + 1]) ** 2) / tot > 1 - 1e-6
+    assert np.sum(np.abs(H[N // 2:]) ** 2) / tot < 1e-9
+
+
+def test_template_matches_library_expression():
+    f0, fd = 1234.5, 333.0
+    t = np.arange(4096) / FS
+    ref = np.hanning(4096) * np.exp(2j * np.pi * (f0 * t + 0.5 * fd * t * t))
+    ref /= np.linalg.norm(ref)
+    assert np.max(np.abs(bo.template(f0, fd, TAU, FS, N)[:4096] - ref)) < 1e-12
+
+
+def test_template_rejects_bad_length():
+    with pytest.raises(ValueError):
+        bo.template(100.0, 0.0, 20.0, FS, N)       # tau*fs > N
+
+
+# -------------------------------------- correlation = definition (PAPER.md:74 eq.3, :81, :89-92 eq.5)
+def _brute_corr(xhat, h, L):
+    """eq.(3) with circular indexing, written with python loops (tiny sizes only)."""
+    n = xhat.size
+    z = np.zeros(n, dtype=complex)
+    for lag in range(n):
+        acc = 0j
+        for s in range(L):
+            acc += np.conj(h[s]) * xhat[(lag + s) % n]
+        z[lag] = acc
+    return z
+
+
+@pytest.mark.parametrize("n", [64, 256, 1024])
+def test_fft_correlation_equals_direct_sum(n):
+    fs, band, L = 256.0, (20.0, 100.0), n // 16
+    rng = np.random.default_rng(n)
+    x = rng.standard_normal(n) + 1j * rng.standard_normal(n)      # general complex x
+    h = bo.template(40.0, 30.0, L / fs, fs, n)
+    X = bo.segment_spectrum(x, fs, *band)
+    z, sigma = bo.correlate(X, h)
+    xhat = bo.fft(X, +1) / n
+    # oracle's direct routine vs python loops, then FFT route vs direct: two independent restatements
+    zd = bo.correlate_direct(xhat, h, L)
+    if n <= 256:
+        assert np.max(np.abs(zd - _brute_corr(xhat, h, L))) < 1e-12
+    assert np.max(np.abs(z - zd)) < 1e-12
+    # PAPER.md:94-100 eq.(6)=(7): Parseval sigma is the rms of the output, identically
+    assert abs(sigma - math.sqrt(np.mean(np.abs(z) ** 2))) < 1e-13
+
+
+def test_correlation_sampled_lags_full_size():
+    x = synth.noise_segment(21).astype(np.complex128)
+    X = bo.segment_spectrum(x, FS, *BAND)
+    h = bo.template(900.0, 150.0, TAU, FS, N)
+    z, sigma = bo.correlate(X, h)
+    lags = np.array([0, 1, 4095, 4096, 29901, N - 4096, N - 1], dtype=np.uint32)   # incl. wrap-around lags
+    zd = bo.correlate_direct(bo.fft(X, +1) / N, h, 4096, lags)
+    assert np.max(np.abs(z[lags] - zd)) < 1e-12
+    assert abs(sigma - math.sqrt(np.mean(np.abs(z) ** 2))) < 1e-13
+
+
+def test_shifted_template_gives_autocorrelation_peak():
+    # x = A * template shifted to n0 (band = everything but DC/Nyquist) => z peaks at n0 with value A
+    n, fs, L, n0, A = 1024, 1024.0, 128, 300, 3.5
+    h = bo.template(200.0, 100.0, L / fs, fs, n)
+    x = A * np.roll(h, n0)
+    X = bo.segment_spectrum(x, fs, 0.5, 511.5)
+    z, _ = bo.correlate(X, h)
+    assert int(np.argmax(np.abs(z))) == n0
+    assert abs(z[n0] - A) < 1e-3          # removed DC/Nyquist bins carry ~nothing
+    assert abs(z[n0].imag) < 1e-6         # conj on the template, not on the data
+
+
+def test_bin_centred_tone_gives_constant_modulus():
+    # fdot = 0 template on a tone at the same bin-centred frequency: |z| independent of lag
+    n, fs, L = 1024, 1024.0, 64
+    x = np.exp(2j * np.pi * 128.0 * np.arange(n) / fs)
+    X = bo.segment_spectrum(x, fs, 10.0, 500.0)
+    z, sigma = bo.correlate(X, bo.template(128.0, 0.0, L / fs, fs, n))
+    assert np.ptp(np.abs(z)) < 1e-12 and abs(sigma - np.abs(z[0])) < 1e-12
+    # and the phase advances with the lag like the tone itself (z[n] ~ x[n]): fixes y(t+s), not y(t-s)
+    assert abs(np.angle(z[1] / z[0]) - 2 * np.pi * 128.0 / fs) < 1e-9
+
+
+# ----------------------------------------- sigma / Gaussian tails (reading 4)
+@pytest.fixture(scope="module")
+def cfg0_interior():
+    """z/sigma of cfg0's 14x14 interior templates (edge templates lose energy out of band)."""
+    w = synth.config0()
+    X = bo.segment_spectrum(w.x[0], FS, *BAND)
+    ids = [i * 16 + j for i in range(1, 15) for j in range(1, 15)]
+    zs, sig = [], []
+    for t in ids:
+        z, s = bo.correlate(X, bo.template(w.f0[t], w.fdot[t], TAU, FS, N))
+        zs.append(z / s)
+        sig.append(s)
+    return np.array(zs), np.array(sig)
+
+
+def test_sigma_predicts_empirical_std_on_noise(cfg0_interior):
+    zs, sig = cfg0_interior
+    L = 4096
+    # rms over the VALID (non wrap-around) lags only: non-trivial version of the "within 1 %" pin
+    rms_valid = np.sqrt(np.mean(np.abs(zs[:, : N - L]) ** 2, axis=1))
+    # pooled over templates within 1 %; a single narrow-band template (small |fdot|: output correlated
+    # over ~1e3 lags, so only ~60 independent samples) scatters by a few % when 1/16 of the lags is dropped
+    assert abs(np.sqrt(np.mean(rms_valid ** 2)) - 1.0) < 0.01
+    assert np.max(np.abs(rms_valid - 1.0)) < 0.05
+    # over ALL lags (circular output) it is an identity, eq.(6)=(7)
+    assert np.max(np.abs(np.sqrt(np.mean(np.abs(zs) ** 2, axis=1)) - 1.0)) < 1e-12
+    # closed form: E[sigma^2] = in-band energy fraction of the unit-norm template on unit white noise
+    assert 0.9 < np.mean(sig ** 2) < 1.1
+
+
+def test_tail_counts_follow_gaussian_laws(cfg0_interior):
+    zs, _ = cfg0_interior
+    n_out = zs.size
+    # circular complex Gaussian: P(|z| > k sigma) = exp(-k^2); each quadrature at sigma/sqrt2 is erfc(k/sqrt2)
+    for k in (2.0, 2.5, 3.0):
+        got = np.count_nonzero(np.abs(zs) > k)
+        exp = n_out * math.exp(-k * k)
+        # outputs are correlated over ~13 lags (band-limited): allow 6 x Poisson on clustered counts
+        assert abs(got - exp) < 6 * math.sqrt(13 * exp) + 0.03 * exp, (k, got, exp)
+        for q in (zs.real, zs.imag):
+            gq = np.count_nonzero(np.abs(q) > k / math.sqrt(2))
+            eq = n_out * math.erfc(k / math.sqrt(2))
+            assert abs(gq - eq) < 6 * math.sqrt(13 * eq) + 0.03 * eq, (k, gq, eq)
+    # circularity: equal variance in both quadratures, no correlation between them
+    assert abs(np.var(zs.real) / np.var(zs.imag) - 1) < 0.01
+    assert abs(np.mean(zs.real * zs.imag)) < 0.005
+
+
+# ------------------------------------------------- injection recovery (BASELINE cfg1; readings 14, 18)
+def test_injected_chirp_recovered_at_true_template_and_lag():
+    w = synth.config1()
+    X = bo.segment_spectrum(w.x[0], FS, *BAND)
+    rows, cols = range(112, 121), range(96, 109)
+    ids = np.array([i * 256 + j for i in rows for j in cols])
+    f0 = np.append(w.f0[ids], 1100.0)            # exact template appended last
+    fd = np.append(w.fdot[ids], -80.0)
+    tails, n_true, sigma, _ = bo.search(X[None, :], f0, fd, TAU, FS, 5.0)
+    assert n_true == tails.size > 0
+    grid = tails[tails["template_id"] < ids.size]
+    best = grid[np.argmax(grid["snr"])]
+    assert ids[best["template_id"]] == w.meta["true_id"] == 29798
+    assert abs(int(best["lag"]) - 29870) <= 2          # chirp degeneracy: n0 + df0*fs/fdot = 29901 - 31
+    assert 9.0 < best["snr"] < 12.5
+    exact = tails[tails["template_id"] == ids.size]
+    assert int(exact[np.argmax(exact["snr"])]["lag"]) == w.meta["n0"] == 29901
+    assert 9.5 < exact["snr"].max() < 12.5             # sigma includes the signal (reading 13)
+    # sigma of the matching template is raised by the injection, a far template stays ~1
+    assert sigma[-1, 0] > 1.05 and 0.9 < sigma[0, 0] < 1.1
+
+
+# ------------------------------------------------------------- search bookkeeping (eq.13)
+def test_search_records_ids_lags_sigma_layout():
+    n, fs, band, tau = 1024, 1024.0, (50.0, 450.0), 0.125
+    xs = np.stack([synth.band_limit(synth.white_noise(s, n), fs, *band) for s in (1, 2, 3)])
+    Xs = np.stack([bo.segment_spectrum(x, fs, *band) for x in xs])
+    f0, fd = synth.bank_grid(3, 2, 100.0, 300.0, -80.0, 80.0)
+    k = 1.7
+    tails, n_true, sigma, used = bo.search(Xs, f0, fd, tau, fs, k)
+    assert used >= 1 and n_true == tails.size and sigma.shape == (6, 3)
+    exp = []
+    for j in range(6):
+        h = bo.template(f0[j], fd[j], tau, fs, n)
+        for m in range(3):
+            z, s = bo.correlate(Xs[m], h)
+            assert abs(s - sigma[j, m]) < 1e-15
+            for lag in np.flatnonzero(np.abs(z) > k * s):
+                exp.append((j, m * n + lag, abs(z[lag]) / s))
+    assert tails.size == len(exp)
+    assert np.array_equal(tails["template_id"], [e[0] for e in exp])
+    assert np.array_equal(tails["lag"], [e[1] for e in exp])
+    assert np.allclose(tails["snr"], [e[2] for e in exp], rtol=1e-13)
+    # cap smaller than the count: true count still returned
+    t2, n2, _, _ = bo.search(Xs, f0, fd, tau, fs, k, cap=5)
+    assert n2 == n_true and t2.size == 5
+
+
+def test_zero_data_gives_no_tails():
+    f0, fd = synth.bank_grid(2, 2, 400.0, 500.0, -10.0, 10.0)
+    tails, n_true, sigma, _ = bo.search(np.zeros((1, 4096), dtype=complex), f0, fd, 0.25, FS, 3.0)
+    assert n_true == 0 and np.all(sigma == 0)
+
+
+def test_search_thread_count_does_not_change_results():
+    n, fs, band = 2048, 1024.0, (50.0, 450.0)
+    X = bo.segment_spectrum(synth.white_noise(9, n), fs, *band)[None, :]
+    f0, fd = synth.bank_grid(4, 4, 100.0, 300.0, -80.0, 80.0)
+    a = bo.search(X, f0, fd, 0.25, fs, 2.0, n_threads=1)
+    b = bo.search(X, f0, fd, 0.25, fs, 2.0, n_threads=4)
+    assert a[1] == b[1] and np.array_equal(a[0], b[0]) and np.array_equal(a[2], b[2])
+
+
+# ------------------------------------------------------------------ the paper's printed arithmetic
+def test_paper_printed_numbers():
+    g = _gold()
+
+    def close(name, val):
+        ref, tol = g[name]
+        assert abs(val - ref) <= tol * ref, (name, val, ref)
+
+    fl = bo.fft_flops(N)
+    close("flops_per_fft_N65536", fl)
+    close("realtime_tflops", fl * 2 ** 23 / 16.0)
+    corr = 2 ** 23 * 288 * 2048
+    close("s6_total_correlations", corr)
+    close("s6_total_flop", corr * fl)
+    close("block_flop_M2", 2048 ** 2 * fl)
+    close("block_output_bytes", 2048 ** 2 * N * 8)
+    close("block_bytes", 2048 * N * 8)
+    close("file_bytes", 8 * 2048 * N * 8)
+    close("segment_bytes", N * 8)
