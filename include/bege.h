@@ -1,0 +1,137 @@
+/*
+ * bege.h -- C ABI of the B200-native hot path of arXiv:1708.01609 (van Putten,
+ * "Deep searches for broadband extended gravitational-wave emission bursts by
+ * heterogeneous computing"): FFT matched filtering of 16 s strain segments against
+ * a bank of one-second chirp templates, Parseval sigma, k-sigma tails.
+ *
+ * Citations are PAPER.md:<line> plus the section / equation they fall in.
+ *
+ * Conventions (all entry points)
+ *   - plain C, no C++/torch types; every call returns a bege_status and never
+ *     throws; on error the outputs are left untouched and bege_last_error(plan)
+ *     describes the failure.
+ *   - "host" / "device" says where a pointer must live; where either is accepted
+ *     the library detects it (cudaPointerGetAttributes).
+ *   - the caller keeps ownership of every array it passes in; the plan owns its
+ *     device state (or borrows the workspace given to bege_plan_set_workspace).
+ *   - one plan = one CUDA device and one stream; a plan is not thread safe.
+ *   - every step of the path runs in the library's own sm_100a kernels; there is
+ *     no CPU fallback.  Without a CUDA device bege_plan_create returns BEGE_ECUDA.
+ */
+#ifndef BEGE_H
+#define BEGE_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct bege_plan bege_plan;   /* opaque */
+
+/* One tail sample, PAPER.md:221 (Table 3: sample offset, rho, template identity). 12 bytes. */
+typedef struct {
+    uint32_t template_id;   /* index into the arrays given to bege_bank_generate          */
+    uint32_t lag;           /* m*N + n: segment m, sample offset n, eq.(13)   */
+    float    snr;           /* |z[n]| / sigma_jm                                          */
+} bege_tail;
+
+typedef enum {
+    BEGE_OK        = 0,
+    BEGE_EINVAL    = 1,   /* bad argument (N not 2^16, band outside (0, fs/2), NULL pointer ...) */
+    BEGE_ESTATE    = 2,   /* call out of order (search before bank / segments are loaded ...)    */
+    BEGE_ENOMEM    = 3,   /* workspace too small / device allocation failed                      */
+    BEGE_ECUDA     = 4,   /* CUDA runtime error; text in bege_last_error                         */
+    BEGE_EOVERFLOW = 5    /* more tails than `cap`; *n_tails is still the true count             */
+} bege_status;
+
+/* Counters for benches (bege_plan_get_stats). */
+typedef struct {
+    uint64_t kernel_launches;      /* kernels of this library launched since plan creation / last reset   */
+    uint64_t correlations;         /* (template, segment) pairs searched since last reset                 */
+    double   fused_kernel_ms;      /* CUDA-event time spent in the dominant search kernel(s), accumulated
+                                      only while profiling is on (bege_plan_set_profiling)               */
+    uint64_t fused_kernel_launches;/* launches that fused_kernel_ms covers                                */
+    uint64_t hbm_bytes_per_template; /* bytes of one stored template spectrum (the algorithmic HBM read)  */
+} bege_stats;
+
+/*
+ * Create a plan for transforms of length N (must be 65536 = 2^16: "FFT_{N,M} of
+ * length N = 2^16") at sampling rate fs [Hz] with the analysis band band_lo_hz <= |f| <= band_hi_hz
+ * (inclusive edges; 350-2000 Hz).  0 < band_lo < band_hi < fs/2.
+ * device: CUDA device ordinal.  cuda_stream: a cudaStream_t (e.g. torch's current stream handle) or
+ * NULL for a stream the plan creates.  All work of the plan is ordered on that stream; a second,
+ * internal stream carries the device->host copy of the tails.
+ */
+int bege_plan_create(bege_plan** out, uint32_t N, double fs, double band_lo_hz, double band_hi_hz,
+                     int device, void* cuda_stream);
+
+/*
+ * Device bytes the plan needs for a bank of n_templates, n_segments segments and room for `cap`
+ * tail records (bank spectra + segment spectra + FFT staging + sigma + records).
+ */
+int bege_plan_workspace_bytes(const bege_plan*, uint64_t n_templates, uint32_t n_segments,
+                              uint64_t cap, uint64_t* bytes);
+
+/*
+ * Lend the plan a device buffer (e.g. a torch tensor's storage, 256-byte aligned) of `bytes` bytes; it
+ * must outlive the plan or the next call of this function.  Loaded banks / segments are forgotten.
+ * dev_ptr == NULL: the plan allocates (cudaMalloc) what it needs on demand and owns it.
+ */
+int bege_plan_set_workspace(bege_plan*, void* dev_ptr, uint64_t bytes);
+
+/*
+ * a1 -- template spectra (PAPER.md:156 step ii: "a chirp template w of duration tau = 1 s is extended by
+ * zeros to length N and its transform w~ is loaded into Global Memory").  For j < n_templates:
+ *   L = round(tau_s*fs); t_n = n/fs; h_j[n] = hann_L[n] * exp(i 2 pi (f0_j t_n + fdot_j t_n^2 / 2)), n < L,
+ *   unit L2 norm, zero padded to N; H_j = DFT_N(h_j).  Phases are formed in fp64, the transform runs in
+ *   fp32.  The in-band rows of H_j are stored in HBM in the tiled layout the search kernel streams.
+ * f0_hz, fdot_hz_s: host arrays of n_templates doubles.  Replaces any previous bank.  1 <= L <= N/16.
+ */
+int bege_bank_generate(bege_plan*, const double* f0_hz, const double* fdot_hz_s,
+                       uint64_t n_templates, double tau_s);
+
+/*
+ * a2 -- segment spectra (PAPER.md:155 step i).  x: n_segments*N complex samples, interleaved
+ * (re, im) fp32, host or device.  X_m = DFT_N(x_m), bins outside the band set to zero.
+ * Replaces previously loaded segments.  n_segments*N must fit 32 bits (lag = m*N + n).
+ */
+int bege_segment_load(bege_plan*, const float* x_interleaved_c64, uint32_t n_segments);
+
+/*
+ * a3-a7 -- the search (PAPER.md:89-100 eq.5-7, :116-120 eq.9, :156-160 steps ii-iv, :162).  For every
+ * template j of the bank and loaded segment m:  R = conj(H_j) X_m;  sigma_jm^2 = N^-2 sum_k |R[k]|^2;
+ * z = IDFT_N(R) (four-step 256x256, never written to HBM);  every n with |z[n]| > k_sigma*sigma_jm is
+ * appended as {j, m*N+n, |z[n]|/sigma_jm}.  Only these records cross PCIe (pinned staging, side stream).
+ * tails_out: host array of `cap` records (pinned memory is copied into directly), may be NULL if cap = 0.
+ * *n_tails: the TRUE number of tails.  If it exceeds cap, exactly cap records are written (which ones
+ * is unspecified) and BEGE_EOVERFLOW is returned.  Record order is unspecified.  Synchronous at return.
+ */
+int bege_search(bege_plan*, float k_sigma, bege_tail* tails_out, uint64_t cap, uint64_t* n_tails);
+
+/* sigma_jm of the last bege_search, host array of n_templates*n_segments floats, template-major. */
+int bege_get_sigma(bege_plan*, float* sigma_out);
+
+/*
+ * Off the timed path, for parity tests: the full correlation z_jm (host, N complex fp32 interleaved)
+ * and its sigma for one (template, segment) pair, computed by the same kernels as bege_search.
+ */
+int bege_debug_correlate(bege_plan*, uint64_t template_id, uint32_t segment, float* z_out_c64,
+                         float* sigma_out);
+
+/* Off the timed path: stored spectrum of one template / one segment, natural order, N complex fp32 (host). */
+int bege_debug_template_spectrum(bege_plan*, uint64_t template_id, float* H_out_c64);
+int bege_debug_segment_spectrum(bege_plan*, uint32_t segment, float* X_out_c64);
+
+int  bege_plan_set_profiling(bege_plan*, int on);    /* CUDA events around the dominant kernel (adds syncs) */
+int  bege_plan_get_stats(const bege_plan*, bege_stats* out);
+int  bege_plan_reset_stats(bege_plan*);
+
+const char* bege_last_error(const bege_plan*);       /* never NULL; valid until the next call on the plan */
+void bege_plan_destroy(bege_plan*);
+const char* bege_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BEGE_H */

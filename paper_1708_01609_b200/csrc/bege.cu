@@ -1,0 +1,770 @@
+// bege.cu -- sm_100a kernels and C ABI (include/bege.h) of the butterfly-filtering hot path of
+// arXiv:1708.01609.  See DESIGN.md for the data layout and the roofline of each kernel.
+//
+// Index conventions (N = 65536 = 256 x 256, w_M = exp(2 pi i / M)):
+//   inverse (search):  k = k1 + 256 k2,  n = 256 n1 + n2
+//     z[256 n1 + n2] = 1/N sum_k1 w256^(k1 n1) [ wN^(k1 n2) sum_k2 R[k1 + 256 k2] w256^(k2 n2) ]
+//     pass 1 (k_inv_cols): 256-point column DFTs over k2 + twiddle wN^(k1 n2) -> scratch T[n2][k1] (L2)
+//     pass 2 (k_inv_rows): 256-point row DFTs over k1, threshold, compaction
+//   forward (bank / segments): n = nl + 256 nh, k = k1 + 256 k2
+//     H[k1 + 256 k2] = sum_nl w256^(-nl k2) [ wN^(-nl k1) sum_nh h[nl + 256 nh] w256^(-nh k1) ]
+//     step A (k_fwd_rows_*): DFT over nh + twiddle -> scratch G (tile layout), step B (k_fwd_cols): DFT over nl
+//   every 256-point DFT is 16 x 16: a half-warp owns one DFT, each lane 16 points in registers.
+//
+// "Tile layout" of a spectrum (bank, segments, forward scratch): for tile b (columns k1 = 16 b + c),
+// kept row-block i (rows k2 = g + 16 i), element index ((b*NI + (i - I0))*16 + c)*16 + g, so that the 16
+// lanes g of a half-warp (and the two half-warps c, c+1 of a warp) read contiguous memory.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "../../include/bege.h"
+#include "cplx.cuh"
+
+namespace bege {
+
+constexpr int kN = 65536;
+constexpr int kBatch = 72;                 // correlations in flight between pass 1 and pass 2 (36 MB of L2)
+constexpr int kGroups = 18;                // persistent CTA groups per tile: 16 tiles x 18 = 288 CTAs ~ 2 per SM
+
+// ------------------------------------------------------------------------------------------------
+// shared-memory exchange index for the column passes: stage-1 thread (c, g) writes its p-th value,
+// stage-2 thread (c, p) reads over g.  XOR swizzle keeps both sides bank-conflict free (8-byte words).
+BEGE_D int xidx(int c, int g, int p) { return ((p << 4) + g) * 16 + (c ^ g); }
+// private 256-element region of a half-warp: lane a writes its p-th value, lane p reads over a
+BEGE_D int pidx(int a, int p) { return (a << 4) + (p ^ a); }
+
+// stage 1 of a 256-point DFT held by a half-warp: 16-point DFT over the register index, then the
+// w256^(DIR * lane * p) twiddles (w1[p] = exp(+2 pi i lane p / 256), conjugated for DIR < 0)
+template <int DIR>
+BEGE_D void stage1(c2 (&v)[16], const float2 (&w1)[16]) {
+    fft16<DIR>(v);
+#pragma unroll
+    for (int p = 1; p < 16; ++p) v[p] = cmul(v[p], w1[p].x, DIR > 0 ? w1[p].y : -w1[p].y);
+}
+
+// full 256-point DFT of a half-warp through its private shared-memory region.
+// in: lane a holds x[a + 16 i] in v[i];  out: lane p holds X[p + 16 q] in v[q].
+template <int DIR>
+BEGE_D void hw_fft256(c2 (&v)[16], const float2 (&w1)[16], c2* priv, int lane16) {
+    stage1<DIR>(v, w1);
+#pragma unroll
+    for (int p = 0; p < 16; ++p) priv[pidx(lane16, p)] = v[p];
+    __syncwarp();
+#pragma unroll
+    for (int a = 0; a < 16; ++a) v[a] = priv[pidx(a, lane16)];
+    __syncwarp();
+    fft16<DIR>(v);
+}
+
+BEGE_D void load_w1(float2 (&w1)[16], const float2* __restrict__ tw256, int lane16) {
+#pragma unroll
+    for (int p = 0; p < 16; ++p) w1[p] = __ldg(tw256 + p * 16 + lane16);
+}
+
+// ------------------------------------------------------------------------------------------------
+// a1, step A: chirp synthesis (fp64 phase) + pruned row DFTs.  grid (16, n_templates_in_batch), 256 thr.
+// CTA (ia, jl): the 16 rows nl = ga + 16 ia (ga = half-warp index); only nh < 16 inputs are non-zero
+// (L <= 4096), so X[k1 = p + 16 q] = sum_nh h[nl + 256 nh] w256^(-nh p) w16^(-nh q): lane p twiddles the
+// 16 samples and runs one 16-point DFT.  Output -> G tile layout, times wN^(-nl k1).
+__global__ void __launch_bounds__(256)
+k_fwd_rows_chirp(const double* __restrict__ f0, const double* __restrict__ fdot, uint64_t j0,
+                 double fs, uint32_t L, double inv_norm,
+                 const float2* __restrict__ tw256, const float2* __restrict__ twN, c2* __restrict__ G)
+{
+    __shared__ c2 samp[16][16];          // [nh][ga]
+    const int t = threadIdx.x, ia = blockIdx.x;
+    const uint64_t jl = blockIdx.y;
+    {
+        const int ga = t & 15, nh = t >> 4;
+        const uint32_t n = ga + 16 * ia + 256 * nh;
+        c2 s = mk(0.f, 0.f);
+        if (n < L) {
+            const double tt = (double)n / fs;
+            const double cyc = f0[j0 + jl] * tt + 0.5 * fdot[j0 + jl] * tt * tt;
+            const double fr = cyc - floor(cyc);
+            double sn, cs;
+            sincospi(2.0 * fr, &sn, &cs);
+            const double w = (0.5 - 0.5 * cospi(2.0 * (double)n / (double)(L - 1))) * inv_norm;
+            s = mk((float)(w * cs), (float)(w * sn));
+        }
+        samp[nh][ga] = s;
+    }
+    __syncthreads();
+    const int ga = t >> 4, p = t & 15;
+    const int nl = ga + 16 * ia;
+    c2 v[16];
+#pragma unroll
+    for (int nh = 0; nh < 16; ++nh) {
+        const float2 w = __ldg(tw256 + p * 16 + nh);           // exp(+2 pi i nh p / 256)
+        v[nh] = cmul(samp[nh][ga], w.x, -w.y);
+    }
+    fft16<-1>(v);
+    c2* out = G + jl * (uint64_t)kN;
+#pragma unroll
+    for (int q = 0; q < 16; ++q) {
+        const int k1 = p + 16 * q;
+        const float2 w = __ldg(twN + nl * 256 + k1);           // exp(+2 pi i nl k1 / N)
+        out[((q * 16 + ia) * 16 + p) * 16 + ga] = cmul(v[q], w.x, -w.y);
+    }
+}
+
+// a2, step A: full row DFTs of a data segment.  grid (16, n_segments), 256 thr.
+__global__ void __launch_bounds__(256)
+k_fwd_rows_data(const c2* __restrict__ x, const float2* __restrict__ tw256, const float2* __restrict__ twN,
+                c2* __restrict__ G)
+{
+    __shared__ c2 sm[16][256];
+    const int t = threadIdx.x, ia = blockIdx.x;
+    const uint64_t m = blockIdx.y;
+    const int ga = t >> 4, a = t & 15;
+    const int nl = ga + 16 * ia;
+    float2 w1[16];
+    load_w1(w1, tw256, a);
+    const c2* xin = x + m * (uint64_t)kN;
+    c2 v[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) v[i] = xin[nl + 256 * (a + 16 * i)];
+    hw_fft256<-1>(v, w1, sm[ga], a);
+    c2* out = G + m * (uint64_t)kN;
+    const int p = a;
+#pragma unroll
+    for (int q = 0; q < 16; ++q) {
+        const int k1 = p + 16 * q;
+        const float2 w = __ldg(twN + nl * 256 + k1);
+        out[((q * 16 + ia) * 16 + p) * 16 + ga] = cmul(v[q], w.x, -w.y);
+    }
+}
+
+// step B of both forward transforms: column DFTs over nl.  grid (16 tiles, batch), 256 thr.
+// Reads G (tile layout, all 16 row-blocks), writes the kept row-blocks [I0, I0+NI) of the spectrum in
+// tile layout.  MASK: zero bins outside klo <= min(k, N-k) <= khi (segments).
+template <bool MASK>
+__global__ void __launch_bounds__(256)
+k_fwd_cols(const c2* __restrict__ G, c2* __restrict__ out, uint64_t out_stride, int I0, int NI,
+           const float2* __restrict__ tw256, uint32_t klo, uint32_t khi)
+{
+    __shared__ c2 sm[16][256];
+    const int t = threadIdx.x, b = blockIdx.x;
+    const uint64_t jl = blockIdx.y;
+    const int c = t >> 4, g = t & 15;
+    float2 w1[16];
+    load_w1(w1, tw256, g);
+    const c2* in = G + jl * (uint64_t)kN + (uint64_t)b * 4096;
+    c2 v[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) v[i] = in[(i * 16 + c) * 16 + g];
+    hw_fft256<-1>(v, w1, sm[c], g);
+    // lane p = g holds k2 = p + 16 q
+    c2* o = out + jl * out_stride + (uint64_t)b * NI * 256;
+    const uint32_t k1 = 16 * b + c;
+#pragma unroll
+    for (int q = 0; q < 16; ++q) {
+        if (q < I0 || q >= I0 + NI) continue;
+        c2 val = v[q];
+        if (MASK) {
+            const uint32_t k = k1 + 256u * (uint32_t)(g + 16 * q);
+            const uint32_t kk = k < (uint32_t)kN / 2 ? k : (uint32_t)kN - k;
+            if (kk < klo || kk > khi) val = mk(0.f, 0.f);
+        }
+        o[((q - I0) * 16 + c) * 16 + g] = val;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a3 + a4 + first half of a5: conj(H) X, Parseval partial sums, column DFTs, four-step twiddle.
+// grid (16 tiles, kGroups); CTA (b, grp) keeps its tile of the segment spectrum (SINGLE) and all its
+// twiddles in registers and loops over the templates of the batch.  256 threads:
+//   stage 1: half-warp c, lane g: k2 = g + 16 i  (coalesced tile-layout loads)
+//   exchange through shared memory (double buffered, one __syncthreads per correlation)
+//   stage 2: lane c, p = warp pair index: n2 = p + 16 q, stores T[n2][16 b + c] (128 B per half-warp)
+template <int I0, int NI, bool SINGLE>
+__global__ void __launch_bounds__(256, 2)
+k_inv_cols(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restrict__ T,
+           float* __restrict__ sigpart, const float2* __restrict__ tw256, const float2* __restrict__ twN,
+           uint64_t j0, int Tb, int m0, int Sb, int S)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    c2* sm = reinterpret_cast<c2*>(smem_raw);                 // [2][4096]
+    float* red = reinterpret_cast<float*>(sm + 2 * 4096);     // [2][8]
+    const int t = threadIdx.x, b = blockIdx.x, grp = blockIdx.y, ngrp = gridDim.y;
+    const int c = t >> 4, g = t & 15;                         // stage-1 role
+    const int c2i = t & 15, p2 = t >> 4;                      // stage-2 role
+    constexpr uint64_t kTile = (uint64_t)NI * 256;            // elements per (spectrum, tile)
+
+    float2 w1[16], wN[16];
+    load_w1(w1, tw256, g);
+#pragma unroll
+    for (int q = 0; q < 16; ++q) wN[q] = __ldg(twN + (p2 + 16 * q) * 256 + 16 * b + c2i);
+
+    c2 xr[NI];
+    if (SINGLE) {
+        const c2* xb = xseg + ((uint64_t)m0 * 16 + b) * kTile;
+#pragma unroll
+        for (int ii = 0; ii < NI; ++ii) xr[ii] = xb[(ii * 16 + c) * 16 + g];
+    }
+    int it = 0;
+    for (int jl = grp; jl < Tb; jl += ngrp) {
+        const c2* hb = bank + ((j0 + jl) * 16 + b) * kTile;
+        c2 h[NI];
+#pragma unroll
+        for (int ii = 0; ii < NI; ++ii) h[ii] = __ldcs(hb + (ii * 16 + c) * 16 + g);
+        for (int ml = 0; ml < Sb; ++ml, ++it) {
+            c2 v[16];
+            c2 acc = mk(0.f, 0.f);
+            if (!SINGLE) {
+                const c2* xb = xseg + ((uint64_t)(m0 + ml) * 16 + b) * kTile;
+#pragma unroll
+                for (int ii = 0; ii < NI; ++ii) xr[ii] = __ldg(xb + (ii * 16 + c) * 16 + g);
+            }
+#pragma unroll
+            for (int i = 0; i < 16; ++i) {
+                if (i >= I0 && i < I0 + NI) {
+                    v[i] = cmulc(xr[i - I0], h[i - I0]);
+                    acc = fma2(v[i], v[i], acc);
+                } else {
+                    v[i] = mk(0.f, 0.f);
+                }
+            }
+            stage1<+1>(v, w1);
+            c2* buf = sm + (it & 1) * 4096;
+            float* rbuf = red + (it & 1) * 8;
+#pragma unroll
+            for (int p = 0; p < 16; ++p) buf[xidx(c, g, p)] = v[p];
+            const float s = warp_sum32(re(acc) + im(acc));
+            if ((t & 31) == 0) rbuf[t >> 5] = s;
+            __syncthreads();
+#pragma unroll
+            for (int gg = 0; gg < 16; ++gg) v[gg] = buf[xidx(c2i, gg, p2)];
+            fft16<+1>(v);
+            c2* out = T + (uint64_t)(jl * Sb + ml) * kN + 16 * b + c2i;
+#pragma unroll
+            for (int q = 0; q < 16; ++q) out[(p2 + 16 * q) * 256] = cmul(v[q], wN[q]);
+            if (t == 0) {
+                float tot = 0.f;
+#pragma unroll
+                for (int w = 0; w < 8; ++w) tot += rbuf[w];
+                sigpart[((j0 + jl) * (uint64_t)S + (m0 + ml)) * 16 + b] = tot;
+            }
+        }
+    }
+}
+
+// second half of a5 + a6 + a7: row DFTs over k1, threshold |Z|^2 > k^2 sum|R|^2, warp-aggregated compaction.
+// grid (16 row tiles, kGroups); half-warp hw of CTA rt owns row n2 = 16 rt + hw; warps never synchronise
+// with each other.  DEBUG additionally writes z = Z/N to zdbg in lag order (off the timed path).
+template <bool DEBUG>
+__global__ void __launch_bounds__(256, 2)
+k_inv_rows(const c2* __restrict__ T, const float* __restrict__ sigpart, const float2* __restrict__ tw256,
+           float k2, bege_tail* __restrict__ rec, unsigned long long cap, unsigned long long* __restrict__ counter,
+           c2* __restrict__ zdbg, uint64_t j0, int Tb, int m0, int Sb, int S)
+{
+    __shared__ c2 sm[16][256];
+    const int t = threadIdx.x, rt = blockIdx.x, grp = blockIdx.y, ngrp = gridDim.y;
+    const int hw = t >> 4, a = t & 15, lane = t & 31;
+    const int n2 = 16 * rt + hw;
+    float2 w1[16];
+    load_w1(w1, tw256, a);
+    const int items = Tb * Sb;
+    for (int item = grp; item < items; item += ngrp) {
+        const int jl = item / Sb, ml = item - jl * Sb;
+        const c2* src = T + (uint64_t)item * kN + n2 * 256 + a;
+        c2 v[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) v[i] = __ldcg(src + 16 * i);
+        const uint64_t pair = (j0 + jl) * (uint64_t)S + (m0 + ml);
+        const float sumR2 = hw_sum16(__ldcg(sigpart + pair * 16 + a));
+        hw_fft256<+1>(v, w1, sm[hw], a);
+        // lane p = a holds Z[n1 = p + 16 q]; lag n = 256 n1 + n2
+        const float thr = k2 * sumR2;
+        unsigned hits = 0;
+        float m2[16];
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+            const c2 sq = mul2(v[q], v[q]);
+            m2[q] = re(sq) + im(sq);
+            if (m2[q] > thr) hits |= 1u << q;
+        }
+        if (DEBUG) {
+            const float invN = 1.0f / (float)kN;
+#pragma unroll
+            for (int q = 0; q < 16; ++q)
+                zdbg[(uint64_t)(a + 16 * q) * 256 + n2] = mul2(v[q], bc(invN));
+        }
+        if (__any_sync(0xffffffffu, hits != 0)) {
+            const int cnt = __popc(hits);
+            int incl = cnt;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int o = __shfl_up_sync(0xffffffffu, incl, d);
+                if (lane >= d) incl += o;
+            }
+            const int total = __shfl_sync(0xffffffffu, incl, 31);
+            unsigned long long base = 0;
+            if (lane == 31) base = atomicAdd(counter, (unsigned long long)total);
+            base = __shfl_sync(0xffffffffu, base, 31);
+            unsigned long long slot = base + (unsigned long long)(incl - cnt);
+            const float inv = 1.0f / sumR2;
+#pragma unroll
+            for (int q = 0; q < 16; ++q) {
+                if (hits & (1u << q)) {
+                    if (slot < cap) {
+                        bege_tail r;
+                        r.template_id = (uint32_t)(j0 + jl);
+                        r.lag = (uint32_t)(m0 + ml) * (uint32_t)kN + (uint32_t)((a + 16 * q) * 256 + n2);
+                        r.snr = sqrtf(m2[q] * inv);
+                        rec[slot] = r;
+                    }
+                    ++slot;
+                }
+            }
+        }
+    }
+}
+
+// sigma_jm = sqrt(sum of the 16 tile partial sums) / N
+__global__ void k_sigma(const float* __restrict__ sigpart, float* __restrict__ sigma, uint64_t n)
+{
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float s = 0.f;
+    // same pairwise order as hw_sum16 (xor 8, 4, 2, 1) so that sigma matches the search bit for bit
+    float v[16];
+    for (int a = 0; a < 16; ++a) v[a] = sigpart[i * 16 + a];
+    for (int d = 8; d >= 1; d >>= 1)
+        for (int a = 0; a < d; ++a) v[a] = v[a] + v[a + d];
+    s = v[0];
+    sigma[i] = sqrtf(s) / (float)kN;
+}
+
+}  // namespace bege
+
+// =================================================================================================
+// host side
+// =================================================================================================
+using namespace bege;
+
+struct Slot { uint64_t off = 0, bytes = 0; void* own = nullptr; };
+
+struct bege_plan {
+    int device = 0;
+    cudaStream_t stream = nullptr, side = nullptr;
+    bool own_stream = false;
+    uint32_t N = 0;
+    double fs = 0, lo = 0, hi = 0;
+    uint32_t klo = 0, khi = 0;
+    int I0 = 0, NI = 16;
+    float2 *tw256 = nullptr, *twN = nullptr;
+    // workspace
+    unsigned char* ws = nullptr; uint64_t ws_bytes = 0, bump = 0; bool user_ws = false;
+    Slot s_bank, s_x, s_scratch, s_sig, s_rec, s_misc, s_par;
+    uint64_t T = 0; uint32_t S = 0; double tau = 0; uint32_t L = 0;
+    bool have_sigma = false;
+    // pinned staging
+    unsigned long long* h_count = nullptr;
+    cudaEvent_t ev_a = nullptr, ev_b = nullptr, ev_done = nullptr;
+    bool profiling = false;
+    bege_stats stats{};
+    std::string err;
+};
+
+static int fail(bege_plan* p, int code, const char* fmt, ...)
+{
+    if (p) {
+        char buf[512];
+        va_list ap; va_start(ap, fmt); vsnprintf(buf, sizeof buf, fmt, ap); va_end(ap);
+        p->err = buf;
+    }
+    return code;
+}
+#define CU(p, call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return fail((p), BEGE_ECUDA, "%s: %s", #call, cudaGetErrorString(e_)); } while (0)
+
+static uint64_t align_up(uint64_t v, uint64_t a) { return (v + a - 1) / a * a; }
+
+// (re)size a slot: reuse if big enough; own memory if no user workspace, else bump-allocate from it
+static int slot_get(bege_plan* p, Slot& s, uint64_t need, void** out)
+{
+    need = align_up(need ? need : 256, 256);
+    if (!p->user_ws) {
+        if (s.bytes < need) {
+            if (s.own) { cudaFree(s.own); s.own = nullptr; s.bytes = 0; }
+            cudaError_t e = cudaMalloc(&s.own, need);
+            if (e != cudaSuccess) { cudaGetLastError(); return fail(p, BEGE_ENOMEM, "cudaMalloc(%llu) failed: %s", (unsigned long long)need, cudaGetErrorString(e)); }
+            s.bytes = need;
+        }
+        *out = s.own;
+        return BEGE_OK;
+    }
+    if (s.bytes < need) {
+        const bool last = s.bytes && s.off + s.bytes == p->bump;
+        if (last) p->bump = s.off;                       // grow the most recent slot in place
+        else if (s.bytes) return fail(p, BEGE_ENOMEM, "workspace slot cannot grow (%llu -> %llu bytes); call bege_plan_set_workspace again",
+                                      (unsigned long long)s.bytes, (unsigned long long)need);
+        if (p->bump + need > p->ws_bytes)
+            return fail(p, BEGE_ENOMEM, "workspace too small: need %llu more bytes, %llu of %llu used",
+                        (unsigned long long)need, (unsigned long long)p->bump, (unsigned long long)p->ws_bytes);
+        s.off = p->bump; s.bytes = need; p->bump += need;
+    }
+    *out = p->ws + s.off;
+    return BEGE_OK;
+}
+static void slot_free(Slot& s) { if (s.own) cudaFree(s.own); s = Slot(); }
+
+static uint64_t tpl_bytes(const bege_plan* p) { return (uint64_t)p->NI * 16 * 256 * sizeof(c2); }
+
+static void count_launch(bege_plan* p, uint64_t n = 1) { p->stats.kernel_launches += n; }
+
+extern "C" const char* bege_version(void) { return "bege 0.1 (sm_100a)"; }
+
+extern "C" const char* bege_last_error(const bege_plan* p) { return p ? p->err.c_str() : "null plan"; }
+
+extern "C" int bege_plan_create(bege_plan** out, uint32_t N, double fs, double lo, double hi, int device, void* stream)
+{
+    if (!out) return BEGE_EINVAL;
+    if (N != (uint32_t)kN || !(fs > 0) || !(lo > 0) || !(hi > lo) || !(hi < 0.5 * fs)) return BEGE_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) { cudaGetLastError(); return BEGE_ECUDA; }
+    bege_plan* p = new bege_plan();
+    p->device = device; p->N = N; p->fs = fs; p->lo = lo; p->hi = hi;
+    auto bail = [&](int code) { bege_plan_destroy(p); return code; };
+    if (cudaSetDevice(device) != cudaSuccess) return bail(BEGE_ECUDA);
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return bail(BEGE_ECUDA);
+    if (prop.major < 10) return bail(BEGE_ECUDA);              // sm_100a code only
+    if (stream) p->stream = (cudaStream_t)stream;
+    else { if (cudaStreamCreateWithFlags(&p->stream, cudaStreamNonBlocking) != cudaSuccess) return bail(BEGE_ECUDA); p->own_stream = true; }
+    if (cudaStreamCreateWithFlags(&p->side, cudaStreamNonBlocking) != cudaSuccess) return bail(BEGE_ECUDA);
+    if (cudaEventCreate(&p->ev_a) != cudaSuccess || cudaEventCreate(&p->ev_b) != cudaSuccess ||
+        cudaEventCreateWithFlags(&p->ev_done, cudaEventDisableTiming) != cudaSuccess) return bail(BEGE_ECUDA);
+    if (cudaMallocHost(&p->h_count, 64) != cudaSuccess) return bail(BEGE_ECUDA);
+
+    // band in bins, inclusive edges: klo = ceil(lo N/fs), khi = floor(hi N/fs)
+    const double df = fs / N;
+    p->klo = (uint32_t)ceil(lo / df - 1e-9);
+    p->khi = (uint32_t)floor(hi / df + 1e-9);
+    // kept row-blocks: block i holds rows k2 = g + 16 i, g < 16, i.e. bins [4096 i, 4096 i + 4095]; a block is
+    // kept when it (or its mirror at N - k) contains an in-band bin
+    bool keep[16];
+    int first = 16, last = -1;
+    for (int i = 0; i < 16; ++i) {
+        const uint32_t a = 4096u * i, b = a + 4095u;
+        auto hit = [&](uint32_t l, uint32_t h) { return !(b < l || a > h); };
+        keep[i] = hit(p->klo, p->khi) || hit(N - p->khi, N - p->klo);
+        if (keep[i]) { if (i < first) first = i; last = i; }
+    }
+    if (first == 1 && last == 14) { p->I0 = 1; p->NI = 14; } else { p->I0 = 0; p->NI = 16; }
+
+    std::vector<float2> w256(256), wN((size_t)256 * 256);
+    for (int pp = 0; pp < 16; ++pp)
+        for (int g = 0; g < 16; ++g) {
+            const double a = 2.0 * M_PI * (double)(g * pp) / 256.0;
+            w256[pp * 16 + g] = make_float2((float)cos(a), (float)sin(a));
+        }
+    for (int n2 = 0; n2 < 256; ++n2)
+        for (int k1 = 0; k1 < 256; ++k1) {
+            const double a = 2.0 * M_PI * (double)(n2 * k1) / (double)N;
+            wN[(size_t)n2 * 256 + k1] = make_float2((float)cos(a), (float)sin(a));
+        }
+    if (cudaMalloc(&p->tw256, w256.size() * sizeof(float2)) != cudaSuccess ||
+        cudaMalloc(&p->twN, wN.size() * sizeof(float2)) != cudaSuccess) return bail(BEGE_ENOMEM);
+    if (cudaMemcpy(p->tw256, w256.data(), w256.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(p->twN, wN.data(), wN.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess) return bail(BEGE_ECUDA);
+
+    const int smem = 2 * 4096 * (int)sizeof(c2) + 64;
+    cudaFuncSetAttribute(k_inv_cols<1, 14, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    cudaFuncSetAttribute(k_inv_cols<1, 14, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    cudaFuncSetAttribute(k_inv_cols<0, 16, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    cudaFuncSetAttribute(k_inv_cols<0, 16, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (cudaGetLastError() != cudaSuccess) return bail(BEGE_ECUDA);
+    p->stats.hbm_bytes_per_template = tpl_bytes(p);
+    *out = p;
+    return BEGE_OK;
+}
+
+extern "C" void bege_plan_destroy(bege_plan* p)
+{
+    if (!p) return;
+    cudaSetDevice(p->device);
+    if (p->stream) cudaStreamSynchronize(p->stream);
+    if (p->side) { cudaStreamSynchronize(p->side); cudaStreamDestroy(p->side); }
+    if (p->own_stream && p->stream) cudaStreamDestroy(p->stream);
+    for (Slot* s : {&p->s_bank, &p->s_x, &p->s_scratch, &p->s_sig, &p->s_rec, &p->s_misc, &p->s_par}) slot_free(*s);
+    if (p->tw256) cudaFree(p->tw256);
+    if (p->twN) cudaFree(p->twN);
+    if (p->h_count) cudaFreeHost(p->h_count);
+    if (p->ev_a) cudaEventDestroy(p->ev_a);
+    if (p->ev_b) cudaEventDestroy(p->ev_b);
+    if (p->ev_done) cudaEventDestroy(p->ev_done);
+    delete p;
+}
+
+static uint64_t scratch_bytes() { return (uint64_t)kBatch * kN * sizeof(c2); }
+
+extern "C" int bege_plan_workspace_bytes(const bege_plan* p, uint64_t T, uint32_t S, uint64_t cap, uint64_t* bytes)
+{
+    if (!p || !bytes) return BEGE_EINVAL;
+    auto al = [](uint64_t v) { return align_up(v ? v : 256, 256); };
+    uint64_t b = 0;
+    b += al(T * tpl_bytes(p));                         // bank
+    b += al(T * 16);                                   // template parameters (f0, fdot)
+    b += al((uint64_t)S * tpl_bytes(p));               // segment spectra
+    b += al(scratch_bytes());                          // four-step staging (stays in L2)
+    b += al(T * S * 16 * sizeof(float));               // Parseval partial sums
+    b += al(cap * sizeof(bege_tail));                  // records
+    b += al(256 + (uint64_t)S * kN * sizeof(c2));      // counter + raw segment staging
+    *bytes = b + 4096;
+    return BEGE_OK;
+}
+
+extern "C" int bege_plan_set_workspace(bege_plan* p, void* dev_ptr, uint64_t bytes)
+{
+    if (!p) return BEGE_EINVAL;
+    if (dev_ptr && ((uintptr_t)dev_ptr & 255)) return fail(p, BEGE_EINVAL, "workspace must be 256-byte aligned");
+    CU(p, cudaSetDevice(p->device));
+    CU(p, cudaStreamSynchronize(p->stream));
+    for (Slot* s : {&p->s_bank, &p->s_x, &p->s_scratch, &p->s_sig, &p->s_rec, &p->s_misc, &p->s_par}) slot_free(*s);
+    p->ws = (unsigned char*)dev_ptr; p->ws_bytes = dev_ptr ? bytes : 0; p->bump = 0; p->user_ws = dev_ptr != nullptr;
+    p->T = 0; p->S = 0; p->have_sigma = false;
+    return BEGE_OK;
+}
+
+extern "C" int bege_bank_generate(bege_plan* p, const double* f0, const double* fdot, uint64_t T, double tau)
+{
+    if (!p) return BEGE_EINVAL;
+    if (!f0 || !fdot || T == 0 || T > 0xffffffffull) return fail(p, BEGE_EINVAL, "bad bank arguments");
+    const long Ll = lround(tau * p->fs);
+    if (Ll < 2 || Ll > kN / 16) return fail(p, BEGE_EINVAL, "tau*fs = %ld outside [2, %d]", Ll, kN / 16);
+    CU(p, cudaSetDevice(p->device));
+    void *bank, *par, *scr;
+    int rc;
+    if ((rc = slot_get(p, p->s_bank, T * tpl_bytes(p), &bank))) return rc;
+    if ((rc = slot_get(p, p->s_par, T * 16, &par))) return rc;
+    if ((rc = slot_get(p, p->s_scratch, scratch_bytes(), &scr))) return rc;
+    p->T = 0; p->have_sigma = false;
+    double* d_f0 = (double*)par; double* d_fd = d_f0 + T;
+    CU(p, cudaMemcpyAsync(d_f0, f0, T * sizeof(double), cudaMemcpyHostToDevice, p->stream));
+    CU(p, cudaMemcpyAsync(d_fd, fdot, T * sizeof(double), cudaMemcpyHostToDevice, p->stream));
+    // unit L2 norm: ||h||^2 = sum_n hann_L[n]^2 (the phase factor has modulus 1)
+    const uint32_t L = (uint32_t)Ll;
+    double n2 = 0;
+    for (uint32_t n = 0; n < L; ++n) { const double w = 0.5 - 0.5 * cos(2.0 * M_PI * n / (double)(L - 1)); n2 += w * w; }
+    const double inv_norm = 1.0 / sqrt(n2);
+    const uint64_t stride = tpl_bytes(p) / sizeof(c2);
+    for (uint64_t j0 = 0; j0 < T; j0 += kBatch) {
+        const unsigned nb = (unsigned)std::min<uint64_t>(kBatch, T - j0);
+        k_fwd_rows_chirp<<<dim3(16, nb), 256, 0, p->stream>>>(d_f0, d_fd, j0, p->fs, L, inv_norm, p->tw256, p->twN, (c2*)scr);
+        k_fwd_cols<false><<<dim3(16, nb), 256, 0, p->stream>>>((const c2*)scr, (c2*)bank + j0 * stride, stride, p->I0, p->NI, p->tw256, 0, 0);
+        count_launch(p, 2);
+    }
+    CU(p, cudaGetLastError());
+    CU(p, cudaStreamSynchronize(p->stream));
+    p->T = T; p->tau = tau; p->L = L;
+    return BEGE_OK;
+}
+
+extern "C" int bege_segment_load(bege_plan* p, const float* x, uint32_t S)
+{
+    if (!p) return BEGE_EINVAL;
+    if (!x || S == 0 || (uint64_t)S * kN > 0xffffffffull) return fail(p, BEGE_EINVAL, "bad segment arguments");
+    CU(p, cudaSetDevice(p->device));
+    void *xs, *misc, *scr;
+    int rc;
+    if ((rc = slot_get(p, p->s_x, (uint64_t)S * tpl_bytes(p), &xs))) return rc;
+    if ((rc = slot_get(p, p->s_misc, 256 + (uint64_t)S * kN * sizeof(c2), &misc))) return rc;
+    if ((rc = slot_get(p, p->s_scratch, scratch_bytes(), &scr))) return rc;
+    p->S = 0; p->have_sigma = false;
+    c2* raw = (c2*)((unsigned char*)misc + 256);
+    cudaPointerAttributes at;
+    cudaError_t e = cudaPointerGetAttributes(&at, x);
+    if (e != cudaSuccess) { cudaGetLastError(); at.type = cudaMemoryTypeUnregistered; }
+    const bool on_dev = at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+    CU(p, cudaMemcpyAsync(raw, x, (uint64_t)S * kN * sizeof(c2), on_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, p->stream));
+    const uint64_t stride = tpl_bytes(p) / sizeof(c2);
+    for (uint32_t m0 = 0; m0 < S; m0 += kBatch) {
+        const unsigned nb = std::min<uint32_t>(kBatch, S - m0);
+        k_fwd_rows_data<<<dim3(16, nb), 256, 0, p->stream>>>(raw + (uint64_t)m0 * kN, p->tw256, p->twN, (c2*)scr);
+        k_fwd_cols<true><<<dim3(16, nb), 256, 0, p->stream>>>((const c2*)scr, (c2*)xs + m0 * stride, stride, p->I0, p->NI, p->tw256, p->klo, p->khi);
+        count_launch(p, 2);
+    }
+    CU(p, cudaGetLastError());
+    CU(p, cudaStreamSynchronize(p->stream));
+    p->S = S;
+    return BEGE_OK;
+}
+
+template <bool DEBUG>
+static void launch_pair(bege_plan* p, const c2* bank, const c2* xs, c2* scr, float* sig, float k2, bege_tail* rec,
+                        uint64_t cap, unsigned long long* counter, c2* zdbg, uint64_t j0, int Tb, int m0, int Sb)
+{
+    const int smem = 2 * 4096 * (int)sizeof(c2) + 64;
+    const dim3 grid(16, kGroups);
+    const bool single = (p->S == 1);
+    if (p->profiling) cudaEventRecord(p->ev_a, p->stream);
+#define BEGE_COLS(I0, NI, SG) k_inv_cols<I0, NI, SG><<<grid, 256, smem, p->stream>>>(bank, xs, scr, sig, p->tw256, p->twN, j0, Tb, m0, Sb, (int)p->S)
+    if (p->NI == 14) { if (single) BEGE_COLS(1, 14, true); else BEGE_COLS(1, 14, false); }
+    else             { if (single) BEGE_COLS(0, 16, true); else BEGE_COLS(0, 16, false); }
+#undef BEGE_COLS
+    k_inv_rows<DEBUG><<<grid, 256, 0, p->stream>>>(scr, sig, p->tw256, k2, rec, cap, counter, zdbg, j0, Tb, m0, Sb, (int)p->S);
+    count_launch(p, 2);
+    if (p->profiling) {
+        cudaEventRecord(p->ev_b, p->stream);
+        cudaEventSynchronize(p->ev_b);
+        float ms = 0; cudaEventElapsedTime(&ms, p->ev_a, p->ev_b);
+        p->stats.fused_kernel_ms += ms; p->stats.fused_kernel_launches += 2;
+    }
+}
+
+extern "C" int bege_search(bege_plan* p, float k_sigma, bege_tail* tails_out, uint64_t cap, uint64_t* n_tails)
+{
+    if (!p) return BEGE_EINVAL;
+    if (!n_tails || (cap && !tails_out) || !(k_sigma >= 0.f)) return fail(p, BEGE_EINVAL, "bad search arguments");
+    if (!p->T || !p->S) return fail(p, BEGE_ESTATE, "bege_search needs a generated bank and loaded segments");
+    CU(p, cudaSetDevice(p->device));
+    void *sig, *rec, *misc, *scr, *bank, *xs;
+    int rc;
+    if ((rc = slot_get(p, p->s_sig, p->T * p->S * 16 * sizeof(float), &sig))) return rc;
+    if ((rc = slot_get(p, p->s_rec, cap * sizeof(bege_tail), &rec))) return rc;
+    if ((rc = slot_get(p, p->s_misc, 256, &misc))) return rc;
+    if ((rc = slot_get(p, p->s_scratch, scratch_bytes(), &scr))) return rc;
+    if ((rc = slot_get(p, p->s_bank, 0, &bank))) return rc;
+    if ((rc = slot_get(p, p->s_x, 0, &xs))) return rc;
+    unsigned long long* counter = (unsigned long long*)misc;
+    CU(p, cudaMemsetAsync(counter, 0, sizeof(unsigned long long), p->stream));
+    const int Sb = (int)std::min<uint32_t>(p->S, kBatch);
+    const int Tbmax = kBatch / Sb;
+    for (uint32_t m0 = 0; m0 < p->S; m0 += Sb) {
+        const int sb = (int)std::min<uint32_t>(Sb, p->S - m0);
+        for (uint64_t j0 = 0; j0 < p->T; j0 += Tbmax) {
+            const int tb = (int)std::min<uint64_t>(Tbmax, p->T - j0);
+            launch_pair<false>(p, (const c2*)bank, (const c2*)xs, (c2*)scr, (float*)sig, k_sigma * k_sigma,
+                               (bege_tail*)rec, cap, counter, nullptr, j0, tb, (int)m0, sb);
+        }
+    }
+    CU(p, cudaGetLastError());
+    // only the tails cross PCIe: count first, then exactly the records, on the side stream
+    CU(p, cudaMemcpyAsync(p->h_count, counter, sizeof(unsigned long long), cudaMemcpyDeviceToHost, p->stream));
+    CU(p, cudaEventRecord(p->ev_done, p->stream));
+    CU(p, cudaStreamWaitEvent(p->side, p->ev_done, 0));
+    CU(p, cudaStreamSynchronize(p->stream));
+    const uint64_t total = *p->h_count;
+    const uint64_t ncopy = std::min<uint64_t>(total, cap);
+    if (ncopy) {
+        CU(p, cudaMemcpyAsync(tails_out, rec, ncopy * sizeof(bege_tail), cudaMemcpyDeviceToHost, p->side));
+        CU(p, cudaStreamSynchronize(p->side));
+    }
+    p->stats.correlations += p->T * p->S;
+    p->have_sigma = true;
+    *n_tails = total;
+    if (total > cap) return fail(p, BEGE_EOVERFLOW, "%llu tails exceed cap %llu", (unsigned long long)total, (unsigned long long)cap);
+    return BEGE_OK;
+}
+
+extern "C" int bege_get_sigma(bege_plan* p, float* sigma_out)
+{
+    if (!p || !sigma_out) return BEGE_EINVAL;
+    if (!p->have_sigma) return fail(p, BEGE_ESTATE, "bege_get_sigma needs a completed bege_search");
+    CU(p, cudaSetDevice(p->device));
+    const uint64_t n = p->T * p->S;
+    float* d = nullptr;
+    CU(p, cudaMalloc(&d, n * sizeof(float)));
+    void* sig; slot_get(p, p->s_sig, 0, &sig);
+    k_sigma<<<(unsigned)((n + 255) / 256), 256, 0, p->stream>>>((const float*)sig, d, n);
+    count_launch(p);
+    cudaError_t e = cudaMemcpyAsync(sigma_out, d, n * sizeof(float), cudaMemcpyDeviceToHost, p->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
+    cudaFree(d);
+    CU(p, e);
+    return BEGE_OK;
+}
+
+extern "C" int bege_debug_correlate(bege_plan* p, uint64_t j, uint32_t m, float* z_out, float* sigma_out)
+{
+    if (!p || !z_out) return BEGE_EINVAL;
+    if (!p->T || !p->S) return fail(p, BEGE_ESTATE, "needs a bank and segments");
+    if (j >= p->T || m >= p->S) return fail(p, BEGE_EINVAL, "pair (%llu, %u) out of range", (unsigned long long)j, m);
+    CU(p, cudaSetDevice(p->device));
+    void *scr, *bank, *xs;
+    int rc;
+    if ((rc = slot_get(p, p->s_scratch, scratch_bytes(), &scr))) return rc;
+    slot_get(p, p->s_bank, 0, &bank); slot_get(p, p->s_x, 0, &xs);
+    c2* zd = nullptr; float* sg = nullptr; unsigned long long* cnt = nullptr;
+    CU(p, cudaMalloc(&zd, kN * sizeof(c2)));
+    CU(p, cudaMalloc(&sg, 16 * sizeof(float)));         // private partial sums of this one pair
+    CU(p, cudaMalloc(&cnt, 8));
+    cudaMemsetAsync(cnt, 0, 8, p->stream);
+    const bool prof = p->profiling; p->profiling = false;
+    // the kernels index the partial sums by (j*S + m)*16: bias the base so that this pair lands on sg[0..15]
+    float* sg_biased = sg - (j * p->S + m) * 16;
+    launch_pair<true>(p, (const c2*)bank, (const c2*)xs, (c2*)scr, sg_biased, 1e30f, nullptr, 0, cnt, zd, j, 1, (int)m, 1);
+    p->profiling = prof;
+    float part[16];
+    cudaError_t e = cudaMemcpyAsync(z_out, zd, kN * sizeof(c2), cudaMemcpyDeviceToHost, p->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(part, sg, sizeof part, cudaMemcpyDeviceToHost, p->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    cudaFree(zd); cudaFree(sg); cudaFree(cnt);
+    CU(p, e);
+    if (sigma_out) {
+        float v[16];
+        for (int a = 0; a < 16; ++a) v[a] = part[a];
+        for (int d = 8; d >= 1; d >>= 1) for (int a = 0; a < d; ++a) v[a] = v[a] + v[a + d];
+        *sigma_out = sqrtf(v[0]) / (float)kN;
+    }
+    return BEGE_OK;
+}
+
+// tile layout -> natural order, on the host (debug only)
+static void untile(const bege_plan* p, const std::vector<float2>& tile, float* out)
+{
+    memset(out, 0, sizeof(float) * 2 * kN);
+    for (int b = 0; b < 16; ++b)
+        for (int ii = 0; ii < p->NI; ++ii)
+            for (int c = 0; c < 16; ++c)
+                for (int g = 0; g < 16; ++g) {
+                    const float2 v = tile[(((size_t)b * p->NI + ii) * 16 + c) * 16 + g];
+                    const size_t k = (size_t)(16 * b + c) + 256 * (size_t)(g + 16 * (ii + p->I0));
+                    out[2 * k] = v.x; out[2 * k + 1] = v.y;
+                }
+}
+
+extern "C" int bege_debug_template_spectrum(bege_plan* p, uint64_t j, float* H_out)
+{
+    if (!p || !H_out) return BEGE_EINVAL;
+    if (j >= p->T) return fail(p, BEGE_EINVAL, "template %llu out of range", (unsigned long long)j);
+    CU(p, cudaSetDevice(p->device));
+    void* bank; slot_get(p, p->s_bank, 0, &bank);
+    std::vector<float2> tile(tpl_bytes(p) / sizeof(float2));
+    CU(p, cudaMemcpyAsync(tile.data(), (unsigned char*)bank + j * tpl_bytes(p), tpl_bytes(p), cudaMemcpyDeviceToHost, p->stream));
+    CU(p, cudaStreamSynchronize(p->stream));
+    untile(p, tile, H_out);
+    return BEGE_OK;
+}
+
+extern "C" int bege_debug_segment_spectrum(bege_plan* p, uint32_t m, float* X_out)
+{
+    if (!p || !X_out) return BEGE_EINVAL;
+    if (m >= p->S) return fail(p, BEGE_EINVAL, "segment %u out of range", m);
+    CU(p, cudaSetDevice(p->device));
+    void* xs; slot_get(p, p->s_x, 0, &xs);
+    std::vector<float2> tile(tpl_bytes(p) / sizeof(float2));
+    CU(p, cudaMemcpyAsync(tile.data(), (unsigned char*)xs + (uint64_t)m * tpl_bytes(p), tpl_bytes(p), cudaMemcpyDeviceToHost, p->stream));
+    CU(p, cudaStreamSynchronize(p->stream));
+    untile(p, tile, X_out);
+    return BEGE_OK;
+}
+
+extern "C" int bege_plan_set_profiling(bege_plan* p, int on) { if (!p) return BEGE_EINVAL; p->profiling = on != 0; return BEGE_OK; }
+extern "C" int bege_plan_get_stats(const bege_plan* p, bege_stats* out) { if (!p || !out) return BEGE_EINVAL; *out = p->stats; return BEGE_OK; }
+extern "C" int bege_plan_reset_stats(bege_plan* p)
+{
+    if (!p) return BEGE_EINVAL;
+    const uint64_t keep = p->stats.hbm_bytes_per_template;
+    p->stats = bege_stats{}; p->stats.hbm_bytes_per_template = keep;
+    return BEGE_OK;
+}

@@ -1,0 +1,115 @@
+// Packed complex fp32 arithmetic for sm_100a.
+//
+// A complex number lives in one 64-bit register pair as (re, im) and is processed with Blackwell's
+// packed fp32x2 instructions (PTX add/sub/mul/fma.rn.f32x2 -> SASS FADD2/FMUL2/FFMA2).  ptxas folds
+// the half swap (mk(im, re)) and the scalar broadcast (mk(s, s)) written below into operand
+// modifiers (.F32x2.LO_HI, .F32), so a complex add is 1 issue slot, a twiddle multiply 2, and a
+// multiplication by +-i fuses into the following add.  Measured on B200: FFMA2 issues at half the
+// rate of FFMA, i.e. the same flops in half the issue slots, which is what leaves room for the
+// load / shared-memory / integer instructions of the FFT passes.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace bege {
+
+typedef unsigned long long c2;   // packed (re, im), fp32 each
+
+#define BEGE_D __device__ __forceinline__
+
+BEGE_D c2 mk(float re, float im) { c2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(re), "f"(im)); return r; }
+BEGE_D float re(c2 v) { float a, b; asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); return a; }
+BEGE_D float im(c2 v) { float a, b; asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); return b; }
+BEGE_D c2 from_f2(float2 v) { return mk(v.x, v.y); }
+BEGE_D float2 to_f2(c2 v) { return make_float2(re(v), im(v)); }
+
+BEGE_D c2 add2(c2 a, c2 b) { c2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+BEGE_D c2 sub2(c2 a, c2 b) { c2 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+BEGE_D c2 mul2(c2 a, c2 b) { c2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+BEGE_D c2 fma2(c2 a, c2 b, c2 c) { c2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+
+BEGE_D c2 swp(c2 a) { return mk(im(a), re(a)); }
+BEGE_D c2 bc(float s) { return mk(s, s); }
+
+// a + i*b and a - i*b
+BEGE_D c2 add_i(c2 a, c2 b) { return fma2(swp(b), mk(-1.f, 1.f), a); }
+BEGE_D c2 sub_i(c2 a, c2 b) { return fma2(swp(b), mk(1.f, -1.f), a); }
+
+// x * (c + i d)
+BEGE_D c2 cmul(c2 x, float c, float d) { return fma2(swp(x), mk(-d, d), mul2(x, bc(c))); }
+BEGE_D c2 cmul(c2 x, float2 w) { return cmul(x, w.x, w.y); }
+// conj(h) * x
+BEGE_D c2 cmulc(c2 x, c2 h) {
+    const float hr = re(h), hi = im(h);
+    return fma2(swp(x), mk(hi, -hi), mul2(x, bc(hr)));
+}
+
+// 4-point DFT, DIR = +1: exp(+2 pi i jk/4) (inverse), DIR = -1: forward.  In place, natural order.
+template <int DIR>
+BEGE_D void fft4(c2& a0, c2& a1, c2& a2, c2& a3) {
+    const c2 s02 = add2(a0, a2), d02 = sub2(a0, a2);
+    const c2 s13 = add2(a1, a3), d13 = sub2(a1, a3);
+    a0 = add2(s02, s13);
+    a2 = sub2(s02, s13);
+    if (DIR > 0) { a1 = add_i(d02, d13); a3 = sub_i(d02, d13); }
+    else         { a1 = sub_i(d02, d13); a3 = add_i(d02, d13); }
+}
+
+// x * exp(DIR * 2 pi i m / 16), m a compile-time constant
+template <int DIR, int M>
+BEGE_D c2 tw16(c2 x) {
+    constexpr int m = ((M % 16) + 16) % 16;
+    constexpr float C1 = 0.92387953251128675613f, S1 = 0.38268343236508977173f, H = 0.70710678118654752440f;
+    if (m == 0) return x;
+    if (m == 4) return DIR > 0 ? mul2(swp(x), mk(-1.f, 1.f)) : mul2(swp(x), mk(1.f, -1.f));     // * (+-i)
+    if (m == 8) return mul2(x, bc(-1.f));
+    if (m == 12) return DIR > 0 ? mul2(swp(x), mk(1.f, -1.f)) : mul2(swp(x), mk(-1.f, 1.f));
+    // cos / sin of 2 pi m / 16
+    constexpr float c = (m == 1 || m == 15) ? C1 : (m == 2 || m == 14) ? H : (m == 3 || m == 13) ? S1
+                      : (m == 5 || m == 11) ? -S1 : (m == 6 || m == 10) ? -H : /* 7, 9 */ -C1;
+    constexpr float s0 = (m == 1 || m == 7) ? S1 : (m == 2 || m == 6) ? H : (m == 3 || m == 5) ? C1
+                       : (m == 9 || m == 15) ? -S1 : (m == 10 || m == 14) ? -H : /* 11, 13 */ -C1;
+    constexpr float s = DIR > 0 ? s0 : -s0;
+    return cmul(x, c, s);
+}
+
+// 16-point DFT in registers: A[k] = sum_i a[i] exp(DIR 2 pi i ik/16); in place, natural order in and out.
+// i = i0 + 4 i1, k = k0 + 4 k1:  radix-4 over i1, twiddle w16^(i0 k0), radix-4 over i0.
+template <int DIR>
+BEGE_D void fft16(c2 (&a)[16]) {
+#pragma unroll
+    for (int i0 = 0; i0 < 4; ++i0) fft4<DIR>(a[i0], a[i0 + 4], a[i0 + 8], a[i0 + 12]);
+    // now a[i0 + 4 k0] holds B[i0][k0]
+    a[1 + 4 * 1] = tw16<DIR, 1>(a[1 + 4 * 1]);
+    a[1 + 4 * 2] = tw16<DIR, 2>(a[1 + 4 * 2]);
+    a[1 + 4 * 3] = tw16<DIR, 3>(a[1 + 4 * 3]);
+    a[2 + 4 * 1] = tw16<DIR, 2>(a[2 + 4 * 1]);
+    a[2 + 4 * 2] = tw16<DIR, 4>(a[2 + 4 * 2]);
+    a[2 + 4 * 3] = tw16<DIR, 6>(a[2 + 4 * 3]);
+    a[3 + 4 * 1] = tw16<DIR, 3>(a[3 + 4 * 1]);
+    a[3 + 4 * 2] = tw16<DIR, 6>(a[3 + 4 * 2]);
+    a[3 + 4 * 3] = tw16<DIR, 9>(a[3 + 4 * 3]);
+    // radix-4 over i0 for each k0: inputs a[0 + 4k0], a[1 + 4k0], a[2 + 4k0], a[3 + 4k0] -> outputs k = k0 + 4 k1
+#pragma unroll
+    for (int k0 = 0; k0 < 4; ++k0) fft4<DIR>(a[4 * k0], a[4 * k0 + 1], a[4 * k0 + 2], a[4 * k0 + 3]);
+    // a[4 k0 + k1] now holds A[k0 + 4 k1]: transpose the 4x4 index (register renaming, free when unrolled)
+#pragma unroll
+    for (int k0 = 0; k0 < 4; ++k0)
+#pragma unroll
+        for (int k1 = k0 + 1; k1 < 4; ++k1) { const c2 t = a[4 * k0 + k1]; a[4 * k0 + k1] = a[4 * k1 + k0]; a[4 * k1 + k0] = t; }
+}
+
+// warp-level sum over the 16 lanes of a half-warp (all lanes get the result), fixed order
+BEGE_D float hw_sum16(float v) {
+    v += __shfl_xor_sync(0xffffffffu, v, 8);
+    v += __shfl_xor_sync(0xffffffffu, v, 4);
+    v += __shfl_xor_sync(0xffffffffu, v, 2);
+    v += __shfl_xor_sync(0xffffffffu, v, 1);
+    return v;
+}
+BEGE_D float warp_sum32(float v) {
+    v += __shfl_xor_sync(0xffffffffu, v, 16);
+    return hw_sum16(v);
+}
+
+}  // namespace bege

@@ -1,0 +1,288 @@
+"""Parity of the CUDA path (through the C ABI) against the fp64 CPU oracle.  `-m gpu` only.
+
+Bars (BASELINE.json north_star): correlation outputs rel-L2 <= 2e-5 per template; tail sets
+identical except for entries within 1e-4*sigma of the threshold; integer fields bit exact.
+"""
+import numpy as np
+import pytest
+
+from paper_1708_01609_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+FS, N, BAND, TAU = synth.FS, synth.N_SEG, synth.BAND, synth.TAU
+REL_L2 = 2e-5          # north_star
+GUARD = 1e-4           # north_star: entries within 1e-4 sigma of the threshold are exempt
+SIGMA_RTOL = 2e-6      # fp32 sum of 5e4 squares + sqrt: derived in DESIGN.md ("Tolerances")
+
+
+@pytest.fixture(scope="module")
+def bo():
+    from oracle import bege_oracle
+    return bege_oracle
+
+
+@pytest.fixture(scope="module")
+def bege():
+    from paper_1708_01609_b200 import bege as m, build
+    build.build_library()           # no-op when the in-tree .so is fresh
+    return m
+
+
+def rel_l2(a, b):
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def check_tail_sets(gpu_tails, n_gpu, oracle_lo, k, guard=GUARD):
+    """oracle_lo: oracle tails found at a threshold slightly below k (fp64 snr)."""
+    assert n_gpu == gpu_tails.size
+    okey = oracle_lo["template_id"].astype(np.uint64) << np.uint64(32) | oracle_lo["lag"].astype(np.uint64)
+    gkey = gpu_tails["template_id"].astype(np.uint64) << np.uint64(32) | gpu_tails["lag"].astype(np.uint64)
+    assert np.unique(gkey).size == gkey.size, "duplicate records"
+    must = okey[oracle_lo["snr"] > k + guard]
+    may = okey[oracle_lo["snr"] > k - guard]
+    missing = np.setdiff1d(must, gkey)
+    extra = np.setdiff1d(gkey, may)
+    assert missing.size == 0, f"{missing.size} oracle tails missing on the GPU"
+    assert extra.size == 0, f"{extra.size} GPU tails not in the oracle set"
+    # snr values of the common records
+    order_o = np.argsort(okey)
+    pos = np.searchsorted(okey[order_o], gkey)
+    snr_o = oracle_lo["snr"][order_o][pos]
+    assert np.max(np.abs(gpu_tails["snr"] - snr_o) / snr_o, initial=0.0) < 2e-5
+    return must.size, may.size
+
+
+# ----------------------------------------------------------------------------- cfg0, everything
+@pytest.fixture(scope="module")
+def cfg0(bo, bege):
+    w = synth.config0()
+    plan = bege.Plan(N, FS, BAND)
+    plan.bank_generate(w.f0, w.fdot, TAU)
+    plan.segment_load(w.x)
+    X = bo.segment_spectrum(w.x[0], FS, *BAND)
+    yield w, plan, X
+    plan.close()
+
+
+def test_segment_spectrum_matches_oracle(cfg0, bo):
+    w, plan, X = cfg0
+    Xg = plan.debug_segment_spectrum(0).astype(np.complex128)
+    assert rel_l2(Xg, X) < 1e-6
+    assert np.array_equal(Xg == 0, X == 0)            # band mask: exactly the same bins are zero
+
+
+def test_template_spectra_match_oracle(cfg0, bo):
+    w, plan, _ = cfg0
+    kept = np.zeros(N, dtype=bool)
+    kept[4096:61440] = True                            # row blocks 1..14 are stored; blocks 0 and 15 hold no in-band bin
+    for j in (0, 17, 100, 255):
+        H = bo.fft(bo.template(w.f0[j], w.fdot[j], TAU, FS, N), -1)
+        Hg = plan.debug_template_spectrum(j).astype(np.complex128)
+        assert np.linalg.norm(Hg[kept] - H[kept]) / np.linalg.norm(H) < 1e-6, j
+
+
+def test_correlations_match_oracle_all_templates(cfg0, bo):
+    w, plan, X = cfg0
+    worst, worst_s = 0.0, 0.0
+    for j in range(w.n_templates):
+        z, s = bo.correlate(X, bo.template(w.f0[j], w.fdot[j], TAU, FS, N))
+        zg, sg = plan.debug_correlate(j, 0)
+        worst = max(worst, rel_l2(zg.astype(np.complex128), z))
+        worst_s = max(worst_s, abs(sg - s) / s)
+    assert worst <= REL_L2, worst
+    assert worst_s <= SIGMA_RTOL, worst_s
+
+
+@pytest.mark.parametrize("k", [2.5, 3.0, 5.0])
+def test_tail_sets_match_oracle(cfg0, bo, k):
+    w, plan, X = cfg0
+    lo_tails, n_lo, sigma_o, _ = bo.search(X[None, :], w.f0, w.fdot, TAU, FS, k - 1e-3, cap=1 << 20)
+    assert n_lo == lo_tails.size
+    tails, n = plan.search(k, cap=1 << 20)
+    must, may = check_tail_sets(tails, n, lo_tails, k)
+    if k < 5:
+        assert must > 1000                              # the comparison is not vacuous
+    else:
+        assert n == 0                                   # reading 4: exp(-25) * 1.7e7 outputs -> empty set
+    sg = plan.get_sigma()
+    assert sg.shape == (w.n_templates, 1)
+    assert np.max(np.abs(sg[:, 0] - sigma_o[:, 0]) / sigma_o[:, 0]) <= SIGMA_RTOL
+
+
+def test_cap_overflow_reports_true_count(cfg0, bege):
+    w, plan, _ = cfg0
+    tails_all, n_all = plan.search(3.0, cap=1 << 20)
+    with pytest.raises(bege.BegeError) as ei:
+        plan.search(3.0, cap=100)
+    assert ei.value.status == bege.EOVERFLOW
+    part, n = plan.search(3.0, cap=100, allow_overflow=True)
+    assert n == n_all and part.size == 100
+    allkeys = set(zip(tails_all["template_id"].tolist(), tails_all["lag"].tolist()))
+    assert all((a, b) in allkeys for a, b in zip(part["template_id"].tolist(), part["lag"].tolist()))
+    _, n0 = plan.search(3.0, cap=0, allow_overflow=True)
+    assert n0 == n_all
+
+
+def test_search_is_repeatable(cfg0):
+    w, plan, _ = cfg0
+    a, na = plan.search(3.0)
+    b, nb = plan.search(3.0)
+    assert na == nb
+    a = a[np.lexsort((a["lag"], a["template_id"]))]
+    b = b[np.lexsort((b["lag"], b["template_id"]))]
+    assert np.array_equal(a, b)                          # partial sums are combined in a fixed order
+
+
+# ----------------------------------------------------------------------------- cfg1: injection, ragged bank
+def test_injection_ridge_subbank(bo, bege):
+    w = synth.config1()
+    rows, cols = range(110, 123), range(98, 107)
+    ids = [i * 256 + j for i in rows for j in cols]      # 117 templates: not a multiple of the batch (72)
+    sub = synth.subsample(w, ids)
+    X = bo.segment_spectrum(w.x[0], FS, *BAND)
+    lo_tails, _, sigma_o, _ = bo.search(X[None, :], sub.f0, sub.fdot, TAU, FS, 5.0 - 1e-3)
+    with bege.Plan(N, FS, BAND) as plan:
+        plan.bank_generate(sub.f0, sub.fdot, TAU)
+        plan.segment_load(w.x)
+        tails, n = plan.search(5.0)
+        must, _ = check_tail_sets(tails, n, lo_tails, 5.0)
+        assert must > 100
+        best = tails[np.argmax(tails["snr"])]
+        assert ids[best["template_id"]] == w.meta["true_id"]
+        assert abs(int(best["lag"]) - 29870) <= 2
+        sg = plan.get_sigma()[:, 0]
+        assert np.max(np.abs(sg - sigma_o[:, 0]) / sigma_o[:, 0]) <= SIGMA_RTOL
+
+
+# ----------------------------------------------------------------------------- several segments
+def test_multi_segment_search(bo, bege):
+    xs = np.stack([synth.noise_segment(s) for s in (40, 41, 42)])
+    x2, n0 = synth.inject_chirp(xs[1].real.astype(np.float64), 800.0, 120.0, 3.0, 10.0)
+    xs[1] = synth.as_segment(x2)
+    f0, fd = synth.bank_grid(5, 5, 780.0, 820.0, 100.0, 140.0)
+    Xs = np.stack([bo.segment_spectrum(x, FS, *BAND) for x in xs])
+    k = 3.0
+    lo_tails, _, sigma_o, _ = bo.search(Xs, f0, fd, TAU, FS, k - 1e-3)
+    with bege.Plan(N, FS, BAND) as plan:
+        plan.bank_generate(f0, fd, TAU)
+        plan.segment_load(xs)
+        tails, n = plan.search(k)
+        check_tail_sets(tails, n, lo_tails, k)
+        sg = plan.get_sigma()
+        assert sg.shape == (25, 3)
+        assert np.max(np.abs(sg - sigma_o) / sigma_o) <= SIGMA_RTOL
+        best = tails[np.argmax(tails["snr"])]
+        assert best["lag"] // N == 1 and abs(int(best["lag"]) % N - n0) <= 2      # lag = m*N + n
+        for (j, m) in ((0, 0), (12, 1), (24, 2)):
+            z, s = bo.correlate(Xs[m], bo.template(f0[j], fd[j], TAU, FS, N))
+            zg, sgj = plan.debug_correlate(j, m)
+            assert rel_l2(zg.astype(np.complex128), z) <= REL_L2
+            assert abs(sgj - s) / s <= SIGMA_RTOL
+
+
+def test_many_segments_batching(bo, bege):
+    """More segments than one batch holds (kBatch = 72): segment sub-batches, lag offsets, sigma layout."""
+    S = 75
+    xs = np.stack([synth.noise_segment(500 + s) for s in range(S)])
+    f0, fd = np.array([600.0, 1500.0]), np.array([50.0, -250.0])
+    with bege.Plan(N, FS, BAND) as plan:
+        plan.bank_generate(f0, fd, TAU)
+        plan.segment_load(xs)
+        tails, n = plan.search(3.3)
+        sg = plan.get_sigma()
+    assert sg.shape == (2, S)
+    for m in (0, 71, 72, 74):
+        X = bo.segment_spectrum(xs[m], FS, *BAND)
+        lo_tails, _, sigma_o, _ = bo.search(X[None, :], f0, fd, TAU, FS, 3.3 - 1e-3)
+        sel = tails[tails["lag"] // N == m].copy()
+        sel["lag"] -= np.uint32(m * N)
+        check_tail_sets(sel, sel.size, lo_tails, 3.3)
+        assert np.max(np.abs(sg[:, m] - sigma_o[:, 0]) / sigma_o[:, 0]) <= SIGMA_RTOL
+
+
+# ----------------------------------------------------------------------------- other band (generic row-block path)
+def test_other_band_uses_full_row_blocks(bo, bege):
+    band = (100.0, 1900.0)                                # bins reach into row-block 0: all 16 blocks are stored
+    x = synth.as_segment(synth.band_limit(synth.white_noise(77), FS, *band))
+    f0, fd = synth.bank_grid(3, 3, 150.0, 1700.0, -100.0, 100.0)
+    X = bo.segment_spectrum(x, FS, *band)
+    lo_tails, _, sigma_o, _ = bo.search(X[None, :], f0, fd, TAU, FS, 2.8 - 1e-3)
+    with bege.Plan(N, FS, band) as plan:
+        plan.bank_generate(f0, fd, TAU)
+        plan.segment_load(x[None, :])
+        tails, n = plan.search(2.8)
+        check_tail_sets(tails, n, lo_tails, 2.8)
+        for j in (0, 8):
+            z, s = bo.correlate(X, bo.template(f0[j], fd[j], TAU, FS, N))
+            zg, sgj = plan.debug_correlate(j, 0)
+            assert rel_l2(zg.astype(np.complex128), z) <= REL_L2 and abs(sgj - s) / s <= SIGMA_RTOL
+
+
+def test_shorter_template_and_complex_data(bo, bege):
+    """tau = 0.25 s (L = 1024) and a genuinely complex segment (the paper packs H1 + i L1)."""
+    r = np.random.default_rng(5)
+    x = synth.band_limit(r.standard_normal(N) + 1j * r.standard_normal(N)).astype(np.complex64)
+    f0, fd = np.array([500.0, 1200.0, 1800.0]), np.array([300.0, -500.0, 0.0])
+    X = bo.segment_spectrum(x, FS, *BAND)
+    with bege.Plan(N, FS, BAND) as plan:
+        plan.bank_generate(f0, fd, 0.25)
+        plan.segment_load(x[None, :])
+        for j in range(3):
+            z, s = bo.correlate(X, bo.template(f0[j], fd[j], 0.25, FS, N))
+            zg, sgj = plan.debug_correlate(j, 0)
+            assert rel_l2(zg.astype(np.complex128), z) <= REL_L2 and abs(sgj - s) / s <= SIGMA_RTOL
+
+
+# ----------------------------------------------------------------------------- degenerate inputs / errors
+def test_zero_segment_gives_no_tails(bege):
+    f0, fd = synth.bank_grid(2, 2, 400.0, 500.0, -10.0, 10.0)
+    with bege.Plan(N, FS, BAND) as plan:
+        plan.bank_generate(f0, fd, TAU)
+        plan.segment_load(np.zeros((1, N), dtype=np.complex64))
+        tails, n = plan.search(0.0)
+        assert n == 0 and tails.size == 0
+        assert np.all(plan.get_sigma() == 0)
+
+
+def test_error_paths(bege):
+    import ctypes
+    L = bege.load_library()
+    h = ctypes.c_void_p()
+    assert L.bege_plan_create(ctypes.byref(h), 4096, FS, 350.0, 2000.0, 0, None) == bege.EINVAL     # N != 2^16
+    assert L.bege_plan_create(ctypes.byref(h), N, FS, 350.0, 3000.0, 0, None) == bege.EINVAL        # band > fs/2
+    assert L.bege_plan_create(ctypes.byref(h), N, FS, 350.0, 2000.0, 99, None) == bege.ECUDA        # no such device
+    with bege.Plan(N, FS, BAND) as plan:
+        with pytest.raises(bege.BegeError) as ei:
+            plan.search(5.0)
+        assert ei.value.status == bege.ESTATE
+        with pytest.raises(bege.BegeError) as ei:
+            plan.bank_generate([500.0], [0.0], 2.0)                                                  # tau*fs > N/16
+        assert ei.value.status == bege.EINVAL
+        plan.bank_generate([500.0], [0.0], TAU)
+        with pytest.raises(bege.BegeError) as ei:
+            plan.get_sigma()
+        assert ei.value.status == bege.ESTATE
+
+
+def test_user_workspace_and_device_input(bo, bege):
+    """Workspace lent by torch, segment given as a CUDA tensor, bank replaced in place."""
+    import torch
+    w = synth.config0()
+    ids = np.arange(0, 256, 7)
+    X = bo.segment_spectrum(w.x[0], FS, *BAND)
+    with bege.Plan(N, FS, BAND) as plan:
+        nbytes = plan.alloc_workspace(ids.size, 1, 1 << 16)
+        assert nbytes > ids.size * 14 * 32768
+        plan.bank_generate(w.f0[ids], w.fdot[ids], TAU)
+        plan.segment_load(torch.from_numpy(w.x).cuda())
+        lo_tails, _, _, _ = bo.search(X[None, :], w.f0[ids], w.fdot[ids], TAU, FS, 3.0 - 1e-3)
+        tails, n = plan.search(3.0, cap=1 << 16)
+        check_tail_sets(tails, n, lo_tails, 3.0)
+        ids2 = ids[::-1].copy()
+        plan.bank_generate(w.f0[ids2], w.fdot[ids2], TAU)           # same size: reuses the bank slot
+        tails2, n2 = plan.search(3.0, cap=1 << 16)
+        assert n2 == n
+        with pytest.raises(bege.BegeError) as ei:
+            plan.bank_generate(w.f0, w.fdot, TAU)                   # does not fit the lent workspace
+        assert ei.value.status == bege.ENOMEM
