@@ -4,8 +4,8 @@
 // Index conventions (N = 65536 = 256 x 256, w_M = exp(2 pi i / M)):
 //   inverse (search):  k = k1 + 256 k2,  n = 256 n1 + n2
 //     z[256 n1 + n2] = 1/N sum_k1 w256^(k1 n1) [ wN^(k1 n2) sum_k2 R[k1 + 256 k2] w256^(k2 n2) ]
-//     pass 1 (k_inv_cols): 256-point column DFTs over k2 + twiddle wN^(k1 n2) -> scratch T[n2][k1] (L2)
-//     pass 2 (k_inv_rows): 256-point row DFTs over k1, threshold, compaction
+//     pass 1 (k_search phase A): 256-point column DFTs over k2 + twiddle wN^(k1 n2) -> ring T[n2][k1] (L2)
+//     pass 2 (k_search phase B): 256-point row DFTs over k1, threshold, compaction
 //   forward (bank / segments): n = nl + 256 nh, k = k1 + 256 k2
 //     H[k1 + 256 k2] = sum_nl w256^(-nl k2) [ wN^(-nl k1) sum_nh h[nl + 256 nh] w256^(-nh k1) ]
 //     step A (k_fwd_rows_*): DFT over nh + twiddle -> scratch G (tile layout), step B (k_fwd_cols): DFT over nl
@@ -30,8 +30,10 @@
 namespace bege {
 
 constexpr int kN = 65536;
-constexpr int kBatch = 72;                 // correlations in flight between pass 1 and pass 2 (36 MB of L2)
-constexpr int kGroups = 18;                // persistent CTA groups per tile: 16 tiles x 18 = 288 CTAs ~ 2 per SM
+constexpr int kBatch = 72;                 // spectra per launch of the forward transforms (36 MB of staging)
+constexpr int kMaxGroups = 32;             // search: persistent CTA groups of 16 tiles (18 on a 148-SM B200)
+constexpr int kSearchSmem = 4096 * 8 + 4096 * 8 + 64;   // exchange buffer + tile twiddles + reduction scratch
+constexpr uint64_t kMiscHdr = 4096;        // counter @0, abort flag @8, done1 @256, done2 @2048 (per group and ring slot)
 
 // ------------------------------------------------------------------------------------------------
 // shared-memory exchange index for the column passes: stage-1 thread (c, g) writes its p-th value,
@@ -178,152 +180,186 @@ k_fwd_cols(const c2* __restrict__ G, c2* __restrict__ out, uint64_t out_stride, 
 }
 
 // ------------------------------------------------------------------------------------------------
-// a3 + a4 + first half of a5: conj(H) X, Parseval partial sums, column DFTs, four-step twiddle.
-// grid (16 tiles, kGroups); CTA (b, grp) keeps its tile of the segment spectrum (SINGLE) and all its
-// twiddles in registers and loops over the templates of the batch.  256 threads:
-//   stage 1: half-warp c, lane g: k2 = g + 16 i  (coalesced tile-layout loads)
-//   exchange through shared memory (double buffered, one __syncthreads per correlation)
-//   stage 2: lane c, p = warp pair index: n2 = p + 16 q, stores T[n2][16 b + c] (128 B per half-warp)
+// a3 - a7, one persistent kernel for a whole search (PAPER.md:156-162 steps ii-iv; eq.5-9, 13).
+// grid (16 tiles, G groups), 256 threads, 2 CTAs per SM, cooperative launch (all CTAs co-resident).
+// The 16 CTAs of a group work through the group's (template, segment) items in lock step; item i of a
+// group is pair (template grp + G (i / S), segment i % S).  Per iteration a CTA runs
+//   phase A (pass 1) of item i:   conj(H) X for its 16 columns k1 = 16 b + c, Parseval partial sum, 256-point
+//            column DFTs over k2, four-step twiddle, store T[n2][k1] into ring slot i % kRing of the group (L2);
+//   phase B (pass 2) of item i-1: 256-point row DFTs over k1 for its 16 rows n2 = 16 b + hw, threshold against
+//            k^2 sum|R|^2, warp-aggregated compaction of the tails.
+// Hand-over between the CTAs of a group goes through two monotone counters per group and
+// per ring slot in global memory (done1: tiles of pass 1 finished, done2: row tiles of pass 2 finished;
+// release/acquire at gpu scope).
+// The ring (G x kRing x 512 KiB) is written and read back within microseconds and stays in L2.
+//   phase A roles: stage 1 half-warp c, lane g: rows k2 = g + 16 i (coalesced tile-layout loads); exchange
+//            through shared memory; stage 2 lane c, p2 = warp pair index: n2 = p2 + 16 q (128 B stores)
+//   phase B roles: half-warp hw owns row n2, lane a holds k1 = a + 16 i; private shared-memory region
+constexpr int kRing = 3;
+constexpr long long kSpinLimit = 6000000000ll;          // ~3 s of SM clocks: a stuck pipeline aborts, never hangs
+
+BEGE_D void signal_inc(unsigned long long* ctr)
+{
+    __syncthreads();
+    if (threadIdx.x == 0) asm volatile("red.release.gpu.global.add.u64 [%0], %1;" :: "l"(ctr), "l"(1ull) : "memory");
+}
+BEGE_D void wait_ge(const unsigned long long* ctr, unsigned long long target, int* abort_flag)
+{
+    if (threadIdx.x == 0) {
+        unsigned long long v;
+        const long long t0 = clock64();
+        for (;;) {
+            asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(ctr) : "memory");
+            if (v >= target) break;
+            if (*(volatile int*)abort_flag) break;
+            if (clock64() - t0 > kSpinLimit) { *(volatile int*)abort_flag = 1; break; }
+        }
+    }
+    __syncthreads();
+}
+
 template <int I0, int NI, bool SINGLE>
 __global__ void __launch_bounds__(256, 2)
-k_inv_cols(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restrict__ T,
-           float* __restrict__ sigpart, const float2* __restrict__ tw256, const float2* __restrict__ twN,
-           uint64_t j0, int Tb, int m0, int Sb, int S)
+k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restrict__ ring,
+         float* __restrict__ sigpart, const float2* __restrict__ tw256, const float2* __restrict__ twN,
+         float k2, bege_tail* __restrict__ rec, unsigned long long cap, unsigned long long* __restrict__ counter,
+         c2* __restrict__ zdbg, uint64_t j0, uint64_t nT, uint32_t m0, uint32_t nS, uint32_t S,
+         unsigned long long* done1, unsigned long long* done2, int* abort_flag)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    c2* sm = reinterpret_cast<c2*>(smem_raw);                 // [2][4096]
-    float* red = reinterpret_cast<float*>(sm + 2 * 4096);     // [2][8]
-    const int t = threadIdx.x, b = blockIdx.x, grp = blockIdx.y, ngrp = gridDim.y;
-    const int c = t >> 4, g = t & 15;                         // stage-1 role
-    const int c2i = t & 15, p2 = t >> 4;                      // stage-2 role
-    constexpr uint64_t kTile = (uint64_t)NI * 256;            // elements per (spectrum, tile)
+    c2* sm = reinterpret_cast<c2*>(smem_raw);                     // [4096] exchange buffer (both phases)
+    float2* wNs = reinterpret_cast<float2*>(sm + 4096);           // [16][256] four-step twiddles of this tile
+    float* red = reinterpret_cast<float*>(wNs + 4096);            // [8]
+    const int t = threadIdx.x, b = blockIdx.x, grp = blockIdx.y, G = gridDim.y;
+    const int c = t >> 4, g = t & 15, lane = t & 31;              // phase A stage 1 (c, g); phase B (hw = c, a = g)
+    const int c2i = t & 15, p2 = t >> 4;                          // phase A stage 2
+    constexpr uint64_t kTile = (uint64_t)NI * 256;                // elements per (spectrum, tile)
 
-    float2 w1[16], wN[16];
+    float2 w1[16];
     load_w1(w1, tw256, g);
 #pragma unroll
-    for (int q = 0; q < 16; ++q) wN[q] = __ldg(twN + (p2 + 16 * q) * 256 + 16 * b + c2i);
+    for (int q = 0; q < 16; ++q) wNs[q * 256 + t] = __ldg(twN + (p2 + 16 * q) * 256 + 16 * b + c2i);
 
-    c2 xr[NI];
+    c2 xr[NI], h[NI];
     if (SINGLE) {
         const c2* xb = xseg + ((uint64_t)m0 * 16 + b) * kTile;
 #pragma unroll
-        for (int ii = 0; ii < NI; ++ii) xr[ii] = xb[(ii * 16 + c) * 16 + g];
+        for (int ii = 0; ii < NI; ++ii) xr[ii] = xb[ii * 256 + t];
     }
-    int it = 0;
-    for (int jl = grp; jl < Tb; jl += ngrp) {
-        const c2* hb = bank + ((j0 + jl) * 16 + b) * kTile;
-        c2 h[NI];
+    __syncthreads();
+
+    const uint64_t nTg = nT > (uint64_t)grp ? (nT - grp + G - 1) / G : 0;   // templates of this group
+    const uint64_t n_items = nTg * nS;
+    c2* myring = ring + (uint64_t)grp * kRing * kN;
+    unsigned long long* d1 = done1 + grp * kRing;             // one counter per ring slot: a count can only
+    unsigned long long* d2 = done2 + grp * kRing;             // come from the item that currently owns the slot
+    const int n2 = 16 * b + c;                                    // phase B row
+
+    for (uint64_t i = 0; i <= n_items; ++i) {
+        if (i < n_items) {
+            // ---------------------------------------------------------------- phase A, item i
+            const uint64_t jl = grp + (uint64_t)G * (i / nS);
+            const uint32_t ml = (uint32_t)(i % nS);
+            if (SINGLE || ml == 0) {
+                const c2* hb = bank + ((j0 + jl) * 16 + b) * kTile;
 #pragma unroll
-        for (int ii = 0; ii < NI; ++ii) h[ii] = __ldcs(hb + (ii * 16 + c) * 16 + g);
-        for (int ml = 0; ml < Sb; ++ml, ++it) {
-            c2 v[16];
-            c2 acc = mk(0.f, 0.f);
+                for (int ii = 0; ii < NI; ++ii) h[ii] = __ldcs(hb + ii * 256 + t);
+            }
             if (!SINGLE) {
                 const c2* xb = xseg + ((uint64_t)(m0 + ml) * 16 + b) * kTile;
 #pragma unroll
-                for (int ii = 0; ii < NI; ++ii) xr[ii] = __ldg(xb + (ii * 16 + c) * 16 + g);
+                for (int ii = 0; ii < NI; ++ii) xr[ii] = __ldg(xb + ii * 256 + t);
             }
+            if (i >= kRing) wait_ge(d2 + i % kRing, 16ull * (i / kRing), abort_flag);   // slot free again
+            c2 v[16];
+            c2 acc = mk(0.f, 0.f);
 #pragma unroll
-            for (int i = 0; i < 16; ++i) {
-                if (i >= I0 && i < I0 + NI) {
-                    v[i] = cmulc(xr[i - I0], h[i - I0]);
-                    acc = fma2(v[i], v[i], acc);
+            for (int r = 0; r < 16; ++r) {
+                if (r >= I0 && r < I0 + NI) {
+                    v[r] = cmulc(xr[r - I0], h[r - I0]);
+                    acc = fma2(v[r], v[r], acc);
                 } else {
-                    v[i] = mk(0.f, 0.f);
+                    v[r] = mk(0.f, 0.f);
                 }
             }
             stage1<+1>(v, w1);
-            c2* buf = sm + (it & 1) * 4096;
-            float* rbuf = red + (it & 1) * 8;
 #pragma unroll
-            for (int p = 0; p < 16; ++p) buf[xidx(c, g, p)] = v[p];
+            for (int p = 0; p < 16; ++p) sm[xidx(c, g, p)] = v[p];
             const float s = warp_sum32(re(acc) + im(acc));
-            if ((t & 31) == 0) rbuf[t >> 5] = s;
+            if (lane == 0) red[t >> 5] = s;
             __syncthreads();
 #pragma unroll
-            for (int gg = 0; gg < 16; ++gg) v[gg] = buf[xidx(c2i, gg, p2)];
+            for (int gg = 0; gg < 16; ++gg) v[gg] = sm[xidx(c2i, gg, p2)];
             fft16<+1>(v);
-            c2* out = T + (uint64_t)(jl * Sb + ml) * kN + 16 * b + c2i;
+            c2* out = myring + (i % kRing) * (uint64_t)kN + 16 * b + c2i;
 #pragma unroll
-            for (int q = 0; q < 16; ++q) out[(p2 + 16 * q) * 256] = cmul(v[q], wN[q]);
+            for (int q = 0; q < 16; ++q) out[(p2 + 16 * q) * 256] = cmul(v[q], wNs[q * 256 + t]);
             if (t == 0) {
                 float tot = 0.f;
 #pragma unroll
-                for (int w = 0; w < 8; ++w) tot += rbuf[w];
+                for (int w = 0; w < 8; ++w) tot += red[w];
                 sigpart[((j0 + jl) * (uint64_t)S + (m0 + ml)) * 16 + b] = tot;
             }
+            signal_inc(d1 + i % kRing);
         }
-    }
-}
-
-// second half of a5 + a6 + a7: row DFTs over k1, threshold |Z|^2 > k^2 sum|R|^2, warp-aggregated compaction.
-// grid (16 row tiles, kGroups); half-warp hw of CTA rt owns row n2 = 16 rt + hw; warps never synchronise
-// with each other.  DEBUG additionally writes z = Z/N to zdbg in lag order (off the timed path).
-template <bool DEBUG>
-__global__ void __launch_bounds__(256, 2)
-k_inv_rows(const c2* __restrict__ T, const float* __restrict__ sigpart, const float2* __restrict__ tw256,
-           float k2, bege_tail* __restrict__ rec, unsigned long long cap, unsigned long long* __restrict__ counter,
-           c2* __restrict__ zdbg, uint64_t j0, int Tb, int m0, int Sb, int S)
-{
-    __shared__ c2 sm[16][256];
-    const int t = threadIdx.x, rt = blockIdx.x, grp = blockIdx.y, ngrp = gridDim.y;
-    const int hw = t >> 4, a = t & 15, lane = t & 31;
-    const int n2 = 16 * rt + hw;
-    float2 w1[16];
-    load_w1(w1, tw256, a);
-    const int items = Tb * Sb;
-    for (int item = grp; item < items; item += ngrp) {
-        const int jl = item / Sb, ml = item - jl * Sb;
-        const c2* src = T + (uint64_t)item * kN + n2 * 256 + a;
-        c2 v[16];
+        if (i >= 1) {
+            // ---------------------------------------------------------------- phase B, item i - 1
+            const uint64_t ib = i - 1;
+            const uint64_t jl = grp + (uint64_t)G * (ib / nS);
+            const uint32_t ml = (uint32_t)(ib % nS);
+            wait_ge(d1 + ib % kRing, 16ull * (ib / kRing + 1), abort_flag);   // all 16 tiles of item i-1 are in the ring
+            const c2* src = myring + (ib % kRing) * (uint64_t)kN + n2 * 256 + g;
+            c2 v[16];
 #pragma unroll
-        for (int i = 0; i < 16; ++i) v[i] = __ldcg(src + 16 * i);
-        const uint64_t pair = (j0 + jl) * (uint64_t)S + (m0 + ml);
-        const float sumR2 = hw_sum16(__ldcg(sigpart + pair * 16 + a));
-        hw_fft256<+1>(v, w1, sm[hw], a);
-        // lane p = a holds Z[n1 = p + 16 q]; lag n = 256 n1 + n2
-        const float thr = k2 * sumR2;
-        unsigned hits = 0;
-        float m2[16];
-#pragma unroll
-        for (int q = 0; q < 16; ++q) {
-            const c2 sq = mul2(v[q], v[q]);
-            m2[q] = re(sq) + im(sq);
-            if (m2[q] > thr) hits |= 1u << q;
-        }
-        if (DEBUG) {
-            const float invN = 1.0f / (float)kN;
-#pragma unroll
-            for (int q = 0; q < 16; ++q)
-                zdbg[(uint64_t)(a + 16 * q) * 256 + n2] = mul2(v[q], bc(invN));
-        }
-        if (__any_sync(0xffffffffu, hits != 0)) {
-            const int cnt = __popc(hits);
-            int incl = cnt;
-#pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
-                const int o = __shfl_up_sync(0xffffffffu, incl, d);
-                if (lane >= d) incl += o;
-            }
-            const int total = __shfl_sync(0xffffffffu, incl, 31);
-            unsigned long long base = 0;
-            if (lane == 31) base = atomicAdd(counter, (unsigned long long)total);
-            base = __shfl_sync(0xffffffffu, base, 31);
-            unsigned long long slot = base + (unsigned long long)(incl - cnt);
-            const float inv = 1.0f / sumR2;
+            for (int r = 0; r < 16; ++r) v[r] = __ldcg(src + 16 * r);
+            const uint64_t pair = (j0 + jl) * (uint64_t)S + (m0 + ml);
+            const float sumR2 = hw_sum16(__ldcg(sigpart + pair * 16 + g));
+            hw_fft256<+1>(v, w1, sm + c * 256, g);
+            // lane a = g holds Z[n1 = a + 16 q]; lag n = 256 n1 + n2
+            const float thr = k2 * sumR2;
+            unsigned hits = 0;
+            float m2[16];
 #pragma unroll
             for (int q = 0; q < 16; ++q) {
-                if (hits & (1u << q)) {
-                    if (slot < cap) {
-                        bege_tail r;
-                        r.template_id = (uint32_t)(j0 + jl);
-                        r.lag = (uint32_t)(m0 + ml) * (uint32_t)kN + (uint32_t)((a + 16 * q) * 256 + n2);
-                        r.snr = sqrtf(m2[q] * inv);
-                        rec[slot] = r;
+                const c2 sq = mul2(v[q], v[q]);
+                m2[q] = re(sq) + im(sq);
+                if (m2[q] > thr) hits |= 1u << q;
+            }
+            if (zdbg != nullptr) {
+                const float invN = 1.0f / (float)kN;
+#pragma unroll
+                for (int q = 0; q < 16; ++q)
+                    zdbg[(uint64_t)(g + 16 * q) * 256 + n2] = mul2(v[q], bc(invN));
+            }
+            if (__any_sync(0xffffffffu, hits != 0)) {
+                const int cnt = __popc(hits);
+                int incl = cnt;
+#pragma unroll
+                for (int d = 1; d < 32; d <<= 1) {
+                    const int o = __shfl_up_sync(0xffffffffu, incl, d);
+                    if (lane >= d) incl += o;
+                }
+                const int total = __shfl_sync(0xffffffffu, incl, 31);
+                unsigned long long base = 0;
+                if (lane == 31) base = atomicAdd(counter, (unsigned long long)total);
+                base = __shfl_sync(0xffffffffu, base, 31);
+                unsigned long long slot = base + (unsigned long long)(incl - cnt);
+                const float inv = 1.0f / sumR2;
+#pragma unroll
+                for (int q = 0; q < 16; ++q) {
+                    if (hits & (1u << q)) {
+                        if (slot < cap) {
+                            bege_tail r;
+                            r.template_id = (uint32_t)(j0 + jl);
+                            r.lag = (uint32_t)(m0 + ml) * (uint32_t)kN + (uint32_t)((g + 16 * q) * 256 + n2);
+                            r.snr = sqrtf(m2[q] * inv);
+                            rec[slot] = r;
+                        }
+                        ++slot;
                     }
-                    ++slot;
                 }
             }
+            signal_inc(d2 + ib % kRing);
         }
     }
 }
@@ -360,6 +396,7 @@ struct bege_plan {
     double fs = 0, lo = 0, hi = 0;
     uint32_t klo = 0, khi = 0;
     int I0 = 0, NI = 16;
+    int G = 0;                      // search groups (16 CTAs each), all co-resident
     float2 *tw256 = nullptr, *twN = nullptr;
     // workspace
     unsigned char* ws = nullptr; uint64_t ws_bytes = 0, bump = 0; bool user_ws = false;
@@ -476,12 +513,19 @@ extern "C" int bege_plan_create(bege_plan** out, uint32_t N, double fs, double l
     if (cudaMemcpy(p->tw256, w256.data(), w256.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess ||
         cudaMemcpy(p->twN, wN.data(), wN.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess) return bail(BEGE_ECUDA);
 
-    const int smem = 2 * 4096 * (int)sizeof(c2) + 64;
-    cudaFuncSetAttribute(k_inv_cols<1, 14, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    cudaFuncSetAttribute(k_inv_cols<1, 14, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    cudaFuncSetAttribute(k_inv_cols<0, 16, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    cudaFuncSetAttribute(k_inv_cols<0, 16, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (cudaGetLastError() != cudaSuccess) return bail(BEGE_ECUDA);
+    // the search kernel needs all its CTAs co-resident (groups hand over through global counters)
+    int occ = 0;
+    for (const void* f : {(const void*)k_search<1, 14, true>, (const void*)k_search<1, 14, false>,
+                          (const void*)k_search<0, 16, true>, (const void*)k_search<0, 16, false>}) {
+        if (cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, kSearchSmem) != cudaSuccess) return bail(BEGE_ECUDA);
+        int o = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, f, 256, kSearchSmem) != cudaSuccess) return bail(BEGE_ECUDA);
+        occ = occ ? std::min(occ, o) : o;
+    }
+    int coop = 0;
+    cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, device);
+    p->G = std::min(kMaxGroups, occ * prop.multiProcessorCount / 16);
+    if (!coop || p->G < 1) return bail(BEGE_ECUDA);
     p->stats.hbm_bytes_per_template = tpl_bytes(p);
     *out = p;
     return BEGE_OK;
@@ -504,7 +548,7 @@ extern "C" void bege_plan_destroy(bege_plan* p)
     delete p;
 }
 
-static uint64_t scratch_bytes() { return (uint64_t)kBatch * kN * sizeof(c2); }
+static uint64_t scratch_bytes() { return (uint64_t)std::max(kBatch, kMaxGroups * kRing) * kN * sizeof(c2); }
 
 extern "C" int bege_plan_workspace_bytes(const bege_plan* p, uint64_t T, uint32_t S, uint64_t cap, uint64_t* bytes)
 {
@@ -517,7 +561,7 @@ extern "C" int bege_plan_workspace_bytes(const bege_plan* p, uint64_t T, uint32_
     b += al(scratch_bytes());                          // four-step staging (stays in L2)
     b += al(T * S * 16 * sizeof(float));               // Parseval partial sums
     b += al(cap * sizeof(bege_tail));                  // records
-    b += al(256 + (uint64_t)S * kN * sizeof(c2));      // counter + raw segment staging
+    b += al(kMiscHdr + (uint64_t)S * kN * sizeof(c2)); // counters + raw segment staging
     *bytes = b + 4096;
     return BEGE_OK;
 }
@@ -576,10 +620,10 @@ extern "C" int bege_segment_load(bege_plan* p, const float* x, uint32_t S)
     void *xs, *misc, *scr;
     int rc;
     if ((rc = slot_get(p, p->s_x, (uint64_t)S * tpl_bytes(p), &xs))) return rc;
-    if ((rc = slot_get(p, p->s_misc, 256 + (uint64_t)S * kN * sizeof(c2), &misc))) return rc;
+    if ((rc = slot_get(p, p->s_misc, kMiscHdr + (uint64_t)S * kN * sizeof(c2), &misc))) return rc;
     if ((rc = slot_get(p, p->s_scratch, scratch_bytes(), &scr))) return rc;
     p->S = 0; p->have_sigma = false;
-    c2* raw = (c2*)((unsigned char*)misc + 256);
+    c2* raw = (c2*)((unsigned char*)misc + kMiscHdr);
     cudaPointerAttributes at;
     cudaError_t e = cudaPointerGetAttributes(&at, x);
     if (e != cudaSuccess) { cudaGetLastError(); at.type = cudaMemoryTypeUnregistered; }
@@ -598,26 +642,44 @@ extern "C" int bege_segment_load(bege_plan* p, const float* x, uint32_t S)
     return BEGE_OK;
 }
 
-template <bool DEBUG>
-static void launch_pair(bege_plan* p, const c2* bank, const c2* xs, c2* scr, float* sig, float k2, bege_tail* rec,
-                        uint64_t cap, unsigned long long* counter, c2* zdbg, uint64_t j0, int Tb, int m0, int Sb)
+// one cooperative launch of the persistent search kernel over templates [j0, j0 + nT) x segments [m0, m0 + nS)
+static int launch_search(bege_plan* p, const c2* bank, const c2* xs, c2* ring, float* sig, float k2, bege_tail* rec,
+                         uint64_t cap, unsigned char* misc, c2* zdbg, uint64_t j0, uint64_t nT, uint32_t m0, uint32_t nS)
 {
-    const int smem = 2 * 4096 * (int)sizeof(c2) + 64;
-    const dim3 grid(16, kGroups);
+    unsigned long long* counter = (unsigned long long*)misc;
+    int* abort_flag = (int*)(misc + 8);
+    unsigned long long* done1 = (unsigned long long*)(misc + 256);
+    unsigned long long* done2 = (unsigned long long*)(misc + 2048);
+    CU(p, cudaMemsetAsync(misc, 0, kMiscHdr, p->stream));
+    const int G = (int)std::min<uint64_t>((uint64_t)p->G, nT);
+    const dim3 grid(16, G);
     const bool single = (p->S == 1);
+    const float2 *tw256 = p->tw256, *twN = p->twN;
+    unsigned long long capll = cap;
+    uint32_t S = p->S;
+    void* args[] = {&bank, &xs, &ring, &sig, &tw256, &twN, &k2, &rec, &capll, &counter, &zdbg, &j0, &nT, &m0, &nS, &S,
+                    &done1, &done2, &abort_flag};
+    const void* f = p->NI == 14 ? (single ? (const void*)k_search<1, 14, true> : (const void*)k_search<1, 14, false>)
+                                : (single ? (const void*)k_search<0, 16, true> : (const void*)k_search<0, 16, false>);
     if (p->profiling) cudaEventRecord(p->ev_a, p->stream);
-#define BEGE_COLS(I0, NI, SG) k_inv_cols<I0, NI, SG><<<grid, 256, smem, p->stream>>>(bank, xs, scr, sig, p->tw256, p->twN, j0, Tb, m0, Sb, (int)p->S)
-    if (p->NI == 14) { if (single) BEGE_COLS(1, 14, true); else BEGE_COLS(1, 14, false); }
-    else             { if (single) BEGE_COLS(0, 16, true); else BEGE_COLS(0, 16, false); }
-#undef BEGE_COLS
-    k_inv_rows<DEBUG><<<grid, 256, 0, p->stream>>>(scr, sig, p->tw256, k2, rec, cap, counter, zdbg, j0, Tb, m0, Sb, (int)p->S);
-    count_launch(p, 2);
+    CU(p, cudaLaunchCooperativeKernel(f, grid, dim3(256), args, kSearchSmem, p->stream));
+    count_launch(p);
     if (p->profiling) {
         cudaEventRecord(p->ev_b, p->stream);
-        cudaEventSynchronize(p->ev_b);
+        CU(p, cudaEventSynchronize(p->ev_b));
         float ms = 0; cudaEventElapsedTime(&ms, p->ev_a, p->ev_b);
-        p->stats.fused_kernel_ms += ms; p->stats.fused_kernel_launches += 2;
+        p->stats.fused_kernel_ms += ms; p->stats.fused_kernel_launches += 1;
     }
+    return BEGE_OK;
+}
+
+static int check_abort(bege_plan* p, unsigned char* misc)
+{
+    int flag = 0;
+    CU(p, cudaMemcpyAsync(&flag, misc + 8, sizeof flag, cudaMemcpyDeviceToHost, p->stream));
+    CU(p, cudaStreamSynchronize(p->stream));
+    if (flag) return fail(p, BEGE_ECUDA, "search pipeline timed out waiting on a group counter");
+    return BEGE_OK;
 }
 
 extern "C" int bege_search(bege_plan* p, float k_sigma, bege_tail* tails_out, uint64_t cap, uint64_t* n_tails)
@@ -630,28 +692,21 @@ extern "C" int bege_search(bege_plan* p, float k_sigma, bege_tail* tails_out, ui
     int rc;
     if ((rc = slot_get(p, p->s_sig, p->T * p->S * 16 * sizeof(float), &sig))) return rc;
     if ((rc = slot_get(p, p->s_rec, cap * sizeof(bege_tail), &rec))) return rc;
-    if ((rc = slot_get(p, p->s_misc, 256, &misc))) return rc;
+    if ((rc = slot_get(p, p->s_misc, kMiscHdr, &misc))) return rc;
     if ((rc = slot_get(p, p->s_scratch, scratch_bytes(), &scr))) return rc;
     if ((rc = slot_get(p, p->s_bank, 0, &bank))) return rc;
     if ((rc = slot_get(p, p->s_x, 0, &xs))) return rc;
     unsigned long long* counter = (unsigned long long*)misc;
-    CU(p, cudaMemsetAsync(counter, 0, sizeof(unsigned long long), p->stream));
-    const int Sb = (int)std::min<uint32_t>(p->S, kBatch);
-    const int Tbmax = kBatch / Sb;
-    for (uint32_t m0 = 0; m0 < p->S; m0 += Sb) {
-        const int sb = (int)std::min<uint32_t>(Sb, p->S - m0);
-        for (uint64_t j0 = 0; j0 < p->T; j0 += Tbmax) {
-            const int tb = (int)std::min<uint64_t>(Tbmax, p->T - j0);
-            launch_pair<false>(p, (const c2*)bank, (const c2*)xs, (c2*)scr, (float*)sig, k_sigma * k_sigma,
-                               (bege_tail*)rec, cap, counter, nullptr, j0, tb, (int)m0, sb);
-        }
-    }
+    if ((rc = launch_search(p, (const c2*)bank, (const c2*)xs, (c2*)scr, (float*)sig, k_sigma * k_sigma,
+                            (bege_tail*)rec, cap, (unsigned char*)misc, nullptr, 0, p->T, 0, p->S))) return rc;
     CU(p, cudaGetLastError());
     // only the tails cross PCIe: count first, then exactly the records, on the side stream
     CU(p, cudaMemcpyAsync(p->h_count, counter, sizeof(unsigned long long), cudaMemcpyDeviceToHost, p->stream));
     CU(p, cudaEventRecord(p->ev_done, p->stream));
     CU(p, cudaStreamWaitEvent(p->side, p->ev_done, 0));
+    CU(p, cudaMemcpyAsync(p->h_count + 1, (unsigned char*)misc + 8, sizeof(int), cudaMemcpyDeviceToHost, p->stream));
     CU(p, cudaStreamSynchronize(p->stream));
+    if (*(volatile int*)(p->h_count + 1)) return fail(p, BEGE_ECUDA, "search pipeline timed out waiting on a group counter");
     const uint64_t total = *p->h_count;
     const uint64_t ncopy = std::min<uint64_t>(total, cap);
     if (ncopy) {
@@ -689,26 +744,27 @@ extern "C" int bege_debug_correlate(bege_plan* p, uint64_t j, uint32_t m, float*
     if (!p->T || !p->S) return fail(p, BEGE_ESTATE, "needs a bank and segments");
     if (j >= p->T || m >= p->S) return fail(p, BEGE_EINVAL, "pair (%llu, %u) out of range", (unsigned long long)j, m);
     CU(p, cudaSetDevice(p->device));
-    void *scr, *bank, *xs;
+    void *scr, *bank, *xs, *misc;
     int rc;
     if ((rc = slot_get(p, p->s_scratch, scratch_bytes(), &scr))) return rc;
+    if ((rc = slot_get(p, p->s_misc, kMiscHdr, &misc))) return rc;
     slot_get(p, p->s_bank, 0, &bank); slot_get(p, p->s_x, 0, &xs);
-    c2* zd = nullptr; float* sg = nullptr; unsigned long long* cnt = nullptr;
+    c2* zd = nullptr; float* sg = nullptr;
     CU(p, cudaMalloc(&zd, kN * sizeof(c2)));
     CU(p, cudaMalloc(&sg, 16 * sizeof(float)));         // private partial sums of this one pair
-    CU(p, cudaMalloc(&cnt, 8));
-    cudaMemsetAsync(cnt, 0, 8, p->stream);
     const bool prof = p->profiling; p->profiling = false;
-    // the kernels index the partial sums by (j*S + m)*16: bias the base so that this pair lands on sg[0..15]
+    // the kernel indexes the partial sums by (j*S + m)*16: bias the base so that this pair lands on sg[0..15]
     float* sg_biased = sg - (j * p->S + m) * 16;
-    launch_pair<true>(p, (const c2*)bank, (const c2*)xs, (c2*)scr, sg_biased, 1e30f, nullptr, 0, cnt, zd, j, 1, (int)m, 1);
+    rc = launch_search(p, (const c2*)bank, (const c2*)xs, (c2*)scr, sg_biased, 1e30f, nullptr, 0, (unsigned char*)misc, zd, j, 1, m, 1);
     p->profiling = prof;
+    if (!rc) rc = check_abort(p, (unsigned char*)misc);
+    if (rc) { cudaFree(zd); cudaFree(sg); return rc; }
     float part[16];
     cudaError_t e = cudaMemcpyAsync(z_out, zd, kN * sizeof(c2), cudaMemcpyDeviceToHost, p->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(part, sg, sizeof part, cudaMemcpyDeviceToHost, p->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
     if (e == cudaSuccess) e = cudaGetLastError();
-    cudaFree(zd); cudaFree(sg); cudaFree(cnt);
+    cudaFree(zd); cudaFree(sg);
     CU(p, e);
     if (sigma_out) {
         float v[16];
