@@ -27,6 +27,10 @@
 #include "../../include/bege.h"
 #include "cplx.cuh"
 
+#ifndef BEGE_LAG
+#define BEGE_LAG 2
+#endif
+
 namespace bege {
 
 constexpr int kN = 65536;
@@ -195,7 +199,8 @@ k_fwd_cols(const c2* __restrict__ G, c2* __restrict__ out, uint64_t out_stride, 
 //   phase A roles: stage 1 half-warp c, lane g: rows k2 = g + 16 i (coalesced tile-layout loads); exchange
 //            through shared memory; stage 2 lane c, p2 = warp pair index: n2 = p2 + 16 q (128 B stores)
 //   phase B roles: half-warp hw owns row n2, lane a holds k1 = a + 16 i; private shared-memory region
-constexpr int kRing = 3;
+constexpr int kLag = BEGE_LAG;                           // phase B runs kLag items behind phase A
+constexpr int kRing = BEGE_LAG + 2;
 constexpr long long kSpinLimit = 6000000000ll;          // ~3 s of SM clocks: a stuck pipeline aborts, never hangs
 
 BEGE_D void signal_inc(unsigned long long* ctr)
@@ -255,7 +260,7 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
     unsigned long long* d2 = done2 + grp * kRing;             // come from the item that currently owns the slot
     const int n2 = 16 * b + c;                                    // phase B row
 
-    for (uint64_t i = 0; i <= n_items; ++i) {
+    for (uint64_t i = 0; i < n_items + kLag; ++i) {
         if (i < n_items) {
             // ---------------------------------------------------------------- phase A, item i
             const uint64_t jl = grp + (uint64_t)G * (i / nS);
@@ -302,9 +307,9 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
             }
             signal_inc(d1 + i % kRing);
         }
-        if (i >= 1) {
-            // ---------------------------------------------------------------- phase B, item i - 1
-            const uint64_t ib = i - 1;
+        if (i >= kLag) {
+            // ---------------------------------------------------------------- phase B, item i - kLag
+            const uint64_t ib = i - kLag;
             const uint64_t jl = grp + (uint64_t)G * (ib / nS);
             const uint32_t ml = (uint32_t)(ib % nS);
             wait_ge(d1 + ib % kRing, 16ull * (ib / kRing + 1), abort_flag);   // all 16 tiles of item i-1 are in the ring
