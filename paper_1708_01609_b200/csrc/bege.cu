@@ -26,17 +26,13 @@
 
 #include "../../include/bege.h"
 #include "cplx.cuh"
-
-#ifndef BEGE_LAG
-#define BEGE_LAG 2
-#endif
+#include "async.cuh"
 
 namespace bege {
 
 constexpr int kN = 65536;
 constexpr int kBatch = 72;                 // spectra per launch of the forward transforms (36 MB of staging)
 constexpr int kMaxGroups = 32;             // search: persistent CTA groups of 16 tiles (18 on a 148-SM B200)
-constexpr int kSearchSmem = 4096 * 8 + 4096 * 8 + 64;   // exchange buffer + tile twiddles + reduction scratch
 constexpr uint64_t kMiscHdr = 4096;        // counter @0, abort flag @8, done1 @256, done2 @2048 (per group and ring slot)
 
 // ------------------------------------------------------------------------------------------------
@@ -184,143 +180,238 @@ k_fwd_cols(const c2* __restrict__ G, c2* __restrict__ out, uint64_t out_stride, 
 }
 
 // ------------------------------------------------------------------------------------------------
-// a3 - a7, one persistent kernel for a whole search (PAPER.md:156-162 steps ii-iv; eq.5-9, 13).
-// grid (16 tiles, G groups), 256 threads, 2 CTAs per SM, cooperative launch (all CTAs co-resident).
-// The 16 CTAs of a group work through the group's (template, segment) items in lock step; item i of a
-// group is pair (template grp + G (i / S), segment i % S).  Per iteration a CTA runs
-//   phase A (pass 1) of item i:   conj(H) X for its 16 columns k1 = 16 b + c, Parseval partial sum, 256-point
-//            column DFTs over k2, four-step twiddle, store T[n2][k1] into ring slot i % kRing of the group (L2);
-//   phase B (pass 2) of item i-1: 256-point row DFTs over k1 for its 16 rows n2 = 16 b + hw, threshold against
-//            k^2 sum|R|^2, warp-aggregated compaction of the tails.
-// Hand-over between the CTAs of a group goes through two monotone counters per group and
-// per ring slot in global memory (done1: tiles of pass 1 finished, done2: row tiles of pass 2 finished;
-// release/acquire at gpu scope).
-// The ring (G x kRing x 512 KiB) is written and read back within microseconds and stays in L2.
-//   phase A roles: stage 1 half-warp c, lane g: rows k2 = g + 16 i (coalesced tile-layout loads); exchange
-//            through shared memory; stage 2 lane c, p2 = warp pair index: n2 = p2 + 16 q (128 B stores)
-//   phase B roles: half-warp hw owns row n2, lane a holds k1 = a + 16 i; private shared-memory region
-constexpr int kLag = BEGE_LAG;                           // phase B runs kLag items behind phase A
-constexpr int kRing = BEGE_LAG + 2;
-constexpr long long kSpinLimit = 6000000000ll;          // ~3 s of SM clocks: a stuck pipeline aborts, never hangs
+// a3 - a7, one persistent warp-specialised kernel for a whole search (PAPER.md:156-162 steps ii-iv; eq.5-9, 13).
+// grid (16 tiles, G groups), one CTA of 20 warps per SM, cooperative launch (all CTAs co-resident).  The kernel
+// is compiled for 96 registers per thread; the A warp groups raise their share to 120 and the S group drops to
+// 48 (setmaxnreg): 2 x 120 + 2 x 96 + 48 = 5 x 96 per SM sub-partition, i.e. exactly the CTA's allocation.
+// The 16 CTAs of a group share the group's (template, segment) items; item `it` of a group is the pair
+// (template grp + G (it / nS), segment it % nS).  CTA (b, grp) owns columns k1 = 16 b + c in pass 1 and rows
+// n2 = 16 b + r in pass 2.  Inside a CTA three roles run concurrently and meet only through mbarriers:
+//   warps 0-7  (A, pass 1): half-warp c takes the template's column tile from shared memory (bulk async copy
+//              from HBM, double buffered, issued one template ahead by warp 0), multiplies by conj() onto its
+//              registers' copy of the segment column, accumulates the Parseval sum, runs the 256-point column
+//              DFT over k2 through a private shared-memory region, applies the four-step twiddle and writes
+//              the 256 x 16 tile into the staging buffer;
+//   warp 16    (S): when the 8 A warps have filled the staging buffer, adds up their Parseval partial sums,
+//              waits until the ring slot is free (done2), sends the tile to the ring with one 32 KiB bulk
+//              async store, and publishes it (done1) once the store has completed;
+//   warps 8-15 (B, pass 2): half-warp r waits for all 16 tiles of an item (done1), loads its row of T from
+//              the ring (L2), runs the 256-point row DFT over k1, thresholds against k^2 sum|R|^2, compacts
+//              the tails with warp-aggregated atomics and releases its share of the slot (done2).
+// The ring holds kRing items per group (G x kRing x 512 KiB), lives in L2, and is laid out per tile as
+// T'[b][n2][c ^ (n2 & 15)] so that both the staging writes and the row reads are bank-conflict free and
+// every tile is one contiguous 32 KiB bulk copy.  Four-step twiddle: wN^(k1 n2) with n2 = p + 16 q is split
+// into wN^(k1 p), folded into the stage-1 twiddles of the column DFT (registers), and wN^(16 k1 q), a
+// 16 x 16 table in shared memory; all twiddles are rounded once from fp64 angles.
+constexpr int kRing = 4;
+constexpr int kSearchThreads = 20 * 32;                    // warp groups: 2 x A, 2 x B, 1 x S (+ 3 idle warps)
+constexpr int kPriv = 16 * 17;                              // padded private region of a half-warp (c2 elements)
 
-BEGE_D void signal_inc(unsigned long long* ctr)
+template <int NI> struct SearchSmem {
+    c2 hbuf[2][NI * 256];                                   // template column tiles (bulk async loads)
+    c2 apriv[16][kPriv];                                    // pass 1: private exchange regions
+    c2 stage[4096];                                         // pass 1 -> ring: T' tile
+    float ssig[16];                                         // Parseval partial sums of the 8 A warps
+    c2 bpriv[16][kPriv];                                    // pass 2: private exchange regions
+    float2 tbl[256];                                        // wN^(16 k1 q), [q][c]
+    uint64_t hfull[2], hempty[2], sfull, sempty;
+};
+
+constexpr int kSearchSmem = (int)sizeof(SearchSmem<16>) + 128;   // one size for both band layouts
+
+// 256-point DFT of a half-warp through its private padded region.  in: lane a holds x[a + 16 i] in v[i];
+// out: lane p holds X[p + 16 q] in v[q].  tw[p] (as given, no conjugation) multiplies stage-1 output p.
+template <int DIR>
+BEGE_D void hw_fft256p(c2 (&v)[16], const float2 (&tw)[16], c2* priv, int lane16)
 {
-    __syncthreads();
-    if (threadIdx.x == 0) asm volatile("red.release.gpu.global.add.u64 [%0], %1;" :: "l"(ctr), "l"(1ull) : "memory");
-}
-BEGE_D void wait_ge(const unsigned long long* ctr, unsigned long long target, int* abort_flag)
-{
-    if (threadIdx.x == 0) {
-        unsigned long long v;
-        const long long t0 = clock64();
-        for (;;) {
-            asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(ctr) : "memory");
-            if (v >= target) break;
-            if (*(volatile int*)abort_flag) break;
-            if (clock64() - t0 > kSpinLimit) { *(volatile int*)abort_flag = 1; break; }
-        }
-    }
-    __syncthreads();
+    fft16<DIR>(v);
+#pragma unroll
+    for (int p = 1; p < 16; ++p) v[p] = cmul(v[p], tw[p].x, tw[p].y);
+    c2* wr = priv + lane16 * 17;
+#pragma unroll
+    for (int p = 0; p < 16; ++p) wr[p] = v[p];
+    __syncwarp();
+    const c2* rd = priv + lane16;
+#pragma unroll
+    for (int a = 0; a < 16; ++a) v[a] = rd[a * 17];
+    __syncwarp();
+    fft16<DIR>(v);
 }
 
 template <int I0, int NI, bool SINGLE>
-__global__ void __launch_bounds__(256, 2)
+__global__ void __launch_bounds__(kSearchThreads, 1)
 k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restrict__ ring,
-         float* __restrict__ sigpart, const float2* __restrict__ tw256, const float2* __restrict__ twN,
-         float k2, bege_tail* __restrict__ rec, unsigned long long cap, unsigned long long* __restrict__ counter,
-         c2* __restrict__ zdbg, uint64_t j0, uint64_t nT, uint32_t m0, uint32_t nS, uint32_t S,
-         unsigned long long* done1, unsigned long long* done2, int* abort_flag)
+         float* __restrict__ sigpart, float k2, bege_tail* __restrict__ rec, unsigned long long cap,
+         unsigned long long* __restrict__ counter, c2* __restrict__ zdbg, uint64_t j0, uint64_t nT,
+         uint32_t m0, uint32_t nS, uint32_t S, unsigned long long* done1, unsigned long long* done2,
+         int* abort_flag)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    c2* sm = reinterpret_cast<c2*>(smem_raw);                     // [4096] exchange buffer (both phases)
-    float2* wNs = reinterpret_cast<float2*>(sm + 4096);           // [16][256] four-step twiddles of this tile
-    float* red = reinterpret_cast<float*>(wNs + 4096);            // [8]
-    const int t = threadIdx.x, b = blockIdx.x, grp = blockIdx.y, G = gridDim.y;
-    const int c = t >> 4, g = t & 15, lane = t & 31;              // phase A stage 1 (c, g); phase B (hw = c, a = g)
-    const int c2i = t & 15, p2 = t >> 4;                          // phase A stage 2
-    constexpr uint64_t kTile = (uint64_t)NI * 256;                // elements per (spectrum, tile)
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    SearchSmem<NI>& sm = *reinterpret_cast<SearchSmem<NI>*>(smem_raw);
+    const int t = threadIdx.x, warp = t >> 5, lane = t & 31;
+    const int b = blockIdx.x, grp = blockIdx.y, G = gridDim.y;
+    constexpr uint32_t kTileBytes = NI * 256 * sizeof(c2);
+    constexpr uint64_t kTile = (uint64_t)NI * 256;
 
-    float2 w1[16];
-    load_w1(w1, tw256, g);
-#pragma unroll
-    for (int q = 0; q < 16; ++q) wNs[q * 256 + t] = __ldg(twN + (p2 + 16 * q) * 256 + 16 * b + c2i);
-
-    c2 xr[NI], h[NI];
-    if (SINGLE) {
-        const c2* xb = xseg + ((uint64_t)m0 * 16 + b) * kTile;
-#pragma unroll
-        for (int ii = 0; ii < NI; ++ii) xr[ii] = xb[ii * 256 + t];
+    if (t == 0) {
+        mbar_init(&sm.hfull[0], 1); mbar_init(&sm.hfull[1], 1);
+        mbar_init(&sm.hempty[0], 8); mbar_init(&sm.hempty[1], 8);
+        mbar_init(&sm.sfull, 8); mbar_init(&sm.sempty, 1);
+        fence_mbar_init();
+    }
+    if (t < 256) {                                           // tbl[q][c] = exp(2 pi i 16 q (16 b + c) / N)
+        const int q = t >> 4, c = t & 15;
+        double sn, cs;
+        sincospi(2.0 * (double)((16 * q * (16 * b + c)) & (kN - 1)) / (double)kN, &sn, &cs);
+        sm.tbl[t] = make_float2((float)cs, (float)sn);
     }
     __syncthreads();
 
     const uint64_t nTg = nT > (uint64_t)grp ? (nT - grp + G - 1) / G : 0;   // templates of this group
     const uint64_t n_items = nTg * nS;
     c2* myring = ring + (uint64_t)grp * kRing * kN;
-    unsigned long long* d1 = done1 + grp * kRing;             // one counter per ring slot: a count can only
-    unsigned long long* d2 = done2 + grp * kRing;             // come from the item that currently owns the slot
-    const int n2 = 16 * b + c;                                    // phase B row
+    unsigned long long* d1 = done1 + grp * kRing;            // one counter pair per ring slot: a count can only
+    unsigned long long* d2 = done2 + grp * kRing;            // come from the item that currently owns the slot
 
-    for (uint64_t i = 0; i < n_items + kLag; ++i) {
-        if (i < n_items) {
-            // ---------------------------------------------------------------- phase A, item i
-            const uint64_t jl = grp + (uint64_t)G * (i / nS);
-            const uint32_t ml = (uint32_t)(i % nS);
-            if (SINGLE || ml == 0) {
-                const c2* hb = bank + ((j0 + jl) * 16 + b) * kTile;
+    if (warp < 8) {
+        // ================================================================ A: pass 1
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 120;");
+        const int c = t >> 4, g = t & 15;                    // column of the tile, lane of its half-warp
+        const int k1 = 16 * b + c;
+        float2 tw[16];                                       // exp(2 pi i (g p / 256 + k1 p / N))
 #pragma unroll
-                for (int ii = 0; ii < NI; ++ii) h[ii] = __ldcs(hb + ii * 256 + t);
+        for (int p = 0; p < 16; ++p) {
+            double sn, cs;
+            sincospi(2.0 * (double)((256 * g * p + k1 * p) & (kN - 1)) / (double)kN, &sn, &cs);
+            tw[p] = make_float2((float)cs, (float)sn);
+        }
+        c2 xr[NI];
+        if (SINGLE) {
+            const c2* xb = xseg + ((uint64_t)m0 * 16 + b) * kTile;
+#pragma unroll
+            for (int ii = 0; ii < NI; ++ii) xr[ii] = xb[ii * 256 + t];
+        }
+        const uint64_t pol = policy_evict_first();
+        if (t == 0 && nTg > 0) {
+            mbar_arrive_expect_tx(&sm.hfull[0], kTileBytes);
+            bulk_load(sm.hbuf[0], bank + ((j0 + grp) * 16 + b) * kTile, kTileBytes, &sm.hfull[0], pol);
+        }
+        c2* priv = sm.apriv[c];
+        uint64_t it = 0;
+        for (uint64_t tj = 0; tj < nTg; ++tj) {
+            const int s = (int)(tj & 1);
+            if (t == 0 && tj + 1 < nTg) {                    // prefetch the next template's tile
+                if (tj >= 1) mbar_wait(&sm.hempty[s ^ 1], (uint32_t)(((tj - 1) >> 1) & 1), abort_flag);
+                mbar_arrive_expect_tx(&sm.hfull[s ^ 1], kTileBytes);
+                bulk_load(sm.hbuf[s ^ 1], bank + ((j0 + grp + (uint64_t)G * (tj + 1)) * 16 + b) * kTile, kTileBytes,
+                          &sm.hfull[s ^ 1], pol);
             }
-            if (!SINGLE) {
-                const c2* xb = xseg + ((uint64_t)(m0 + ml) * 16 + b) * kTile;
+            __syncwarp();
+            mbar_wait(&sm.hfull[s], (uint32_t)((tj >> 1) & 1), abort_flag);
+            const c2* hb = sm.hbuf[s];
+            for (uint32_t ml = 0; ml < nS; ++ml, ++it) {
+                if (!SINGLE) {
+                    const c2* xb = xseg + ((uint64_t)(m0 + ml) * 16 + b) * kTile;
 #pragma unroll
-                for (int ii = 0; ii < NI; ++ii) xr[ii] = __ldg(xb + ii * 256 + t);
-            }
-            if (i >= kRing) wait_ge(d2 + i % kRing, 16ull * (i / kRing), abort_flag);   // slot free again
-            c2 v[16];
-            c2 acc = mk(0.f, 0.f);
-#pragma unroll
-            for (int r = 0; r < 16; ++r) {
-                if (r >= I0 && r < I0 + NI) {
-                    v[r] = cmulc(xr[r - I0], h[r - I0]);
-                    acc = fma2(v[r], v[r], acc);
-                } else {
-                    v[r] = mk(0.f, 0.f);
+                    for (int ii = 0; ii < NI; ++ii) xr[ii] = __ldg(xb + ii * 256 + t);
                 }
+                c2 v[16];
+                c2 acc = mk(0.f, 0.f);
+#pragma unroll
+                for (int r = 0; r < 16; ++r) {
+                    if (r >= I0 && r < I0 + NI) {
+                        v[r] = cmulc(xr[r - I0], hb[(r - I0) * 256 + t]);
+                        acc = fma2(v[r], v[r], acc);
+                    } else {
+                        v[r] = mk(0.f, 0.f);
+                    }
+                }
+                if (ml + 1 == nS) {                          // this warp is done with the template tile
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&sm.hempty[s]);
+                }
+                hw_fft256p<+1>(v, tw, priv, g);
+                // lane p = g holds n2 = p + 16 q of column c
+                if (it >= 1) mbar_wait(&sm.sempty, (uint32_t)((it - 1) & 1), abort_flag);
+                c2* st = sm.stage + g * 16 + (c ^ g);
+#pragma unroll
+                for (int q = 0; q < 16; ++q) st[q * 256] = cmul(v[q], sm.tbl[q * 16 + c]);
+                const float sw = warp_sum32(re(acc) + im(acc));
+                if (lane == 0) sm.ssig[warp] = sw;
+                fence_proxy_async_smem();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&sm.sfull);
             }
-            stage1<+1>(v, w1);
-#pragma unroll
-            for (int p = 0; p < 16; ++p) sm[xidx(c, g, p)] = v[p];
-            const float s = warp_sum32(re(acc) + im(acc));
-            if (lane == 0) red[t >> 5] = s;
-            __syncthreads();
-#pragma unroll
-            for (int gg = 0; gg < 16; ++gg) v[gg] = sm[xidx(c2i, gg, p2)];
-            fft16<+1>(v);
-            c2* out = myring + (i % kRing) * (uint64_t)kN + 16 * b + c2i;
-#pragma unroll
-            for (int q = 0; q < 16; ++q) out[(p2 + 16 * q) * 256] = cmul(v[q], wNs[q * 256 + t]);
-            if (t == 0) {
+        }
+    } else if (warp >= 16) {
+        // ================================================================ S: staging buffer -> ring
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 48;");
+        if (warp == 16 && lane == 0) {
+            const uint64_t pol = policy_evict_last();
+            for (uint64_t it = 0; it < n_items; ++it) {
+                const int slot = (int)(it % kRing);
+                const uint64_t use = it / kRing;
+                const uint64_t jl = grp + (uint64_t)G * (it / nS);
+                const uint32_t ml = (uint32_t)(it % nS);
+                mbar_wait(&sm.sfull, (uint32_t)(it & 1), abort_flag);
                 float tot = 0.f;
 #pragma unroll
-                for (int w = 0; w < 8; ++w) tot += red[w];
+                for (int w = 0; w < 8; ++w) tot += sm.ssig[w];
                 sigpart[((j0 + jl) * (uint64_t)S + (m0 + ml)) * 16 + b] = tot;
+                if (use >= 1) counter_wait_ge(d2 + slot, 128ull * use, abort_flag);   // slot read out by pass 2
+                fence_proxy_async();
+                bulk_store(myring + (uint64_t)slot * kN + (uint64_t)b * 4096, sm.stage, 4096 * sizeof(c2), pol);
+                bulk_commit();
+                bulk_wait_read0();
+                mbar_arrive(&sm.sempty);
+                bulk_wait0();
+                fence_proxy_async();
+                counter_add_release(d1 + slot, 1ull);
             }
-            signal_inc(d1 + i % kRing);
         }
-        if (i >= kLag) {
-            // ---------------------------------------------------------------- phase B, item i - kLag
-            const uint64_t ib = i - kLag;
+    } else {
+        // ================================================================ B: pass 2
+        const int hw = (t - 256) >> 4, a = t & 15;           // row of the row tile, lane of its half-warp
+        const int n2 = 16 * b + hw;
+        float2 w1[16];                                       // exp(2 pi i a p / 256)
+#pragma unroll
+        for (int p = 0; p < 16; ++p) {
+            double sn, cs;
+            sincospi(2.0 * (double)((a * p) & 255) / 256.0, &sn, &cs);
+            w1[p] = make_float2((float)cs, (float)sn);
+        }
+        c2* priv = sm.bpriv[hw];
+        const uint64_t row_off = (uint64_t)n2 * 16 + (uint64_t)(a ^ hw);      // T'[i][n2][a ^ (n2 & 15)]
+        for (uint64_t ib = 0; ib < n_items; ++ib) {
+            const int slot = (int)(ib % kRing);
+            const uint64_t use = ib / kRing;
             const uint64_t jl = grp + (uint64_t)G * (ib / nS);
             const uint32_t ml = (uint32_t)(ib % nS);
-            wait_ge(d1 + ib % kRing, 16ull * (ib / kRing + 1), abort_flag);   // all 16 tiles of item i-1 are in the ring
-            const c2* src = myring + (ib % kRing) * (uint64_t)kN + n2 * 256 + g;
+            if (lane == 0) counter_wait_ge(d1 + slot, 16ull * (use + 1), abort_flag);   // all 16 tiles are in the ring
+            __syncwarp();
+            const c2* src = myring + (uint64_t)slot * kN + row_off;
             c2 v[16];
 #pragma unroll
-            for (int r = 0; r < 16; ++r) v[r] = __ldcg(src + 16 * r);
+            for (int r = 0; r < 16; ++r) v[r] = __ldcg(src + r * 4096);
             const uint64_t pair = (j0 + jl) * (uint64_t)S + (m0 + ml);
-            const float sumR2 = hw_sum16(__ldcg(sigpart + pair * 16 + g));
-            hw_fft256<+1>(v, w1, sm + c * 256, g);
-            // lane a = g holds Z[n1 = a + 16 q]; lag n = 256 n1 + n2
+            const float sumR2 = hw_sum16(__ldcg(sigpart + pair * 16 + a));
+            fft16<+1>(v);
+            __syncwarp();
+            if (lane == 0) counter_add_release(d2 + slot, 1ull);             // this warp's rows are in registers
+#pragma unroll
+            for (int p = 1; p < 16; ++p) v[p] = cmul(v[p], w1[p].x, w1[p].y);
+            {
+                c2* wr = priv + a * 17;
+#pragma unroll
+                for (int p = 0; p < 16; ++p) wr[p] = v[p];
+                __syncwarp();
+                const c2* rd = priv + a;
+#pragma unroll
+                for (int aa = 0; aa < 16; ++aa) v[aa] = rd[aa * 17];
+                __syncwarp();
+                fft16<+1>(v);
+            }
+            // lane a holds Z[n1 = a + 16 q]; lag n = 256 n1 + n2
             const float thr = k2 * sumR2;
             unsigned hits = 0;
             float m2[16];
@@ -334,7 +425,7 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
                 const float invN = 1.0f / (float)kN;
 #pragma unroll
                 for (int q = 0; q < 16; ++q)
-                    zdbg[(uint64_t)(g + 16 * q) * 256 + n2] = mul2(v[q], bc(invN));
+                    zdbg[(uint64_t)(a + 16 * q) * 256 + n2] = mul2(v[q], bc(invN));
             }
             if (__any_sync(0xffffffffu, hits != 0)) {
                 const int cnt = __popc(hits);
@@ -348,23 +439,22 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
                 unsigned long long base = 0;
                 if (lane == 31) base = atomicAdd(counter, (unsigned long long)total);
                 base = __shfl_sync(0xffffffffu, base, 31);
-                unsigned long long slot = base + (unsigned long long)(incl - cnt);
+                unsigned long long slot_r = base + (unsigned long long)(incl - cnt);
                 const float inv = 1.0f / sumR2;
 #pragma unroll
                 for (int q = 0; q < 16; ++q) {
                     if (hits & (1u << q)) {
-                        if (slot < cap) {
+                        if (slot_r < cap) {
                             bege_tail r;
                             r.template_id = (uint32_t)(j0 + jl);
-                            r.lag = (uint32_t)(m0 + ml) * (uint32_t)kN + (uint32_t)((g + 16 * q) * 256 + n2);
+                            r.lag = (uint32_t)(m0 + ml) * (uint32_t)kN + (uint32_t)((a + 16 * q) * 256 + n2);
                             r.snr = sqrtf(m2[q] * inv);
-                            rec[slot] = r;
+                            rec[slot_r] = r;
                         }
-                        ++slot;
+                        ++slot_r;
                     }
                 }
             }
-            signal_inc(d2 + ib % kRing);
         }
     }
 }
@@ -524,7 +614,7 @@ extern "C" int bege_plan_create(bege_plan** out, uint32_t N, double fs, double l
                           (const void*)k_search<0, 16, true>, (const void*)k_search<0, 16, false>}) {
         if (cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, kSearchSmem) != cudaSuccess) return bail(BEGE_ECUDA);
         int o = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, f, 256, kSearchSmem) != cudaSuccess) return bail(BEGE_ECUDA);
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, f, kSearchThreads, kSearchSmem) != cudaSuccess) return bail(BEGE_ECUDA);
         occ = occ ? std::min(occ, o) : o;
     }
     int coop = 0;
@@ -659,15 +749,14 @@ static int launch_search(bege_plan* p, const c2* bank, const c2* xs, c2* ring, f
     const int G = (int)std::min<uint64_t>((uint64_t)p->G, nT);
     const dim3 grid(16, G);
     const bool single = (p->S == 1);
-    const float2 *tw256 = p->tw256, *twN = p->twN;
     unsigned long long capll = cap;
     uint32_t S = p->S;
-    void* args[] = {&bank, &xs, &ring, &sig, &tw256, &twN, &k2, &rec, &capll, &counter, &zdbg, &j0, &nT, &m0, &nS, &S,
+    void* args[] = {&bank, &xs, &ring, &sig, &k2, &rec, &capll, &counter, &zdbg, &j0, &nT, &m0, &nS, &S,
                     &done1, &done2, &abort_flag};
     const void* f = p->NI == 14 ? (single ? (const void*)k_search<1, 14, true> : (const void*)k_search<1, 14, false>)
                                 : (single ? (const void*)k_search<0, 16, true> : (const void*)k_search<0, 16, false>);
     if (p->profiling) cudaEventRecord(p->ev_a, p->stream);
-    CU(p, cudaLaunchCooperativeKernel(f, grid, dim3(256), args, kSearchSmem, p->stream));
+    CU(p, cudaLaunchCooperativeKernel(f, grid, dim3(kSearchThreads), args, kSearchSmem, p->stream));
     count_launch(p);
     if (p->profiling) {
         cudaEventRecord(p->ev_b, p->stream);
