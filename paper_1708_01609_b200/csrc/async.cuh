@@ -90,6 +90,39 @@ BEGE_DA unsigned long long counter_load_acquire(const unsigned long long* ctr)
     asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(ctr) : "memory");
     return v;
 }
+BEGE_DA void counter_add_relaxed(unsigned long long* ctr, unsigned long long v)
+{
+    asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" :: "l"(ctr), "l"(v) : "memory");
+}
+BEGE_DA unsigned long long counter_load_relaxed(const unsigned long long* ctr)
+{
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(ctr) : "memory");
+    return v;
+}
+// whole warp waits until *ctr >= target: lane 0 polls (relaxed, L2), the value is broadcast so that the loop is
+// warp-uniform and the warp stays converged.  The data guarded by the counter must be read with ld.global.cg
+// (L2 is the point of coherence; the producer publishes with a gpu-scope release after its writes completed).
+BEGE_DA void warp_counter_wait_ge(const unsigned long long* ctr, unsigned long long target, int* abort_flag, int lane)
+{
+    const long long t0 = clock64();
+    for (;;) {
+        unsigned long long v = 0;
+        int bail = 0;
+        if (lane == 0) {
+            v = counter_load_relaxed(ctr);
+            if (v < target) {
+                bail = *(volatile int*)abort_flag;
+                if (clock64() - t0 > kSpinLimit) { *(volatile int*)abort_flag = 1; bail = 1; }
+            }
+        }
+        v = __shfl_sync(0xffffffffu, v, 0);
+        bail = __shfl_sync(0xffffffffu, bail, 0);
+        if (v >= target || bail) break;
+        __nanosleep(100);
+    }
+    __syncwarp();
+}
 // one thread spins until *ctr >= target
 BEGE_DA void counter_wait_ge(const unsigned long long* ctr, unsigned long long target, int* abort_flag)
 {

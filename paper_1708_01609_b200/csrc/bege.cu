@@ -210,11 +210,11 @@ constexpr int kPriv = 16 * 17;                              // padded private re
 template <int NI> struct SearchSmem {
     c2 hbuf[2][NI * 256];                                   // template column tiles (bulk async loads)
     c2 apriv[16][kPriv];                                    // pass 1: private exchange regions
-    c2 stage[4096];                                         // pass 1 -> ring: T' tile
-    float ssig[16];                                         // Parseval partial sums of the 8 A warps
+    c2 stage[2][4096];                                      // pass 1 -> ring: T' tile, double buffered
+    float ssig[2][8];                                       // Parseval partial sums of the 8 A warps
     c2 bpriv[16][kPriv];                                    // pass 2: private exchange regions
     float2 tbl[256];                                        // wN^(16 k1 q), [q][c]
-    uint64_t hfull[2], hempty[2], sfull, sempty;
+    uint64_t hfull[2], hempty[2], sfull[2], sempty[2];
 };
 
 constexpr int kSearchSmem = (int)sizeof(SearchSmem<16>) + 128;   // one size for both band layouts
@@ -256,7 +256,8 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
     if (t == 0) {
         mbar_init(&sm.hfull[0], 1); mbar_init(&sm.hfull[1], 1);
         mbar_init(&sm.hempty[0], 8); mbar_init(&sm.hempty[1], 8);
-        mbar_init(&sm.sfull, 8); mbar_init(&sm.sempty, 1);
+        mbar_init(&sm.sfull[0], 8); mbar_init(&sm.sfull[1], 8);
+        mbar_init(&sm.sempty[0], 1); mbar_init(&sm.sempty[1], 1);
         fence_mbar_init();
     }
     if (t < 256) {                                           // tbl[q][c] = exp(2 pi i 16 q (16 b + c) / N)
@@ -332,15 +333,16 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
                 }
                 hw_fft256p<+1>(v, tw, priv, g);
                 // lane p = g holds n2 = p + 16 q of column c
-                if (it >= 1) mbar_wait(&sm.sempty, (uint32_t)((it - 1) & 1), abort_flag);
-                c2* st = sm.stage + g * 16 + (c ^ g);
+                const int sb = (int)(it & 1);                // staging buffer of this item
+                if (it >= 2) mbar_wait(&sm.sempty[sb], (uint32_t)(((it - 2) >> 1) & 1), abort_flag);
+                c2* st = sm.stage[sb] + g * 16 + (c ^ g);
 #pragma unroll
                 for (int q = 0; q < 16; ++q) st[q * 256] = cmul(v[q], sm.tbl[q * 16 + c]);
                 const float sw = warp_sum32(re(acc) + im(acc));
-                if (lane == 0) sm.ssig[warp] = sw;
+                if (lane == 0) sm.ssig[sb][warp] = sw;
                 fence_proxy_async_smem();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&sm.sfull);
+                if (lane == 0) mbar_arrive(&sm.sfull[sb]);
             }
         }
     } else if (warp >= 16) {
@@ -348,25 +350,34 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
         asm volatile("setmaxnreg.dec.sync.aligned.u32 48;");
         if (warp == 16 && lane == 0) {
             const uint64_t pol = policy_evict_last();
+            // one bulk store per item; the store of item it-1 is retired (staging buffer handed back, tile
+            // published) only after the store of item it has been issued, so S never idles on a store
             for (uint64_t it = 0; it < n_items; ++it) {
-                const int slot = (int)(it % kRing);
+                const int slot = (int)(it % kRing), sb = (int)(it & 1);
                 const uint64_t use = it / kRing;
                 const uint64_t jl = grp + (uint64_t)G * (it / nS);
                 const uint32_t ml = (uint32_t)(it % nS);
-                mbar_wait(&sm.sfull, (uint32_t)(it & 1), abort_flag);
+                mbar_wait(&sm.sfull[sb], (uint32_t)((it >> 1) & 1), abort_flag);
                 float tot = 0.f;
 #pragma unroll
-                for (int w = 0; w < 8; ++w) tot += sm.ssig[w];
+                for (int w = 0; w < 8; ++w) tot += sm.ssig[sb][w];
                 sigpart[((j0 + jl) * (uint64_t)S + (m0 + ml)) * 16 + b] = tot;
                 if (use >= 1) counter_wait_ge(d2 + slot, 128ull * use, abort_flag);   // slot read out by pass 2
                 fence_proxy_async();
-                bulk_store(myring + (uint64_t)slot * kN + (uint64_t)b * 4096, sm.stage, 4096 * sizeof(c2), pol);
+                bulk_store(myring + (uint64_t)slot * kN + (uint64_t)b * 4096, sm.stage[sb], 4096 * sizeof(c2), pol);
                 bulk_commit();
-                bulk_wait_read0();
-                mbar_arrive(&sm.sempty);
+                if (it >= 1) {
+                    asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
+                    mbar_arrive(&sm.sempty[sb ^ 1]);
+                    asm volatile("cp.async.bulk.wait_group 1;" ::: "memory");
+                    fence_proxy_async();
+                    counter_add_release(d1 + (int)((it - 1) % kRing), 1ull);
+                }
+            }
+            if (n_items > 0) {
                 bulk_wait0();
                 fence_proxy_async();
-                counter_add_release(d1 + slot, 1ull);
+                counter_add_release(d1 + (int)((n_items - 1) % kRing), 1ull);
             }
         }
     } else {
@@ -387,8 +398,7 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
             const uint64_t use = ib / kRing;
             const uint64_t jl = grp + (uint64_t)G * (ib / nS);
             const uint32_t ml = (uint32_t)(ib % nS);
-            if (lane == 0) counter_wait_ge(d1 + slot, 16ull * (use + 1), abort_flag);   // all 16 tiles are in the ring
-            __syncwarp();
+            warp_counter_wait_ge(d1 + slot, 16ull * (use + 1), abort_flag, lane);     // all 16 tiles are in the ring
             const c2* src = myring + (uint64_t)slot * kN + row_off;
             c2 v[16];
 #pragma unroll
@@ -397,7 +407,8 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
             const float sumR2 = hw_sum16(__ldcg(sigpart + pair * 16 + a));
             fft16<+1>(v);
             __syncwarp();
-            if (lane == 0) counter_add_release(d2 + slot, 1ull);             // this warp's rows are in registers
+            if (lane == 0) counter_add_relaxed(d2 + slot, 1ull);             // this warp's rows are in registers (the
+                                                                             // loads have returned: fft16 consumed them)
 #pragma unroll
             for (int p = 1; p < 16; ++p) v[p] = cmul(v[p], w1[p].x, w1[p].y);
             {
