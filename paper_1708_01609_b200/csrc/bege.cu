@@ -28,6 +28,10 @@
 #include "cplx.cuh"
 #include "async.cuh"
 
+#ifndef BEGE_ABL
+#define BEGE_ABL 0          // ablation switches for timing experiments (never set in the product build)
+#endif
+
 namespace bege {
 
 constexpr int kN = 65536;
@@ -181,62 +185,46 @@ k_fwd_cols(const c2* __restrict__ G, c2* __restrict__ out, uint64_t out_stride, 
 
 // ------------------------------------------------------------------------------------------------
 // a3 - a7, one persistent warp-specialised kernel for a whole search (PAPER.md:156-162 steps ii-iv; eq.5-9, 13).
-// grid (16 tiles, G groups), one CTA of 20 warps per SM, cooperative launch (all CTAs co-resident).  The kernel
-// is compiled for 96 registers per thread; the A warp groups raise their share to 120 and the S group drops to
-// 48 (setmaxnreg): 2 x 120 + 2 x 96 + 48 = 5 x 96 per SM sub-partition, i.e. exactly the CTA's allocation.
-// The 16 CTAs of a group share the group's (template, segment) items; item `it` of a group is the pair
-// (template grp + G (it / nS), segment it % nS).  CTA (b, grp) owns columns k1 = 16 b + c in pass 1 and rows
-// n2 = 16 b + r in pass 2.  Inside a CTA three roles run concurrently and meet only through mbarriers:
-//   warps 0-7  (A, pass 1): half-warp c takes the template's column tile from shared memory (bulk async copy
-//              from HBM, double buffered, issued one template ahead by warp 0), multiplies by conj() onto its
-//              registers' copy of the segment column, accumulates the Parseval sum, runs the 256-point column
-//              DFT over k2 through a private shared-memory region, applies the four-step twiddle and writes
-//              the 256 x 16 tile into the staging buffer;
-//   warp 16    (S): when the 8 A warps have filled the staging buffer, adds up their Parseval partial sums,
-//              waits until the ring slot is free (done2), sends the tile to the ring with one 32 KiB bulk
-//              async store, and publishes it (done1) once the store has completed;
-//   warps 8-15 (B, pass 2): half-warp r waits for all 16 tiles of an item (done1), loads its row of T from
-//              the ring (L2), runs the 256-point row DFT over k1, thresholds against k^2 sum|R|^2, compacts
-//              the tails with warp-aggregated atomics and releases its share of the slot (done2).
-// The ring holds kRing items per group (G x kRing x 512 KiB), lives in L2, and is laid out per tile as
-// T'[b][n2][c ^ (n2 & 15)] so that both the staging writes and the row reads are bank-conflict free and
-// every tile is one contiguous 32 KiB bulk copy.  Four-step twiddle: wN^(k1 n2) with n2 = p + 16 q is split
-// into wN^(k1 p), folded into the stage-1 twiddles of the column DFT (registers), and wN^(16 k1 q), a
-// 16 x 16 table in shared memory; all twiddles are rounded once from fp64 angles.
-constexpr int kRing = 4;
-constexpr int kSearchThreads = 20 * 32;                    // warp groups: 2 x A, 2 x B, 1 x S (+ 3 idle warps)
+// grid (16 tiles, G groups), one CTA of 32 warps (64 registers per thread) per SM, cooperative launch (all CTAs
+// co-resident).  The 16 CTAs of a group share the group's (template, segment) items; item `it` of a group is the
+// pair (template grp + G (it / nS), segment it % nS).  CTA (b, grp) owns columns k1 = 16 b + c in pass 1 and rows
+// n2 = 16 b + r in pass 2.  The path is latency bound, not pipe bound (profiles/), so the kernel is built for
+// warps in flight: four teams of 8 warps, two per pass, team k of a pass taking the items it = k (mod 2).
+//   A teams (pass 1): the template's column tile arrives in shared memory by bulk async copy from HBM (one
+//              buffer per team, refilled as soon as the team has read it, mbarrier-tracked).  Stage 1: half-warp
+//              c, lane g holds rows k2 = g + 16 i of column c: conj(H) X against the segment tile (shared
+//              memory), Parseval partial sum, 16-point DFTs, twiddles theta^p generated from one complex number
+//              per thread.  One exchange through shared memory (two named barriers of the team per item).
+//              Stage 2: lane c, p = warp-pair index: 16-point DFTs, second twiddle factor, and
+//              T[n2 = p + 16 q][16 b + c] goes straight from registers to the ring in L2 (128 B per half-warp
+//              and store).  The tile is published (done1) with a release issued one item later.
+//   B teams (pass 2): half-warp r waits for all 16 tiles of an item (done1), loads its row of T from the ring,
+//              runs the 256-point row DFT over k1 through a private shared-memory region, thresholds against
+//              k^2 sum|R|^2, compacts the tails with warp-aggregated atomics, and releases its share of the
+//              ring slot (done2) as soon as the row is in registers.
+// The ring holds kRing items per group (G x kRing x 512 KiB) and lives in L2.  Four-step twiddle wN^(k1 n2) with
+// n2 = p + 16 q is split into wN^(k1 p), folded into theta = exp(2 pi i (256 g + k1) / N), and wN^(16 k1 q), a
+// 16 x 16 table in shared memory; theta and the tables are rounded once from fp64 angles.
+constexpr int kRing = 8;
+constexpr int kSearchThreads = 32 * 32;
 constexpr int kPriv = 16 * 17;                              // padded private region of a half-warp (c2 elements)
+constexpr int kXch = 16 * 16 * 17;                          // padded exchange buffer of pass 1 (c2 elements)
 
-template <int NI> struct SearchSmem {
-    c2 hbuf[2][NI * 256];                                   // template column tiles (bulk async loads)
-    c2 apriv[16][kPriv];                                    // pass 1: private exchange regions
-    c2 stage[2][4096];                                      // pass 1 -> ring: T' tile, double buffered
-    float ssig[2][8];                                       // Parseval partial sums of the 8 A warps
-    c2 bpriv[16][kPriv];                                    // pass 2: private exchange regions
+template <int NI, bool XS> struct SearchSmem {
+    c2 hbuf[2][NI * 256];                                   // template column tile of each A team
+    c2 xs[XS ? NI * 256 : 2];                               // segment column tile (single-segment searches)
+    c2 xch[2][kXch];                                        // pass 1 of each A team: stage 1 -> stage 2, [p][g][c]
+    c2 bpriv[32][kPriv];                                    // pass 2: private exchange regions
     float2 tbl[256];                                        // wN^(16 k1 q), [q][c]
-    uint64_t hfull[2], hempty[2], sfull[2], sempty[2];
+    float2 w1t[256];                                        // w256^(a p), [p][a]
+    float ssig[2][8];                                       // Parseval partial sums of the 8 warps of an A team
+    uint64_t hfull[2];
 };
+template <int NI, bool SINGLE> __host__ __device__ constexpr bool search_xs() { return SINGLE && NI <= 14; }
+template <int NI, bool SINGLE> constexpr int search_smem() { return (int)sizeof(SearchSmem<NI, search_xs<NI, SINGLE>()>) + 128; }
 
-constexpr int kSearchSmem = (int)sizeof(SearchSmem<16>) + 128;   // one size for both band layouts
-
-// 256-point DFT of a half-warp through its private padded region.  in: lane a holds x[a + 16 i] in v[i];
-// out: lane p holds X[p + 16 q] in v[q].  tw[p] (as given, no conjugation) multiplies stage-1 output p.
-template <int DIR>
-BEGE_D void hw_fft256p(c2 (&v)[16], const float2 (&tw)[16], c2* priv, int lane16)
-{
-    fft16<DIR>(v);
-#pragma unroll
-    for (int p = 1; p < 16; ++p) v[p] = cmul(v[p], tw[p].x, tw[p].y);
-    c2* wr = priv + lane16 * 17;
-#pragma unroll
-    for (int p = 0; p < 16; ++p) wr[p] = v[p];
-    __syncwarp();
-    const c2* rd = priv + lane16;
-#pragma unroll
-    for (int a = 0; a < 16; ++a) v[a] = rd[a * 17];
-    __syncwarp();
-    fft16<DIR>(v);
-}
+BEGE_D void bar_team(int id) { asm volatile("bar.sync %0, 256;" :: "r"(id) : "memory"); }   // the 8 warps of a team
+BEGE_D c2 cmul2(c2 x, c2 w) { return cmul(x, re(w), im(w)); }                               // x * w
 
 template <int I0, int NI, bool SINGLE>
 __global__ void __launch_bounds__(kSearchThreads, 1)
@@ -246,25 +234,32 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
          uint32_t m0, uint32_t nS, uint32_t S, unsigned long long* done1, unsigned long long* done2,
          int* abort_flag)
 {
+    constexpr bool XS = search_xs<NI, SINGLE>();
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    SearchSmem<NI>& sm = *reinterpret_cast<SearchSmem<NI>*>(smem_raw);
-    const int t = threadIdx.x, warp = t >> 5, lane = t & 31;
+    SearchSmem<NI, XS>& sm = *reinterpret_cast<SearchSmem<NI, XS>*>(smem_raw);
+    const int team = threadIdx.x >> 8;                       // 0, 1: A teams; 2, 3: B teams
+    const int t = threadIdx.x & 255, warp = t >> 5, lane = t & 31;   // within the team
     const int b = blockIdx.x, grp = blockIdx.y, G = gridDim.y;
     constexpr uint32_t kTileBytes = NI * 256 * sizeof(c2);
     constexpr uint64_t kTile = (uint64_t)NI * 256;
 
-    if (t == 0) {
+    if (threadIdx.x == 0) {
         mbar_init(&sm.hfull[0], 1); mbar_init(&sm.hfull[1], 1);
-        mbar_init(&sm.hempty[0], 8); mbar_init(&sm.hempty[1], 8);
-        mbar_init(&sm.sfull[0], 8); mbar_init(&sm.sfull[1], 8);
-        mbar_init(&sm.sempty[0], 1); mbar_init(&sm.sempty[1], 1);
         fence_mbar_init();
     }
-    if (t < 256) {                                           // tbl[q][c] = exp(2 pi i 16 q (16 b + c) / N)
+    if (team == 0) {                                         // tbl[q][c] = exp(2 pi i 16 q (16 b + c) / N)
         const int q = t >> 4, c = t & 15;
         double sn, cs;
         sincospi(2.0 * (double)((16 * q * (16 * b + c)) & (kN - 1)) / (double)kN, &sn, &cs);
         sm.tbl[t] = make_float2((float)cs, (float)sn);
+    } else if (team == 1) {                                  // w1t[p][a] = exp(2 pi i a p / 256)
+        const int p = t >> 4, a = t & 15;
+        double sn, cs;
+        sincospi(2.0 * (double)((a * p) & 255) / 256.0, &sn, &cs);
+        sm.w1t[t] = make_float2((float)cs, (float)sn);
+    } else if (XS && team == 2) {
+        const c2* xb = xseg + ((uint64_t)m0 * 16 + b) * kTile;
+        for (int ii = 0; ii < NI; ++ii) sm.xs[XS ? ii * 256 + t : 0] = xb[ii * 256 + t];
     }
     __syncthreads();
 
@@ -274,135 +269,137 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
     unsigned long long* d1 = done1 + grp * kRing;            // one counter pair per ring slot: a count can only
     unsigned long long* d2 = done2 + grp * kRing;            // come from the item that currently owns the slot
 
-    if (warp < 8) {
-        // ================================================================ A: pass 1
-        asm volatile("setmaxnreg.inc.sync.aligned.u32 120;");
-        const int c = t >> 4, g = t & 15;                    // column of the tile, lane of its half-warp
-        const int k1 = 16 * b + c;
-        float2 tw[16];                                       // exp(2 pi i (g p / 256 + k1 p / N))
-#pragma unroll
-        for (int p = 0; p < 16; ++p) {
+    if ((BEGE_ABL & 16) && team < 2) return;
+    if ((BEGE_ABL & 32) && team >= 2) return;
+    if (team < 2) {
+        // ================================================================ A: pass 1, items it = team (mod 2)
+        const int c = t >> 4, g = t & 15;                    // stage 1: column of the tile, lane of its half-warp
+        const int c2i = t & 15, p2 = t >> 4;                 // stage 2: column, index p of n2 = p + 16 q
+        c2 theta;                                            // exp(2 pi i (256 g + k1) / N), k1 = 16 b + c
+        {
             double sn, cs;
-            sincospi(2.0 * (double)((256 * g * p + k1 * p) & (kN - 1)) / (double)kN, &sn, &cs);
-            tw[p] = make_float2((float)cs, (float)sn);
-        }
-        c2 xr[NI];
-        if (SINGLE) {
-            const c2* xb = xseg + ((uint64_t)m0 * 16 + b) * kTile;
-#pragma unroll
-            for (int ii = 0; ii < NI; ++ii) xr[ii] = xb[ii * 256 + t];
+            sincospi(2.0 * (double)(256 * g + 16 * b + c) / (double)kN, &sn, &cs);
+            theta = mk((float)cs, (float)sn);
         }
         const uint64_t pol = policy_evict_first();
-        if (t == 0 && nTg > 0) {
-            mbar_arrive_expect_tx(&sm.hfull[0], kTileBytes);
-            bulk_load(sm.hbuf[0], bank + ((j0 + grp) * 16 + b) * kTile, kTileBytes, &sm.hfull[0], pol);
+        uint64_t* hfull = &sm.hfull[team];
+        c2* hb = sm.hbuf[team];
+        if (t == 0 && (uint64_t)team < n_items && !(BEGE_ABL & 2)) {
+            mbar_arrive_expect_tx(hfull, kTileBytes);
+            bulk_load(hb, bank + ((j0 + grp + (uint64_t)G * (SINGLE ? (uint64_t)team : team / nS)) * 16 + b) * kTile,
+                      kTileBytes, hfull, pol);
         }
-        c2* priv = sm.apriv[c];
-        uint64_t it = 0;
-        for (uint64_t tj = 0; tj < nTg; ++tj) {
-            const int s = (int)(tj & 1);
-            if (t == 0 && tj + 1 < nTg) {                    // prefetch the next template's tile
-                if (tj >= 1) mbar_wait(&sm.hempty[s ^ 1], (uint32_t)(((tj - 1) >> 1) & 1), abort_flag);
-                mbar_arrive_expect_tx(&sm.hfull[s ^ 1], kTileBytes);
-                bulk_load(sm.hbuf[s ^ 1], bank + ((j0 + grp + (uint64_t)G * (tj + 1)) * 16 + b) * kTile, kTileBytes,
-                          &sm.hfull[s ^ 1], pol);
+        c2* xw = sm.xch[team] + g * 17 + c;                  // + p * 272: element [p][g][c] of the exchange buffer
+        const c2* xrd = sm.xch[team] + p2 * 272 + c2i;       // + gg * 17
+        const int bar_id = 1 + team;
+        int pending = -1;                                    // ring slot whose tile this warp has yet to publish
+        uint32_t nload = 0;                                  // tiles this team has waited for so far
+        uint64_t tj_prev = ~0ull;
+        for (uint64_t it = team; it < n_items; it += 2) {
+            const uint64_t tj = SINGLE ? it : it / nS;
+            const uint32_t ml = SINGLE ? 0u : (uint32_t)(it - tj * nS);
+            const int slot = (int)(it % kRing);
+            if (tj != tj_prev) {                             // a new template tile was ordered for this item
+#if !(BEGE_ABL & 2)
+                mbar_wait(hfull, nload & 1, abort_flag);
+#endif
+                ++nload;
+                tj_prev = tj;
             }
-            __syncwarp();
-            mbar_wait(&sm.hfull[s], (uint32_t)((tj >> 1) & 1), abort_flag);
-            const c2* hb = sm.hbuf[s];
-            for (uint32_t ml = 0; ml < nS; ++ml, ++it) {
-                if (!SINGLE) {
-                    const c2* xb = xseg + ((uint64_t)(m0 + ml) * 16 + b) * kTile;
-#pragma unroll
-                    for (int ii = 0; ii < NI; ++ii) xr[ii] = __ldg(xb + ii * 256 + t);
-                }
-                c2 v[16];
-                c2 acc = mk(0.f, 0.f);
+            c2 v[16];
+            c2 acc = mk(0.f, 0.f);
+            {
+                const c2* xb = xseg + ((uint64_t)(m0 + ml) * 16 + b) * kTile;
 #pragma unroll
                 for (int r = 0; r < 16; ++r) {
                     if (r >= I0 && r < I0 + NI) {
-                        v[r] = cmulc(xr[r - I0], hb[(r - I0) * 256 + t]);
+                        const c2 xv = XS ? sm.xs[XS ? (r - I0) * 256 + t : 0] : __ldg(xb + (r - I0) * 256 + t);
+                        v[r] = cmulc(xv, hb[(r - I0) * 256 + t]);
                         acc = fma2(v[r], v[r], acc);
                     } else {
                         v[r] = mk(0.f, 0.f);
                     }
                 }
-                if (ml + 1 == nS) {                          // this warp is done with the template tile
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(&sm.hempty[s]);
-                }
-                hw_fft256p<+1>(v, tw, priv, g);
-                // lane p = g holds n2 = p + 16 q of column c
-                const int sb = (int)(it & 1);                // staging buffer of this item
-                if (it >= 2) mbar_wait(&sm.sempty[sb], (uint32_t)(((it - 2) >> 1) & 1), abort_flag);
-                c2* st = sm.stage[sb] + g * 16 + (c ^ g);
+            }
+            fft16<+1>(v);
+            {   // v[p] *= theta^p, powers by a depth-4 product tree
+                const c2 t2 = cmul2(theta, theta), t4 = cmul2(t2, t2), t8 = cmul2(t4, t4);
+                const c2 t3 = cmul2(t2, theta), t5 = cmul2(t4, theta), t6 = cmul2(t4, t2), t7 = cmul2(t4, t3);
+                v[1] = cmul2(v[1], theta); v[2] = cmul2(v[2], t2); v[3] = cmul2(v[3], t3); v[4] = cmul2(v[4], t4);
+                v[5] = cmul2(v[5], t5); v[6] = cmul2(v[6], t6); v[7] = cmul2(v[7], t7); v[8] = cmul2(v[8], t8);
+                v[9] = cmul2(v[9], cmul2(t8, theta)); v[10] = cmul2(v[10], cmul2(t8, t2));
+                v[11] = cmul2(v[11], cmul2(t8, t3)); v[12] = cmul2(v[12], cmul2(t8, t4));
+                v[13] = cmul2(v[13], cmul2(t8, t5)); v[14] = cmul2(v[14], cmul2(t8, t6));
+                v[15] = cmul2(v[15], cmul2(t8, t7));
+            }
 #pragma unroll
-                for (int q = 0; q < 16; ++q) st[q * 256] = cmul(v[q], sm.tbl[q * 16 + c]);
-                const float sw = warp_sum32(re(acc) + im(acc));
-                if (lane == 0) sm.ssig[sb][warp] = sw;
-                fence_proxy_async_smem();
+            for (int p = 0; p < 16; ++p) xw[p * 272] = v[p];
+            const float sw = warp_sum32(re(acc) + im(acc));
+            if (lane == 0) sm.ssig[team][warp] = sw;
+            bar_team(bar_id);                                // exchange buffer complete, template tile read out
+            if (t == 0 && !(BEGE_ABL & 2)) {                 // order the tile of this team's next item
+                const uint64_t it2 = it + 2;
+                if (it2 < n_items) {
+                    const uint64_t tj2 = SINGLE ? it2 : it2 / nS;
+                    if (tj2 != tj) {
+                        mbar_arrive_expect_tx(hfull, kTileBytes);
+                        bulk_load(hb, bank + ((j0 + grp + (uint64_t)G * tj2) * 16 + b) * kTile, kTileBytes, hfull, pol);
+                    }
+                }
+            }
+#pragma unroll
+            for (int gg = 0; gg < 16; ++gg) v[gg] = xrd[gg * 17];
+            float tot = 0.f;
+            if (t == 0) {
+#pragma unroll
+                for (int w = 0; w < 8; ++w) tot += sm.ssig[team][w];
+            }
+            bar_team(bar_id);                                // exchange buffer free for the team's next item
+            if (pending >= 0) {                              // the previous item's stores have long landed
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&sm.sfull[sb]);
+                if (lane == 0) counter_add_release(d1 + pending, 1ull);
             }
-        }
-    } else if (warp >= 16) {
-        // ================================================================ S: staging buffer -> ring
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 48;");
-        if (warp == 16 && lane == 0) {
-            const uint64_t pol = policy_evict_last();
-            // one bulk store per item; the store of item it-1 is retired (staging buffer handed back, tile
-            // published) only after the store of item it has been issued, so S never idles on a store
-            for (uint64_t it = 0; it < n_items; ++it) {
-                const int slot = (int)(it % kRing), sb = (int)(it & 1);
-                const uint64_t use = it / kRing;
-                const uint64_t jl = grp + (uint64_t)G * (it / nS);
-                const uint32_t ml = (uint32_t)(it % nS);
-                mbar_wait(&sm.sfull[sb], (uint32_t)((it >> 1) & 1), abort_flag);
-                float tot = 0.f;
+            fft16<+1>(v);
+#if !(BEGE_ABL & 1)
+            if (it >= kRing)                                 // ring slot read out by pass 2 of item it - kRing
+                warp_counter_wait_ge(d2 + slot, 128ull * (it / kRing), abort_flag, lane);
+#endif
+            c2* out = myring + (uint64_t)slot * kN + 16 * b + c2i + p2 * 256;
 #pragma unroll
-                for (int w = 0; w < 8; ++w) tot += sm.ssig[sb][w];
-                sigpart[((j0 + jl) * (uint64_t)S + (m0 + ml)) * 16 + b] = tot;
-                if (use >= 1) counter_wait_ge(d2 + slot, 128ull * use, abort_flag);   // slot read out by pass 2
-                fence_proxy_async();
-                bulk_store(myring + (uint64_t)slot * kN + (uint64_t)b * 4096, sm.stage[sb], 4096 * sizeof(c2), pol);
-                bulk_commit();
-                if (it >= 1) {
-                    asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
-                    mbar_arrive(&sm.sempty[sb ^ 1]);
-                    asm volatile("cp.async.bulk.wait_group 1;" ::: "memory");
-                    fence_proxy_async();
-                    counter_add_release(d1 + (int)((it - 1) % kRing), 1ull);
-                }
+            for (int q = 0; q < 16; ++q) {
+                const c2 o = cmul(v[q], sm.tbl[q * 16 + c2i]);
+                if (!(BEGE_ABL & 4) || re(o) == 1.2345e-30f) out[q * 4096] = o;
             }
-            if (n_items > 0) {
-                bulk_wait0();
-                fence_proxy_async();
-                counter_add_release(d1 + (int)((n_items - 1) % kRing), 1ull);
-            }
+            if (t == 0) sigpart[((j0 + grp + (uint64_t)G * tj) * (uint64_t)S + (m0 + ml)) * 16 + b] = tot;
+            pending = slot;
+        }
+        if (pending >= 0) {
+            __syncwarp();
+            if (lane == 0) counter_add_release(d1 + pending, 1ull);
         }
     } else {
-        // ================================================================ B: pass 2
-        const int hw = (t - 256) >> 4, a = t & 15;           // row of the row tile, lane of its half-warp
+        // ================================================================ B: pass 2, items ib = team - 2 (mod 2)
+        const int kb = team - 2;
+        const int hw = t >> 4, a = t & 15;                   // row of the row tile, lane of its half-warp
         const int n2 = 16 * b + hw;
-        float2 w1[16];                                       // exp(2 pi i a p / 256)
-#pragma unroll
-        for (int p = 0; p < 16; ++p) {
-            double sn, cs;
-            sincospi(2.0 * (double)((a * p) & 255) / 256.0, &sn, &cs);
-            w1[p] = make_float2((float)cs, (float)sn);
-        }
-        c2* priv = sm.bpriv[hw];
-        const uint64_t row_off = (uint64_t)n2 * 16 + (uint64_t)(a ^ hw);      // T'[i][n2][a ^ (n2 & 15)]
-        for (uint64_t ib = 0; ib < n_items; ++ib) {
+        c2* priv = sm.bpriv[kb * 16 + hw];
+        c2* pwr = priv + a * 17;                             // + p:      stage-1 output p of lane a
+        const c2* prd = priv + a;                            // + 17 aa:  stage-2 input from lane aa
+        const float2* w1 = sm.w1t + a;                       // + 16 p:   exp(2 pi i a p / 256)
+        const uint64_t row_off = (uint64_t)n2 * 256 + (uint64_t)a;           // T[n2][k1 = a + 16 r]
+        for (uint64_t ib = kb; ib < n_items; ib += 2) {
             const int slot = (int)(ib % kRing);
             const uint64_t use = ib / kRing;
-            const uint64_t jl = grp + (uint64_t)G * (ib / nS);
-            const uint32_t ml = (uint32_t)(ib % nS);
-            warp_counter_wait_ge(d1 + slot, 16ull * (use + 1), abort_flag, lane);     // all 16 tiles are in the ring
+            const uint64_t tj = SINGLE ? ib : ib / nS;
+            const uint32_t ml = SINGLE ? 0u : (uint32_t)(ib - tj * nS);
+            const uint64_t jl = grp + (uint64_t)G * tj;
+#if !(BEGE_ABL & 1)
+            warp_counter_wait_ge(d1 + slot, 128ull * (use + 1), abort_flag, lane);    // all 16 tiles are in the ring
+#endif
             const c2* src = myring + (uint64_t)slot * kN + row_off;
             c2 v[16];
 #pragma unroll
-            for (int r = 0; r < 16; ++r) v[r] = __ldcg(src + r * 4096);
+            for (int r = 0; r < 16; ++r) v[r] = (BEGE_ABL & 8) ? mk((float)(r + a), (float)ib) : __ldcg(src + 16 * r);
             const uint64_t pair = (j0 + jl) * (uint64_t)S + (m0 + ml);
             const float sumR2 = hw_sum16(__ldcg(sigpart + pair * 16 + a));
             fft16<+1>(v);
@@ -410,27 +407,21 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
             if (lane == 0) counter_add_relaxed(d2 + slot, 1ull);             // this warp's rows are in registers (the
                                                                              // loads have returned: fft16 consumed them)
 #pragma unroll
-            for (int p = 1; p < 16; ++p) v[p] = cmul(v[p], w1[p].x, w1[p].y);
-            {
-                c2* wr = priv + a * 17;
+            for (int p = 1; p < 16; ++p) v[p] = cmul(v[p], w1[16 * p]);
 #pragma unroll
-                for (int p = 0; p < 16; ++p) wr[p] = v[p];
-                __syncwarp();
-                const c2* rd = priv + a;
+            for (int p = 0; p < 16; ++p) pwr[p] = v[p];
+            __syncwarp();
 #pragma unroll
-                for (int aa = 0; aa < 16; ++aa) v[aa] = rd[aa * 17];
-                __syncwarp();
-                fft16<+1>(v);
-            }
+            for (int aa = 0; aa < 16; ++aa) v[aa] = prd[aa * 17];
+            __syncwarp();
+            fft16<+1>(v);
             // lane a holds Z[n1 = a + 16 q]; lag n = 256 n1 + n2
             const float thr = k2 * sumR2;
             unsigned hits = 0;
-            float m2[16];
 #pragma unroll
             for (int q = 0; q < 16; ++q) {
                 const c2 sq = mul2(v[q], v[q]);
-                m2[q] = re(sq) + im(sq);
-                if (m2[q] > thr) hits |= 1u << q;
+                if (re(sq) + im(sq) > thr) hits |= 1u << q;
             }
             if (zdbg != nullptr) {
                 const float invN = 1.0f / (float)kN;
@@ -438,6 +429,9 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
                 for (int q = 0; q < 16; ++q)
                     zdbg[(uint64_t)(a + 16 * q) * 256 + n2] = mul2(v[q], bc(invN));
             }
+#if BEGE_ABL
+            if (thr == -1.f)                                 // timing experiment only: never emit
+#endif
             if (__any_sync(0xffffffffu, hits != 0)) {
                 const int cnt = __popc(hits);
                 int incl = cnt;
@@ -456,10 +450,11 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
                 for (int q = 0; q < 16; ++q) {
                     if (hits & (1u << q)) {
                         if (slot_r < cap) {
+                            const c2 sq = mul2(v[q], v[q]);
                             bege_tail r;
                             r.template_id = (uint32_t)(j0 + jl);
                             r.lag = (uint32_t)(m0 + ml) * (uint32_t)kN + (uint32_t)((a + 16 * q) * 256 + n2);
-                            r.snr = sqrtf(m2[q] * inv);
+                            r.snr = sqrtf((re(sq) + im(sq)) * inv);
                             rec[slot_r] = r;
                         }
                         ++slot_r;
@@ -621,12 +616,16 @@ extern "C" int bege_plan_create(bege_plan** out, uint32_t N, double fs, double l
 
     // the search kernel needs all its CTAs co-resident (groups hand over through global counters)
     int occ = 0;
-    for (const void* f : {(const void*)k_search<1, 14, true>, (const void*)k_search<1, 14, false>,
-                          (const void*)k_search<0, 16, true>, (const void*)k_search<0, 16, false>}) {
-        if (cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, kSearchSmem) != cudaSuccess) return bail(BEGE_ECUDA);
-        int o = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, f, kSearchThreads, kSearchSmem) != cudaSuccess) return bail(BEGE_ECUDA);
-        occ = occ ? std::min(occ, o) : o;
+    {
+        const void* fs[4] = {(const void*)k_search<1, 14, true>, (const void*)k_search<1, 14, false>,
+                             (const void*)k_search<0, 16, true>, (const void*)k_search<0, 16, false>};
+        const int sms[4] = {search_smem<14, true>(), search_smem<14, false>(), search_smem<16, true>(), search_smem<16, false>()};
+        for (int i = 0; i < 4; ++i) {
+            if (cudaFuncSetAttribute(fs[i], cudaFuncAttributeMaxDynamicSharedMemorySize, sms[i]) != cudaSuccess) return bail(BEGE_ECUDA);
+            int o = 0;
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, fs[i], kSearchThreads, sms[i]) != cudaSuccess) return bail(BEGE_ECUDA);
+            occ = i ? std::min(occ, o) : o;
+        }
     }
     int coop = 0;
     cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, device);
@@ -766,6 +765,8 @@ static int launch_search(bege_plan* p, const c2* bank, const c2* xs, c2* ring, f
                     &done1, &done2, &abort_flag};
     const void* f = p->NI == 14 ? (single ? (const void*)k_search<1, 14, true> : (const void*)k_search<1, 14, false>)
                                 : (single ? (const void*)k_search<0, 16, true> : (const void*)k_search<0, 16, false>);
+    const int kSearchSmem = p->NI == 14 ? (single ? search_smem<14, true>() : search_smem<14, false>())
+                                        : (single ? search_smem<16, true>() : search_smem<16, false>());
     if (p->profiling) cudaEventRecord(p->ev_a, p->stream);
     CU(p, cudaLaunchCooperativeKernel(f, grid, dim3(kSearchThreads), args, kSearchSmem, p->stream));
     count_launch(p);
