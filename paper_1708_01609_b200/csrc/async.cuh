@@ -119,7 +119,7 @@ BEGE_DA void warp_counter_wait_ge(const unsigned long long* ctr, unsigned long l
         v = __shfl_sync(0xffffffffu, v, 0);
         bail = __shfl_sync(0xffffffffu, bail, 0);
         if (v >= target || bail) break;
-        __nanosleep(100);
+        __nanosleep(400);
     }
     __syncwarp();
 }

@@ -306,6 +306,8 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
                 ++nload;
                 tj_prev = tj;
             }
+            unsigned long long d2v = ~0ull;                  // slot-free counter, polled early: the load is in flight
+            if (it >= kRing && lane == 0 && !(BEGE_ABL & 1)) d2v = counter_load_relaxed(d2 + slot);   // during stage 1
             c2 v[16];
             c2 acc = mk(0.f, 0.f);
             {
@@ -355,14 +357,14 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
                 for (int w = 0; w < 8; ++w) tot += sm.ssig[team][w];
             }
             bar_team(bar_id);                                // exchange buffer free for the team's next item
-            if (pending >= 0) {                              // the previous item's stores have long landed
-                __syncwarp();
-                if (lane == 0) counter_add_release(d1 + pending, 1ull);
-            }
+            if (pending >= 0 && t == 0)                      // the team's stores of its previous item were all issued
+                counter_add_release(d1 + pending, 1ull);     // before this barrier and have long landed
             fft16<+1>(v);
 #if !(BEGE_ABL & 1)
-            if (it >= kRing)                                 // ring slot read out by pass 2 of item it - kRing
-                warp_counter_wait_ge(d2 + slot, 128ull * (it / kRing), abort_flag, lane);
+            if (it >= kRing) {                               // ring slot read out by pass 2 of item it - kRing
+                d2v = __shfl_sync(0xffffffffu, d2v, 0);
+                if (d2v < 128ull * (it / kRing)) warp_counter_wait_ge(d2 + slot, 128ull * (it / kRing), abort_flag, lane);
+            }
 #endif
             c2* out = myring + (uint64_t)slot * kN + 16 * b + c2i + p2 * 256;
 #pragma unroll
@@ -373,10 +375,8 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
             if (t == 0) sigpart[((j0 + grp + (uint64_t)G * tj) * (uint64_t)S + (m0 + ml)) * 16 + b] = tot;
             pending = slot;
         }
-        if (pending >= 0) {
-            __syncwarp();
-            if (lane == 0) counter_add_release(d1 + pending, 1ull);
-        }
+        bar_team(bar_id);
+        if (pending >= 0 && t == 0) counter_add_release(d1 + pending, 1ull);
     } else {
         // ================================================================ B: pass 2, items ib = team - 2 (mod 2)
         const int kb = team - 2;
@@ -394,7 +394,7 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
             const uint32_t ml = SINGLE ? 0u : (uint32_t)(ib - tj * nS);
             const uint64_t jl = grp + (uint64_t)G * tj;
 #if !(BEGE_ABL & 1)
-            warp_counter_wait_ge(d1 + slot, 128ull * (use + 1), abort_flag, lane);    // all 16 tiles are in the ring
+            warp_counter_wait_ge(d1 + slot, 16ull * (use + 1), abort_flag, lane);     // all 16 tiles are in the ring
 #endif
             const c2* src = myring + (uint64_t)slot * kN + row_off;
             c2 v[16];
