@@ -195,7 +195,7 @@ k_fwd_cols(const c2* __restrict__ G, c2* __restrict__ out, uint64_t out_stride, 
 //              c, lane g holds rows k2 = g + 16 i of column c: conj(H) X against the segment tile (shared
 //              memory), Parseval partial sum, 16-point DFTs, twiddles theta^p generated from one complex number
 //              per thread.  One exchange through shared memory (two named barriers of the team per item).
-//              Stage 2: lane c, p = warp-pair index: 16-point DFTs, second twiddle factor, and
+//              Stage 2: lane c, p = warp-pair index: 16-point DFTs, and
 //              T[n2 = p + 16 q][16 b + c] goes straight from registers to the ring in L2 (128 B per half-warp
 //              and store).  The tile is published (done1) with a release issued one item later.
 //   B teams (pass 2): half-warp r waits for all 16 tiles of an item (done1), loads its row of T from the ring,
@@ -203,8 +203,9 @@ k_fwd_cols(const c2* __restrict__ G, c2* __restrict__ out, uint64_t out_stride, 
 //              k^2 sum|R|^2, compacts the tails with warp-aggregated atomics, and releases its share of the
 //              ring slot (done2) as soon as the row is in registers.
 // The ring holds kRing items per group (G x kRing x 512 KiB) and lives in L2.  Four-step twiddle wN^(k1 n2) with
-// n2 = p + 16 q is split into wN^(k1 p), folded into theta = exp(2 pi i (256 g + k1) / N), and wN^(16 k1 q), a
-// 16 x 16 table in shared memory; theta and the tables are rounded once from fp64 angles.
+// n2 = p + 16 q is split into wN^(k1 p), folded into theta = exp(2 pi i (256 g + k1) / N) of pass 1, and
+// wN^(16 k1 q), applied by pass 2 to its inputs (q = n2 >> 4 is the CTA's tile index there: a 16 x 16 table in
+// shared memory); theta and the tables are rounded once from fp64 angles.
 constexpr int kRing = 8;
 constexpr int kSearchThreads = 32 * 32;
 constexpr int kPriv = 16 * 17;                              // padded private region of a half-warp (c2 elements)
@@ -215,7 +216,7 @@ template <int NI, bool XS> struct SearchSmem {
     c2 xs[XS ? NI * 256 : 2];                               // segment column tile (single-segment searches)
     c2 xch[2][kXch];                                        // pass 1 of each A team: stage 1 -> stage 2, [p][g][c]
     c2 bpriv[32][kPriv];                                    // pass 2: private exchange regions
-    float2 tbl[256];                                        // wN^(16 k1 q), [q][c]
+    float2 tbl[256];                                        // wN^(16 b k1), k1 = a + 16 r, [r][a] (pass 2)
     float2 w1t[256];                                        // w256^(a p), [p][a]
     float ssig[2][8];                                       // Parseval partial sums of the 8 warps of an A team
     uint64_t hfull[2];
@@ -247,10 +248,10 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
         mbar_init(&sm.hfull[0], 1); mbar_init(&sm.hfull[1], 1);
         fence_mbar_init();
     }
-    if (team == 0) {                                         // tbl[q][c] = exp(2 pi i 16 q (16 b + c) / N)
-        const int q = t >> 4, c = t & 15;
+    if (team == 0) {                                         // tbl[r][a] = exp(2 pi i 16 b (a + 16 r) / N)
+        const int r = t >> 4, a = t & 15;
         double sn, cs;
-        sincospi(2.0 * (double)((16 * q * (16 * b + c)) & (kN - 1)) / (double)kN, &sn, &cs);
+        sincospi(2.0 * (double)((16 * b * (a + 16 * r)) & (kN - 1)) / (double)kN, &sn, &cs);
         sm.tbl[t] = make_float2((float)cs, (float)sn);
     } else if (team == 1) {                                  // w1t[p][a] = exp(2 pi i a p / 256)
         const int p = t >> 4, a = t & 15;
@@ -263,8 +264,8 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
     }
     __syncthreads();
 
-    const uint64_t nTg = nT > (uint64_t)grp ? (nT - grp + G - 1) / G : 0;   // templates of this group
-    const uint64_t n_items = nTg * nS;
+    const uint32_t nTg = nT > (uint64_t)grp ? (uint32_t)((nT - grp + G - 1) / G) : 0u;   // templates of this group
+    const uint32_t n_items = nTg * nS;                      // < 2^31: the host splits larger searches
     c2* myring = ring + (uint64_t)grp * kRing * kN;
     unsigned long long* d1 = done1 + grp * kRing;            // one counter pair per ring slot: a count can only
     unsigned long long* d2 = done2 + grp * kRing;            // come from the item that currently owns the slot
@@ -284,9 +285,9 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
         const uint64_t pol = policy_evict_first();
         uint64_t* hfull = &sm.hfull[team];
         c2* hb = sm.hbuf[team];
-        if (t == 0 && (uint64_t)team < n_items && !(BEGE_ABL & 2)) {
+        if (t == 0 && (uint32_t)team < n_items && !(BEGE_ABL & 2)) {
             mbar_arrive_expect_tx(hfull, kTileBytes);
-            bulk_load(hb, bank + ((j0 + grp + (uint64_t)G * (SINGLE ? (uint64_t)team : team / nS)) * 16 + b) * kTile,
+            bulk_load(hb, bank + ((j0 + grp + (uint64_t)G * (SINGLE ? (uint32_t)team : team / nS)) * 16 + b) * kTile,
                       kTileBytes, hfull, pol);
         }
         c2* xw = sm.xch[team] + g * 17 + c;                  // + p * 272: element [p][g][c] of the exchange buffer
@@ -294,9 +295,9 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
         const int bar_id = 1 + team;
         int pending = -1;                                    // ring slot whose tile this warp has yet to publish
         uint32_t nload = 0;                                  // tiles this team has waited for so far
-        uint64_t tj_prev = ~0ull;
-        for (uint64_t it = team; it < n_items; it += 2) {
-            const uint64_t tj = SINGLE ? it : it / nS;
+        uint32_t tj_prev = ~0u;
+        for (uint32_t it = team; it < n_items; it += 2) {
+            const uint32_t tj = SINGLE ? it : it / nS;
             const uint32_t ml = SINGLE ? 0u : (uint32_t)(it - tj * nS);
             const int slot = (int)(it % kRing);
             if (tj != tj_prev) {                             // a new template tile was ordered for this item
@@ -340,9 +341,9 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
             if (lane == 0) sm.ssig[team][warp] = sw;
             bar_team(bar_id);                                // exchange buffer complete, template tile read out
             if (t == 0 && !(BEGE_ABL & 2)) {                 // order the tile of this team's next item
-                const uint64_t it2 = it + 2;
+                const uint32_t it2 = it + 2;
                 if (it2 < n_items) {
-                    const uint64_t tj2 = SINGLE ? it2 : it2 / nS;
+                    const uint32_t tj2 = SINGLE ? it2 : it2 / nS;
                     if (tj2 != tj) {
                         mbar_arrive_expect_tx(hfull, kTileBytes);
                         bulk_load(hb, bank + ((j0 + grp + (uint64_t)G * tj2) * 16 + b) * kTile, kTileBytes, hfull, pol);
@@ -369,7 +370,7 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
             c2* out = myring + (uint64_t)slot * kN + 16 * b + c2i + p2 * 256;
 #pragma unroll
             for (int q = 0; q < 16; ++q) {
-                const c2 o = cmul(v[q], sm.tbl[q * 16 + c2i]);
+                const c2 o = v[q];
                 if (!(BEGE_ABL & 4) || re(o) == 1.2345e-30f) out[q * 4096] = o;
             }
             if (t == 0) sigpart[((j0 + grp + (uint64_t)G * tj) * (uint64_t)S + (m0 + ml)) * 16 + b] = tot;
@@ -387,10 +388,10 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
         const c2* prd = priv + a;                            // + 17 aa:  stage-2 input from lane aa
         const float2* w1 = sm.w1t + a;                       // + 16 p:   exp(2 pi i a p / 256)
         const uint64_t row_off = (uint64_t)n2 * 256 + (uint64_t)a;           // T[n2][k1 = a + 16 r]
-        for (uint64_t ib = kb; ib < n_items; ib += 2) {
+        for (uint32_t ib = kb; ib < n_items; ib += 2) {
             const int slot = (int)(ib % kRing);
-            const uint64_t use = ib / kRing;
-            const uint64_t tj = SINGLE ? ib : ib / nS;
+            const uint32_t use = ib / kRing;
+            const uint32_t tj = SINGLE ? ib : ib / nS;
             const uint32_t ml = SINGLE ? 0u : (uint32_t)(ib - tj * nS);
             const uint64_t jl = grp + (uint64_t)G * tj;
 #if !(BEGE_ABL & 1)
@@ -400,6 +401,8 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
             c2 v[16];
 #pragma unroll
             for (int r = 0; r < 16; ++r) v[r] = (BEGE_ABL & 8) ? mk((float)(r + a), (float)ib) : __ldcg(src + 16 * r);
+#pragma unroll
+            for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], sm.tbl[16 * r + a]);          // wN^(16 k1 q), q = b
             const uint64_t pair = (j0 + jl) * (uint64_t)S + (m0 + ml);
             const float sumR2 = hw_sum16(__ldcg(sigpart + pair * 16 + a));
             fft16<+1>(v);
@@ -749,13 +752,15 @@ extern "C" int bege_segment_load(bege_plan* p, const float* x, uint32_t S)
 
 // one cooperative launch of the persistent search kernel over templates [j0, j0 + nT) x segments [m0, m0 + nS)
 static int launch_search(bege_plan* p, const c2* bank, const c2* xs, c2* ring, float* sig, float k2, bege_tail* rec,
-                         uint64_t cap, unsigned char* misc, c2* zdbg, uint64_t j0, uint64_t nT, uint32_t m0, uint32_t nS)
+                         uint64_t cap, unsigned char* misc, c2* zdbg, uint64_t j0, uint64_t nT, uint32_t m0, uint32_t nS,
+                         bool first = true)
 {
     unsigned long long* counter = (unsigned long long*)misc;
     int* abort_flag = (int*)(misc + 8);
     unsigned long long* done1 = (unsigned long long*)(misc + 256);
     unsigned long long* done2 = (unsigned long long*)(misc + 2048);
-    CU(p, cudaMemsetAsync(misc, 0, kMiscHdr, p->stream));
+    // the first launch of a search also clears the record counter and the abort flag (first 16 bytes)
+    CU(p, cudaMemsetAsync(misc + (first ? 0 : 16), 0, kMiscHdr - (first ? 0 : 16), p->stream));
     const int G = (int)std::min<uint64_t>((uint64_t)p->G, nT);
     const dim3 grid(16, G);
     const bool single = (p->S == 1);
@@ -803,8 +808,13 @@ extern "C" int bege_search(bege_plan* p, float k_sigma, bege_tail* tails_out, ui
     if ((rc = slot_get(p, p->s_bank, 0, &bank))) return rc;
     if ((rc = slot_get(p, p->s_x, 0, &xs))) return rc;
     unsigned long long* counter = (unsigned long long*)misc;
-    if ((rc = launch_search(p, (const c2*)bank, (const c2*)xs, (c2*)scr, (float*)sig, k_sigma * k_sigma,
-                            (bege_tail*)rec, cap, (unsigned char*)misc, nullptr, 0, p->T, 0, p->S))) return rc;
+    // the kernel counts a group's (template, segment) items in 32 bits: split longer searches
+    const uint64_t maxT = std::max<uint64_t>(1, ((1ull << 31) - 1) / p->S / 2) * (uint64_t)p->G;
+    for (uint64_t jj = 0; jj < p->T; jj += maxT) {
+        if ((rc = launch_search(p, (const c2*)bank, (const c2*)xs, (c2*)scr, (float*)sig, k_sigma * k_sigma,
+                                (bege_tail*)rec, cap, (unsigned char*)misc, nullptr, jj, std::min(maxT, p->T - jj), 0, p->S,
+                                jj == 0))) return rc;
+    }
     CU(p, cudaGetLastError());
     // only the tails cross PCIe: count first, then exactly the records, on the side stream
     CU(p, cudaMemcpyAsync(p->h_count, counter, sizeof(unsigned long long), cudaMemcpyDeviceToHost, p->stream));
