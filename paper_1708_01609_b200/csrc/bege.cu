@@ -27,6 +27,7 @@
 #include "../../include/bege.h"
 #include "cplx.cuh"
 #include "async.cuh"
+#include "bank64.cuh"
 
 #ifndef BEGE_ABL
 #define BEGE_ABL 0          // ablation switches for timing experiments (never set in the product build)
@@ -75,51 +76,7 @@ BEGE_D void load_w1(float2 (&w1)[16], const float2* __restrict__ tw256, int lane
 }
 
 // ------------------------------------------------------------------------------------------------
-// a1, step A: chirp synthesis (fp64 phase) + pruned row DFTs.  grid (16, n_templates_in_batch), 256 thr.
-// CTA (ia, jl): the 16 rows nl = ga + 16 ia (ga = half-warp index); only nh < 16 inputs are non-zero
-// (L <= 4096), so X[k1 = p + 16 q] = sum_nh h[nl + 256 nh] w256^(-nh p) w16^(-nh q): lane p twiddles the
-// 16 samples and runs one 16-point DFT.  Output -> G tile layout, times wN^(-nl k1).
-__global__ void __launch_bounds__(256)
-k_fwd_rows_chirp(const double* __restrict__ f0, const double* __restrict__ fdot, uint64_t j0,
-                 double fs, uint32_t L, double inv_norm,
-                 const float2* __restrict__ tw256, const float2* __restrict__ twN, c2* __restrict__ G)
-{
-    __shared__ c2 samp[16][16];          // [nh][ga]
-    const int t = threadIdx.x, ia = blockIdx.x;
-    const uint64_t jl = blockIdx.y;
-    {
-        const int ga = t & 15, nh = t >> 4;
-        const uint32_t n = ga + 16 * ia + 256 * nh;
-        c2 s = mk(0.f, 0.f);
-        if (n < L) {
-            const double tt = (double)n / fs;
-            const double cyc = f0[j0 + jl] * tt + 0.5 * fdot[j0 + jl] * tt * tt;
-            const double fr = cyc - floor(cyc);
-            double sn, cs;
-            sincospi(2.0 * fr, &sn, &cs);
-            const double w = (0.5 - 0.5 * cospi(2.0 * (double)n / (double)(L - 1))) * inv_norm;
-            s = mk((float)(w * cs), (float)(w * sn));
-        }
-        samp[nh][ga] = s;
-    }
-    __syncthreads();
-    const int ga = t >> 4, p = t & 15;
-    const int nl = ga + 16 * ia;
-    c2 v[16];
-#pragma unroll
-    for (int nh = 0; nh < 16; ++nh) {
-        const float2 w = __ldg(tw256 + p * 16 + nh);           // exp(+2 pi i nh p / 256)
-        v[nh] = cmul(samp[nh][ga], w.x, -w.y);
-    }
-    fft16<-1>(v);
-    c2* out = G + jl * (uint64_t)kN;
-#pragma unroll
-    for (int q = 0; q < 16; ++q) {
-        const int k1 = p + 16 * q;
-        const float2 w = __ldg(twN + nl * 256 + k1);           // exp(+2 pi i nl k1 / N)
-        out[((q * 16 + ia) * 16 + p) * 16 + ga] = cmul(v[q], w.x, -w.y);
-    }
-}
+// a1 (template spectra) lives in bank64.cuh: fp64 arithmetic, one fp32 rounding per stored bin.
 
 // a2, step A: full row DFTs of a data segment.  grid (16, n_segments), 256 thr.
 __global__ void __launch_bounds__(256)
@@ -502,6 +459,7 @@ struct bege_plan {
     int I0 = 0, NI = 16;
     int G = 0;                      // search groups (16 CTAs each), all co-resident
     float2 *tw256 = nullptr, *twN = nullptr;
+    d2 *tw256d = nullptr, *twNd = nullptr;   // exp(2 pi i m / 256), exp(2 pi i m / N) in fp64 (bank generation)
     // workspace
     unsigned char* ws = nullptr; uint64_t ws_bytes = 0, bump = 0; bool user_ws = false;
     Slot s_bank, s_x, s_scratch, s_sig, s_rec, s_misc, s_par;
@@ -612,6 +570,15 @@ extern "C" int bege_plan_create(bege_plan** out, uint32_t N, double fs, double l
             const double a = 2.0 * M_PI * (double)(n2 * k1) / (double)N;
             wN[(size_t)n2 * 256 + k1] = make_float2((float)cos(a), (float)sin(a));
         }
+    {
+        std::vector<d2> t256(256), tN(N);
+        for (int m = 0; m < 256; ++m) { t256[m].x = cos(2.0 * M_PI * m / 256.0); t256[m].y = sin(2.0 * M_PI * m / 256.0); }
+        for (uint32_t m = 0; m < N; ++m) { tN[m].x = cos(2.0 * M_PI * m / (double)N); tN[m].y = sin(2.0 * M_PI * m / (double)N); }
+        if (cudaMalloc(&p->tw256d, 256 * sizeof(d2)) != cudaSuccess || cudaMalloc(&p->twNd, N * sizeof(d2)) != cudaSuccess) return bail(BEGE_ENOMEM);
+        if (cudaMemcpy(p->tw256d, t256.data(), 256 * sizeof(d2), cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(p->twNd, tN.data(), N * sizeof(d2), cudaMemcpyHostToDevice) != cudaSuccess) return bail(BEGE_ECUDA);
+        if (cudaFuncSetAttribute(k_bank_cols64, cudaFuncAttributeMaxDynamicSharedMemorySize, 16 * 256 * (int)sizeof(d2)) != cudaSuccess) return bail(BEGE_ECUDA);
+    }
     if (cudaMalloc(&p->tw256, w256.size() * sizeof(float2)) != cudaSuccess ||
         cudaMalloc(&p->twN, wN.size() * sizeof(float2)) != cudaSuccess) return bail(BEGE_ENOMEM);
     if (cudaMemcpy(p->tw256, w256.data(), w256.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess ||
@@ -649,6 +616,8 @@ extern "C" void bege_plan_destroy(bege_plan* p)
     for (Slot* s : {&p->s_bank, &p->s_x, &p->s_scratch, &p->s_sig, &p->s_rec, &p->s_misc, &p->s_par}) slot_free(*s);
     if (p->tw256) cudaFree(p->tw256);
     if (p->twN) cudaFree(p->twN);
+    if (p->tw256d) cudaFree(p->tw256d);
+    if (p->twNd) cudaFree(p->twNd);
     if (p->h_count) cudaFreeHost(p->h_count);
     if (p->ev_a) cudaEventDestroy(p->ev_a);
     if (p->ev_b) cudaEventDestroy(p->ev_b);
@@ -710,8 +679,9 @@ extern "C" int bege_bank_generate(bege_plan* p, const double* f0, const double* 
     const uint64_t stride = tpl_bytes(p) / sizeof(c2);
     for (uint64_t j0 = 0; j0 < T; j0 += kBatch) {
         const unsigned nb = (unsigned)std::min<uint64_t>(kBatch, T - j0);
-        k_fwd_rows_chirp<<<dim3(16, nb), 256, 0, p->stream>>>(d_f0, d_fd, j0, p->fs, L, inv_norm, p->tw256, p->twN, (c2*)scr);
-        k_fwd_cols<false><<<dim3(16, nb), 256, 0, p->stream>>>((const c2*)scr, (c2*)bank + j0 * stride, stride, p->I0, p->NI, p->tw256, 0, 0);
+        k_bank_rows64<<<dim3(16, nb), 256, 0, p->stream>>>(d_f0, d_fd, j0, p->fs, L, inv_norm, p->tw256d, p->twNd, (d2*)scr);
+        k_bank_cols64<<<dim3(16, nb), 256, 16 * 256 * sizeof(d2), p->stream>>>((const d2*)scr, (float2*)bank + j0 * stride, stride,
+                                                                            p->I0, p->NI, p->tw256d);
         count_launch(p, 2);
     }
     CU(p, cudaGetLastError());

@@ -286,3 +286,54 @@ def test_user_workspace_and_device_input(bo, bege):
         with pytest.raises(bege.BegeError) as ei:
             plan.bank_generate(w.f0, w.fdot, TAU)                   # does not fit the lent workspace
         assert ei.value.status == bege.ENOMEM
+
+
+# ----------------------------------------------------------------------------- cfg4: glitches, tail heavy
+def test_glitch_segment_tail_heavy_subbank(bo, bege):
+    """configs[4] data (40 Q=9 sine-Gaussians) at k = 3 on a strided sub-bank: tens of thousands of records
+    per launch through the warp-aggregated compaction, many per warp and per row."""
+    w = synth.config4()
+    ids = np.arange(0, w.n_templates, 2731)[:96]           # 96 templates strided over the 512 x 512 grid
+    sub = synth.subsample(w, ids)
+    X = bo.segment_spectrum(w.x[0], FS, *BAND)
+    lo_tails, _, sigma_o, _ = bo.search(X[None, :], sub.f0, sub.fdot, TAU, FS, 3.0 - 1e-3)
+    with bege.Plan(N, FS, BAND) as plan:
+        plan.bank_generate(sub.f0, sub.fdot, TAU)
+        plan.segment_load(w.x)
+        tails, n = plan.search(3.0, cap=1 << 21)
+        must, _ = check_tail_sets(tails, n, lo_tails, 3.0)
+        assert must > 5000
+        sg = plan.get_sigma()[:, 0]
+        assert np.max(np.abs(sg - sigma_o[:, 0]) / sigma_o[:, 0]) <= SIGMA_RTOL
+
+
+# ----------------------------------------------------------------------------- bench-scale launch, sampled outputs
+def test_bench_scale_launch_sampled_against_oracle(bo, bege):
+    """The launch configuration bench.py times (one persistent launch over tens of thousands of templates of the
+    configs[2] bank, all groups and ring slots cycling thousands of times), checked on sampled templates: their
+    tails and sigma against the oracle, and properties that hold for every record."""
+    f0, fd = synth.config2_bank()
+    T = 36864
+    j_lo = 500_000                                          # a slice from the middle of the 2^20 bank
+    x = synth.noise_segment(2)[None, :]
+    k = 3.5                                                 # e^-12.25 per output: thousands of tails in this slice
+    X = bo.segment_spectrum(x[0], FS, *BAND)
+    with bege.Plan(N, FS, BAND) as plan:
+        plan.bank_generate(f0[j_lo:j_lo + T], fd[j_lo:j_lo + T], TAU)
+        plan.segment_load(x)
+        tails, n = plan.search(k, cap=1 << 21)
+        sg = plan.get_sigma()[:, 0]
+        tails2, n2 = plan.search(k, cap=1 << 21)
+    assert n == tails.size and n > 20
+    key = lambda tt: np.sort(tt["template_id"].astype(np.uint64) << np.uint64(32) | tt["lag"].astype(np.uint64))
+    assert n2 == n and np.array_equal(key(tails), key(tails2))                # deterministic set
+    assert tails["template_id"].max() < T and tails["lag"].max() < N
+    assert np.all(tails["snr"] > k) and np.all(np.isfinite(sg)) and np.all(sg > 0)
+    # sampled templates: every template that fired (up to 24) plus 24 strided ones that mostly did not
+    fired = np.unique(tails["template_id"])[:24]
+    sample = np.unique(np.concatenate([fired, np.arange(7, T, T // 24)]))
+    lo_tails, _, sigma_o, _ = bo.search(X[None, :], f0[j_lo + sample], fd[j_lo + sample], TAU, FS, k - 1e-3)
+    sel = tails[np.isin(tails["template_id"], sample)].copy()
+    sel["template_id"] = np.searchsorted(sample, sel["template_id"]).astype(np.uint32)
+    check_tail_sets(sel, sel.size, lo_tails, k)
+    assert np.max(np.abs(sg[sample] - sigma_o[:, 0]) / sigma_o[:, 0]) <= SIGMA_RTOL
