@@ -36,6 +36,9 @@ METRIC = "template correlations/sec at N=2^16 C2C fp32"
 UNIT = "correlations/s"
 FFT_FLOP = 5.0 * 65536 * 16                       # PAPER.md:134 eq.(10): 5 N log2 N
 ALG_BYTES_PER_CORR = 52802 * 8                    # two-sided in-band template spectrum, S = 1
+# dram__bytes_read.sum + dram__bytes_write.sum of k_search per correlation, from the ncu --set full capture summarised
+# in profiles/r1e_search_kernel.md (36,864-template launch: 16.914 GB read + 1.546 GB written)
+NCU_DRAM_BYTES_PER_CORR = (16.913704e9 + 1.546495e9) / 36864
 FP32_PEAK = 148 * 128 * 2 * 1.965e9               # SMs x fp32 lanes x 2 flop x max SM clock
 
 
@@ -173,6 +176,7 @@ def run_ours(args, rank, world, local_rank):
         for ci, (a, b) in enumerate(chunks):
             plan.bank_generate(f0[a:b], fdot[a:b], synth.TAU)              # untimed (configs[2])
             barrier()
+            l0 = plan.stats()["kernel_launches"]
             t0 = time.perf_counter()
             plan.segment_load(x_host)                                        # H2D of the segment + forward FFT
             t1 = time.perf_counter()
@@ -188,10 +192,11 @@ def run_ours(args, rank, world, local_rank):
                 acc["e2e_s"] += t2 - t0
                 acc["d2h"] += 8 + 12 * min(n, cap)
                 acc["h2d"] += x_host.numel() * 8
+                acc["launches"] += plan.stats()["kernel_launches"] - l0
         return n_tails
 
     sampler.start()
-    acc = {"search_ms": 0.0, "e2e_s": 0.0, "d2h": 0, "h2d": 0}
+    acc = {"search_ms": 0.0, "e2e_s": 0.0, "d2h": 0, "h2d": 0, "launches": 0}
     windows = []
     for _ in range(args.warmup):
         one_step(False, windows, acc)
@@ -252,13 +257,15 @@ def run_ours(args, rank, world, local_rank):
         "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": acc["h2d"] // args.steps,
                 "d2h_bytes_per_step": acc["d2h"] // args.steps,
                 "what": "per chunk: bege_segment_load from pinned host memory + bege_search into pinned host memory"},
-        "gpu_launches": int(st["kernel_launches"]),
+        "gpu_launches": int(acc["launches"]),
+        "gpu_launches_note": "kernels of libbege.so launched inside the timed calls (per chunk: 2 segment-load kernels + 1 persistent search kernel); the untimed bank generation launched %d more" % (int(st["kernel_launches"]) - int(acc["launches"])),
         "clocks": sampler.summary(windows),
         "gflops_equiv": value * FFT_FLOP * 1e-9,
         "roofline": {"bound": "alu", "achieved": alu_achieved, "peak": FP32_PEAK * 1e-12, "unit": "TFLOP/s",
-                     "frac": alu_achieved / (FP32_PEAK * 1e-12), "traffic": None,
-                     "kernel": "k_inv_cols + k_inv_rows (one search batch pair), CUDA events, "
-                               f"{pst['fused_kernel_launches']} launches over {kern_corr} correlations",
+                     "frac": alu_achieved / (FP32_PEAK * 1e-12), "traffic": NCU_DRAM_BYTES_PER_CORR * kern_corr,
+                     "traffic_note": "bytes per launch = ncu dram bytes per correlation (profiles/r1e_search_kernel.md) x correlations of the timed launch",
+                     "kernel": "k_search (persistent warp-specialised search kernel, one launch per bank chunk), CUDA events on the plan's stream, "
+                               f"{pst['fused_kernel_launches']} launch over {kern_corr} correlations",
                      "peak_source": "derived: 148 SM x 128 fp32 lanes x 2 x 1.965 GHz (DESIGN.md); "
                                     "flops = 5 N log2 N per correlation (PAPER.md:134)",
                      "hbm": {"achieved": hbm_achieved, "peak": hbm_peak, "unit": "GB/s",
@@ -279,8 +286,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--templates", type=int, default=1 << 20, help="templates per GPU (default: configs[2])")
     ap.add_argument("--chunk", type=int, default=0, help="bank chunk size (default: what fits HBM)")
-    ap.add_argument("--cpu-sample", type=int, default=2048)
-    ap.add_argument("--ref-sample", type=int, default=2048)
+    ap.add_argument("--cpu-sample", type=int, default=24576)
+    ap.add_argument("--ref-sample", type=int, default=8192)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
