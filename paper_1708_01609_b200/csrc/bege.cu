@@ -239,13 +239,12 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
             sincospi(2.0 * (double)(256 * g + 16 * b + c) / (double)kN, &sn, &cs);
             theta = mk((float)cs, (float)sn);
         }
-        const uint64_t pol = policy_evict_first();
         uint64_t* hfull = &sm.hfull[team];
         c2* hb = sm.hbuf[team];
         if (t == 0 && (uint32_t)team < n_items && !(BEGE_ABL & 2)) {
             mbar_arrive_expect_tx(hfull, kTileBytes);
             bulk_load(hb, bank + ((j0 + grp + (uint64_t)G * (SINGLE ? (uint32_t)team : team / nS)) * 16 + b) * kTile,
-                      kTileBytes, hfull, pol);
+                      kTileBytes, hfull, policy_evict_first());
         }
         c2* xw = sm.xch[team] + g * 17 + c;                  // + p * 272: element [p][g][c] of the exchange buffer
         const c2* xrd = sm.xch[team] + p2 * 272 + c2i;       // + gg * 17
@@ -264,8 +263,6 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
                 ++nload;
                 tj_prev = tj;
             }
-            unsigned long long d2v = ~0ull;                  // slot-free counter, polled early: the load is in flight
-            if (it >= kRing && lane == 0 && !(BEGE_ABL & 1)) d2v = counter_load_relaxed(d2 + slot);   // during stage 1
             c2 v[16];
             c2 acc = mk(0.f, 0.f);
             {
@@ -303,10 +300,13 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
                     const uint32_t tj2 = SINGLE ? it2 : it2 / nS;
                     if (tj2 != tj) {
                         mbar_arrive_expect_tx(hfull, kTileBytes);
-                        bulk_load(hb, bank + ((j0 + grp + (uint64_t)G * tj2) * 16 + b) * kTile, kTileBytes, hfull, pol);
+                        bulk_load(hb, bank + ((j0 + grp + (uint64_t)G * tj2) * 16 + b) * kTile, kTileBytes, hfull,
+                                  policy_evict_first());
                     }
                 }
             }
+            unsigned long long d2v = ~0ull;                  // slot-free counter, polled early: the load is in flight
+            if (it >= kRing && lane == 0 && !(BEGE_ABL & 1)) d2v = counter_load_relaxed(d2 + slot);   // during stage 2
 #pragma unroll
             for (int gg = 0; gg < 16; ++gg) v[gg] = xrd[gg * 17];
             float tot = 0.f;
