@@ -469,6 +469,7 @@ struct bege_plan {
     unsigned long long* h_count = nullptr;
     cudaEvent_t ev_a = nullptr, ev_b = nullptr, ev_done = nullptr;
     bool profiling = false;
+    void* l2_window = nullptr;      // ring region currently marked persisting in L2 (access policy window of the stream)
     bege_stats stats{};
     std::string err;
 };
@@ -733,6 +734,21 @@ static int launch_search(bege_plan* p, const c2* bank, const c2* xs, c2* ring, f
     CU(p, cudaMemsetAsync(misc + (first ? 0 : 16), 0, kMiscHdr - (first ? 0 : 16), p->stream));
     const int G = (int)std::min<uint64_t>((uint64_t)p->G, nT);
     const dim3 grid(16, G);
+    if (p->l2_window != (void*)ring) {
+        // keep the ring's lines resident: they are rewritten every few microseconds and must not be written back
+        // to HBM in between (ncu: 31 KB of write-back per correlation without this); best effort, errors ignored
+        const size_t bytes = (size_t)p->G * kRing * kN * sizeof(c2);
+        cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, bytes);
+        cudaStreamAttrValue av{};
+        av.accessPolicyWindow.base_ptr = (void*)ring;
+        av.accessPolicyWindow.num_bytes = bytes;
+        av.accessPolicyWindow.hitRatio = 1.0f;
+        av.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
+        av.accessPolicyWindow.missProp = cudaAccessPropertyStreaming;
+        cudaStreamSetAttribute(p->stream, cudaStreamAttributeAccessPolicyWindow, &av);
+        cudaGetLastError();
+        p->l2_window = (void*)ring;
+    }
     const bool single = (p->S == 1);
     unsigned long long capll = cap;
     uint32_t S = p->S;
