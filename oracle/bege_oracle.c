@@ -279,6 +279,43 @@ uint64_t bo_search(const double* Xs, uint32_t S, const double* f0, const double*
     return bad ? UINT64_MAX : count;
 }
 
+
+/* ------------------------------------------------------- max projection -- */
+/*
+ * The paper's default output, eq.(13)-(17) and Fig.4: per sample offset m*N + n keep only the
+ * largest rho over all templates, with the template it came from ("In collecting B, we select data with maximal
+ * rho values at t_{n+mN}"), provided it is a tail (eq.14, read with kappa as in eq.15; DESIGN.md
+ * reading 6).  snr_out[m*N+n] = max_j |z_jm[n]|/sigma_jm over the templates with |z| > k sigma (0 if none),
+ * id_out[m*N+n] = that template (UINT32_MAX if none); equal values go to the smaller template id, which makes the
+ * result unique where the paper's racy update is not.  Plain serial loops, no threads.
+ */
+int bo_search_maxproj(const double* Xs, uint32_t S, const double* f0, const double* fdot, uint64_t T,
+                      double tau, double fs, uint32_t N, double k_sigma, double* snr_out, uint32_t* id_out)
+{
+    double* Hs = (double*)malloc(sizeof(double) * 2 * (size_t)N);
+    double* z  = (double*)malloc(sizeof(double) * 2 * (size_t)N);
+    if (!Hs || !z) { free(Hs); free(z); return 2; }
+    for (size_t i = 0; i < (size_t)S * N; ++i) { snr_out[i] = 0.0; id_out[i] = UINT32_MAX; }
+    for (uint64_t j = 0; j < T; ++j) {
+        if (bo_template(f0[j], fdot[j], tau, fs, N, Hs) || bo_fft(Hs, N, -1)) { free(Hs); free(z); return 1; }
+        for (uint32_t m = 0; m < S; ++m) {
+            double sigma = 0.0;
+            bo_correlate_spectra(Xs + 2 * (size_t)m * N, Hs, N, z, &sigma);
+            if (!(sigma > 0.0)) continue;
+            for (uint32_t n = 0; n < N; ++n) {
+                double a = hypot(z[2 * n], z[2 * n + 1]);
+                if (a > k_sigma * sigma) {
+                    double r = a / sigma;
+                    size_t i = (size_t)m * N + n;
+                    if (r > snr_out[i]) { snr_out[i] = r; id_out[i] = (uint32_t)j; }   /* j ascending: ties keep the smaller id */
+                }
+            }
+        }
+    }
+    free(Hs); free(z);
+    return 0;
+}
+
 /* PAPER.md:134 eq.(10), :160: nominal flops of one FFT_N. */
 double bo_fft_flops(uint32_t N)
 {

@@ -64,6 +64,8 @@ def lib():
                                 ctypes.POINTER(_Tail), u64, dp, ctypes.c_int,
                                 ctypes.POINTER(ctypes.c_int)]
         L.bo_search.restype = u64
+        L.bo_search_maxproj.argtypes = [dp, u32, dp, dp, u64, dbl, dbl, u32, dbl, dp, ctypes.POINTER(u32)]
+        L.bo_search_maxproj.restype = ctypes.c_int
         L.bo_fft_flops.argtypes = [u32]
         L.bo_fft_flops.restype = dbl
         _lib = L
@@ -161,6 +163,21 @@ def search(Xs, f0, fdot, tau: float, fs: float, k_sigma: float, cap: int = 1 << 
     tails = tails[: min(n, cap)]
     tails = tails[np.lexsort((tails["lag"], tails["template_id"]))]
     return tails, int(n), sigma, used.value
+
+
+def search_maxproj(Xs, f0, fdot, tau: float, fs: float, k_sigma: float):
+    """Max projection over the bank (bo_search_maxproj): (snr[S, N] fp64, template_id[S, N] uint32)."""
+    Xs = np.atleast_2d(_c128(Xs))
+    S, N = Xs.shape
+    f0 = np.ascontiguousarray(np.asarray(f0, dtype=np.float64))
+    fdot = np.ascontiguousarray(np.asarray(fdot, dtype=np.float64))
+    snr = np.zeros((S, N), dtype=np.float64)
+    ids = np.zeros((S, N), dtype=np.uint32)
+    rc = lib().bo_search_maxproj(_dp(Xs.view(np.float64)), S, _dp(f0), _dp(fdot), f0.size, float(tau), float(fs), N,
+                                 float(k_sigma), _dp(snr), ids.ctypes.data_as(ctypes.POINTER(ctypes.c_uint32)))
+    if rc:
+        raise RuntimeError(f"bo_search_maxproj rc={rc}")
+    return snr, ids
 
 
 def fft_flops(N: int) -> float:

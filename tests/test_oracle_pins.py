@@ -339,3 +339,34 @@ def test_paper_printed_numbers():
     close("block_bytes", 2048 * N * 8)
     close("file_bytes", 8 * 2048 * N * 8)
     close("segment_bytes", N * 8)
+
+
+# ----------------------------------------------------------------------------- max projection
+def test_max_projection_is_the_per_lag_maximum_of_the_extended_output():
+    """eq.(15)-(17): B keeps, per sample offset m*N+n, the largest rho over the bank and its template.  Pinned by
+    brute force against the (separately pinned) extended output of bo_search on two segments and 40 templates,
+    with a planted tie to check that equal values go to the smaller template id."""
+    w = synth.config0()
+    x2, _ = synth.inject_chirp(synth.band_limit(synth.white_noise(9)), 1000.0, 50.0, 5.0, 9.0)
+    xs = np.stack([w.x[0], synth.as_segment(x2)])
+    Xs = np.stack([bo.segment_spectrum(x, FS, *BAND) for x in xs])
+    f0 = np.concatenate([w.f0[::8], [1000.0, 1000.0], w.f0[3:8]])       # templates 32 and 33 are identical
+    fd = np.concatenate([w.fdot[::8], [50.0, 50.0], w.fdot[3:8]])
+    k = 2.8
+    tails, n, _, _ = bo.search(Xs, f0, fd, TAU, FS, k)
+    snr, ids = bo.search_maxproj(Xs, f0, fd, TAU, FS, k)
+    assert snr.shape == (2, N) and ids.shape == (2, N)
+    want_snr = np.zeros(2 * N)
+    want_id = np.full(2 * N, np.iinfo(np.uint32).max, dtype=np.uint32)
+    for rec in tails:                                                   # tails are sorted by (template_id, lag)
+        if rec["snr"] > want_snr[rec["lag"]]:
+            want_snr[rec["lag"]] = rec["snr"]
+            want_id[rec["lag"]] = rec["template_id"]
+    assert np.array_equal(snr.ravel(), want_snr)
+    assert np.array_equal(ids.ravel(), want_id)
+    assert (snr > 0).sum() < n                                          # several templates share lags
+    assert np.all((snr == 0) == (ids == np.iinfo(np.uint32).max))
+    # the planted duplicate never wins, the first copy does at the injection
+    assert not np.any(ids == 33)
+    peak = np.unravel_index(np.argmax(snr), snr.shape)
+    assert peak[0] == 1 and ids[peak] == 32
