@@ -109,6 +109,18 @@ int bege_segment_load(bege_plan*, const float* x_interleaved_c64, uint32_t n_seg
  */
 int bege_search(bege_plan*, float k_sigma, bege_tail* tails_out, uint64_t cap, uint64_t* n_tails);
 
+/*
+ * NEXT row of the scope table -- the paper's default output mode (eq.13-17, Fig.4): the tails of
+ * the whole bank projected onto the sample offsets.  For every offset i = m*N + n of the loaded segments:
+ * snr_out[i] = max over the templates j with |z_jm[n]| > k_sigma*sigma_jm of |z_jm[n]|/sigma_jm (0 if none) and
+ * id_out[i] = the template that attains it (UINT32_MAX if none); equal values go to the smaller template id, so the
+ * result is unique (the paper accepts a data race here; this implementation has none: one 64-bit
+ * atomicMax per tail).  A fixed n_segments*N*8 bytes cross PCIe instead of a variable record list.
+ * snr_out, id_out: host arrays of n_segments*N entries.  *n_hits (may be NULL): offsets that hold a tail.
+ * Same kernels, sigma and threshold as bege_search; bege_get_sigma is valid afterwards.  Synchronous at return.
+ */
+int bege_search_maxproj(bege_plan*, float k_sigma, float* snr_out, uint32_t* id_out, uint64_t* n_hits);
+
 /* sigma_jm of the last bege_search, host array of n_templates*n_segments floats, template-major. */
 int bege_get_sigma(bege_plan*, float* sigma_out);
 

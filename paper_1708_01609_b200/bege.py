@@ -23,7 +23,7 @@ _STATUS = {0: "BEGE_OK", 1: "BEGE_EINVAL", 2: "BEGE_ESTATE", 3: "BEGE_ENOMEM", 4
 # every symbol include/bege.h declares (tests check that the library exports all of them)
 SYMBOLS = [
     "bege_plan_create", "bege_plan_workspace_bytes", "bege_plan_set_workspace", "bege_bank_generate",
-    "bege_segment_load", "bege_search", "bege_get_sigma", "bege_debug_correlate",
+    "bege_segment_load", "bege_search", "bege_search_maxproj", "bege_get_sigma", "bege_debug_correlate",
     "bege_debug_template_spectrum", "bege_debug_segment_spectrum", "bege_plan_set_profiling",
     "bege_plan_get_stats", "bege_plan_reset_stats", "bege_last_error", "bege_plan_destroy", "bege_version",
 ]
@@ -60,6 +60,7 @@ def load_library() -> ctypes.CDLL:
     L.bege_bank_generate.argtypes = [vp, vp, vp, u64, dbl]
     L.bege_segment_load.argtypes = [vp, vp, u32]
     L.bege_search.argtypes = [vp, ctypes.c_float, vp, u64, ctypes.POINTER(u64)]
+    L.bege_search_maxproj.argtypes = [vp, ctypes.c_float, vp, vp, ctypes.POINTER(u64)]
     L.bege_get_sigma.argtypes = [vp, vp]
     L.bege_debug_correlate.argtypes = [vp, u64, u32, vp, ctypes.POINTER(ctypes.c_float)]
     L.bege_debug_template_spectrum.argtypes = [vp, u64, vp]
@@ -193,6 +194,15 @@ class Plan:
         got = min(n.value, cap)
         view = buf.numpy()[: got * 12].view(TAIL_DTYPE)
         return (view.copy() if copy else view), int(n.value)
+
+    def search_maxproj(self, k_sigma: float):
+        """Max projection over the bank: (snr[S, N] float32, template_id[S, N] uint32, n_hits)."""
+        snr = np.empty((self.n_segments, self.N), dtype=np.float32)
+        ids = np.empty((self.n_segments, self.N), dtype=np.uint32)
+        n = ctypes.c_uint64()
+        self._check(self._L.bege_search_maxproj(self._h, ctypes.c_float(k_sigma), snr.ctypes.data, ids.ctypes.data,
+                                                ctypes.byref(n)))
+        return snr, ids, int(n.value)
 
     def get_sigma(self) -> np.ndarray:
         out = np.empty((self.n_templates, self.n_segments), dtype=np.float32)

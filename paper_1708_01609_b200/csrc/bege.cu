@@ -393,31 +393,48 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
             if (thr == -1.f)                                 // timing experiment only: never emit
 #endif
             if (__any_sync(0xffffffffu, hits != 0)) {
-                const int cnt = __popc(hits);
-                int incl = cnt;
-#pragma unroll
-                for (int d = 1; d < 32; d <<= 1) {
-                    const int o = __shfl_up_sync(0xffffffffu, incl, d);
-                    if (lane >= d) incl += o;
-                }
-                const int total = __shfl_sync(0xffffffffu, incl, 31);
-                unsigned long long base = 0;
-                if (lane == 31) base = atomicAdd(counter, (unsigned long long)total);
-                base = __shfl_sync(0xffffffffu, base, 31);
-                unsigned long long slot_r = base + (unsigned long long)(incl - cnt);
                 const float inv = 1.0f / sumR2;
+                if (cap == ~0ull) {
+                    // max projection: per sample offset the largest |z|/sigma over the bank and
+                    // its template, race free: one 64-bit atomicMax on (snr bits, ~template_id); positive floats
+                    // order like their bit patterns, equal values go to the smaller template id
+                    unsigned long long* proj = reinterpret_cast<unsigned long long*>(rec);
 #pragma unroll
-                for (int q = 0; q < 16; ++q) {
-                    if (hits & (1u << q)) {
-                        if (slot_r < cap) {
+                    for (int q = 0; q < 16; ++q) {
+                        if (hits & (1u << q)) {
                             const c2 sq = mul2(v[q], v[q]);
-                            bege_tail r;
-                            r.template_id = (uint32_t)(j0 + jl);
-                            r.lag = (uint32_t)(m0 + ml) * (uint32_t)kN + (uint32_t)((a + 16 * q) * 256 + n2);
-                            r.snr = sqrtf((re(sq) + im(sq)) * inv);
-                            rec[slot_r] = r;
+                            const float snr = sqrtf((re(sq) + im(sq)) * inv);
+                            const uint32_t lag = (uint32_t)(m0 + ml) * (uint32_t)kN + (uint32_t)((a + 16 * q) * 256 + n2);
+                            atomicMax(proj + lag, ((unsigned long long)__float_as_uint(snr) << 32) |
+                                                      (unsigned long long)(0xffffffffu - (uint32_t)(j0 + jl)));
                         }
-                        ++slot_r;
+                    }
+                } else {
+                    const int cnt = __popc(hits);
+                    int incl = cnt;
+#pragma unroll
+                    for (int d = 1; d < 32; d <<= 1) {
+                        const int o = __shfl_up_sync(0xffffffffu, incl, d);
+                        if (lane >= d) incl += o;
+                    }
+                    const int total = __shfl_sync(0xffffffffu, incl, 31);
+                    unsigned long long base = 0;
+                    if (lane == 31) base = atomicAdd(counter, (unsigned long long)total);
+                    base = __shfl_sync(0xffffffffu, base, 31);
+                    unsigned long long slot_r = base + (unsigned long long)(incl - cnt);
+#pragma unroll
+                    for (int q = 0; q < 16; ++q) {
+                        if (hits & (1u << q)) {
+                            if (slot_r < cap) {
+                                const c2 sq = mul2(v[q], v[q]);
+                                bege_tail r;
+                                r.template_id = (uint32_t)(j0 + jl);
+                                r.lag = (uint32_t)(m0 + ml) * (uint32_t)kN + (uint32_t)((a + 16 * q) * 256 + n2);
+                                r.snr = sqrtf((re(sq) + im(sq)) * inv);
+                                rec[slot_r] = r;
+                            }
+                            ++slot_r;
+                        }
                     }
                 }
             }
@@ -462,7 +479,7 @@ struct bege_plan {
     d2 *tw256d = nullptr, *twNd = nullptr;   // exp(2 pi i m / 256), exp(2 pi i m / N) in fp64 (bank generation)
     // workspace
     unsigned char* ws = nullptr; uint64_t ws_bytes = 0, bump = 0; bool user_ws = false;
-    Slot s_bank, s_x, s_scratch, s_sig, s_rec, s_misc, s_par;
+    Slot s_bank, s_x, s_scratch, s_sig, s_rec, s_misc, s_par, s_proj;
     uint64_t T = 0; uint32_t S = 0; double tau = 0; uint32_t L = 0;
     bool have_sigma = false;
     // pinned staging
@@ -614,7 +631,7 @@ extern "C" void bege_plan_destroy(bege_plan* p)
     if (p->stream) cudaStreamSynchronize(p->stream);
     if (p->side) { cudaStreamSynchronize(p->side); cudaStreamDestroy(p->side); }
     if (p->own_stream && p->stream) cudaStreamDestroy(p->stream);
-    for (Slot* s : {&p->s_bank, &p->s_x, &p->s_scratch, &p->s_sig, &p->s_rec, &p->s_misc, &p->s_par}) slot_free(*s);
+    for (Slot* s : {&p->s_bank, &p->s_x, &p->s_scratch, &p->s_sig, &p->s_rec, &p->s_misc, &p->s_par, &p->s_proj}) slot_free(*s);
     if (p->tw256) cudaFree(p->tw256);
     if (p->twN) cudaFree(p->twN);
     if (p->tw256d) cudaFree(p->tw256d);
@@ -638,7 +655,7 @@ extern "C" int bege_plan_workspace_bytes(const bege_plan* p, uint64_t T, uint32_
     b += al((uint64_t)S * tpl_bytes(p));               // segment spectra
     b += al(scratch_bytes());                          // four-step staging (stays in L2)
     b += al(T * S * 16 * sizeof(float));               // Parseval partial sums
-    b += al(cap * sizeof(bege_tail));                  // records
+    b += al(std::max<uint64_t>(cap * sizeof(bege_tail), (uint64_t)S * kN * 8));   // records / max-projection array
     b += al(kMiscHdr + (uint64_t)S * kN * sizeof(c2)); // counters + raw segment staging
     *bytes = b + 4096;
     return BEGE_OK;
@@ -650,7 +667,7 @@ extern "C" int bege_plan_set_workspace(bege_plan* p, void* dev_ptr, uint64_t byt
     if (dev_ptr && ((uintptr_t)dev_ptr & 255)) return fail(p, BEGE_EINVAL, "workspace must be 256-byte aligned");
     CU(p, cudaSetDevice(p->device));
     CU(p, cudaStreamSynchronize(p->stream));
-    for (Slot* s : {&p->s_bank, &p->s_x, &p->s_scratch, &p->s_sig, &p->s_rec, &p->s_misc, &p->s_par}) slot_free(*s);
+    for (Slot* s : {&p->s_bank, &p->s_x, &p->s_scratch, &p->s_sig, &p->s_rec, &p->s_misc, &p->s_par, &p->s_proj}) slot_free(*s);
     p->ws = (unsigned char*)dev_ptr; p->ws_bytes = dev_ptr ? bytes : 0; p->bump = 0; p->user_ws = dev_ptr != nullptr;
     p->T = 0; p->S = 0; p->have_sigma = false;
     return BEGE_OK;
@@ -819,6 +836,53 @@ extern "C" int bege_search(bege_plan* p, float k_sigma, bege_tail* tails_out, ui
     p->have_sigma = true;
     *n_tails = total;
     if (total > cap) return fail(p, BEGE_EOVERFLOW, "%llu tails exceed cap %llu", (unsigned long long)total, (unsigned long long)cap);
+    return BEGE_OK;
+}
+
+
+extern "C" int bege_search_maxproj(bege_plan* p, float k_sigma, float* snr_out, uint32_t* id_out, uint64_t* n_hits)
+{
+    if (!p) return BEGE_EINVAL;
+    if (!snr_out || !id_out || !(k_sigma >= 0.f)) return fail(p, BEGE_EINVAL, "bad search arguments");
+    if (!p->T || !p->S) return fail(p, BEGE_ESTATE, "bege_search_maxproj needs a generated bank and loaded segments");
+    CU(p, cudaSetDevice(p->device));
+    void *sig, *proj, *misc, *scr, *bank, *xs;
+    int rc;
+    const uint64_t n = (uint64_t)p->S * kN;
+    if ((rc = slot_get(p, p->s_sig, p->T * p->S * 16 * sizeof(float), &sig))) return rc;
+    if ((rc = slot_get(p, p->s_rec, n * sizeof(unsigned long long), &proj))) return rc;
+    if ((rc = slot_get(p, p->s_misc, kMiscHdr, &misc))) return rc;
+    if ((rc = slot_get(p, p->s_scratch, scratch_bytes(), &scr))) return rc;
+    if ((rc = slot_get(p, p->s_bank, 0, &bank))) return rc;
+    if ((rc = slot_get(p, p->s_x, 0, &xs))) return rc;
+    CU(p, cudaMemsetAsync(proj, 0, n * sizeof(unsigned long long), p->stream));
+    const uint64_t maxT = std::max<uint64_t>(1, ((1ull << 31) - 1) / p->S / 2) * (uint64_t)p->G;
+    for (uint64_t jj = 0; jj < p->T; jj += maxT) {
+        // cap = ~0 switches the kernel's epilogue from appending records to the projection array passed as `rec`
+        if ((rc = launch_search(p, (const c2*)bank, (const c2*)xs, (c2*)scr, (float*)sig, k_sigma * k_sigma,
+                                (bege_tail*)proj, ~0ull, (unsigned char*)misc, nullptr, jj, std::min(maxT, p->T - jj), 0, p->S,
+                                jj == 0))) return rc;
+    }
+    CU(p, cudaGetLastError());
+    std::vector<unsigned long long> host(n);
+    CU(p, cudaMemcpyAsync(host.data(), proj, n * sizeof(unsigned long long), cudaMemcpyDeviceToHost, p->stream));
+    if ((rc = check_abort(p, (unsigned char*)misc))) return rc;      // synchronises the stream
+    uint64_t hits = 0;
+    for (uint64_t i = 0; i < n; ++i) {
+        const unsigned long long key = host[i];
+        if (key) {
+            const uint32_t bits = (uint32_t)(key >> 32);
+            memcpy(&snr_out[i], &bits, sizeof(float));
+            id_out[i] = 0xffffffffu - (uint32_t)key;
+            ++hits;
+        } else {
+            snr_out[i] = 0.f;
+            id_out[i] = 0xffffffffu;
+        }
+    }
+    p->stats.correlations += p->T * p->S;
+    p->have_sigma = true;
+    if (n_hits) *n_hits = hits;
     return BEGE_OK;
 }
 

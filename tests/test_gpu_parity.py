@@ -337,3 +337,50 @@ def test_bench_scale_launch_sampled_against_oracle(bo, bege):
     sel["template_id"] = np.searchsorted(sample, sel["template_id"]).astype(np.uint32)
     check_tail_sets(sel, sel.size, lo_tails, k)
     assert np.max(np.abs(sg[sample] - sigma_o[:, 0]) / sigma_o[:, 0]) <= SIGMA_RTOL
+
+
+# ----------------------------------------------------------------------------- max projection
+def check_maxproj(bo, snr_g, id_g, snr_o, id_o, Xs, f0, fd, k, guard=GUARD):
+    """Offsets whose oracle maximum is clear of the threshold must be present with the same value; the winning
+    template must be the oracle's, or one whose own (fp64) value is within fp32 resolution of the maximum."""
+    none = np.iinfo(np.uint32).max
+    assert np.all((snr_g == 0) == (id_g == none))
+    must = snr_o > k + guard
+    may = snr_o > k - guard
+    assert not np.any(must & (snr_g == 0)), "oracle offsets missing on the GPU"
+    assert not np.any((snr_g > 0) & ~may), "GPU offsets the oracle does not have"
+    both = must & (snr_g > 0)
+    assert np.max(np.abs(snr_g[both] - snr_o[both]) / snr_o[both], initial=0.0) < 2e-5
+    diff = both & (id_g != id_o)
+    for m, n in zip(*np.nonzero(diff)):                       # near-ties: the other template must be as good
+        z, s = bo.correlate(Xs[m], bo.template(f0[id_g[m, n]], fd[id_g[m, n]], TAU, FS, N))
+        assert abs(abs(z[n]) / s - snr_o[m, n]) / snr_o[m, n] < 2e-6
+    return int(both.sum()), int(diff.sum())
+
+
+def test_max_projection_matches_oracle(bo, bege):
+    w = synth.config0()
+    x2, n0 = synth.inject_chirp(synth.band_limit(synth.white_noise(9)), 1000.0, 50.0, 5.0, 9.0)
+    xs = np.stack([w.x[0], synth.as_segment(x2)])
+    Xs = np.stack([bo.segment_spectrum(x, FS, *BAND) for x in xs])
+    f0 = np.concatenate([w.f0[::4], [1000.0, 1000.0]])       # 66 templates, the last two identical (a planted tie)
+    fd = np.concatenate([w.fdot[::4], [50.0, 50.0]])
+    k = 2.8
+    snr_o, id_o = bo.search_maxproj(Xs, f0, fd, TAU, FS, k - 1e-3)
+    with bege.Plan(N, FS, BAND) as plan:
+        plan.bank_generate(f0, fd, TAU)
+        plan.segment_load(xs)
+        snr_g, id_g, nh = plan.search_maxproj(k)
+        tails, n = plan.search(k, cap=1 << 21)               # the extended output of the same call sequence
+        sg = plan.get_sigma()
+    assert nh == int((snr_g > 0).sum()) and 0 < nh < n
+    n_both, n_diff = check_maxproj(bo, snr_g, id_g, snr_o, id_o, Xs, f0, fd, k)
+    assert n_both > 1000
+    assert not np.any(id_g == 65)                            # equal values go to the smaller template id
+    peak = np.unravel_index(np.argmax(snr_g), snr_g.shape)
+    assert peak[0] == 1 and id_g[peak] == 64 and abs(int(peak[1]) - n0) <= 2
+    # the projection is exactly the per-offset maximum of the GPU's own extended output (same fp32 values)
+    best = np.zeros(2 * N, dtype=np.float32)
+    np.maximum.at(best, tails["lag"], tails["snr"])
+    assert np.array_equal(best, snr_g.ravel())
+    assert np.all(np.isfinite(sg)) and sg.shape == (66, 2)
