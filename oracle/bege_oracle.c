@@ -316,6 +316,43 @@ int bo_search_maxproj(const double* Xs, uint32_t S, const double* f0, const doub
     return 0;
 }
 
+
+/* ------------------------------------------------------- band threshold -- */
+/*
+ * PAPER.md:281 (sec.5): "excess tail sizes can conceivably be curtailed by generalising (9) to a finite band,
+ * kappa_1 sigma > rho(t_n) > kappa_2 sigma".  Same loops as bo_search (serial), with both inequalities strict:
+ * keep n iff k_lo*sigma < |z[n]| < k_hi*sigma.  Returns the true count; records beyond cap are not stored.
+ */
+uint64_t bo_search_band(const double* Xs, uint32_t S, const double* f0, const double* fdot, uint64_t T,
+                        double tau, double fs, uint32_t N, double k_lo, double k_hi, bo_tail* tails, uint64_t cap)
+{
+    double* Hs = (double*)malloc(sizeof(double) * 2 * (size_t)N);
+    double* z  = (double*)malloc(sizeof(double) * 2 * (size_t)N);
+    if (!Hs || !z) { free(Hs); free(z); return UINT64_MAX; }
+    uint64_t count = 0;
+    for (uint64_t j = 0; j < T; ++j) {
+        if (bo_template(f0[j], fdot[j], tau, fs, N, Hs) || bo_fft(Hs, N, -1)) { free(Hs); free(z); return UINT64_MAX; }
+        for (uint32_t m = 0; m < S; ++m) {
+            double sigma = 0.0;
+            bo_correlate_spectra(Xs + 2 * (size_t)m * N, Hs, N, z, &sigma);
+            if (!(sigma > 0.0)) continue;
+            for (uint32_t n = 0; n < N; ++n) {
+                double a = hypot(z[2 * n], z[2 * n + 1]);
+                if (a > k_lo * sigma && a < k_hi * sigma) {
+                    if (count < cap) {
+                        tails[count].template_id = (uint32_t)j;
+                        tails[count].lag = m * N + n;
+                        tails[count].snr = a / sigma;
+                    }
+                    ++count;
+                }
+            }
+        }
+    }
+    free(Hs); free(z);
+    return count;
+}
+
 /* PAPER.md:134 eq.(10), :160: nominal flops of one FFT_N. */
 double bo_fft_flops(uint32_t N)
 {

@@ -66,6 +66,8 @@ def lib():
         L.bo_search.restype = u64
         L.bo_search_maxproj.argtypes = [dp, u32, dp, dp, u64, dbl, dbl, u32, dbl, dp, ctypes.POINTER(u32)]
         L.bo_search_maxproj.restype = ctypes.c_int
+        L.bo_search_band.argtypes = [dp, u32, dp, dp, u64, dbl, dbl, u32, dbl, dbl, ctypes.POINTER(_Tail), u64]
+        L.bo_search_band.restype = u64
         L.bo_fft_flops.argtypes = [u32]
         L.bo_fft_flops.restype = dbl
         _lib = L
@@ -178,6 +180,21 @@ def search_maxproj(Xs, f0, fdot, tau: float, fs: float, k_sigma: float):
     if rc:
         raise RuntimeError(f"bo_search_maxproj rc={rc}")
     return snr, ids
+
+
+def search_band(Xs, f0, fdot, tau: float, fs: float, k_lo: float, k_hi: float, cap: int = 1 << 22):
+    """Band threshold k_lo*sigma < |z| < k_hi*sigma (bo_search_band): (tails sorted by (id, lag), n_true)."""
+    Xs = np.atleast_2d(_c128(Xs))
+    S, N = Xs.shape
+    f0 = np.ascontiguousarray(np.asarray(f0, dtype=np.float64))
+    fdot = np.ascontiguousarray(np.asarray(fdot, dtype=np.float64))
+    tails = np.zeros(max(cap, 1), dtype=TAIL_DTYPE)
+    n = lib().bo_search_band(_dp(Xs.view(np.float64)), S, _dp(f0), _dp(fdot), f0.size, float(tau), float(fs), N,
+                             float(k_lo), float(k_hi), tails.ctypes.data_as(ctypes.POINTER(_Tail)), cap)
+    if n == 2**64 - 1:
+        raise RuntimeError("bo_search_band failed")
+    tails = tails[: min(n, cap)]
+    return tails[np.lexsort((tails["lag"], tails["template_id"]))], int(n)
 
 
 def fft_flops(N: int) -> float:

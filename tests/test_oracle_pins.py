@@ -370,3 +370,22 @@ def test_max_projection_is_the_per_lag_maximum_of_the_extended_output():
     assert not np.any(ids == 33)
     peak = np.unravel_index(np.argmax(snr), snr.shape)
     assert peak[0] == 1 and ids[peak] == 32
+
+
+# ----------------------------------------------------------------------------- band threshold
+def test_band_threshold_is_the_extended_output_minus_its_top():
+    """kappa_1 sigma > rho > kappa_2 sigma: pinned against the (separately pinned) one-sided search -- the band
+    result is its tail set with the entries at or above kappa_1 removed; a band up to infinity changes nothing."""
+    w = synth.config0()
+    X = bo.segment_spectrum(w.x[0], FS, *BAND)
+    ids = np.arange(0, 256, 8)
+    full, n_full, _, _ = bo.search(X[None, :], w.f0[ids], w.fdot[ids], TAU, FS, 2.5)
+    band, n_band = bo.search_band(X[None, :], w.f0[ids], w.fdot[ids], TAU, FS, 2.5, 3.0)
+    keep = full[full["snr"] < 3.0]
+    assert 0 < n_band == keep.size < n_full
+    for f in ("template_id", "lag", "snr"):
+        assert np.array_equal(band[f], keep[f])
+    same, n_same = bo.search_band(X[None, :], w.f0[ids], w.fdot[ids], TAU, FS, 2.5, np.inf)
+    assert n_same == n_full and np.array_equal(same["lag"], full["lag"])
+    _, n_none = bo.search_band(X[None, :], w.f0[ids], w.fdot[ids], TAU, FS, 3.0, 3.0)
+    assert n_none == 0
