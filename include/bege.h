@@ -110,6 +110,13 @@ int bege_segment_load(bege_plan*, const float* x_interleaved_c64, uint32_t n_seg
 int bege_search(bege_plan*, float k_sigma, bege_tail* tails_out, uint64_t cap, uint64_t* n_tails);
 
 /*
+ * NEXT row of the scope table -- band threshold ("generalising (9) to a finite band, kappa_1 sigma >
+ * rho(t_n) > kappa_2 sigma", to curtail the tails of very deep searches): as bege_search, but a lag n is kept only if
+ * k_lo*sigma_jm < |z[n]| < k_hi*sigma_jm (both strict).  k_hi >= k_lo; k_hi = INFINITY is bege_search.
+ */
+int bege_search_band(bege_plan*, float k_lo, float k_hi, bege_tail* tails_out, uint64_t cap, uint64_t* n_tails);
+
+/*
  * NEXT row of the scope table -- the paper's default output mode (eq.13-17, Fig.4): the tails of
  * the whole bank projected onto the sample offsets.  For every offset i = m*N + n of the loaded segments:
  * snr_out[i] = max over the templates j with |z_jm[n]| > k_sigma*sigma_jm of |z_jm[n]|/sigma_jm (0 if none) and

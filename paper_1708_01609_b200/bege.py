@@ -23,7 +23,7 @@ _STATUS = {0: "BEGE_OK", 1: "BEGE_EINVAL", 2: "BEGE_ESTATE", 3: "BEGE_ENOMEM", 4
 # every symbol include/bege.h declares (tests check that the library exports all of them)
 SYMBOLS = [
     "bege_plan_create", "bege_plan_workspace_bytes", "bege_plan_set_workspace", "bege_bank_generate",
-    "bege_segment_load", "bege_search", "bege_search_maxproj", "bege_get_sigma", "bege_debug_correlate",
+    "bege_segment_load", "bege_search", "bege_search_band", "bege_search_maxproj", "bege_get_sigma", "bege_debug_correlate",
     "bege_debug_template_spectrum", "bege_debug_segment_spectrum", "bege_plan_set_profiling",
     "bege_plan_get_stats", "bege_plan_reset_stats", "bege_last_error", "bege_plan_destroy", "bege_version",
 ]
@@ -60,6 +60,7 @@ def load_library() -> ctypes.CDLL:
     L.bege_bank_generate.argtypes = [vp, vp, vp, u64, dbl]
     L.bege_segment_load.argtypes = [vp, vp, u32]
     L.bege_search.argtypes = [vp, ctypes.c_float, vp, u64, ctypes.POINTER(u64)]
+    L.bege_search_band.argtypes = [vp, ctypes.c_float, ctypes.c_float, vp, u64, ctypes.POINTER(u64)]
     L.bege_search_maxproj.argtypes = [vp, ctypes.c_float, vp, vp, ctypes.POINTER(u64)]
     L.bege_get_sigma.argtypes = [vp, vp]
     L.bege_debug_correlate.argtypes = [vp, u64, u32, vp, ctypes.POINTER(ctypes.c_float)]
@@ -191,6 +192,16 @@ class Plan:
         rc = self._check(self._L.bege_search(self._h, ctypes.c_float(k_sigma), ctypes.c_void_p(buf.data_ptr()),
                                              cap, ctypes.byref(n)),
                          allow=(EOVERFLOW,) if allow_overflow else ())
+        got = min(n.value, cap)
+        view = buf.numpy()[: got * 12].view(TAIL_DTYPE)
+        return (view.copy() if copy else view), int(n.value)
+
+    def search_band(self, k_lo: float, k_hi: float, cap: int = 1 << 20, copy: bool = True):
+        """Band threshold k_lo*sigma < |z| < k_hi*sigma: (tails, n_tails) as `search`."""
+        buf = self.pinned_tails(cap)
+        n = ctypes.c_uint64()
+        self._check(self._L.bege_search_band(self._h, ctypes.c_float(k_lo), ctypes.c_float(k_hi),
+                                             ctypes.c_void_p(buf.data_ptr()), cap, ctypes.byref(n)))
         got = min(n.value, cap)
         view = buf.numpy()[: got * 12].view(TAIL_DTYPE)
         return (view.copy() if copy else view), int(n.value)

@@ -187,7 +187,7 @@ BEGE_D c2 cmul2(c2 x, c2 w) { return cmul(x, re(w), im(w)); }                   
 template <int I0, int NI, bool SINGLE>
 __global__ void __launch_bounds__(kSearchThreads, 1)
 k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restrict__ ring,
-         float* __restrict__ sigpart, float k2, bege_tail* __restrict__ rec, unsigned long long cap,
+         float* __restrict__ sigpart, float k2, float k2hi, bege_tail* __restrict__ rec, unsigned long long cap,
          unsigned long long* __restrict__ counter, c2* __restrict__ zdbg, uint64_t j0, uint64_t nT,
          uint32_t m0, uint32_t nS, uint32_t S, unsigned long long* done1, unsigned long long* done2,
          int* abort_flag)
@@ -394,6 +394,14 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
 #endif
             if (__any_sync(0xffffffffu, hits != 0)) {
                 const float inv = 1.0f / sumR2;
+                if (k2hi < 3.0e38f) {                        // band threshold: drop |z| >= k_hi sigma
+                    const float thr_hi = k2hi * sumR2;
+#pragma unroll
+                    for (int q = 0; q < 16; ++q) {
+                        const c2 sq = mul2(v[q], v[q]);
+                        if (!(re(sq) + im(sq) < thr_hi)) hits &= ~(1u << q);
+                    }
+                }
                 if (cap == ~0ull) {
                     // max projection: per sample offset the largest |z|/sigma over the bank and
                     // its template, race free: one 64-bit atomicMax on (snr bits, ~template_id); positive floats
@@ -739,7 +747,7 @@ extern "C" int bege_segment_load(bege_plan* p, const float* x, uint32_t S)
 }
 
 // one cooperative launch of the persistent search kernel over templates [j0, j0 + nT) x segments [m0, m0 + nS)
-static int launch_search(bege_plan* p, const c2* bank, const c2* xs, c2* ring, float* sig, float k2, bege_tail* rec,
+static int launch_search(bege_plan* p, const c2* bank, const c2* xs, c2* ring, float* sig, float k2, float k2hi, bege_tail* rec,
                          uint64_t cap, unsigned char* misc, c2* zdbg, uint64_t j0, uint64_t nT, uint32_t m0, uint32_t nS,
                          bool first = true)
 {
@@ -769,7 +777,7 @@ static int launch_search(bege_plan* p, const c2* bank, const c2* xs, c2* ring, f
     const bool single = (p->S == 1);
     unsigned long long capll = cap;
     uint32_t S = p->S;
-    void* args[] = {&bank, &xs, &ring, &sig, &k2, &rec, &capll, &counter, &zdbg, &j0, &nT, &m0, &nS, &S,
+    void* args[] = {&bank, &xs, &ring, &sig, &k2, &k2hi, &rec, &capll, &counter, &zdbg, &j0, &nT, &m0, &nS, &S,
                     &done1, &done2, &abort_flag};
     const void* f = p->NI == 14 ? (single ? (const void*)k_search<1, 14, true> : (const void*)k_search<1, 14, false>)
                                 : (single ? (const void*)k_search<0, 16, true> : (const void*)k_search<0, 16, false>);
@@ -796,10 +804,11 @@ static int check_abort(bege_plan* p, unsigned char* misc)
     return BEGE_OK;
 }
 
-extern "C" int bege_search(bege_plan* p, float k_sigma, bege_tail* tails_out, uint64_t cap, uint64_t* n_tails)
+static int search_impl(bege_plan* p, float k_sigma, float k_hi, bege_tail* tails_out, uint64_t cap, uint64_t* n_tails)
 {
     if (!p) return BEGE_EINVAL;
-    if (!n_tails || (cap && !tails_out) || !(k_sigma >= 0.f)) return fail(p, BEGE_EINVAL, "bad search arguments");
+    if (!n_tails || (cap && !tails_out) || !(k_sigma >= 0.f) || !(k_hi >= k_sigma) || cap == ~0ull)
+        return fail(p, BEGE_EINVAL, "bad search arguments");
     if (!p->T || !p->S) return fail(p, BEGE_ESTATE, "bege_search needs a generated bank and loaded segments");
     CU(p, cudaSetDevice(p->device));
     void *sig, *rec, *misc, *scr, *bank, *xs;
@@ -814,7 +823,7 @@ extern "C" int bege_search(bege_plan* p, float k_sigma, bege_tail* tails_out, ui
     // the kernel counts a group's (template, segment) items in 32 bits: split longer searches
     const uint64_t maxT = std::max<uint64_t>(1, ((1ull << 31) - 1) / p->S / 2) * (uint64_t)p->G;
     for (uint64_t jj = 0; jj < p->T; jj += maxT) {
-        if ((rc = launch_search(p, (const c2*)bank, (const c2*)xs, (c2*)scr, (float*)sig, k_sigma * k_sigma,
+        if ((rc = launch_search(p, (const c2*)bank, (const c2*)xs, (c2*)scr, (float*)sig, k_sigma * k_sigma, k_hi * k_hi,
                                 (bege_tail*)rec, cap, (unsigned char*)misc, nullptr, jj, std::min(maxT, p->T - jj), 0, p->S,
                                 jj == 0))) return rc;
     }
@@ -840,6 +849,16 @@ extern "C" int bege_search(bege_plan* p, float k_sigma, bege_tail* tails_out, ui
 }
 
 
+extern "C" int bege_search(bege_plan* p, float k_sigma, bege_tail* tails_out, uint64_t cap, uint64_t* n_tails)
+{
+    return search_impl(p, k_sigma, INFINITY, tails_out, cap, n_tails);
+}
+
+extern "C" int bege_search_band(bege_plan* p, float k_lo, float k_hi, bege_tail* tails_out, uint64_t cap, uint64_t* n_tails)
+{
+    return search_impl(p, k_lo, k_hi, tails_out, cap, n_tails);
+}
+
 extern "C" int bege_search_maxproj(bege_plan* p, float k_sigma, float* snr_out, uint32_t* id_out, uint64_t* n_hits)
 {
     if (!p) return BEGE_EINVAL;
@@ -859,7 +878,7 @@ extern "C" int bege_search_maxproj(bege_plan* p, float k_sigma, float* snr_out, 
     const uint64_t maxT = std::max<uint64_t>(1, ((1ull << 31) - 1) / p->S / 2) * (uint64_t)p->G;
     for (uint64_t jj = 0; jj < p->T; jj += maxT) {
         // cap = ~0 switches the kernel's epilogue from appending records to the projection array passed as `rec`
-        if ((rc = launch_search(p, (const c2*)bank, (const c2*)xs, (c2*)scr, (float*)sig, k_sigma * k_sigma,
+        if ((rc = launch_search(p, (const c2*)bank, (const c2*)xs, (c2*)scr, (float*)sig, k_sigma * k_sigma, INFINITY,
                                 (bege_tail*)proj, ~0ull, (unsigned char*)misc, nullptr, jj, std::min(maxT, p->T - jj), 0, p->S,
                                 jj == 0))) return rc;
     }
@@ -921,7 +940,7 @@ extern "C" int bege_debug_correlate(bege_plan* p, uint64_t j, uint32_t m, float*
     const bool prof = p->profiling; p->profiling = false;
     // the kernel indexes the partial sums by (j*S + m)*16: bias the base so that this pair lands on sg[0..15]
     float* sg_biased = sg - (j * p->S + m) * 16;
-    rc = launch_search(p, (const c2*)bank, (const c2*)xs, (c2*)scr, sg_biased, 1e30f, nullptr, 0, (unsigned char*)misc, zd, j, 1, m, 1);
+    rc = launch_search(p, (const c2*)bank, (const c2*)xs, (c2*)scr, sg_biased, 1e30f, INFINITY, nullptr, 0, (unsigned char*)misc, zd, j, 1, m, 1);
     p->profiling = prof;
     if (!rc) rc = check_abort(p, (unsigned char*)misc);
     if (rc) { cudaFree(zd); cudaFree(sg); return rc; }

@@ -384,3 +384,24 @@ def test_max_projection_matches_oracle(bo, bege):
     np.maximum.at(best, tails["lag"], tails["snr"])
     assert np.array_equal(best, snr_g.ravel())
     assert np.all(np.isfinite(sg)) and sg.shape == (66, 2)
+
+
+# ----------------------------------------------------------------------------- band threshold
+def test_band_threshold_matches_oracle(cfg0, bo):
+    """kappa_1 sigma > |z| > kappa_2 sigma: both edges get the 1e-4 sigma guard band of the north_star."""
+    w, plan, X = cfg0
+    k_lo, k_hi = 2.5, 3.0
+    wide, _ = bo.search_band(X[None, :], w.f0, w.fdot, TAU, FS, k_lo - 1e-3, k_hi + 1e-3)
+    tails, n = plan.search_band(k_lo, k_hi, cap=1 << 20)
+    assert n == tails.size and n > 10000
+    key = lambda tt: tt["template_id"].astype(np.uint64) << np.uint64(32) | tt["lag"].astype(np.uint64)
+    okey, gkey = key(wide), key(tails)
+    assert np.unique(gkey).size == gkey.size
+    must = okey[(wide["snr"] > k_lo + GUARD) & (wide["snr"] < k_hi - GUARD)]
+    may = okey[(wide["snr"] > k_lo - GUARD) & (wide["snr"] < k_hi + GUARD)]
+    assert np.setdiff1d(must, gkey).size == 0 and np.setdiff1d(gkey, may).size == 0
+    assert np.all((tails["snr"] > k_lo) & (tails["snr"] < k_hi))
+    # an open band is the plain search
+    t_all, n_all = plan.search(k_lo, cap=1 << 20)
+    t_inf, n_inf = plan.search_band(k_lo, float("inf"), cap=1 << 20)
+    assert n_inf == n_all and np.array_equal(np.sort(key(t_inf)), np.sort(key(t_all)))
