@@ -37,8 +37,8 @@ UNIT = "correlations/s"
 FFT_FLOP = 5.0 * 65536 * 16                       # PAPER.md:134 eq.(10): 5 N log2 N
 ALG_BYTES_PER_CORR = 52802 * 8                    # two-sided in-band template spectrum, S = 1
 # dram__bytes_read.sum + dram__bytes_write.sum of k_search per correlation, from the ncu --set full capture summarised
-# in profiles/r1e_search_kernel.md (36,864-template launch: 16.914 GB read + 1.546 GB written)
-NCU_DRAM_BYTES_PER_CORR = (16.913704e9 + 1.546495e9) / 36864
+# in profiles/r1g_search_kernel_final.md (36,864-template launch: 16.914 GB read + 0.365 GB written)
+NCU_DRAM_BYTES_PER_CORR = (16.913879e9 + 0.365349e9) / 36864
 FP32_PEAK = 148 * 128 * 2 * 1.965e9               # SMs x fp32 lanes x 2 flop x max SM clock
 
 
@@ -263,7 +263,7 @@ def run_ours(args, rank, world, local_rank):
         "gflops_equiv": value * FFT_FLOP * 1e-9,
         "roofline": {"bound": "alu", "achieved": alu_achieved, "peak": FP32_PEAK * 1e-12, "unit": "TFLOP/s",
                      "frac": alu_achieved / (FP32_PEAK * 1e-12), "traffic": NCU_DRAM_BYTES_PER_CORR * kern_corr,
-                     "traffic_note": "bytes per launch = ncu dram bytes per correlation (profiles/r1e_search_kernel.md) x correlations of the timed launch",
+                     "traffic_note": "bytes per launch = ncu dram bytes per correlation (profiles/r1g_search_kernel_final.md) x correlations of the timed launch",
                      "kernel": "k_search (persistent warp-specialised search kernel, one launch per bank chunk), CUDA events on the plan's stream, "
                                f"{pst['fused_kernel_launches']} launch over {kern_corr} correlations",
                      "peak_source": "derived: 148 SM x 128 fp32 lanes x 2 x 1.965 GHz (DESIGN.md); "
