@@ -651,7 +651,12 @@ extern "C" void bege_plan_destroy(bege_plan* p)
     delete p;
 }
 
-static uint64_t scratch_bytes() { return (uint64_t)std::max(kBatch, kMaxGroups * kRing) * kN * sizeof(c2); }
+// one region serves the fp64 staging of the bank generation (kBatch spectra of 16-byte elements), the fp32 staging of
+// the segment transform and the search ring (G groups x kRing items)
+static uint64_t scratch_bytes(const bege_plan* p)
+{
+    return std::max<uint64_t>((uint64_t)kBatch * kN * sizeof(d2), (uint64_t)p->G * kRing * kN * sizeof(c2));
+}
 
 extern "C" int bege_plan_workspace_bytes(const bege_plan* p, uint64_t T, uint32_t S, uint64_t cap, uint64_t* bytes)
 {
@@ -661,7 +666,7 @@ extern "C" int bege_plan_workspace_bytes(const bege_plan* p, uint64_t T, uint32_
     b += al(T * tpl_bytes(p));                         // bank
     b += al(T * 16);                                   // template parameters (f0, fdot)
     b += al((uint64_t)S * tpl_bytes(p));               // segment spectra
-    b += al(scratch_bytes());                          // four-step staging (stays in L2)
+    b += al(scratch_bytes(p));                          // four-step staging (stays in L2)
     b += al(T * S * 16 * sizeof(float));               // Parseval partial sums
     b += al(std::max<uint64_t>(cap * sizeof(bege_tail), (uint64_t)S * kN * 8));   // records / max-projection array
     b += al(kMiscHdr + (uint64_t)S * kN * sizeof(c2)); // counters + raw segment staging
@@ -692,7 +697,7 @@ extern "C" int bege_bank_generate(bege_plan* p, const double* f0, const double* 
     int rc;
     if ((rc = slot_get(p, p->s_bank, T * tpl_bytes(p), &bank))) return rc;
     if ((rc = slot_get(p, p->s_par, T * 16, &par))) return rc;
-    if ((rc = slot_get(p, p->s_scratch, scratch_bytes(), &scr))) return rc;
+    if ((rc = slot_get(p, p->s_scratch, scratch_bytes(p), &scr))) return rc;
     p->T = 0; p->have_sigma = false;
     double* d_f0 = (double*)par; double* d_fd = d_f0 + T;
     CU(p, cudaMemcpyAsync(d_f0, f0, T * sizeof(double), cudaMemcpyHostToDevice, p->stream));
@@ -725,7 +730,7 @@ extern "C" int bege_segment_load(bege_plan* p, const float* x, uint32_t S)
     int rc;
     if ((rc = slot_get(p, p->s_x, (uint64_t)S * tpl_bytes(p), &xs))) return rc;
     if ((rc = slot_get(p, p->s_misc, kMiscHdr + (uint64_t)S * kN * sizeof(c2), &misc))) return rc;
-    if ((rc = slot_get(p, p->s_scratch, scratch_bytes(), &scr))) return rc;
+    if ((rc = slot_get(p, p->s_scratch, scratch_bytes(p), &scr))) return rc;
     p->S = 0; p->have_sigma = false;
     c2* raw = (c2*)((unsigned char*)misc + kMiscHdr);
     cudaPointerAttributes at;
@@ -816,7 +821,7 @@ static int search_impl(bege_plan* p, float k_sigma, float k_hi, bege_tail* tails
     if ((rc = slot_get(p, p->s_sig, p->T * p->S * 16 * sizeof(float), &sig))) return rc;
     if ((rc = slot_get(p, p->s_rec, cap * sizeof(bege_tail), &rec))) return rc;
     if ((rc = slot_get(p, p->s_misc, kMiscHdr, &misc))) return rc;
-    if ((rc = slot_get(p, p->s_scratch, scratch_bytes(), &scr))) return rc;
+    if ((rc = slot_get(p, p->s_scratch, scratch_bytes(p), &scr))) return rc;
     if ((rc = slot_get(p, p->s_bank, 0, &bank))) return rc;
     if ((rc = slot_get(p, p->s_x, 0, &xs))) return rc;
     unsigned long long* counter = (unsigned long long*)misc;
@@ -871,7 +876,7 @@ extern "C" int bege_search_maxproj(bege_plan* p, float k_sigma, float* snr_out, 
     if ((rc = slot_get(p, p->s_sig, p->T * p->S * 16 * sizeof(float), &sig))) return rc;
     if ((rc = slot_get(p, p->s_rec, n * sizeof(unsigned long long), &proj))) return rc;
     if ((rc = slot_get(p, p->s_misc, kMiscHdr, &misc))) return rc;
-    if ((rc = slot_get(p, p->s_scratch, scratch_bytes(), &scr))) return rc;
+    if ((rc = slot_get(p, p->s_scratch, scratch_bytes(p), &scr))) return rc;
     if ((rc = slot_get(p, p->s_bank, 0, &bank))) return rc;
     if ((rc = slot_get(p, p->s_x, 0, &xs))) return rc;
     CU(p, cudaMemsetAsync(proj, 0, n * sizeof(unsigned long long), p->stream));
@@ -931,7 +936,7 @@ extern "C" int bege_debug_correlate(bege_plan* p, uint64_t j, uint32_t m, float*
     CU(p, cudaSetDevice(p->device));
     void *scr, *bank, *xs, *misc;
     int rc;
-    if ((rc = slot_get(p, p->s_scratch, scratch_bytes(), &scr))) return rc;
+    if ((rc = slot_get(p, p->s_scratch, scratch_bytes(p), &scr))) return rc;
     if ((rc = slot_get(p, p->s_misc, kMiscHdr, &misc))) return rc;
     slot_get(p, p->s_bank, 0, &bank); slot_get(p, p->s_x, 0, &xs);
     c2* zd = nullptr; float* sg = nullptr;
