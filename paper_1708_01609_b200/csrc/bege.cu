@@ -499,6 +499,22 @@ struct bege_plan {
     std::string err;
 };
 
+// take the ring's persisting-L2 window off the plan's stream again (the stream may be the caller's)
+static void drop_l2_window(bege_plan* p)
+{
+    if (!p->l2_window || !p->stream) return;
+    cudaStreamAttrValue av{};
+    av.accessPolicyWindow.base_ptr = nullptr;
+    av.accessPolicyWindow.num_bytes = 0;
+    av.accessPolicyWindow.hitRatio = 0.f;
+    av.accessPolicyWindow.hitProp = cudaAccessPropertyNormal;
+    av.accessPolicyWindow.missProp = cudaAccessPropertyNormal;
+    cudaStreamSetAttribute(p->stream, cudaStreamAttributeAccessPolicyWindow, &av);
+    cudaCtxResetPersistingL2Cache();
+    cudaGetLastError();
+    p->l2_window = nullptr;
+}
+
 static int fail(bege_plan* p, int code, const char* fmt, ...)
 {
     if (p) {
@@ -637,6 +653,7 @@ extern "C" void bege_plan_destroy(bege_plan* p)
     if (!p) return;
     cudaSetDevice(p->device);
     if (p->stream) cudaStreamSynchronize(p->stream);
+    drop_l2_window(p);
     if (p->side) { cudaStreamSynchronize(p->side); cudaStreamDestroy(p->side); }
     if (p->own_stream && p->stream) cudaStreamDestroy(p->stream);
     for (Slot* s : {&p->s_bank, &p->s_x, &p->s_scratch, &p->s_sig, &p->s_rec, &p->s_misc, &p->s_par, &p->s_proj}) slot_free(*s);
@@ -680,6 +697,7 @@ extern "C" int bege_plan_set_workspace(bege_plan* p, void* dev_ptr, uint64_t byt
     if (dev_ptr && ((uintptr_t)dev_ptr & 255)) return fail(p, BEGE_EINVAL, "workspace must be 256-byte aligned");
     CU(p, cudaSetDevice(p->device));
     CU(p, cudaStreamSynchronize(p->stream));
+    drop_l2_window(p);
     for (Slot* s : {&p->s_bank, &p->s_x, &p->s_scratch, &p->s_sig, &p->s_rec, &p->s_misc, &p->s_par, &p->s_proj}) slot_free(*s);
     p->ws = (unsigned char*)dev_ptr; p->ws_bytes = dev_ptr ? bytes : 0; p->bump = 0; p->user_ws = dev_ptr != nullptr;
     p->T = 0; p->S = 0; p->have_sigma = false;
