@@ -13,6 +13,7 @@ each bracketed by a device synchronize and CUDA events on the plan's stream.
 N > 1 (torchrun): every rank searches its own 2^20-template shard of an N-times finer fdot grid (weak
 scaling, no data-path collective); tail records are gathered on rank 0 after the timed region.
 --impl reference times the fp64 CPU oracle (oracle/) on the host cores, on a bounded sample.
+--impl cufft times the same steps built from library kernels (torch + cuFFT): a reference point for context only.
 """
 from __future__ import annotations
 
@@ -129,6 +130,54 @@ def run_reference(args, rank):
         "gflops_equiv": value * FFT_FLOP * 1e-9,
     }
     print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------ library reference point
+def run_cufft(args, rank, local_rank):
+    """Context only (north_star: "cuFFT used only as a timed reference point, not as the product"): the same steps
+    with library kernels -- torch elementwise product, torch reductions, torch.fft.ifft (cuFFT batched C2C, N = 2^16),
+    torch compare + count -- on a resident batch of template spectra produced by the product's own bank generation."""
+    if rank != 0:
+        return
+    import torch
+    from paper_1708_01609_b200 import bege
+    dev = torch.device("cuda", local_rank)
+    torch.cuda.set_device(dev)
+    Tb = args.cufft_batch
+    f0, fdot = synth.config2_bank()
+    ids = np.linspace(0, f0.size - 1, Tb).astype(np.int64)
+    x = synth.noise_segment(2)[None, :]
+    with bege.Plan(synth.N_SEG, synth.FS, synth.BAND, device=local_rank) as plan:
+        plan.bank_generate(f0[ids], fdot[ids], synth.TAU)
+        plan.segment_load(x)
+        H = torch.from_numpy(np.stack([plan.debug_template_spectrum(j) for j in range(Tb)])).to(dev)
+        X = torch.from_numpy(plan.debug_segment_spectrum(0)).to(dev)
+    k2 = 36.0
+    def step():
+        R = torch.conj(H) * X                                        # a3
+        s2 = (R.real * R.real + R.imag * R.imag).sum(dim=1) / float(synth.N_SEG) ** 2     # a4
+        z = torch.fft.ifft(R, dim=1)                                 # a5 (1/N inside)
+        hit = (z.real * z.real + z.imag * z.imag) > (k2 * s2)[:, None]                   # a6
+        return int(hit.sum().item())                                 # a7: count only (records not materialised)
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize(dev)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    n = 0
+    for _ in range(args.steps):
+        n = step()
+    e1.record()
+    torch.cuda.synchronize(dev)
+    ms = e0.elapsed_time(e1) / args.steps
+    value = Tb / (ms * 1e-3)
+    print(json.dumps({"impl": "cufft", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+                      "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "dtype": "f32",
+                      "data": "synthetic", "config": {"workload": f"{Tb} templates of configs[2] x 1 segment, resident full "
+                      "spectra (512 KiB each), torch elementwise + torch.fft.ifft (cuFFT) + torch reductions", "tails": n},
+                      "gflops_equiv": value * FFT_FLOP * 1e-9,
+                      "note": "library reference point for context; not the product, not the driver's reference arm"}),
+          flush=True)
 
 
 # ------------------------------------------------------------------------------------------ our arm
@@ -283,18 +332,22 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference", "cufft"])
     ap.add_argument("--templates", type=int, default=1 << 20, help="templates per GPU (default: configs[2])")
     ap.add_argument("--chunk", type=int, default=0, help="bank chunk size (default: what fits HBM)")
     ap.add_argument("--cpu-sample", type=int, default=24576)
     ap.add_argument("--ref-sample", type=int, default=8192)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cufft-batch", type=int, default=2048, help="templates per step of the --impl cufft reference point")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
         run_reference(args, rank)
+        return
+    if args.impl == "cufft":
+        run_cufft(args, rank, local_rank)
         return
     if world > 1:
         import torch.distributed as dist
