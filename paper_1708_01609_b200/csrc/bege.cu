@@ -4,8 +4,8 @@
 // Index conventions (N = 65536 = 256 x 256, w_M = exp(2 pi i / M)):
 //   inverse (search):  k = k1 + 256 k2,  n = 256 n1 + n2
 //     z[256 n1 + n2] = 1/N sum_k1 w256^(k1 n1) [ wN^(k1 n2) sum_k2 R[k1 + 256 k2] w256^(k2 n2) ]
-//     pass 1 (k_search phase A): 256-point column DFTs over k2 + twiddle wN^(k1 n2) -> ring T[n2][k1] (L2)
-//     pass 2 (k_search phase B): 256-point row DFTs over k1, threshold, compaction
+//     pass 1 (k_search A teams): 256-point column DFTs over k2 + first twiddle factor -> ring T[n2][k1] (L2)
+//     pass 2 (k_search B teams): second twiddle factor, 256-point row DFTs over k1, threshold, compaction
 //   forward (bank / segments): n = nl + 256 nh, k = k1 + 256 k2
 //     H[k1 + 256 k2] = sum_nl w256^(-nl k2) [ wN^(-nl k1) sum_nh h[nl + 256 nh] w256^(-nh k1) ]
 //     step A (k_fwd_rows_*): DFT over nh + twiddle -> scratch G (tile layout), step B (k_fwd_cols): DFT over nl
@@ -30,14 +30,17 @@
 #include "bank64.cuh"
 
 #ifndef BEGE_ABL
-#define BEGE_ABL 0          // ablation switches for timing experiments (never set in the product build)
+// Ablation switches for timing experiments (profiles/r1e_search_kernel.md); never set in the product build, results
+// are garbage when any is set: 1 no cross-CTA waits, 2 no template tile loads, 4 no ring stores, 8 no ring loads,
+// 16 pass-1 teams off, 32 pass-2 teams off.
+#define BEGE_ABL 0
 #endif
 
 namespace bege {
 
 constexpr int kN = 65536;
-constexpr int kBatch = 72;                 // spectra per launch of the forward transforms (36 MB of staging)
-constexpr int kMaxGroups = 32;             // search: persistent CTA groups of 16 tiles (18 on a 148-SM B200)
+constexpr int kBatch = 72;                 // spectra per launch of the forward transforms (fp64 bank staging: 75 MB)
+constexpr int kMaxGroups = 32;             // search: persistent CTA groups of 16 tiles (9 on a 148-SM B200)
 constexpr uint64_t kMiscHdr = 4096;        // counter @0, abort flag @8, done1 @256, done2 @2048 (per group and ring slot)
 
 // ------------------------------------------------------------------------------------------------
