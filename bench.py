@@ -33,7 +33,7 @@ if ROOT not in sys.path:
 
 from paper_1708_01609_b200 import synth  # noqa: E402
 
-METRIC = "template correlations/sec at N=2^16 C2C fp32"
+METRIC = "template correlations/sec at N=2^16 C2C fp32 on 1 B200; % of FFT roofline"   # BASELINE.json, verbatim
 UNIT = "correlations/s"
 FFT_FLOP = 5.0 * 65536 * 16                       # PAPER.md:134 eq.(10): 5 N log2 N
 ALG_BYTES_PER_CORR = 52802 * 8                    # two-sided in-band template spectrum, S = 1
