@@ -59,9 +59,11 @@ typedef struct {
  * Create a plan for transforms of length N (must be 65536 = 2^16: "FFT_{N,M} of
  * length N = 2^16") at sampling rate fs [Hz] with the analysis band band_lo_hz <= |f| <= band_hi_hz
  * (inclusive edges; 350-2000 Hz).  0 < band_lo < band_hi < fs/2.
- * device: CUDA device ordinal.  cuda_stream: a cudaStream_t (e.g. torch's current stream handle) or
- * NULL for a stream the plan creates.  All work of the plan is ordered on that stream; a second,
- * internal stream carries the device->host copy of the tails.
+ * device: CUDA device ordinal.  cuda_stream: a cudaStream_t (e.g. torch's current stream handle; pass
+ * cudaStreamLegacy, not 0, for the legacy default stream) or NULL for a non-blocking stream the plan creates.
+ * All work of the plan is ordered on that stream: device inputs (bege_segment_load) must have been produced on
+ * it or be complete before the call.  A second, internal stream carries the device->host copy of the tails
+ * while the search goes on.
  */
 int bege_plan_create(bege_plan** out, uint32_t N, double fs, double band_lo_hz, double band_hi_hz,
                      int device, void* cuda_stream);
@@ -84,8 +86,9 @@ int bege_plan_set_workspace(bege_plan*, void* dev_ptr, uint64_t bytes);
  * a1 -- template spectra (PAPER.md:156 step ii: "a chirp template w of duration tau = 1 s is extended by
  * zeros to length N and its transform w~ is loaded into Global Memory").  For j < n_templates:
  *   L = round(tau_s*fs); t_n = n/fs; h_j[n] = hann_L[n] * exp(i 2 pi (f0_j t_n + fdot_j t_n^2 / 2)), n < L,
- *   unit L2 norm, zero padded to N; H_j = DFT_N(h_j).  Phases are formed in fp64, the transform runs in
- *   fp32.  The in-band rows of H_j are stored in HBM in the tiled layout the search kernel streams.
+ *   unit L2 norm, zero padded to N; H_j = DFT_N(h_j).  Phases and the whole transform run in fp64; each stored
+ *   bin is rounded to fp32 once.  The in-band rows of H_j are stored in HBM in the tiled layout the search
+ *   kernel streams.
  * f0_hz, fdot_hz_s: host arrays of n_templates doubles.  Replaces any previous bank.  1 <= L <= N/16.
  */
 int bege_bank_generate(bege_plan*, const double* f0_hz, const double* fdot_hz_s,
@@ -102,7 +105,8 @@ int bege_segment_load(bege_plan*, const float* x_interleaved_c64, uint32_t n_seg
  * a3-a7 -- the search (PAPER.md:89-100 eq.5-7, :116-120 eq.9, :156-160 steps ii-iv, :162).  For every
  * template j of the bank and loaded segment m:  R = conj(H_j) X_m;  sigma_jm^2 = N^-2 sum_k |R[k]|^2;
  * z = IDFT_N(R) (four-step 256x256, never written to HBM);  every n with |z[n]| > k_sigma*sigma_jm is
- * appended as {j, m*N+n, |z[n]|/sigma_jm}.  Only these records cross PCIe (pinned staging, side stream).
+ * appended as {j, m*N+n, |z[n]|/sigma_jm}.  Only these records cross PCIe (side stream; for large searches the
+ * bank is searched in up to 8 slices and the records of slice i are copied while slice i+1 is searched).
  * tails_out: host array of `cap` records (pinned memory is copied into directly), may be NULL if cap = 0.
  * *n_tails: the TRUE number of tails.  If it exceeds cap, exactly cap records are written (which ones
  * is unspecified) and BEGE_EOVERFLOW is returned.  Record order is unspecified.  Synchronous at return.
@@ -141,6 +145,14 @@ int bege_debug_correlate(bege_plan*, uint64_t template_id, uint32_t segment, flo
 /* Off the timed path: stored spectrum of one template / one segment, natural order, N complex fp32 (host). */
 int bege_debug_template_spectrum(bege_plan*, uint64_t template_id, float* H_out_c64);
 int bege_debug_segment_spectrum(bege_plan*, uint32_t segment, float* X_out_c64);
+
+/*
+ * Off the timed path, for tests: the search kernel counts the (template, segment) items of a CTA group in 32 bits, so
+ * bege_search splits a search of more than 2^30 items per group into several launches.  This lowers that limit
+ * (1 <= max_items < 2^30; default 2^30 - 1) so that a test can reach the split with a small bank.  Results do not
+ * depend on it.
+ */
+int bege_debug_set_max_items(bege_plan*, uint64_t max_items);
 
 int  bege_plan_set_profiling(bege_plan*, int on);    /* CUDA events around the dominant kernel (adds syncs) */
 int  bege_plan_get_stats(const bege_plan*, bege_stats* out);

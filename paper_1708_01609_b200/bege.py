@@ -18,13 +18,14 @@ TAIL_DTYPE = np.dtype([("template_id", "<u4"), ("lag", "<u4"), ("snr", "<f4")])
 assert TAIL_DTYPE.itemsize == 12
 
 OK, EINVAL, ESTATE, ENOMEM, ECUDA, EOVERFLOW = range(6)
+CUDA_STREAM_LEGACY = 0x1          # cudaStreamLegacy (driver_types.h): the legacy default stream as an explicit handle
 _STATUS = {0: "BEGE_OK", 1: "BEGE_EINVAL", 2: "BEGE_ESTATE", 3: "BEGE_ENOMEM", 4: "BEGE_ECUDA", 5: "BEGE_EOVERFLOW"}
 
 # every symbol include/bege.h declares (tests check that the library exports all of them)
 SYMBOLS = [
     "bege_plan_create", "bege_plan_workspace_bytes", "bege_plan_set_workspace", "bege_bank_generate",
     "bege_segment_load", "bege_search", "bege_search_band", "bege_search_maxproj", "bege_get_sigma", "bege_debug_correlate",
-    "bege_debug_template_spectrum", "bege_debug_segment_spectrum", "bege_plan_set_profiling",
+    "bege_debug_template_spectrum", "bege_debug_segment_spectrum", "bege_debug_set_max_items", "bege_plan_set_profiling",
     "bege_plan_get_stats", "bege_plan_reset_stats", "bege_last_error", "bege_plan_destroy", "bege_version",
 ]
 
@@ -66,6 +67,7 @@ def load_library() -> ctypes.CDLL:
     L.bege_debug_correlate.argtypes = [vp, u64, u32, vp, ctypes.POINTER(ctypes.c_float)]
     L.bege_debug_template_spectrum.argtypes = [vp, u64, vp]
     L.bege_debug_segment_spectrum.argtypes = [vp, u32, vp]
+    L.bege_debug_set_max_items.argtypes = [vp, u64]
     L.bege_plan_set_profiling.argtypes = [vp, i32]
     L.bege_plan_get_stats.argtypes = [vp, ctypes.POINTER(Stats)]
     L.bege_plan_reset_stats.argtypes = [vp]
@@ -94,6 +96,11 @@ class Plan:
         self.N, self.fs, self.band, self.device = int(N), float(fs), tuple(band), int(device)
         if stream is None:
             stream = torch.cuda.current_stream(self.device).cuda_stream
+        if stream == 0:
+            # torch's default stream is the legacy default stream; handle 0 would read as "no stream given" and make
+            # the plan create a private non-blocking stream that is NOT ordered after work torch has queued (e.g. the
+            # kernel that produced a CUDA tensor passed to segment_load).  cudaStreamLegacy names it explicitly.
+            stream = CUDA_STREAM_LEGACY
         h = ctypes.c_void_p()
         rc = self._L.bege_plan_create(ctypes.byref(h), self.N, self.fs, float(band[0]), float(band[1]),
                                       self.device, ctypes.c_void_p(stream))
@@ -235,6 +242,10 @@ class Plan:
         X = np.empty(self.N, dtype=np.complex64)
         self._check(self._L.bege_debug_segment_spectrum(self._h, segment, X.ctypes.data))
         return X
+
+    def debug_set_max_items(self, max_items: int):
+        """(template, segment) items one kernel launch may take per CTA group; tests lower it to reach the launch split."""
+        self._check(self._L.bege_debug_set_max_items(self._h, int(max_items)))
 
     def set_profiling(self, on: bool):
         self._check(self._L.bege_plan_set_profiling(self._h, int(bool(on))))

@@ -10,7 +10,8 @@ HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 LIB = HERE / "libbege.so"
 SOURCES = [CSRC / "bege.cu"]
-HEADERS = [CSRC / "cplx.cuh", HERE.parent / "include" / "bege.h"]
+# everything the library is compiled from: a change to any of these makes the built .so stale
+HEADERS = sorted(CSRC.glob("*.cuh")) + [HERE.parent / "include" / "bege.h"]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC", "--use_fast_math=false"]

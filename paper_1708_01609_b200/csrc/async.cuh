@@ -1,8 +1,11 @@
-// mbarrier, bulk async copy (TMA engine, 1-D) and gpu-scope counter primitives for sm_100a (inline PTX).
+// mbarrier, bulk async copy (TMA engine, 1-D), shared-memory accessors and gpu-scope counter primitives
+// for sm_100a (inline PTX).
 //
 // Loads:  cp.async.bulk global -> shared, completion counted in bytes on an mbarrier (SASS UBLKCP).
-// Stores: cp.async.bulk shared -> global as a bulk async-group of the issuing thread.
-// Cross-CTA hand-over: monotone 64-bit counters in global memory, red.release / ld.acquire at gpu scope.
+// Cross-CTA hand-over: monotone 64-bit counters in global memory.  The PTX memory-model ordering every arrow
+// of the protocol relies on is listed in DESIGN.md section 5 ("hand-over"); in short:
+//   producer:  data stores -> (CTA barrier) -> red.release.gpu by one thread   (release is cumulative)
+//   consumer:  ld.acquire.gpu by one thread sees the count -> (CTA barrier) -> data loads of all threads
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -13,23 +16,38 @@ namespace bege {
 
 BEGE_DA uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
-BEGE_DA void mbar_init(uint64_t* bar, uint32_t count)
+// ---- shared memory by 32-bit address + immediate byte offset (keeps one base register per access pattern)
+template <int OFF> BEGE_DA unsigned long long lds64(uint32_t a)
 {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(smem_u32(bar)), "r"(count) : "memory");
+    unsigned long long v;
+    asm volatile("ld.shared.b64 %0, [%1+%2];" : "=l"(v) : "r"(a), "n"(OFF));
+    return v;
 }
-BEGE_DA void mbar_arrive(uint64_t* bar)
+template <int OFF> BEGE_DA void lds128(uint32_t a, unsigned long long& v0, unsigned long long& v1)
 {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(smem_u32(bar)) : "memory");
+    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2+%3];" : "=l"(v0), "=l"(v1) : "r"(a), "n"(OFF));
 }
-BEGE_DA void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes)
+template <int OFF> BEGE_DA void sts64(uint32_t a, unsigned long long v)
 {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(smem_u32(bar)), "r"(bytes) : "memory");
+    asm volatile("st.shared.b64 [%0+%1], %2;" :: "r"(a), "n"(OFF), "l"(v) : "memory");
 }
-BEGE_DA bool mbar_try_wait(uint64_t* bar, uint32_t parity)
+BEGE_DA float lds32(uint32_t a) { float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a)); return v; }
+BEGE_DA void sts32(uint32_t a, float v) { asm volatile("st.shared.f32 [%0], %1;" :: "r"(a), "f"(v) : "memory"); }
+
+// ---- mbarrier
+BEGE_DA void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(bar), "r"(count) : "memory");
+}
+BEGE_DA void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory");
+}
+BEGE_DA bool mbar_try_wait(uint32_t bar, uint32_t parity)
 {
     uint32_t ok;
     asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                 : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
     return ok != 0;
 }
 
@@ -37,7 +55,7 @@ BEGE_DA bool mbar_try_wait(uint64_t* bar, uint32_t parity)
 // abort flag (checked by the host after the launch) and lets the caller run on with whatever it has
 constexpr long long kSpinLimit = 1000000000ll;
 
-BEGE_DA void mbar_wait(uint64_t* bar, uint32_t parity, int* abort_flag)
+BEGE_DA void mbar_wait(uint32_t bar, uint32_t parity, int* abort_flag)
 {
     if (mbar_try_wait(bar, parity)) return;
     const long long t0 = clock64();
@@ -47,8 +65,6 @@ BEGE_DA void mbar_wait(uint64_t* bar, uint32_t parity, int* abort_flag)
     }
 }
 
-BEGE_DA void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
-BEGE_DA void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 BEGE_DA void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 
 BEGE_DA uint64_t policy_evict_first()
@@ -65,21 +81,58 @@ BEGE_DA uint64_t policy_evict_last()
 }
 
 // global -> shared, `bytes` a multiple of 16, both addresses 16-byte aligned; completes on `bar`
-BEGE_DA void bulk_load(void* smem_dst, const void* gmem_src, uint32_t bytes, uint64_t* bar, uint64_t policy)
+BEGE_DA void bulk_load(uint32_t smem_dst, const void* gmem_src, uint32_t bytes, uint32_t bar, uint64_t policy)
 {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
-                 :: "r"(smem_u32(smem_dst)), "l"(gmem_src), "r"(bytes), "r"(smem_u32(bar)), "l"(policy) : "memory");
+                 :: "r"(smem_dst), "l"(gmem_src), "r"(bytes), "r"(bar), "l"(policy) : "memory");
 }
-// shared -> global, joins the issuing thread's current bulk async-group
-BEGE_DA void bulk_store(void* gmem_dst, const void* smem_src, uint32_t bytes, uint64_t policy)
-{
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;"
-                 :: "l"(gmem_dst), "r"(smem_u32(smem_src)), "r"(bytes), "l"(policy) : "memory");
-}
-BEGE_DA void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
-BEGE_DA void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }   // source reusable
-BEGE_DA void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }             // writes done
 
+// ---- tensor memory (TMEM, 512 columns x 128 lanes x 32 bit per SM), used here as a second register file for
+// loop-invariant per-thread tables: tcgen05.ld/st have their own datapath and take nothing from the L1/LSU data pipe
+// that the FFT exchanges saturate.  Shape 32x32b: thread i of a warp reads/writes lane 32 (warp % 4) + i, N columns.
+template <int NCOLS> BEGE_DA void tmem_alloc(uint32_t smem_dst)          // one whole warp; address -> shared memory
+{
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_dst), "n"(NCOLS) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+template <int NCOLS> BEGE_DA void tmem_dealloc(uint32_t taddr)           // the same warp
+{
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(taddr), "n"(NCOLS) : "memory");
+}
+BEGE_DA void tmem_fence_before_sync() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+BEGE_DA void tmem_fence_after_sync() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+BEGE_DA void tmem_st8(uint32_t taddr, const uint32_t (&r)[8])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};"
+                 :: "r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]) : "memory");
+}
+BEGE_DA void tmem_st4(uint32_t taddr, const uint32_t (&r)[4])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};"
+                 :: "r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]) : "memory");
+}
+BEGE_DA void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+// asynchronous load of 4 complex numbers (8 columns); the values may be used only after tmem_wait_ld on the same array
+BEGE_DA void tmem_ld8(uint32_t taddr, unsigned long long (&w)[4])
+{
+    uint32_t r0, r1, r2, r3, r4, r5, r6, r7;
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3), "=r"(r4), "=r"(r5), "=r"(r6), "=r"(r7) : "r"(taddr));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(w[0]) : "r"(r0), "r"(r1));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(w[1]) : "r"(r2), "r"(r3));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(w[2]) : "r"(r4), "r"(r5));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(w[3]) : "r"(r6), "r"(r7));
+}
+// waits for all tcgen05.ld of this thread; the array is an in/out operand so that no use can be scheduled above it
+BEGE_DA void tmem_wait_ld(unsigned long long (&w)[4])
+{
+    asm volatile("tcgen05.wait::ld.sync.aligned;" : "+l"(w[0]), "+l"(w[1]), "+l"(w[2]), "+l"(w[3]) :: "memory");
+}
+
+// ---- named barrier of `nthreads` threads
+BEGE_DA void bar_named(int id, int nthreads) { asm volatile("bar.sync %0, %1;" :: "r"(id), "r"(nthreads) : "memory"); }
+
+// ---- gpu-scope counters
 BEGE_DA void counter_add_release(unsigned long long* ctr, unsigned long long v)
 {
     asm volatile("red.release.gpu.global.add.u64 [%0], %1;" :: "l"(ctr), "l"(v) : "memory");
@@ -90,49 +143,17 @@ BEGE_DA unsigned long long counter_load_acquire(const unsigned long long* ctr)
     asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(ctr) : "memory");
     return v;
 }
-BEGE_DA void counter_add_relaxed(unsigned long long* ctr, unsigned long long v)
-{
-    asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" :: "l"(ctr), "l"(v) : "memory");
-}
-BEGE_DA unsigned long long counter_load_relaxed(const unsigned long long* ctr)
-{
-    unsigned long long v;
-    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(ctr) : "memory");
-    return v;
-}
-// whole warp waits until *ctr >= target: lane 0 polls (relaxed, L2), the value is broadcast so that the loop is
-// warp-uniform and the warp stays converged.  The data guarded by the counter must be read with ld.global.cg
-// (L2 is the point of coherence; the producer publishes with a gpu-scope release after its writes completed).
-BEGE_DA void warp_counter_wait_ge(const unsigned long long* ctr, unsigned long long target, int* abort_flag, int lane)
-{
-    const long long t0 = clock64();
-    for (;;) {
-        unsigned long long v = 0;
-        int bail = 0;
-        if (lane == 0) {
-            v = counter_load_relaxed(ctr);
-            if (v < target) {
-                bail = *(volatile int*)abort_flag;
-                if (clock64() - t0 > kSpinLimit) { *(volatile int*)abort_flag = 1; bail = 1; }
-            }
-        }
-        v = __shfl_sync(0xffffffffu, v, 0);
-        bail = __shfl_sync(0xffffffffu, bail, 0);
-        if (v >= target || bail) break;
-        __nanosleep(400);
-    }
-    __syncwarp();
-}
-// one thread spins until *ctr >= target
+// ONE thread spins until *ctr >= target; every probe is an acquire load, so whatever the thread (and, after a
+// CTA barrier, its team) reads afterwards is ordered after the producers' released writes.
 BEGE_DA void counter_wait_ge(const unsigned long long* ctr, unsigned long long target, int* abort_flag)
 {
     if (counter_load_acquire(ctr) >= target) return;
     const long long t0 = clock64();
     for (;;) {
+        __nanosleep(100);
         if (counter_load_acquire(ctr) >= target) return;
         if (*(volatile int*)abort_flag) return;
         if (clock64() - t0 > kSpinLimit) { *(volatile int*)abort_flag = 1; return; }
-        __nanosleep(64);
     }
 }
 

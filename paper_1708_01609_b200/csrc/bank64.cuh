@@ -55,7 +55,7 @@ BEGE_DD void dfft16f(d2 (&a)[16])
 }
 
 // step A: chirp synthesis (fp64 phase) + pruned row DFTs.  grid (16, templates in batch), 256 threads.
-// Same index map as k_fwd_rows_chirp: CTA (ia, jl) owns the rows nl = ga + 16 ia; only nh < 16 inputs are
+// Same index map as k_fwd_rows_data (bege.cu): CTA (ia, jl) owns the rows nl = ga + 16 ia; only nh < 16 inputs are
 // non-zero (L <= 4096); output G[k1 = p + 16 q][nl] times wN^(-nl k1), tile layout, fp64.
 // tw256d[m] = exp(2 pi i m / 256), twNd[m] = exp(2 pi i m / N) (host-built double tables).
 __global__ void __launch_bounds__(256)
@@ -126,12 +126,18 @@ k_bank_cols64(const d2* __restrict__ G, float2* __restrict__ out, uint64_t out_s
     for (int a = 0; a < 16; ++a) v[a] = priv[(a << 4) + (g ^ a)];
     __syncwarp();
     dfft16f(v);
-    // lane p = g holds k2 = p + 16 q
-    float2* o = out + jl * out_stride + (uint64_t)b * NI * 256;
+    // lane p = g holds k2 = p + 16 q; stored layout: row-blocks in pairs, one 16-byte word per thread and pair
+    float4* o = reinterpret_cast<float4*>(out + jl * out_stride + (uint64_t)b * NI * 256) + t;
 #pragma unroll
-    for (int q = 0; q < 16; ++q) {
-        if (q < I0 || q >= I0 + NI) continue;
-        o[((q - I0) * 16 + c) * 16 + g] = make_float2((float)v[q].x, (float)v[q].y);
+    for (int ip = 0; ip < 8; ++ip) {
+        if (2 * ip < NI) {
+            float4 w;
+            if (I0 == 1) { w = make_float4((float)v[(2 * ip + 1) & 15].x, (float)v[(2 * ip + 1) & 15].y,
+                                           (float)v[(2 * ip + 2) & 15].x, (float)v[(2 * ip + 2) & 15].y); }
+            else         { w = make_float4((float)v[2 * ip].x, (float)v[2 * ip].y,
+                                           (float)v[(2 * ip + 1) & 15].x, (float)v[(2 * ip + 1) & 15].y); }
+            o[ip * 256] = w;
+        }
     }
 }
 

@@ -11,9 +11,11 @@
 //     step A (k_fwd_rows_*): DFT over nh + twiddle -> scratch G (tile layout), step B (k_fwd_cols): DFT over nl
 //   every 256-point DFT is 16 x 16: a half-warp owns one DFT, each lane 16 points in registers.
 //
-// "Tile layout" of a spectrum (bank, segments, forward scratch): for tile b (columns k1 = 16 b + c),
-// kept row-block i (rows k2 = g + 16 i), element index ((b*NI + (i - I0))*16 + c)*16 + g, so that the 16
-// lanes g of a half-warp (and the two half-warps c, c+1 of a warp) read contiguous memory.
+// "Tile layout" of a stored spectrum (bank, segments): for tile b (columns k1 = 16 b + c), kept row-block i
+// (rows k2 = g + 16 i, i in [I0, I0 + NI)), thread t = 16 c + g of a pass-1 team, element index
+// ((b*NI/2 + (i - I0)/2)*256 + t)*2 + ((i - I0) & 1): a thread's two row-blocks of a pair are one 16-byte word, a
+// team reads 4 KiB per 128-bit load, conflict free.  The forward scratch G keeps the plain order
+// ((b*16 + i)*16 + c)*16 + g over all 16 row-blocks.
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -41,12 +43,11 @@ namespace bege {
 constexpr int kN = 65536;
 constexpr int kBatch = 72;                 // spectra per launch of the forward transforms (fp64 bank staging: 75 MB)
 constexpr int kMaxGroups = 32;             // search: persistent CTA groups of 16 tiles (9 on a 148-SM B200)
-constexpr uint64_t kMiscHdr = 4096;        // counter @0, abort flag @8, done1 @256, done2 @2048 (per group and ring slot)
+constexpr uint64_t kMiscHdr = 4096;        // counter @0, abort flag @8, hits @16, done1 @256, done2 @2048 (per group and ring slot)
+constexpr int kMaxSlices = 8;              // launches per search whose record copies overlap the next launch
+constexpr uint64_t kSliceMinCorr = 32768;  // do not slice below this many correlations per slice
 
 // ------------------------------------------------------------------------------------------------
-// shared-memory exchange index for the column passes: stage-1 thread (c, g) writes its p-th value,
-// stage-2 thread (c, p) reads over g.  XOR swizzle keeps both sides bank-conflict free (8-byte words).
-BEGE_D int xidx(int c, int g, int p) { return ((p << 4) + g) * 16 + (c ^ g); }
 // private 256-element region of a half-warp: lane a writes its p-th value, lane p reads over a
 BEGE_D int pidx(int a, int p) { return (a << 4) + (p ^ a); }
 
@@ -56,7 +57,7 @@ template <int DIR>
 BEGE_D void stage1(c2 (&v)[16], const float2 (&w1)[16]) {
     fft16<DIR>(v);
 #pragma unroll
-    for (int p = 1; p < 16; ++p) v[p] = cmul(v[p], w1[p].x, DIR > 0 ? w1[p].y : -w1[p].y);
+    for (int p = 1; p < 16; ++p) v[p] = cmulw(v[p], w1[p].x, DIR > 0 ? w1[p].y : -w1[p].y);
 }
 
 // full 256-point DFT of a half-warp through its private shared-memory region.
@@ -104,7 +105,7 @@ k_fwd_rows_data(const c2* __restrict__ x, const float2* __restrict__ tw256, cons
     for (int q = 0; q < 16; ++q) {
         const int k1 = p + 16 * q;
         const float2 w = __ldg(twN + nl * 256 + k1);
-        out[((q * 16 + ia) * 16 + p) * 16 + ga] = cmul(v[q], w.x, -w.y);
+        out[((q * 16 + ia) * 16 + p) * 16 + ga] = cmulw(v[q], w.x, -w.y);
     }
 }
 
@@ -127,19 +128,26 @@ k_fwd_cols(const c2* __restrict__ G, c2* __restrict__ out, uint64_t out_stride, 
 #pragma unroll
     for (int i = 0; i < 16; ++i) v[i] = in[(i * 16 + c) * 16 + g];
     hw_fft256<-1>(v, w1, sm[c], g);
-    // lane p = g holds k2 = p + 16 q
-    c2* o = out + jl * out_stride + (uint64_t)b * NI * 256;
+    // lane p = g holds k2 = p + 16 q; row-blocks are stored in pairs (one 16-byte word per thread and pair)
+    ulonglong2* o = reinterpret_cast<ulonglong2*>(out + jl * out_stride + (uint64_t)b * NI * 256) + t;
     const uint32_t k1 = 16 * b + c;
 #pragma unroll
     for (int q = 0; q < 16; ++q) {
-        if (q < I0 || q >= I0 + NI) continue;
-        c2 val = v[q];
         if (MASK) {
             const uint32_t k = k1 + 256u * (uint32_t)(g + 16 * q);
             const uint32_t kk = k < (uint32_t)kN / 2 ? k : (uint32_t)kN - k;
-            if (kk < klo || kk > khi) val = mk(0.f, 0.f);
+            if (kk < klo || kk > khi) v[q] = mk(0.f, 0.f);
         }
-        o[((q - I0) * 16 + c) * 16 + g] = val;
+    }
+#pragma unroll
+    for (int ip = 0; ip < 8; ++ip) {
+        if (2 * ip < NI) {
+            ulonglong2 w;
+            // (I0, NI) is (1, 14) or (0, 16): both spelled out so that v is indexed with compile-time constants
+            if (I0 == 1) { w.x = v[(2 * ip + 1) & 15]; w.y = v[(2 * ip + 2) & 15]; }
+            else         { w.x = v[2 * ip]; w.y = v[(2 * ip + 1) & 15]; }
+            o[ip * 256] = w;
+        }
     }
 }
 
@@ -148,276 +156,492 @@ k_fwd_cols(const c2* __restrict__ G, c2* __restrict__ out, uint64_t out_stride, 
 // grid (16 tiles, G groups), one CTA of 32 warps (64 registers per thread) per SM, cooperative launch (all CTAs
 // co-resident).  The 16 CTAs of a group share the group's (template, segment) items; item `it` of a group is the
 // pair (template grp + G (it / nS), segment it % nS).  CTA (b, grp) owns columns k1 = 16 b + c in pass 1 and rows
-// n2 = 16 b + r in pass 2.  The path is latency bound, not pipe bound (profiles/), so the kernel is built for
-// warps in flight: four teams of 8 warps, two per pass, team k of a pass taking the items it = k (mod 2).
-//   A teams (pass 1): the template's column tile arrives in shared memory by bulk async copy from HBM (one
-//              buffer per team, refilled as soon as the team has read it, mbarrier-tracked).  Stage 1: half-warp
-//              c, lane g holds rows k2 = g + 16 i of column c: conj(H) X against the segment tile (shared
-//              memory), Parseval partial sum, 16-point DFTs, twiddles theta^p generated from one complex number
+// n2 = 16 b + r in pass 2.  Four teams of 8 warps, two per pass, team k of a pass taking the items it = k (mod 2).
+//   A teams (pass 1): R = conj(H) X needs one column tile of the template spectrum and one of the segment spectrum.
+//              One of them is STATIONARY in shared memory, the other STREAMS through a per-team buffer by bulk
+//              async copy (mbarrier-tracked, refilled as soon as the team has read it):
+//                single-segment calls (nS = 1): X stationary (loaded once per launch), H streams from HBM;
+//                batched calls (nS >= 2):       H stationary (one load per template, it serves all nS segments --
+//                                               PAPER.md:156 "loaded once per M inverse FFTs"), X streams from L2.
+//              Stage 1: half-warp c, lane g holds rows k2 = g + 16 i of column c: 128-bit loads of both tiles,
+//              conj(H) X, Parseval partial sum, 16-point DFTs, twiddles theta^p generated from one complex number
 //              per thread.  One exchange through shared memory (two named barriers of the team per item).
-//              Stage 2: lane c, p = warp-pair index: 16-point DFTs, and
-//              T[n2 = p + 16 q][16 b + c] goes straight from registers to the ring in L2 (128 B per half-warp
-//              and store).  The tile is published (done1) with a release issued one item later.
-//   B teams (pass 2): half-warp r waits for all 16 tiles of an item (done1), loads its row of T from the ring,
+//              Stage 2: lane c, p = warp-pair index: 16-point DFTs, and T[n2 = p + 16 q][16 b + c] goes straight
+//              from registers to the ring in L2 (128 B per half-warp and store).
+//   B teams (pass 2): wait for all 16 tiles of an item, half-warp r loads its row of T from the ring,
 //              runs the 256-point row DFT over k1 through a private shared-memory region, thresholds against
-//              k^2 sum|R|^2, compacts the tails with warp-aggregated atomics, and releases its share of the
-//              ring slot (done2) as soon as the row is in registers.
+//              k^2 sum|R|^2 and compacts the tails with warp-aggregated atomics.
+// Hand-over (PTX memory model): per group and ring slot two monotone counters.
+//   done1 (tiles in the ring): every A team adds 1 per item with red.release.gpu by ONE thread after a team barrier
+//              that follows all the team's ring stores (release is cumulative over the barrier).  ONE thread of the
+//              B team spins on ld.acquire.gpu until 16 tiles have arrived, then the team barrier releases the other
+//              seven warps, which sleep in hardware meanwhile (no polling instructions).
+//   done2 (ring slot read out): one thread of the B team adds 1 with red.release.gpu after the team barrier of the
+//              team's NEXT item, which every warp reaches only after its loads of this item have returned.  ONE
+//              thread of the A team acquires 16 of them before the barrier that precedes the team's ring stores.
 // The ring holds kRing items per group (G x kRing x 512 KiB) and lives in L2.  Four-step twiddle wN^(k1 n2) with
 // n2 = p + 16 q is split into wN^(k1 p), folded into theta = exp(2 pi i (256 g + k1) / N) of pass 1, and
 // wN^(16 k1 q), applied by pass 2 to its inputs (q = n2 >> 4 is the CTA's tile index there: a 16 x 16 table in
 // shared memory); theta and the tables are rounded once from fp64 angles.
 constexpr int kRing = 8;
 constexpr int kSearchThreads = 32 * 32;
-constexpr int kPriv = 16 * 17;                              // padded private region of a half-warp (c2 elements)
-constexpr int kXch = 16 * 16 * 17;                          // padded exchange buffer of pass 1 (c2 elements)
 
-template <int NI, bool XS> struct SearchSmem {
-    c2 hbuf[2][NI * 256];                                   // template column tile of each A team
-    c2 xs[XS ? NI * 256 : 2];                               // segment column tile (single-segment searches)
-    c2 xch[2][kXch];                                        // pass 1 of each A team: stage 1 -> stage 2, [p][g][c]
-    c2 bpriv[32][kPriv];                                    // pass 2: private exchange regions
-    float2 tbl[256];                                        // wN^(16 b k1), k1 = a + 16 r, [r][a] (pass 2)
-    float2 w1t[256];                                        // w256^(a p), [p][a]
-    float ssig[2][8];                                       // Parseval partial sums of the 8 warps of an A team
-    uint64_t hfull[2];
+// Loop-invariant per-thread tables live in tensor memory (read with tcgen05.ld: no L1/LSU wavefronts):
+//   columns [0, 32):    pass 2: delta_p = exp(2 pi i a (b + 16 p) / 4096), p < 16 -- the lane-dependent part of the
+//                       four-step factor wN^(16 b k1) times the inner twiddle w256^(a p); all four lane quadrants
+//   columns [32, 96):   pass 1: the stationary tile, 28 columns per thread (14 complex), 32 per warp of a lane quadrant
+//   columns [96, 160):  pass 1: theta^p, p = 1 .. 15, same arrangement
+// The CTA-uniform part of the four-step factor, w256^(b r), comes from constant memory (uniform loads).
+#ifndef BEGE_TM
+#define BEGE_TM 7          // 1: pass-2 twiddles, 2: stationary tile, 4: theta powers (timing experiments switch them off)
+#endif
+constexpr int kTmemCols = 256;
+constexpr uint32_t kTmDelta = 0, kTmStat = 32, kTmTheta = 96;
+__constant__ float2 c_w256[256];           // exp(2 pi i m / 256), rounded from fp64 (host, bege_plan_create)
+
+struct SearchArgs {
+    const c2* bank; const c2* xseg; c2* ring; float* sigpart; bege_tail* rec; c2* zdbg;
+    unsigned long long cap; unsigned long long* counter; unsigned long long* done1; unsigned long long* done2;
+    int* abort_flag;
+    uint64_t j0, nT, sig_pair0;
+    uint32_t m0, nS, S;
+    float k2, k2hi;
 };
-template <int NI, bool SINGLE> __host__ __device__ constexpr bool search_xs() { return SINGLE && NI <= 14; }
-template <int NI, bool SINGLE> constexpr int search_smem() { return (int)sizeof(SearchSmem<NI, search_xs<NI, SINGLE>()>) + 128; }
 
-BEGE_D void bar_team(int id) { asm volatile("bar.sync %0, 256;" :: "r"(id) : "memory"); }   // the 8 warps of a team
-BEGE_D c2 cmul2(c2 x, c2 w) { return cmul(x, re(w), im(w)); }                               // x * w
+// shared-memory map of k_search (byte offsets from the 128-byte aligned base)
+template <int NI, bool STAT> struct SearchSmem {
+    static constexpr uint32_t kTile = NI * 256 * 8;              // one column tile of a spectrum
+    static constexpr uint32_t kXch = 16 * 16 * 17 * 8;           // padded pass-1 exchange buffer, [p][g][c]
+    static constexpr uint32_t kPriv = 16 * 17 * 8;               // padded private region of a pass-2 half-warp
+    static constexpr uint32_t stream = 0;                        // [2]  streaming tile of each A team
+    static constexpr uint32_t stat = stream + 2 * kTile;         //      stationary tile (if STAT)
+    static constexpr uint32_t xch = stat + (STAT ? kTile : 0);   // [2]
+    static constexpr uint32_t bpriv = xch + 2 * kXch;            // [32]
+    static constexpr uint32_t tbl = bpriv + 32 * kPriv;          // wN^(16 b k1), k1 = a + 16 r, [r/2][a][r&1] (pass 2)
+    static constexpr uint32_t w1t = tbl + 2048;                  // w256^(a p), [p/2][a][p&1]
+    static constexpr uint32_t ssig = w1t + 2048;                 // [2][8] Parseval partial sums of the A warps
+    static constexpr uint32_t bars = ssig + 64;                  // mbarriers: stream[2], stat; TMEM base address @ +24
+    static constexpr uint32_t total = bars + 32;
+};
+// the stationary tile fits next to everything else only for bands that need 14 of the 16 row-blocks
+template <int NI> __host__ __device__ constexpr bool search_stat() { return NI <= 14; }
+template <int NI> constexpr int search_smem() { return (int)SearchSmem<NI, search_stat<NI>()>::total + 128; }
 
-template <int I0, int NI, bool SINGLE>
-__global__ void __launch_bounds__(kSearchThreads, 1)
-k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restrict__ ring,
-         float* __restrict__ sigpart, float k2, float k2hi, bege_tail* __restrict__ rec, unsigned long long cap,
-         unsigned long long* __restrict__ counter, c2* __restrict__ zdbg, uint64_t j0, uint64_t nT,
-         uint32_t m0, uint32_t nS, uint32_t S, unsigned long long* done1, unsigned long long* done2,
-         int* abort_flag)
+// 16 values to shared memory at a + p * STRIDE bytes
+template <int STRIDE, int P = 0> BEGE_D void sts16(uint32_t a, const c2 (&v)[16])
 {
-    constexpr bool XS = search_xs<NI, SINGLE>();
+    if constexpr (P < 16) { sts64<P * STRIDE>(a, v[P]); sts16<STRIDE, P + 1>(a, v); }
+}
+template <int STRIDE, int P = 0> BEGE_D void lds16(uint32_t a, c2 (&v)[16])
+{
+    if constexpr (P < 16) { v[P] = lds64<P * STRIDE>(a); lds16<STRIDE, P + 1>(a, v); }
+}
+// v[2 i], v[2 i + 1] *= table entries (2 i, 2 i + 1) at a + i * 256 bytes (one 128-bit load per pair); FIRST: skip entry 0
+template <bool FIRST, int IP = 0> BEGE_D void twiddle16(uint32_t a, c2 (&v)[16])
+{
+    if constexpr (IP < 8) {
+        c2 w0, w1;
+        lds128<IP * 256>(a, w0, w1);
+        if (!(FIRST && IP == 0)) v[2 * IP] = cmulw(v[2 * IP], w0);
+        v[2 * IP + 1] = cmulw(v[2 * IP + 1], w1);
+        twiddle16<FIRST, IP + 1>(a, v);
+    }
+}
+// stage 1 of pass 1: v[I0 + 2 ip], v[I0 + 2 ip + 1] = conj(H) X for the row-block pair ip, acc += |.|^2 (packed)
+template <int I0, int NI, bool SINGLE, bool STAT, int IP = 0>
+BEGE_D void load_products(uint32_t stream_a, uint32_t stat_a, const ulonglong2* __restrict__ statg, c2 (&v)[16], c2& acc)
+{
+    if constexpr (IP < NI / 2) {
+        c2 s0, s1, q0, q1;
+        lds128<IP * 4096>(stream_a, s0, s1);
+        if constexpr (STAT) lds128<IP * 4096>(stat_a, q0, q1);
+        else { const ulonglong2 q = __ldg(statg + IP * 256); q0 = q.x; q1 = q.y; }
+        // SINGLE: the template streams, the segment is stationary; batched: the other way round
+        const c2 r0 = SINGLE ? cmulc(q0, s0) : cmulc(s0, q0);
+        const c2 r1 = SINGLE ? cmulc(q1, s1) : cmulc(s1, q1);
+        v[I0 + 2 * IP] = r0; v[I0 + 2 * IP + 1] = r1;
+        acc = fma2(r0, r0, acc);
+        acc = fma2(r1, r1, acc);
+        load_products<I0, NI, SINGLE, STAT, IP + 1>(stream_a, stat_a, statg, v, acc);
+    }
+}
+
+// v[4 j + k] *= w[k]
+template <int J> BEGE_D void mul4(c2 (&v)[16], const c2 (&w)[4])
+{
+#pragma unroll
+    for (int k = 0; k < 4; ++k) v[4 * J + k] = cmulw(v[4 * J + k], w[k]);
+}
+// products of two row-block pairs: streaming tile from shared memory, stationary values q[0..3] from tensor memory
+template <int I0, bool SINGLE, int IP> BEGE_D void products2(uint32_t stream_a, const c2 (&q)[4], c2 (&v)[16], c2& acc, bool second = true)
+{
+    c2 s0, s1;
+    lds128<IP * 4096>(stream_a, s0, s1);
+    c2 r0 = SINGLE ? cmulc(q[0], s0) : cmulc(s0, q[0]);
+    c2 r1 = SINGLE ? cmulc(q[1], s1) : cmulc(s1, q[1]);
+    v[I0 + 2 * IP] = r0; v[I0 + 2 * IP + 1] = r1;
+    acc = fma2(r0, r0, acc); acc = fma2(r1, r1, acc);
+    if (second) {
+        lds128<(IP + 1) * 4096>(stream_a, s0, s1);
+        r0 = SINGLE ? cmulc(q[2], s0) : cmulc(s0, q[2]);
+        r1 = SINGLE ? cmulc(q[3], s1) : cmulc(s1, q[3]);
+        v[(I0 + 2 * IP + 2) & 15] = r0; v[(I0 + 2 * IP + 3) & 15] = r1;
+        acc = fma2(r0, r0, acc); acc = fma2(r1, r1, acc);
+    }
+}
+
+template <int I0, int NI, bool SINGLE, bool DBG>
+__global__ void __launch_bounds__(kSearchThreads, 1)
+k_search(const __grid_constant__ SearchArgs A)
+{
+    constexpr bool STAT = search_stat<NI>();
+    constexpr bool TM_TW = (BEGE_TM & 1) != 0;               // pass-2 twiddles from TMEM + constant memory
+    constexpr bool TM_ST = STAT && (BEGE_TM & 2) != 0;       // stationary tile in TMEM instead of shared memory
+    constexpr bool TM_TH = (BEGE_TM & 4) != 0;               // theta powers from TMEM instead of the product tree
+    using SM = SearchSmem<NI, STAT>;
+    static_assert(NI % 2 == 0, "row-blocks are stored in pairs");
+    static_assert(!TM_ST || NI == 14, "TMEM arrangement of the stationary tile is written out for 14 row-blocks");
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    SearchSmem<NI, XS>& sm = *reinterpret_cast<SearchSmem<NI, XS>*>(smem_raw);
+    const uint32_t sb = smem_u32(smem_raw);
     const int team = threadIdx.x >> 8;                       // 0, 1: A teams; 2, 3: B teams
     const int t = threadIdx.x & 255, warp = t >> 5, lane = t & 31;   // within the team
     const int b = blockIdx.x, grp = blockIdx.y, G = gridDim.y;
-    constexpr uint32_t kTileBytes = NI * 256 * sizeof(c2);
-    constexpr uint64_t kTile = (uint64_t)NI * 256;
+    constexpr uint32_t kTileBytes = SM::kTile;
+    constexpr uint64_t kTile = (uint64_t)NI * 256;           // elements
+    int* const abort_flag = A.abort_flag;
+
+    const uint32_t nS = SINGLE ? 1u : A.nS;
+    const uint32_t nTg = A.nT > (uint64_t)grp ? (uint32_t)((A.nT - grp + G - 1) / G) : 0u;   // templates of this group
+    const uint32_t n_items = nTg * nS;                      // < 2^31: the host splits larger searches
+    c2* const myring = A.ring + (uint64_t)grp * kRing * kN;
+    unsigned long long* const d1 = A.done1 + grp * kRing;    // one counter pair per ring slot: a count can only
+    unsigned long long* const d2 = A.done2 + grp * kRing;    // come from the item that currently owns the slot
+    // tile b of template (group-local index tj) / of segment ml
+    auto tpl_tile = [&](uint32_t tj) { return A.bank + ((A.j0 + grp + (uint64_t)G * tj) * 16 + b) * kTile; };
+    auto seg_tile = [&](uint32_t ml) { return A.xseg + ((uint64_t)(A.m0 + ml) * 16 + b) * kTile; };
 
     if (threadIdx.x == 0) {
-        mbar_init(&sm.hfull[0], 1); mbar_init(&sm.hfull[1], 1);
+        mbar_init(sb + SM::bars, 1); mbar_init(sb + SM::bars + 8, 1); mbar_init(sb + SM::bars + 16, 1);
         fence_mbar_init();
     }
-    if (team == 0) {                                         // tbl[r][a] = exp(2 pi i 16 b (a + 16 r) / N)
-        const int r = t >> 4, a = t & 15;
-        double sn, cs;
-        sincospi(2.0 * (double)((16 * b * (a + 16 * r)) & (kN - 1)) / (double)kN, &sn, &cs);
-        sm.tbl[t] = make_float2((float)cs, (float)sn);
-    } else if (team == 1) {                                  // w1t[p][a] = exp(2 pi i a p / 256)
-        const int p = t >> 4, a = t & 15;
-        double sn, cs;
-        sincospi(2.0 * (double)((a * p) & 255) / 256.0, &sn, &cs);
-        sm.w1t[t] = make_float2((float)cs, (float)sn);
-    } else if (XS && team == 2) {
-        const c2* xb = xseg + ((uint64_t)m0 * 16 + b) * kTile;
-        for (int ii = 0; ii < NI; ++ii) sm.xs[XS ? ii * 256 + t : 0] = xb[ii * 256 + t];
+    if (threadIdx.x < 32) tmem_alloc<kTmemCols>(sb + SM::bars + 24);
+    if (!TM_TW) {
+        if (team == 2) {                                     // tbl: exp(2 pi i 16 b (a + 16 r) / N)
+            const int r = t >> 4, a = t & 15;
+            double sn, cs;
+            sincospi(2.0 * (double)((16 * b * (a + 16 * r)) & (kN - 1)) / (double)kN, &sn, &cs);
+            reinterpret_cast<float2*>(smem_raw + SM::tbl)[((r >> 1) * 16 + a) * 2 + (r & 1)] = make_float2((float)cs, (float)sn);
+        } else if (team == 3) {                              // w1t: exp(2 pi i a p / 256)
+            const int p = t >> 4, a = t & 15;
+            double sn, cs;
+            sincospi(2.0 * (double)((a * p) & 255) / 256.0, &sn, &cs);
+            reinterpret_cast<float2*>(smem_raw + SM::w1t)[((p >> 1) * 16 + a) * 2 + (p & 1)] = make_float2((float)cs, (float)sn);
+        }
     }
+    tmem_fence_before_sync();
     __syncthreads();
+    tmem_fence_after_sync();
+    // this warp's lane quadrant of the tensor memory (lane field = bits 16 and up)
+    const uint32_t tq = *reinterpret_cast<volatile uint32_t*>(smem_raw + SM::bars + 24) + ((uint32_t)(warp & 3) << 21);
+    const uint32_t tq_a = tq + 32u * (uint32_t)(warp >> 2);  // pass 1: column block of this warp inside a table
+    // the stationary tile of pass 1 goes from global memory to this thread's TMEM columns (team 0 does it for both)
+    auto stat_to_tmem = [&](const c2* tile) {
+        const ulonglong2* src = reinterpret_cast<const ulonglong2*>(tile) + t;
+#pragma unroll
+        for (int ip = 0; ip < NI / 2; ++ip) {
+            const ulonglong2 q = __ldcg(src + ip * 256);
+            const uint32_t r[4] = {(uint32_t)q.x, (uint32_t)(q.x >> 32), (uint32_t)q.y, (uint32_t)(q.y >> 32)};
+            tmem_st4(tq_a + kTmStat + 4 * ip, r);
+        }
+        tmem_wait_st();
+    };
+    if (team == 0) {
+        if (TM_TW && warp < 4) {                             // delta_p, one copy per lane quadrant
+            const int a = lane & 15;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                uint32_t r[8];
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    double sn, cs;
+                    sincospi(2.0 * (double)((a * (b + 16 * (4 * j + k))) & 4095) / 4096.0, &sn, &cs);
+                    r[2 * k] = __float_as_uint((float)cs); r[2 * k + 1] = __float_as_uint((float)sn);
+                }
+                tmem_st8(tq + kTmDelta + 8 * j, r);
+            }
+        }
+        if (TM_TH) {                                         // theta^p, p = 1 .. 15 (+ one unused entry)
+            const int c = t >> 4, g = t & 15;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                uint32_t r[8];
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const int pp = 4 * j + k + 1;
+                    double sn, cs;
+                    sincospi(2.0 * (double)((pp * (256 * g + 16 * b + c)) & (kN - 1)) / (double)kN, &sn, &cs);
+                    r[2 * k] = __float_as_uint((float)cs); r[2 * k + 1] = __float_as_uint((float)sn);
+                }
+                tmem_st8(tq_a + kTmTheta + 8 * j, r);
+            }
+        }
+        if (TM_ST && n_items > 0) stat_to_tmem(SINGLE ? seg_tile(0) : tpl_tile(0));
+        tmem_wait_st();
+    }
+    tmem_fence_before_sync();
+    __syncthreads();
+    tmem_fence_after_sync();
 
-    const uint32_t nTg = nT > (uint64_t)grp ? (uint32_t)((nT - grp + G - 1) / G) : 0u;   // templates of this group
-    const uint32_t n_items = nTg * nS;                      // < 2^31: the host splits larger searches
-    c2* myring = ring + (uint64_t)grp * kRing * kN;
-    unsigned long long* d1 = done1 + grp * kRing;            // one counter pair per ring slot: a count can only
-    unsigned long long* d2 = done2 + grp * kRing;            // come from the item that currently owns the slot
-
-    if ((BEGE_ABL & 16) && team < 2) return;
-    if ((BEGE_ABL & 32) && team >= 2) return;
-    if (team < 2) {
+    if (team < 2 && !(BEGE_ABL & 16)) {
         // ================================================================ A: pass 1, items it = team (mod 2)
         const int c = t >> 4, g = t & 15;                    // stage 1: column of the tile, lane of its half-warp
         const int c2i = t & 15, p2 = t >> 4;                 // stage 2: column, index p of n2 = p + 16 q
-        c2 theta;                                            // exp(2 pi i (256 g + k1) / N), k1 = 16 b + c
-        {
+        c2 theta = mk(1.f, 0.f);                             // exp(2 pi i (256 g + k1) / N), k1 = 16 b + c
+        if (!TM_TH) {
             double sn, cs;
             sincospi(2.0 * (double)(256 * g + 16 * b + c) / (double)kN, &sn, &cs);
             theta = mk((float)cs, (float)sn);
         }
-        uint64_t* hfull = &sm.hfull[team];
-        c2* hb = sm.hbuf[team];
-        if (t == 0 && (uint32_t)team < n_items && !(BEGE_ABL & 2)) {
-            mbar_arrive_expect_tx(hfull, kTileBytes);
-            bulk_load(hb, bank + ((j0 + grp + (uint64_t)G * (SINGLE ? (uint32_t)team : team / nS)) * 16 + b) * kTile,
-                      kTileBytes, hfull, policy_evict_first());
-        }
-        c2* xw = sm.xch[team] + g * 17 + c;                  // + p * 272: element [p][g][c] of the exchange buffer
-        const c2* xrd = sm.xch[team] + p2 * 272 + c2i;       // + gg * 17
+        const uint32_t bar_stream = sb + SM::bars + 8 * team, bar_stat = sb + SM::bars + 16;
+        const uint32_t stream_buf = sb + SM::stream + team * kTileBytes;
+        const uint32_t stream_a = stream_buf + t * 16, stat_a = sb + SM::stat + t * 16;
+        const uint32_t xw_a = sb + SM::xch + team * SM::kXch + (g * 17 + c) * 8;       // + p * 2176: element [p][g][c]
+        const uint32_t xr_a = sb + SM::xch + team * SM::kXch + (p2 * 272 + c2i) * 8;   // + gg * 136
+        const uint32_t ssig_a = sb + SM::ssig + team * 32;
         const int bar_id = 1 + team;
-        int pending = -1;                                    // ring slot whose tile this warp has yet to publish
+        auto stream_src = [&](uint32_t it) { return SINGLE ? tpl_tile(it) : seg_tile(it % nS); };
+        const ulonglong2* statg = nullptr;
+        if (n_items > 0) {
+            if (STAT && !TM_ST && team == 0 && t == 0) {     // first stationary tile
+                mbar_arrive_expect_tx(bar_stat, kTileBytes);
+                bulk_load(sb + SM::stat, SINGLE ? seg_tile(0) : tpl_tile(0), kTileBytes, bar_stat, policy_evict_last());
+            }
+            if (!STAT) statg = reinterpret_cast<const ulonglong2*>(SINGLE ? seg_tile(0) : tpl_tile(0)) + t;
+            if (t == 0 && (uint32_t)team < n_items && !(BEGE_ABL & 2)) {
+                mbar_arrive_expect_tx(bar_stream, kTileBytes);
+                bulk_load(stream_buf, stream_src(team), kTileBytes, bar_stream, SINGLE ? policy_evict_first() : policy_evict_last());
+            }
+        }
+        int pending = -1;                                    // ring slot whose tile this team has yet to publish
         uint32_t nload = 0;                                  // tiles this team has waited for so far
-        uint32_t tj_prev = ~0u;
+        uint32_t tj_prev = 0;
+        if (STAT && !TM_ST && n_items > 0) mbar_wait(bar_stat, 0, abort_flag);
         for (uint32_t it = team; it < n_items; it += 2) {
             const uint32_t tj = SINGLE ? it : it / nS;
             const uint32_t ml = SINGLE ? 0u : (uint32_t)(it - tj * nS);
             const int slot = (int)(it % kRing);
-            if (tj != tj_prev) {                             // a new template tile was ordered for this item
+            // slot-free counter (ring slot read out by pass 2 of item it - kRing, all 16 CTAs of the group): ONE thread
+            // acquires it, early, so that the L2 round trip is hidden behind stage 1
+            unsigned long long d2v = ~0ull;
+            if (!(BEGE_ABL & 1) && t == 32 && it >= (uint32_t)kRing) d2v = counter_load_acquire(d2 + slot);
+            c2 qa[4], qb[4];                                 // TMEM staging (stationary values, then theta powers)
+            if (TM_ST) tmem_ld8(tq_a + kTmStat, qa);
 #if !(BEGE_ABL & 2)
-                mbar_wait(hfull, nload & 1, abort_flag);
+            mbar_wait(bar_stream, nload & 1, abort_flag);
 #endif
-                ++nload;
+            ++nload;
+            if (!SINGLE && tj != tj_prev) {                  // first item of a template for this team (not the first)
+                if (STAT && !TM_ST) mbar_wait(bar_stat, tj & 1, abort_flag);
+                if (!STAT) statg = reinterpret_cast<const ulonglong2*>(tpl_tile(tj)) + t;
                 tj_prev = tj;
             }
             c2 v[16];
             c2 acc = mk(0.f, 0.f);
-            {
-                const c2* xb = xseg + ((uint64_t)(m0 + ml) * 16 + b) * kTile;
 #pragma unroll
-                for (int r = 0; r < 16; ++r) {
-                    if (r >= I0 && r < I0 + NI) {
-                        const c2 xv = XS ? sm.xs[XS ? (r - I0) * 256 + t : 0] : __ldg(xb + (r - I0) * 256 + t);
-                        v[r] = cmulc(xv, hb[(r - I0) * 256 + t]);
-                        acc = fma2(v[r], v[r], acc);
-                    } else {
-                        v[r] = mk(0.f, 0.f);
-                    }
-                }
+            for (int r = 0; r < 16; ++r) if (r < I0 || r >= I0 + NI) v[r] = mk(0.f, 0.f);
+            if (TM_ST) {
+                tmem_wait_ld(qa); tmem_ld8(tq_a + kTmStat + 8, qb);
+                products2<I0, SINGLE, 0>(stream_a, qa, v, acc);
+                tmem_wait_ld(qb); tmem_ld8(tq_a + kTmStat + 16, qa);
+                products2<I0, SINGLE, 2>(stream_a, qb, v, acc);
+                tmem_wait_ld(qa); tmem_ld8(tq_a + kTmStat + 24, qb);
+                products2<I0, SINGLE, 4>(stream_a, qa, v, acc);
+                tmem_wait_ld(qb);
+                if (TM_TH) tmem_ld8(tq_a + kTmTheta, qa);
+                products2<I0, SINGLE, 6>(stream_a, qb, v, acc, false);
+            } else {
+                if (TM_TH) tmem_ld8(tq_a + kTmTheta, qa);
+                load_products<I0, NI, SINGLE, STAT>(stream_a, stat_a, statg, v, acc);
             }
             fft16<+1>(v);
-            {   // v[p] *= theta^p, powers by a depth-4 product tree
-                const c2 t2 = cmul2(theta, theta), t4 = cmul2(t2, t2), t8 = cmul2(t4, t4);
-                const c2 t3 = cmul2(t2, theta), t5 = cmul2(t4, theta), t6 = cmul2(t4, t2), t7 = cmul2(t4, t3);
-                v[1] = cmul2(v[1], theta); v[2] = cmul2(v[2], t2); v[3] = cmul2(v[3], t3); v[4] = cmul2(v[4], t4);
-                v[5] = cmul2(v[5], t5); v[6] = cmul2(v[6], t6); v[7] = cmul2(v[7], t7); v[8] = cmul2(v[8], t8);
-                v[9] = cmul2(v[9], cmul2(t8, theta)); v[10] = cmul2(v[10], cmul2(t8, t2));
-                v[11] = cmul2(v[11], cmul2(t8, t3)); v[12] = cmul2(v[12], cmul2(t8, t4));
-                v[13] = cmul2(v[13], cmul2(t8, t5)); v[14] = cmul2(v[14], cmul2(t8, t6));
-                v[15] = cmul2(v[15], cmul2(t8, t7));
+            if (TM_TH) {                                     // v[p] *= theta^p, p = 1 .. 15
+                tmem_wait_ld(qa); tmem_ld8(tq_a + kTmTheta + 8, qb);
+                v[1] = cmulw(v[1], qa[0]); v[2] = cmulw(v[2], qa[1]); v[3] = cmulw(v[3], qa[2]); v[4] = cmulw(v[4], qa[3]);
+                tmem_wait_ld(qb); tmem_ld8(tq_a + kTmTheta + 16, qa);
+                v[5] = cmulw(v[5], qb[0]); v[6] = cmulw(v[6], qb[1]); v[7] = cmulw(v[7], qb[2]); v[8] = cmulw(v[8], qb[3]);
+                tmem_wait_ld(qa); tmem_ld8(tq_a + kTmTheta + 24, qb);
+                v[9] = cmulw(v[9], qa[0]); v[10] = cmulw(v[10], qa[1]); v[11] = cmulw(v[11], qa[2]); v[12] = cmulw(v[12], qa[3]);
+                tmem_wait_ld(qb);
+                v[13] = cmulw(v[13], qb[0]); v[14] = cmulw(v[14], qb[1]); v[15] = cmulw(v[15], qb[2]);
+            } else {   // powers by a depth-4 product tree
+                const c2 t2 = cmulw(theta, theta), t3 = cmulw(t2, theta);
+                const c2 t4 = cmulw(t2, t2), t5 = cmulw(t3, t2), t6 = cmulw(t2, t4), t7 = cmulw(t3, t4), t8 = cmulw(t4, t4);
+                v[1] = cmulw(v[1], theta); v[2] = cmulw(v[2], t2); v[3] = cmulw(v[3], t3); v[4] = cmulw(v[4], t4);
+                v[5] = cmulw(v[5], t5); v[6] = cmulw(v[6], t6); v[7] = cmulw(v[7], t7); v[8] = cmulw(v[8], t8);
+                v[9] = cmulw(v[9], cmulw(theta, t8)); v[10] = cmulw(v[10], cmulw(t2, t8));
+                v[11] = cmulw(v[11], cmulw(t3, t8)); v[12] = cmulw(v[12], cmulw(t4, t8));
+                v[13] = cmulw(v[13], cmulw(t5, t8)); v[14] = cmulw(v[14], cmulw(t6, t8));
+                v[15] = cmulw(v[15], cmulw(t7, t8));
             }
-#pragma unroll
-            for (int p = 0; p < 16; ++p) xw[p * 272] = v[p];
+            sts16<2176>(xw_a, v);
             const float sw = warp_sum32(re(acc) + im(acc));
-            if (lane == 0) sm.ssig[team][warp] = sw;
-            bar_team(bar_id);                                // exchange buffer complete, template tile read out
-            if (t == 0 && !(BEGE_ABL & 2)) {                 // order the tile of this team's next item
+            if (lane == 0) sts32(ssig_a + 4 * warp, sw);
+            bar_named(bar_id, 256);                          // exchange buffer complete, both tiles read out
+            if (t == 0 && !(BEGE_ABL & 2)) {                 // order the streaming tile of this team's next item
                 const uint32_t it2 = it + 2;
                 if (it2 < n_items) {
-                    const uint32_t tj2 = SINGLE ? it2 : it2 / nS;
-                    if (tj2 != tj) {
-                        mbar_arrive_expect_tx(hfull, kTileBytes);
-                        bulk_load(hb, bank + ((j0 + grp + (uint64_t)G * tj2) * 16 + b) * kTile, kTileBytes, hfull,
-                                  policy_evict_first());
+                    mbar_arrive_expect_tx(bar_stream, kTileBytes);
+                    bulk_load(stream_buf, stream_src(it2), kTileBytes, bar_stream,
+                              SINGLE ? policy_evict_first() : policy_evict_last());
+                }
+            }
+            if (!SINGLE && STAT) {                           // last item of this template for this team: once both A
+                if (it + 2 >= (tj + 1) * nS && tj + 1 < nTg) {   // teams are past it, bring in the next template's tile
+                    bar_named(3, 512);
+                    if (TM_ST) {
+                        if (team == 0) stat_to_tmem(tpl_tile(tj + 1));
+                        tmem_fence_before_sync();
+                        bar_named(3, 512);
+                        tmem_fence_after_sync();
+                    } else if (team == 0 && t == 0) {
+                        mbar_arrive_expect_tx(bar_stat, kTileBytes);
+                        bulk_load(sb + SM::stat, tpl_tile(tj + 1), kTileBytes, bar_stat, policy_evict_first());
                     }
                 }
             }
-            unsigned long long d2v = ~0ull;                  // slot-free counter, polled early: the load is in flight
-            if (it >= kRing && lane == 0 && !(BEGE_ABL & 1)) d2v = counter_load_relaxed(d2 + slot);   // during stage 2
-#pragma unroll
-            for (int gg = 0; gg < 16; ++gg) v[gg] = xrd[gg * 17];
+            lds16<136>(xr_a, v);
             float tot = 0.f;
-            if (t == 0) {
+            if (t == 64) {
 #pragma unroll
-                for (int w = 0; w < 8; ++w) tot += sm.ssig[team][w];
+                for (int w = 0; w < 8; ++w) tot += lds32(ssig_a + 4 * w);
             }
-            bar_team(bar_id);                                // exchange buffer free for the team's next item
-            if (pending >= 0 && t == 0)                      // the team's stores of its previous item were all issued
-                counter_add_release(d1 + pending, 1ull);     // before this barrier and have long landed
+            if (t == 32 && d2v < 16ull * (it / kRing)) counter_wait_ge(d2 + slot, 16ull * (it / kRing), abort_flag);
+            __syncwarp();
+            bar_named(bar_id, 256);                          // exchange buffer free for the team's next item; slot free
+            // the team's ring stores of its previous item were all issued before the FIRST barrier of this item and
+            // have long landed: the release fence does not wait
+            if (t == 0 && pending >= 0) counter_add_release(d1 + pending, 1ull);
             fft16<+1>(v);
-#if !(BEGE_ABL & 1)
-            if (it >= kRing) {                               // ring slot read out by pass 2 of item it - kRing
-                d2v = __shfl_sync(0xffffffffu, d2v, 0);
-                if (d2v < 128ull * (it / kRing)) warp_counter_wait_ge(d2 + slot, 128ull * (it / kRing), abort_flag, lane);
-            }
-#endif
             c2* out = myring + (uint64_t)slot * kN + 16 * b + c2i + p2 * 256;
 #pragma unroll
             for (int q = 0; q < 16; ++q) {
                 const c2 o = v[q];
                 if (!(BEGE_ABL & 4) || re(o) == 1.2345e-30f) out[q * 4096] = o;
             }
-            if (t == 0) sigpart[((j0 + grp + (uint64_t)G * tj) * (uint64_t)S + (m0 + ml)) * 16 + b] = tot;
+            if (t == 64)
+                A.sigpart[((A.j0 + grp + (uint64_t)G * tj) * (uint64_t)A.S + (A.m0 + ml) - A.sig_pair0) * 16 + b] = tot;
             pending = slot;
         }
-        bar_team(bar_id);
+        bar_named(bar_id, 256);
         if (pending >= 0 && t == 0) counter_add_release(d1 + pending, 1ull);
-    } else {
+    } else if (team >= 2 && !(BEGE_ABL & 32)) {
         // ================================================================ B: pass 2, items ib = team - 2 (mod 2)
         const int kb = team - 2;
         const int hw = t >> 4, a = t & 15;                   // row of the row tile, lane of its half-warp
         const int n2 = 16 * b + hw;
-        c2* priv = sm.bpriv[kb * 16 + hw];
-        c2* pwr = priv + a * 17;                             // + p:      stage-1 output p of lane a
-        const c2* prd = priv + a;                            // + 17 aa:  stage-2 input from lane aa
-        const float2* w1 = sm.w1t + a;                       // + 16 p:   exp(2 pi i a p / 256)
+        const uint32_t priv = sb + SM::bpriv + (kb * 16 + hw) * SM::kPriv;
+        const uint32_t pw_a = priv + a * 136;                // + 8 p:    stage-1 output p of lane a
+        const uint32_t pr_a = priv + a * 8;                  // + 136 aa: stage-2 input from lane aa
+        const uint32_t tbl_a = sb + SM::tbl + a * 16, w1_a = sb + SM::w1t + a * 16;
         const uint64_t row_off = (uint64_t)n2 * 256 + (uint64_t)a;           // T[n2][k1 = a + 16 r]
+        const int bar_id = 4 + kb;
+        int prev_slot = -1;
+        unsigned long long d1v = 0;                          // t == 0: last acquired value of the item's counter
         for (uint32_t ib = kb; ib < n_items; ib += 2) {
             const int slot = (int)(ib % kRing);
-            const uint32_t use = ib / kRing;
             const uint32_t tj = SINGLE ? ib : ib / nS;
             const uint32_t ml = SINGLE ? 0u : (uint32_t)(ib - tj * nS);
             const uint64_t jl = grp + (uint64_t)G * tj;
 #if !(BEGE_ABL & 1)
-            warp_counter_wait_ge(d1 + slot, 16ull * (use + 1), abort_flag, lane);     // all 16 tiles are in the ring
+            if (t == 0 && d1v < 16ull * (ib / kRing + 1))    // all 16 tiles are in the ring
+                counter_wait_ge(d1 + slot, 16ull * (ib / kRing + 1), abort_flag);
 #endif
+            __syncwarp();
+            bar_named(bar_id, 256);                          // ... and every warp of the team is done with its
+            if (t == 224 && prev_slot >= 0)                  // loads of the team's previous item: free that slot
+                counter_add_release(d2 + prev_slot, 1ull);
             const c2* src = myring + (uint64_t)slot * kN + row_off;
             c2 v[16];
 #pragma unroll
             for (int r = 0; r < 16; ++r) v[r] = (BEGE_ABL & 8) ? mk((float)(r + a), (float)ib) : __ldcg(src + 16 * r);
+            const uint64_t pair = (A.j0 + jl) * (uint64_t)A.S + (A.m0 + ml);
+            const float part = __ldcg(A.sigpart + (pair - A.sig_pair0) * 16 + a);
+            // look at the counter of the team's next item now: the answer is there when the item starts
+            d1v = 0;
+            if (!(BEGE_ABL & 1) && t == 0 && ib + 2 < n_items) d1v = counter_load_acquire(d1 + (ib + 2) % kRing);
+            c2 wa[4], wb[4];
+            if (TM_TW) {
+                tmem_ld8(tq + kTmDelta, wa);
+                // four-step factor wN^(16 b k1), k1 = a + 16 r: its CTA-uniform part w256^(b r) here, the rest in delta_p
 #pragma unroll
-            for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], sm.tbl[16 * r + a]);          // wN^(16 k1 q), q = b
-            const uint64_t pair = (j0 + jl) * (uint64_t)S + (m0 + ml);
-            const float sumR2 = hw_sum16(__ldcg(sigpart + pair * 16 + a));
+                for (int r = 1; r < 16; ++r) { const float2 w = c_w256[(b * r) & 255]; v[r] = cmulw(v[r], w.x, w.y); }
+            } else {
+                twiddle16<false>(tbl_a, v);                  // wN^(16 k1 q), q = b
+            }
+            const float sumR2 = hw_sum16(part);
             fft16<+1>(v);
+            if (TM_TW) {                                     // v[p] *= delta_p = wN^(16 b a) w256^(a p)
+                tmem_wait_ld(wa); tmem_ld8(tq + kTmDelta + 8, wb);
+                mul4<0>(v, wa);
+                tmem_wait_ld(wb); tmem_ld8(tq + kTmDelta + 16, wa);
+                mul4<1>(v, wb);
+                tmem_wait_ld(wa); tmem_ld8(tq + kTmDelta + 24, wb);
+                mul4<2>(v, wa);
+                tmem_wait_ld(wb);
+                mul4<3>(v, wb);
+            } else {
+                twiddle16<true>(w1_a, v);                    // w256^(a p)
+            }
+            sts16<8>(pw_a, v);
             __syncwarp();
-            if (lane == 0) counter_add_relaxed(d2 + slot, 1ull);             // this warp's rows are in registers (the
-                                                                             // loads have returned: fft16 consumed them)
-#pragma unroll
-            for (int p = 1; p < 16; ++p) v[p] = cmul(v[p], w1[16 * p]);
-#pragma unroll
-            for (int p = 0; p < 16; ++p) pwr[p] = v[p];
-            __syncwarp();
-#pragma unroll
-            for (int aa = 0; aa < 16; ++aa) v[aa] = prd[aa * 17];
+            lds16<136>(pr_a, v);
             __syncwarp();
             fft16<+1>(v);
             // lane a holds Z[n1 = a + 16 q]; lag n = 256 n1 + n2
-            const float thr = k2 * sumR2;
-            unsigned hits = 0;
+            const float thr = A.k2 * sumR2;
+            bool any = false;
 #pragma unroll
             for (int q = 0; q < 16; ++q) {
-                const c2 sq = mul2(v[q], v[q]);
-                if (re(sq) + im(sq) > thr) hits |= 1u << q;
+                const float zr = re(v[q]), zi = im(v[q]);
+                any |= fmaf(zi, zi, zr * zr) > thr;
             }
-            if (zdbg != nullptr) {
+            if (DBG) {
                 const float invN = 1.0f / (float)kN;
 #pragma unroll
                 for (int q = 0; q < 16; ++q)
-                    zdbg[(uint64_t)(a + 16 * q) * 256 + n2] = mul2(v[q], bc(invN));
+                    A.zdbg[(uint64_t)(a + 16 * q) * 256 + n2] = mul2(v[q], bc(invN));
             }
 #if BEGE_ABL
             if (thr == -1.f)                                 // timing experiment only: never emit
 #endif
-            if (__any_sync(0xffffffffu, hits != 0)) {
-                const float inv = 1.0f / sumR2;
-                if (k2hi < 3.0e38f) {                        // band threshold: drop |z| >= k_hi sigma
-                    const float thr_hi = k2hi * sumR2;
+            if (__any_sync(0xffffffffu, any)) {
+                unsigned hits = 0;
+                float mag[16];
 #pragma unroll
-                    for (int q = 0; q < 16; ++q) {
-                        const c2 sq = mul2(v[q], v[q]);
-                        if (!(re(sq) + im(sq) < thr_hi)) hits &= ~(1u << q);
-                    }
+                for (int q = 0; q < 16; ++q) {
+                    const float zr = re(v[q]), zi = im(v[q]);
+                    mag[q] = fmaf(zi, zi, zr * zr);
+                    if (mag[q] > thr) hits |= 1u << q;
                 }
-                if (cap == ~0ull) {
+                const float inv = 1.0f / sumR2;
+                if (A.k2hi < 3.0e38f) {                      // band threshold: drop |z| >= k_hi sigma
+                    const float thr_hi = A.k2hi * sumR2;
+#pragma unroll
+                    for (int q = 0; q < 16; ++q)
+                        if (!(mag[q] < thr_hi)) hits &= ~(1u << q);
+                }
+                const uint32_t lag0 = (uint32_t)(A.m0 + ml) * (uint32_t)kN + (uint32_t)(a * 256 + n2);   // + 4096 q
+                if (A.cap == ~0ull) {
                     // max projection: per sample offset the largest |z|/sigma over the bank and
                     // its template, race free: one 64-bit atomicMax on (snr bits, ~template_id); positive floats
                     // order like their bit patterns, equal values go to the smaller template id
-                    unsigned long long* proj = reinterpret_cast<unsigned long long*>(rec);
+                    unsigned long long* proj = reinterpret_cast<unsigned long long*>(A.rec);
 #pragma unroll
                     for (int q = 0; q < 16; ++q) {
                         if (hits & (1u << q)) {
-                            const c2 sq = mul2(v[q], v[q]);
-                            const float snr = sqrtf((re(sq) + im(sq)) * inv);
-                            const uint32_t lag = (uint32_t)(m0 + ml) * (uint32_t)kN + (uint32_t)((a + 16 * q) * 256 + n2);
-                            atomicMax(proj + lag, ((unsigned long long)__float_as_uint(snr) << 32) |
-                                                      (unsigned long long)(0xffffffffu - (uint32_t)(j0 + jl)));
+                            const float snr = sqrtf(mag[q] * inv);
+                            atomicMax(proj + lag0 + 4096u * q, ((unsigned long long)__float_as_uint(snr) << 32) |
+                                                                   (unsigned long long)(0xffffffffu - (uint32_t)(A.j0 + jl)));
                         }
                     }
                 } else {
@@ -430,27 +654,33 @@ k_search(const c2* __restrict__ bank, const c2* __restrict__ xseg, c2* __restric
                     }
                     const int total = __shfl_sync(0xffffffffu, incl, 31);
                     unsigned long long base = 0;
-                    if (lane == 31) base = atomicAdd(counter, (unsigned long long)total);
+                    if (lane == 31) base = atomicAdd(A.counter, (unsigned long long)total);
                     base = __shfl_sync(0xffffffffu, base, 31);
                     unsigned long long slot_r = base + (unsigned long long)(incl - cnt);
 #pragma unroll
                     for (int q = 0; q < 16; ++q) {
                         if (hits & (1u << q)) {
-                            if (slot_r < cap) {
-                                const c2 sq = mul2(v[q], v[q]);
+                            if (slot_r < A.cap) {
                                 bege_tail r;
-                                r.template_id = (uint32_t)(j0 + jl);
-                                r.lag = (uint32_t)(m0 + ml) * (uint32_t)kN + (uint32_t)((a + 16 * q) * 256 + n2);
-                                r.snr = sqrtf((re(sq) + im(sq)) * inv);
-                                rec[slot_r] = r;
+                                r.template_id = (uint32_t)(A.j0 + jl);
+                                r.lag = lag0 + 4096u * q;
+                                r.snr = sqrtf(mag[q] * inv);
+                                A.rec[slot_r] = r;
                             }
                             ++slot_r;
                         }
                     }
                 }
             }
+            prev_slot = slot;
         }
+        bar_named(bar_id, 256);
+        if (t == 224 && prev_slot >= 0) counter_add_release(d2 + prev_slot, 1ull);
     }
+    // every warp is done with the tensor memory: give it back
+    tmem_fence_before_sync();
+    __syncthreads();
+    if (threadIdx.x < 32) tmem_dealloc<kTmemCols>(tq);
 }
 
 // sigma_jm = sqrt(sum of the 16 tile partial sums) / N
@@ -490,7 +720,8 @@ struct bege_plan {
     d2 *tw256d = nullptr, *twNd = nullptr;   // exp(2 pi i m / 256), exp(2 pi i m / N) in fp64 (bank generation)
     // workspace
     unsigned char* ws = nullptr; uint64_t ws_bytes = 0, bump = 0; bool user_ws = false;
-    Slot s_bank, s_x, s_scratch, s_sig, s_rec, s_misc, s_par, s_proj;
+    Slot s_bank, s_x, s_scratch, s_sig, s_rec, s_misc, s_par, s_tmp;
+    std::vector<cudaEvent_t> ev_slice;
     uint64_t T = 0; uint32_t S = 0; double tau = 0; uint32_t L = 0;
     bool have_sigma = false;
     // pinned staging
@@ -498,6 +729,8 @@ struct bege_plan {
     cudaEvent_t ev_a = nullptr, ev_b = nullptr, ev_done = nullptr;
     bool profiling = false;
     void* l2_window = nullptr;      // ring region currently marked persisting in L2 (access policy window of the stream)
+    size_t l2_limit_prev = 0; bool l2_limit_saved = false;   // device limit found before the first search
+    uint64_t max_items = ((1ull << 31) - 1) / 2;   // per group and launch (the kernel counts items in 32 bits)
     bege_stats stats{};
     std::string err;
 };
@@ -514,6 +747,7 @@ static void drop_l2_window(bege_plan* p)
     av.accessPolicyWindow.missProp = cudaAccessPropertyNormal;
     cudaStreamSetAttribute(p->stream, cudaStreamAttributeAccessPolicyWindow, &av);
     cudaCtxResetPersistingL2Cache();
+    if (p->l2_limit_saved) cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, p->l2_limit_prev);
     cudaGetLastError();
     p->l2_window = nullptr;
 }
@@ -564,7 +798,18 @@ static uint64_t tpl_bytes(const bege_plan* p) { return (uint64_t)p->NI * 16 * 25
 
 static void count_launch(bege_plan* p, uint64_t n = 1) { p->stats.kernel_launches += n; }
 
-extern "C" const char* bege_version(void) { return "bege 0.1 (sm_100a)"; }
+// the eight instantiations of the search kernel: row-blocks kept (14 / 16), single-segment or batched, debug z output
+static const void* search_variant(int NI, bool single, bool dbg)
+{
+    if (NI == 14) {
+        if (single) return dbg ? (const void*)k_search<1, 14, true, true> : (const void*)k_search<1, 14, true, false>;
+        return dbg ? (const void*)k_search<1, 14, false, true> : (const void*)k_search<1, 14, false, false>;
+    }
+    if (single) return dbg ? (const void*)k_search<0, 16, true, true> : (const void*)k_search<0, 16, true, false>;
+    return dbg ? (const void*)k_search<0, 16, false, true> : (const void*)k_search<0, 16, false, false>;
+}
+
+extern "C" const char* bege_version(void) { return "bege 0.2 (sm_100a)"; }
 
 extern "C" const char* bege_last_error(const bege_plan* p) { return p ? p->err.c_str() : "null plan"; }
 
@@ -581,12 +826,13 @@ extern "C" int bege_plan_create(bege_plan** out, uint32_t N, double fs, double l
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return bail(BEGE_ECUDA);
     if (prop.major < 10) return bail(BEGE_ECUDA);              // sm_100a code only
+    // a caller on the legacy default stream passes cudaStreamLegacy (handle 0 would be indistinguishable from NULL)
     if (stream) p->stream = (cudaStream_t)stream;
     else { if (cudaStreamCreateWithFlags(&p->stream, cudaStreamNonBlocking) != cudaSuccess) return bail(BEGE_ECUDA); p->own_stream = true; }
     if (cudaStreamCreateWithFlags(&p->side, cudaStreamNonBlocking) != cudaSuccess) return bail(BEGE_ECUDA);
     if (cudaEventCreate(&p->ev_a) != cudaSuccess || cudaEventCreate(&p->ev_b) != cudaSuccess ||
         cudaEventCreateWithFlags(&p->ev_done, cudaEventDisableTiming) != cudaSuccess) return bail(BEGE_ECUDA);
-    if (cudaMallocHost(&p->h_count, 64) != cudaSuccess) return bail(BEGE_ECUDA);
+    if (cudaMallocHost(&p->h_count, 8 * (2 + kMaxSlices)) != cudaSuccess) return bail(BEGE_ECUDA);
 
     // band in bins, inclusive edges: klo = ceil(lo N/fs), khi = floor(hi N/fs)
     const double df = fs / N;
@@ -624,6 +870,11 @@ extern "C" int bege_plan_create(bege_plan** out, uint32_t N, double fs, double l
             cudaMemcpy(p->twNd, tN.data(), N * sizeof(d2), cudaMemcpyHostToDevice) != cudaSuccess) return bail(BEGE_ECUDA);
         if (cudaFuncSetAttribute(k_bank_cols64, cudaFuncAttributeMaxDynamicSharedMemorySize, 16 * 256 * (int)sizeof(d2)) != cudaSuccess) return bail(BEGE_ECUDA);
     }
+    {   // exp(2 pi i m / 256) for the search kernel's CTA-uniform twiddles (constant memory of this device's context)
+        std::vector<float2> lin(256);
+        for (int m = 0; m < 256; ++m) lin[m] = make_float2((float)cos(2.0 * M_PI * m / 256.0), (float)sin(2.0 * M_PI * m / 256.0));
+        if (cudaMemcpyToSymbol(c_w256, lin.data(), sizeof(float2) * 256) != cudaSuccess) return bail(BEGE_ECUDA);
+    }
     if (cudaMalloc(&p->tw256, w256.size() * sizeof(float2)) != cudaSuccess ||
         cudaMalloc(&p->twN, wN.size() * sizeof(float2)) != cudaSuccess) return bail(BEGE_ENOMEM);
     if (cudaMemcpy(p->tw256, w256.data(), w256.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess ||
@@ -631,16 +882,13 @@ extern "C" int bege_plan_create(bege_plan** out, uint32_t N, double fs, double l
 
     // the search kernel needs all its CTAs co-resident (groups hand over through global counters)
     int occ = 0;
-    {
-        const void* fs[4] = {(const void*)k_search<1, 14, true>, (const void*)k_search<1, 14, false>,
-                             (const void*)k_search<0, 16, true>, (const void*)k_search<0, 16, false>};
-        const int sms[4] = {search_smem<14, true>(), search_smem<14, false>(), search_smem<16, true>(), search_smem<16, false>()};
-        for (int i = 0; i < 4; ++i) {
-            if (cudaFuncSetAttribute(fs[i], cudaFuncAttributeMaxDynamicSharedMemorySize, sms[i]) != cudaSuccess) return bail(BEGE_ECUDA);
-            int o = 0;
-            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, fs[i], kSearchThreads, sms[i]) != cudaSuccess) return bail(BEGE_ECUDA);
-            occ = i ? std::min(occ, o) : o;
-        }
+    for (int i = 0; i < 8; ++i) {
+        const void* f = search_variant(i >> 2 ? 16 : 14, (i >> 1) & 1, i & 1);
+        const int sm = (i >> 2) ? search_smem<16>() : search_smem<14>();
+        if (cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, sm) != cudaSuccess) return bail(BEGE_ECUDA);
+        int o = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, f, kSearchThreads, sm) != cudaSuccess) return bail(BEGE_ECUDA);
+        occ = i ? std::min(occ, o) : o;
     }
     int coop = 0;
     cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, device);
@@ -659,7 +907,7 @@ extern "C" void bege_plan_destroy(bege_plan* p)
     drop_l2_window(p);
     if (p->side) { cudaStreamSynchronize(p->side); cudaStreamDestroy(p->side); }
     if (p->own_stream && p->stream) cudaStreamDestroy(p->stream);
-    for (Slot* s : {&p->s_bank, &p->s_x, &p->s_scratch, &p->s_sig, &p->s_rec, &p->s_misc, &p->s_par, &p->s_proj}) slot_free(*s);
+    for (Slot* s : {&p->s_bank, &p->s_x, &p->s_scratch, &p->s_sig, &p->s_rec, &p->s_misc, &p->s_par, &p->s_tmp}) slot_free(*s);
     if (p->tw256) cudaFree(p->tw256);
     if (p->twN) cudaFree(p->twN);
     if (p->tw256d) cudaFree(p->tw256d);
@@ -668,6 +916,7 @@ extern "C" void bege_plan_destroy(bege_plan* p)
     if (p->ev_a) cudaEventDestroy(p->ev_a);
     if (p->ev_b) cudaEventDestroy(p->ev_b);
     if (p->ev_done) cudaEventDestroy(p->ev_done);
+    for (cudaEvent_t e : p->ev_slice) cudaEventDestroy(e);
     delete p;
 }
 
@@ -690,6 +939,7 @@ extern "C" int bege_plan_workspace_bytes(const bege_plan* p, uint64_t T, uint32_
     b += al(T * S * 16 * sizeof(float));               // Parseval partial sums
     b += al(std::max<uint64_t>(cap * sizeof(bege_tail), (uint64_t)S * kN * 8));   // records / max-projection array
     b += al(kMiscHdr + (uint64_t)S * kN * sizeof(c2)); // counters + raw segment staging
+    b += al(std::max<uint64_t>(std::max<uint64_t>(T * S * sizeof(float), (uint64_t)S * kN * 8), kN * sizeof(c2) + 256));   // sigma / projection / debug output
     *bytes = b + 4096;
     return BEGE_OK;
 }
@@ -701,7 +951,7 @@ extern "C" int bege_plan_set_workspace(bege_plan* p, void* dev_ptr, uint64_t byt
     CU(p, cudaSetDevice(p->device));
     CU(p, cudaStreamSynchronize(p->stream));
     drop_l2_window(p);
-    for (Slot* s : {&p->s_bank, &p->s_x, &p->s_scratch, &p->s_sig, &p->s_rec, &p->s_misc, &p->s_par, &p->s_proj}) slot_free(*s);
+    for (Slot* s : {&p->s_bank, &p->s_x, &p->s_scratch, &p->s_sig, &p->s_rec, &p->s_misc, &p->s_par, &p->s_tmp}) slot_free(*s);
     p->ws = (unsigned char*)dev_ptr; p->ws_bytes = dev_ptr ? bytes : 0; p->bump = 0; p->user_ws = dev_ptr != nullptr;
     p->T = 0; p->S = 0; p->have_sigma = false;
     return BEGE_OK;
@@ -772,45 +1022,46 @@ extern "C" int bege_segment_load(bege_plan* p, const float* x, uint32_t S)
     return BEGE_OK;
 }
 
-// one cooperative launch of the persistent search kernel over templates [j0, j0 + nT) x segments [m0, m0 + nS)
-static int launch_search(bege_plan* p, const c2* bank, const c2* xs, c2* ring, float* sig, float k2, float k2hi, bege_tail* rec,
-                         uint64_t cap, unsigned char* misc, c2* zdbg, uint64_t j0, uint64_t nT, uint32_t m0, uint32_t nS,
-                         bool first = true)
+// keep the ring's lines resident in L2 for the duration of a search: they are rewritten every few microseconds and
+// must not be written back to HBM in between (ncu: 31 KB of write-back per correlation without this).  Best effort,
+// errors ignored.  The window is taken off the stream again when the search returns (the stream may be the caller's).
+static void set_l2_window(bege_plan* p, void* ring)
 {
-    unsigned long long* counter = (unsigned long long*)misc;
-    int* abort_flag = (int*)(misc + 8);
-    unsigned long long* done1 = (unsigned long long*)(misc + 256);
-    unsigned long long* done2 = (unsigned long long*)(misc + 2048);
+    if (p->l2_window == ring) return;
+    const size_t bytes = (size_t)p->G * kRing * kN * sizeof(c2);
+    if (!p->l2_limit_saved) { cudaDeviceGetLimit(&p->l2_limit_prev, cudaLimitPersistingL2CacheSize); p->l2_limit_saved = true; }
+    cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, bytes);
+    cudaStreamAttrValue av{};
+    av.accessPolicyWindow.base_ptr = ring;
+    av.accessPolicyWindow.num_bytes = bytes;
+    av.accessPolicyWindow.hitRatio = 1.0f;
+    av.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
+    av.accessPolicyWindow.missProp = cudaAccessPropertyStreaming;
+    cudaStreamSetAttribute(p->stream, cudaStreamAttributeAccessPolicyWindow, &av);
+    cudaGetLastError();
+    p->l2_window = ring;
+}
+
+// one cooperative launch of the persistent search kernel over templates [j0, j0 + nT) x segments [m0, m0 + nS)
+static int launch_search(bege_plan* p, const c2* bank, const c2* xs, c2* ring, float* sig, uint64_t sig_pair0, float k2, float k2hi,
+                         bege_tail* rec, uint64_t cap, unsigned char* misc, c2* zdbg, uint64_t j0, uint64_t nT, uint32_t m0,
+                         uint32_t nS, bool first = true)
+{
     // the first launch of a search also clears the record counter and the abort flag (first 16 bytes)
     CU(p, cudaMemsetAsync(misc + (first ? 0 : 16), 0, kMiscHdr - (first ? 0 : 16), p->stream));
     const int G = (int)std::min<uint64_t>((uint64_t)p->G, nT);
     const dim3 grid(16, G);
-    if (p->l2_window != (void*)ring) {
-        // keep the ring's lines resident: they are rewritten every few microseconds and must not be written back
-        // to HBM in between (ncu: 31 KB of write-back per correlation without this); best effort, errors ignored
-        const size_t bytes = (size_t)p->G * kRing * kN * sizeof(c2);
-        cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, bytes);
-        cudaStreamAttrValue av{};
-        av.accessPolicyWindow.base_ptr = (void*)ring;
-        av.accessPolicyWindow.num_bytes = bytes;
-        av.accessPolicyWindow.hitRatio = 1.0f;
-        av.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
-        av.accessPolicyWindow.missProp = cudaAccessPropertyStreaming;
-        cudaStreamSetAttribute(p->stream, cudaStreamAttributeAccessPolicyWindow, &av);
-        cudaGetLastError();
-        p->l2_window = (void*)ring;
-    }
-    const bool single = (p->S == 1);
-    unsigned long long capll = cap;
-    uint32_t S = p->S;
-    void* args[] = {&bank, &xs, &ring, &sig, &k2, &k2hi, &rec, &capll, &counter, &zdbg, &j0, &nT, &m0, &nS, &S,
-                    &done1, &done2, &abort_flag};
-    const void* f = p->NI == 14 ? (single ? (const void*)k_search<1, 14, true> : (const void*)k_search<1, 14, false>)
-                                : (single ? (const void*)k_search<0, 16, true> : (const void*)k_search<0, 16, false>);
-    const int kSearchSmem = p->NI == 14 ? (single ? search_smem<14, true>() : search_smem<14, false>())
-                                        : (single ? search_smem<16, true>() : search_smem<16, false>());
+    set_l2_window(p, (void*)ring);
+    SearchArgs a{};
+    a.bank = bank; a.xseg = xs; a.ring = ring; a.sigpart = sig; a.rec = rec; a.zdbg = zdbg;
+    a.cap = cap; a.counter = (unsigned long long*)misc; a.abort_flag = (int*)(misc + 8);
+    a.done1 = (unsigned long long*)(misc + 256); a.done2 = (unsigned long long*)(misc + 2048);
+    a.j0 = j0; a.nT = nT; a.sig_pair0 = sig_pair0; a.m0 = m0; a.nS = nS; a.S = p->S; a.k2 = k2; a.k2hi = k2hi;
+    void* args[] = {&a};
+    const void* f = search_variant(p->NI, nS == 1, zdbg != nullptr);
+    const int smem = p->NI == 14 ? search_smem<14>() : search_smem<16>();
     if (p->profiling) cudaEventRecord(p->ev_a, p->stream);
-    CU(p, cudaLaunchCooperativeKernel(f, grid, dim3(kSearchThreads), args, kSearchSmem, p->stream));
+    CU(p, cudaLaunchCooperativeKernel(f, grid, dim3(kSearchThreads), args, smem, p->stream));
     count_launch(p);
     if (p->profiling) {
         cudaEventRecord(p->ev_b, p->stream);
@@ -830,6 +1081,19 @@ static int check_abort(bege_plan* p, unsigned char* misc)
     return BEGE_OK;
 }
 
+// template slices of one search: each slice is one launch of the persistent kernel.  Several slices let the copy of
+// slice i's records to the host (side stream) run while slice i + 1 is searched (only the tails cross
+// the bus, and they must not hold up the search); one slice never exceeds the kernel's 32-bit item count per group.
+static uint64_t slice_templates(const bege_plan* p, bool want_overlap)
+{
+    const uint64_t maxT = std::max<uint64_t>(1, p->max_items / p->S) * (uint64_t)p->G;
+    uint64_t n = 1;
+    if (want_overlap) n = std::min<uint64_t>(kMaxSlices, std::max<uint64_t>(1, p->T * p->S / kSliceMinCorr));
+    uint64_t per = (p->T + n - 1) / n;
+    per = (per + p->G - 1) / p->G * p->G;            // whole rounds of the groups
+    return std::min(per, maxT);
+}
+
 static int search_impl(bege_plan* p, float k_sigma, float k_hi, bege_tail* tails_out, uint64_t cap, uint64_t* n_tails)
 {
     if (!p) return BEGE_EINVAL;
@@ -846,27 +1110,50 @@ static int search_impl(bege_plan* p, float k_sigma, float k_hi, bege_tail* tails
     if ((rc = slot_get(p, p->s_bank, 0, &bank))) return rc;
     if ((rc = slot_get(p, p->s_x, 0, &xs))) return rc;
     unsigned long long* counter = (unsigned long long*)misc;
-    // the kernel counts a group's (template, segment) items in 32 bits: split longer searches
-    const uint64_t maxT = std::max<uint64_t>(1, ((1ull << 31) - 1) / p->S / 2) * (uint64_t)p->G;
-    for (uint64_t jj = 0; jj < p->T; jj += maxT) {
-        if ((rc = launch_search(p, (const c2*)bank, (const c2*)xs, (c2*)scr, (float*)sig, k_sigma * k_sigma, k_hi * k_hi,
-                                (bege_tail*)rec, cap, (unsigned char*)misc, nullptr, jj, std::min(maxT, p->T - jj), 0, p->S,
-                                jj == 0))) return rc;
+    const uint64_t per = slice_templates(p, cap > 0);
+    const uint64_t nsl = (p->T + per - 1) / per;
+    // all slices are enqueued at once; after each one its running record count goes to pinned host memory
+    std::vector<cudaEvent_t>& ev = p->ev_slice;
+    while (ev.size() < std::min<uint64_t>(nsl, kMaxSlices)) {
+        cudaEvent_t e; CU(p, cudaEventCreateWithFlags(&e, cudaEventDisableTiming)); ev.push_back(e);
+    }
+    const bool overlap = nsl <= (uint64_t)kMaxSlices;      // more slices only for > 2^31-item searches: no overlap then
+    for (uint64_t i = 0; i < nsl; ++i) {
+        const uint64_t jj = i * per;
+        if ((rc = launch_search(p, (const c2*)bank, (const c2*)xs, (c2*)scr, (float*)sig, 0, k_sigma * k_sigma, k_hi * k_hi,
+                                (bege_tail*)rec, cap, (unsigned char*)misc, nullptr, jj, std::min(per, p->T - jj), 0, p->S,
+                                i == 0))) { drop_l2_window(p); return rc; }
+        if (overlap) {
+            CU(p, cudaMemcpyAsync(p->h_count + 2 + i, counter, sizeof(unsigned long long), cudaMemcpyDeviceToHost, p->stream));
+            CU(p, cudaEventRecord(ev[i], p->stream));
+        }
     }
     CU(p, cudaGetLastError());
-    // only the tails cross PCIe: count first, then exactly the records, on the side stream
     CU(p, cudaMemcpyAsync(p->h_count, counter, sizeof(unsigned long long), cudaMemcpyDeviceToHost, p->stream));
-    CU(p, cudaEventRecord(p->ev_done, p->stream));
-    CU(p, cudaStreamWaitEvent(p->side, p->ev_done, 0));
     CU(p, cudaMemcpyAsync(p->h_count + 1, (unsigned char*)misc + 8, sizeof(int), cudaMemcpyDeviceToHost, p->stream));
+    // only the tails cross PCIe: the records of slice i are complete once slice i has finished, and are
+    // copied on the side stream while the main stream searches slice i + 1
+    uint64_t copied = 0;
+    if (overlap && cap) {
+        for (uint64_t i = 0; i < nsl; ++i) {
+            CU(p, cudaEventSynchronize(ev[i]));
+            const uint64_t upto = std::min<uint64_t>(p->h_count[2 + i], cap);
+            if (upto > copied) {
+                CU(p, cudaMemcpyAsync(tails_out + copied, (bege_tail*)rec + copied, (upto - copied) * sizeof(bege_tail),
+                                      cudaMemcpyDeviceToHost, p->side));
+                copied = upto;
+            }
+        }
+    }
     CU(p, cudaStreamSynchronize(p->stream));
+    drop_l2_window(p);
     if (*(volatile int*)(p->h_count + 1)) return fail(p, BEGE_ECUDA, "search pipeline timed out waiting on a group counter");
     const uint64_t total = *p->h_count;
     const uint64_t ncopy = std::min<uint64_t>(total, cap);
-    if (ncopy) {
-        CU(p, cudaMemcpyAsync(tails_out, rec, ncopy * sizeof(bege_tail), cudaMemcpyDeviceToHost, p->side));
-        CU(p, cudaStreamSynchronize(p->side));
-    }
+    if (ncopy > copied)
+        CU(p, cudaMemcpyAsync(tails_out + copied, (bege_tail*)rec + copied, (ncopy - copied) * sizeof(bege_tail),
+                              cudaMemcpyDeviceToHost, p->side));
+    CU(p, cudaStreamSynchronize(p->side));
     p->stats.correlations += p->T * p->S;
     p->have_sigma = true;
     *n_tails = total;
@@ -885,49 +1172,60 @@ extern "C" int bege_search_band(bege_plan* p, float k_lo, float k_hi, bege_tail*
     return search_impl(p, k_lo, k_hi, tails_out, cap, n_tails);
 }
 
+// max projection: unpack (snr bits, ~template_id) keys into the two output arrays and count the offsets that hold a tail
+__global__ void k_proj_decode(const unsigned long long* __restrict__ proj, float* __restrict__ snr, uint32_t* __restrict__ id,
+                              unsigned long long* __restrict__ hits, uint64_t n)
+{
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    bool hit = false;
+    if (i < n) {
+        const unsigned long long key = proj[i];
+        hit = key != 0ull;
+        snr[i] = hit ? __uint_as_float((uint32_t)(key >> 32)) : 0.f;
+        id[i] = hit ? 0xffffffffu - (uint32_t)key : 0xffffffffu;
+    }
+    const unsigned m = __ballot_sync(0xffffffffu, hit);
+    if ((threadIdx.x & 31) == 0 && m) atomicAdd(hits, (unsigned long long)__popc(m));
+}
+
 extern "C" int bege_search_maxproj(bege_plan* p, float k_sigma, float* snr_out, uint32_t* id_out, uint64_t* n_hits)
 {
     if (!p) return BEGE_EINVAL;
     if (!snr_out || !id_out || !(k_sigma >= 0.f)) return fail(p, BEGE_EINVAL, "bad search arguments");
     if (!p->T || !p->S) return fail(p, BEGE_ESTATE, "bege_search_maxproj needs a generated bank and loaded segments");
     CU(p, cudaSetDevice(p->device));
-    void *sig, *proj, *misc, *scr, *bank, *xs;
+    void *sig, *proj, *misc, *scr, *bank, *xs, *tmp;
     int rc;
     const uint64_t n = (uint64_t)p->S * kN;
     if ((rc = slot_get(p, p->s_sig, p->T * p->S * 16 * sizeof(float), &sig))) return rc;
     if ((rc = slot_get(p, p->s_rec, n * sizeof(unsigned long long), &proj))) return rc;
     if ((rc = slot_get(p, p->s_misc, kMiscHdr, &misc))) return rc;
     if ((rc = slot_get(p, p->s_scratch, scratch_bytes(p), &scr))) return rc;
+    if ((rc = slot_get(p, p->s_tmp, n * 8, &tmp))) return rc;
     if ((rc = slot_get(p, p->s_bank, 0, &bank))) return rc;
     if ((rc = slot_get(p, p->s_x, 0, &xs))) return rc;
     CU(p, cudaMemsetAsync(proj, 0, n * sizeof(unsigned long long), p->stream));
-    const uint64_t maxT = std::max<uint64_t>(1, ((1ull << 31) - 1) / p->S / 2) * (uint64_t)p->G;
-    for (uint64_t jj = 0; jj < p->T; jj += maxT) {
+    const uint64_t per = slice_templates(p, false);
+    for (uint64_t jj = 0; jj < p->T; jj += per) {
         // cap = ~0 switches the kernel's epilogue from appending records to the projection array passed as `rec`
-        if ((rc = launch_search(p, (const c2*)bank, (const c2*)xs, (c2*)scr, (float*)sig, k_sigma * k_sigma, INFINITY,
-                                (bege_tail*)proj, ~0ull, (unsigned char*)misc, nullptr, jj, std::min(maxT, p->T - jj), 0, p->S,
-                                jj == 0))) return rc;
+        if ((rc = launch_search(p, (const c2*)bank, (const c2*)xs, (c2*)scr, (float*)sig, 0, k_sigma * k_sigma, INFINITY,
+                                (bege_tail*)proj, ~0ull, (unsigned char*)misc, nullptr, jj, std::min(per, p->T - jj), 0, p->S,
+                                jj == 0))) { drop_l2_window(p); return rc; }
     }
     CU(p, cudaGetLastError());
-    std::vector<unsigned long long> host(n);
-    CU(p, cudaMemcpyAsync(host.data(), proj, n * sizeof(unsigned long long), cudaMemcpyDeviceToHost, p->stream));
-    if ((rc = check_abort(p, (unsigned char*)misc))) return rc;      // synchronises the stream
-    uint64_t hits = 0;
-    for (uint64_t i = 0; i < n; ++i) {
-        const unsigned long long key = host[i];
-        if (key) {
-            const uint32_t bits = (uint32_t)(key >> 32);
-            memcpy(&snr_out[i], &bits, sizeof(float));
-            id_out[i] = 0xffffffffu - (uint32_t)key;
-            ++hits;
-        } else {
-            snr_out[i] = 0.f;
-            id_out[i] = 0xffffffffu;
-        }
-    }
+    float* d_snr = (float*)tmp; uint32_t* d_id = (uint32_t*)(d_snr + n);
+    unsigned long long* d_hits = (unsigned long long*)((unsigned char*)misc + 16);      // cleared by the first launch
+    k_proj_decode<<<(unsigned)((n + 255) / 256), 256, 0, p->stream>>>((const unsigned long long*)proj, d_snr, d_id, d_hits, n);
+    count_launch(p);
+    CU(p, cudaMemcpyAsync(snr_out, d_snr, n * sizeof(float), cudaMemcpyDeviceToHost, p->stream));
+    CU(p, cudaMemcpyAsync(id_out, d_id, n * sizeof(uint32_t), cudaMemcpyDeviceToHost, p->stream));
+    CU(p, cudaMemcpyAsync(p->h_count, d_hits, sizeof(unsigned long long), cudaMemcpyDeviceToHost, p->stream));
+    rc = check_abort(p, (unsigned char*)misc);      // synchronises the stream
+    drop_l2_window(p);
+    if (rc) return rc;
     p->stats.correlations += p->T * p->S;
     p->have_sigma = true;
-    if (n_hits) *n_hits = hits;
+    if (n_hits) *n_hits = *p->h_count;
     return BEGE_OK;
 }
 
@@ -937,15 +1235,14 @@ extern "C" int bege_get_sigma(bege_plan* p, float* sigma_out)
     if (!p->have_sigma) return fail(p, BEGE_ESTATE, "bege_get_sigma needs a completed bege_search");
     CU(p, cudaSetDevice(p->device));
     const uint64_t n = p->T * p->S;
-    float* d = nullptr;
-    CU(p, cudaMalloc(&d, n * sizeof(float)));
-    void* sig; slot_get(p, p->s_sig, 0, &sig);
-    k_sigma<<<(unsigned)((n + 255) / 256), 256, 0, p->stream>>>((const float*)sig, d, n);
+    void *sig, *tmp;
+    int rc;
+    if ((rc = slot_get(p, p->s_sig, 0, &sig))) return rc;
+    if ((rc = slot_get(p, p->s_tmp, n * sizeof(float), &tmp))) return rc;
+    k_sigma<<<(unsigned)((n + 255) / 256), 256, 0, p->stream>>>((const float*)sig, (float*)tmp, n);
     count_launch(p);
-    cudaError_t e = cudaMemcpyAsync(sigma_out, d, n * sizeof(float), cudaMemcpyDeviceToHost, p->stream);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
-    cudaFree(d);
-    CU(p, e);
+    CU(p, cudaMemcpyAsync(sigma_out, tmp, n * sizeof(float), cudaMemcpyDeviceToHost, p->stream));
+    CU(p, cudaStreamSynchronize(p->stream));
     return BEGE_OK;
 }
 
@@ -955,34 +1252,41 @@ extern "C" int bege_debug_correlate(bege_plan* p, uint64_t j, uint32_t m, float*
     if (!p->T || !p->S) return fail(p, BEGE_ESTATE, "needs a bank and segments");
     if (j >= p->T || m >= p->S) return fail(p, BEGE_EINVAL, "pair (%llu, %u) out of range", (unsigned long long)j, m);
     CU(p, cudaSetDevice(p->device));
-    void *scr, *bank, *xs, *misc;
+    void *scr, *bank, *xs, *misc, *tmp;
     int rc;
     if ((rc = slot_get(p, p->s_scratch, scratch_bytes(p), &scr))) return rc;
     if ((rc = slot_get(p, p->s_misc, kMiscHdr, &misc))) return rc;
-    slot_get(p, p->s_bank, 0, &bank); slot_get(p, p->s_x, 0, &xs);
-    c2* zd = nullptr; float* sg = nullptr;
-    CU(p, cudaMalloc(&zd, kN * sizeof(c2)));
-    CU(p, cudaMalloc(&sg, 16 * sizeof(float)));         // private partial sums of this one pair
+    if ((rc = slot_get(p, p->s_tmp, kN * sizeof(c2) + 256, &tmp))) return rc;
+    if ((rc = slot_get(p, p->s_bank, 0, &bank))) return rc;
+    if ((rc = slot_get(p, p->s_x, 0, &xs))) return rc;
+    c2* zd = (c2*)tmp;
+    float* sg = (float*)((unsigned char*)tmp + kN * sizeof(c2));     // private partial sums of this one pair
     const bool prof = p->profiling; p->profiling = false;
-    // the kernel indexes the partial sums by (j*S + m)*16: bias the base so that this pair lands on sg[0..15]
-    float* sg_biased = sg - (j * p->S + m) * 16;
-    rc = launch_search(p, (const c2*)bank, (const c2*)xs, (c2*)scr, sg_biased, 1e30f, INFINITY, nullptr, 0, (unsigned char*)misc, zd, j, 1, m, 1);
+    // sig_pair0 = this pair's index, so that its partial sums land on sg[0..15]
+    rc = launch_search(p, (const c2*)bank, (const c2*)xs, (c2*)scr, sg, j * p->S + m, 1e30f, INFINITY, nullptr, 0,
+                       (unsigned char*)misc, zd, j, 1, m, 1);
     p->profiling = prof;
     if (!rc) rc = check_abort(p, (unsigned char*)misc);
-    if (rc) { cudaFree(zd); cudaFree(sg); return rc; }
+    drop_l2_window(p);
+    if (rc) return rc;
     float part[16];
-    cudaError_t e = cudaMemcpyAsync(z_out, zd, kN * sizeof(c2), cudaMemcpyDeviceToHost, p->stream);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(part, sg, sizeof part, cudaMemcpyDeviceToHost, p->stream);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
-    if (e == cudaSuccess) e = cudaGetLastError();
-    cudaFree(zd); cudaFree(sg);
-    CU(p, e);
+    CU(p, cudaMemcpyAsync(z_out, zd, kN * sizeof(c2), cudaMemcpyDeviceToHost, p->stream));
+    CU(p, cudaMemcpyAsync(part, sg, sizeof part, cudaMemcpyDeviceToHost, p->stream));
+    CU(p, cudaStreamSynchronize(p->stream));
     if (sigma_out) {
         float v[16];
         for (int a = 0; a < 16; ++a) v[a] = part[a];
         for (int d = 8; d >= 1; d >>= 1) for (int a = 0; a < d; ++a) v[a] = v[a] + v[a + d];
         *sigma_out = sqrtf(v[0]) / (float)kN;
     }
+    return BEGE_OK;
+}
+
+extern "C" int bege_debug_set_max_items(bege_plan* p, uint64_t max_items)
+{
+    if (!p) return BEGE_EINVAL;
+    if (max_items == 0 || max_items > ((1ull << 31) - 1) / 2) return fail(p, BEGE_EINVAL, "max_items outside [1, 2^30)");
+    p->max_items = max_items;
     return BEGE_OK;
 }
 
@@ -994,7 +1298,7 @@ static void untile(const bege_plan* p, const std::vector<float2>& tile, float* o
         for (int ii = 0; ii < p->NI; ++ii)
             for (int c = 0; c < 16; ++c)
                 for (int g = 0; g < 16; ++g) {
-                    const float2 v = tile[(((size_t)b * p->NI + ii) * 16 + c) * 16 + g];
+                    const float2 v = tile[((((size_t)b * (p->NI / 2) + ii / 2) * 256) + 16 * c + g) * 2 + (ii & 1)];
                     const size_t k = (size_t)(16 * b + c) + 256 * (size_t)(g + 16 * (ii + p->I0));
                     out[2 * k] = v.x; out[2 * k + 1] = v.y;
                 }

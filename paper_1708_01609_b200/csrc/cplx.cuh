@@ -3,10 +3,13 @@
 // A complex number lives in one 64-bit register pair as (re, im) and is processed with Blackwell's
 // packed fp32x2 instructions (PTX add/sub/mul/fma.rn.f32x2 -> SASS FADD2/FMUL2/FFMA2).  ptxas folds
 // the half swap (mk(im, re)) and the scalar broadcast (mk(s, s)) written below into operand
-// modifiers (.F32x2.LO_HI, .F32), so a complex add is 1 issue slot, a twiddle multiply 2, and a
-// multiplication by +-i fuses into the following add.  Measured on B200: FFMA2 issues at half the
-// rate of FFMA, i.e. the same flops in half the issue slots, which is what leaves room for the
-// load / shared-memory / integer instructions of the FFT passes.
+// modifiers (.F32x2.LO_HI, .F32), so a complex add is 1 issue slot and a twiddle multiply 2.
+// Measured on B200: FFMA2 issues at half the rate of FFMA, i.e. the same flops in half the issue
+// slots, which is what leaves room for the load / shared-memory / integer instructions of the FFT.
+//
+// The packed instructions have no per-half sign, so the cross terms of a multiplication by a RUN-TIME complex
+// number w = (c, d) are two scalar FFMAs (free operand negation, same FMA-pipe time as one FFMA2): 3 issue slots
+// and no sign/pack moves.  Compile-time twiddles keep the 2-slot packed form with an immediate (-d, d) pair.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -18,8 +21,8 @@ typedef unsigned long long c2;   // packed (re, im), fp32 each
 #define BEGE_D __device__ __forceinline__
 
 BEGE_D c2 mk(float re, float im) { c2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(re), "f"(im)); return r; }
-BEGE_D float re(c2 v) { float a, b; asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); return a; }
-BEGE_D float im(c2 v) { float a, b; asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); return b; }
+BEGE_D float re(c2 v) { float a, b; asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); (void)b; return a; }
+BEGE_D float im(c2 v) { float a, b; asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); (void)a; return b; }
 BEGE_D c2 from_f2(float2 v) { return mk(v.x, v.y); }
 BEGE_D float2 to_f2(c2 v) { return make_float2(re(v), im(v)); }
 
@@ -35,13 +38,19 @@ BEGE_D c2 bc(float s) { return mk(s, s); }
 BEGE_D c2 add_i(c2 a, c2 b) { return fma2(swp(b), mk(-1.f, 1.f), a); }
 BEGE_D c2 sub_i(c2 a, c2 b) { return fma2(swp(b), mk(1.f, -1.f), a); }
 
-// x * (c + i d)
+// x * (c + i d), c and d compile-time constants (the pair is an immediate)
 BEGE_D c2 cmul(c2 x, float c, float d) { return fma2(swp(x), mk(-d, d), mul2(x, bc(c))); }
-BEGE_D c2 cmul(c2 x, float2 w) { return cmul(x, w.x, w.y); }
-// conj(h) * x
+// x * w, w a run-time number:  (xr c, xi c) + (-xi d, xr d)
+BEGE_D c2 cmulw(c2 x, float c, float d) {
+    const c2 t = mul2(x, bc(c));
+    return mk(fmaf(-im(x), d, re(t)), fmaf(re(x), d, im(t)));
+}
+BEGE_D c2 cmulw(c2 x, c2 w) { return cmulw(x, re(w), im(w)); }
+BEGE_D c2 cmul(c2 x, float2 w) { return cmulw(x, w.x, w.y); }
+// conj(h) * x = x * conj(h):  (xr hr, xi hr) + (xi hi, -xr hi)
 BEGE_D c2 cmulc(c2 x, c2 h) {
-    const float hr = re(h), hi = im(h);
-    return fma2(swp(x), mk(hi, -hi), mul2(x, bc(hr)));
+    const c2 t = mul2(x, bc(re(h)));
+    return mk(fmaf(im(x), im(h), re(t)), fmaf(-re(x), im(h), im(t)));
 }
 
 // 4-point DFT, DIR = +1: exp(+2 pi i jk/4) (inverse), DIR = -1: forward.  In place, natural order.
