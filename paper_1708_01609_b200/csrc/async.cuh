@@ -43,6 +43,17 @@ BEGE_DA void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes)
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory");
 }
+BEGE_DA void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(bar) : "memory");
+}
+BEGE_DA bool mbar_test_wait(uint32_t bar, uint32_t parity)      // non-blocking probe
+{
+    uint32_t ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0;
+}
 BEGE_DA bool mbar_try_wait(uint32_t bar, uint32_t parity)
 {
     uint32_t ok;
@@ -87,6 +98,17 @@ BEGE_DA void bulk_load(uint32_t smem_dst, const void* gmem_src, uint32_t bytes, 
                  :: "r"(smem_dst), "l"(gmem_src), "r"(bytes), "r"(bar), "l"(policy) : "memory");
 }
 
+// shared -> global, joins the issuing thread's current bulk async-group (the TMA engine drains it in the background)
+BEGE_DA void bulk_store(void* gmem_dst, uint32_t smem_src, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" :: "l"(gmem_dst), "r"(smem_src), "r"(bytes) : "memory");
+}
+BEGE_DA void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+BEGE_DA void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }   // sources reusable
+BEGE_DA void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }             // writes performed
+// generic-proxy writes to shared memory -> visible to the async proxy (TMA) of this CTA
+BEGE_DA void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
 // ---- tensor memory (TMEM, 512 columns x 128 lanes x 32 bit per SM), used here as a second register file for
 // loop-invariant per-thread tables: tcgen05.ld/st have their own datapath and take nothing from the L1/LSU data pipe
 // that the FFT exchanges saturate.  Shape 32x32b: thread i of a warp reads/writes lane 32 (warp % 4) + i, N columns.
@@ -112,21 +134,19 @@ BEGE_DA void tmem_st4(uint32_t taddr, const uint32_t (&r)[4])
                  :: "r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]) : "memory");
 }
 BEGE_DA void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
-// asynchronous load of 4 complex numbers (8 columns); the values may be used only after tmem_wait_ld on the same array
-BEGE_DA void tmem_ld8(uint32_t taddr, unsigned long long (&w)[4])
+// asynchronous load of 2 complex numbers (4 columns); the values may be used only after tmem_wait_ld on the same array
+BEGE_DA void tmem_ld4(uint32_t taddr, unsigned long long (&w)[2])
 {
-    uint32_t r0, r1, r2, r3, r4, r5, r6, r7;
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
-                 : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3), "=r"(r4), "=r"(r5), "=r"(r6), "=r"(r7) : "r"(taddr));
+    uint32_t r0, r1, r2, r3;
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3) : "r"(taddr));
     asm("mov.b64 %0, {%1, %2};" : "=l"(w[0]) : "r"(r0), "r"(r1));
     asm("mov.b64 %0, {%1, %2};" : "=l"(w[1]) : "r"(r2), "r"(r3));
-    asm("mov.b64 %0, {%1, %2};" : "=l"(w[2]) : "r"(r4), "r"(r5));
-    asm("mov.b64 %0, {%1, %2};" : "=l"(w[3]) : "r"(r6), "r"(r7));
 }
 // waits for all tcgen05.ld of this thread; the array is an in/out operand so that no use can be scheduled above it
-BEGE_DA void tmem_wait_ld(unsigned long long (&w)[4])
+BEGE_DA void tmem_wait_ld(unsigned long long (&w)[2])
 {
-    asm volatile("tcgen05.wait::ld.sync.aligned;" : "+l"(w[0]), "+l"(w[1]), "+l"(w[2]), "+l"(w[3]) :: "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" : "+l"(w[0]), "+l"(w[1]) :: "memory");
 }
 
 // ---- named barrier of `nthreads` threads
@@ -136,6 +156,11 @@ BEGE_DA void bar_named(int id, int nthreads) { asm volatile("bar.sync %0, %1;" :
 BEGE_DA void counter_add_release(unsigned long long* ctr, unsigned long long v)
 {
     asm volatile("red.release.gpu.global.add.u64 [%0], %1;" :: "l"(ctr), "l"(v) : "memory");
+}
+BEGE_DA void fence_acq_rel_gpu() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
+BEGE_DA void counter_add_relaxed(unsigned long long* ctr, unsigned long long v)
+{
+    asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" :: "l"(ctr), "l"(v) : "memory");
 }
 BEGE_DA unsigned long long counter_load_acquire(const unsigned long long* ctr)
 {

@@ -183,7 +183,19 @@ k_fwd_cols(const c2* __restrict__ G, c2* __restrict__ out, uint64_t out_stride, 
 // n2 = p + 16 q is split into wN^(k1 p), folded into theta = exp(2 pi i (256 g + k1) / N) of pass 1, and
 // wN^(16 k1 q), applied by pass 2 to its inputs (q = n2 >> 4 is the CTA's tile index there: a 16 x 16 table in
 // shared memory); theta and the tables are rounded once from fp64 angles.
-constexpr int kRing = 8;
+#ifndef BEGE_BTMA
+#define BEGE_BTMA 1        // 1: pass 2 gets its 16 ring rows by one bulk copy into shared memory (0: global loads)
+#endif
+#ifndef BEGE_TMAST
+#define BEGE_TMAST 0       // 1: ring tiles leave through per-warp bulk copies from the exchange buffer instead of direct stores
+#endif
+#ifndef BEGE_X
+#define BEGE_X 0           // timing experiments only (results invalid): 1 publish before the copy completes, 2 no fences
+#endif
+#ifndef BEGE_RING
+#define BEGE_RING 8
+#endif
+constexpr int kRing = BEGE_RING;
 constexpr int kSearchThreads = 32 * 32;
 
 // Loop-invariant per-thread tables live in tensor memory (read with tcgen05.ld: no L1/LSU wavefronts):
@@ -212,16 +224,24 @@ struct SearchArgs {
 template <int NI, bool STAT> struct SearchSmem {
     static constexpr uint32_t kTile = NI * 256 * 8;              // one column tile of a spectrum
     static constexpr uint32_t kXch = 16 * 16 * 17 * 8;           // padded pass-1 exchange buffer, [p][g][c]
-    static constexpr uint32_t kPriv = 16 * 17 * 8;               // padded private region of a pass-2 half-warp
+    static constexpr uint32_t kPriv = 16 * 17 * 8;               // padded private region of a pass-2 half-warp (BEGE_BTMA = 0)
+    static constexpr int kNB = NI <= 14 ? 3 : 2;                 // 32 KiB row tiles of pass 2 (BEGE_BTMA = 1)
     static constexpr uint32_t stream = 0;                        // [2]  streaming tile of each A team
-    static constexpr uint32_t stat = stream + 2 * kTile;         //      stationary tile (if STAT)
-    static constexpr uint32_t xch = stat + (STAT ? kTile : 0);   // [2]
-    static constexpr uint32_t bpriv = xch + 2 * kXch;            // [32]
-    static constexpr uint32_t tbl = bpriv + 32 * kPriv;          // wN^(16 b k1), k1 = a + 16 r, [r/2][a][r&1] (pass 2)
-    static constexpr uint32_t w1t = tbl + 2048;                  // w256^(a p), [p/2][a][p&1]
-    static constexpr uint32_t ssig = w1t + 2048;                 // [2][8] Parseval partial sums of the A warps
+    static constexpr uint32_t xch = stream + 2 * kTile;          // [2]
+    static constexpr uint32_t bpriv = xch + 2 * kXch;            // [32] private regions / [kNB] row tiles
+    static constexpr uint32_t kBBytes = BEGE_BTMA ? kNB * 32768 : 32 * kPriv;
+    static constexpr uint32_t stat = bpriv + kBBytes;            //      stationary tile in shared memory (only if !TMEM)
+    static constexpr uint32_t tbl = stat + ((STAT && !(BEGE_TM & 2)) ? kTile : 0);   // (BEGE_TM & 1) == 0 only
+    static constexpr uint32_t w1t = tbl + ((BEGE_TM & 1) ? 0 : 2048);
+    static constexpr uint32_t ssig = w1t + ((BEGE_TM & 1) ? 0 : 2048);   // [2][8] Parseval partial sums of the A warps
     static constexpr uint32_t bars = ssig + 64;                  // mbarriers: stream[2], stat; TMEM base address @ +24
-    static constexpr uint32_t total = bars + 32;
+    static constexpr uint32_t amb = bars + 32;                   // [kRing] mbarriers: tile of ring slot stored (8 A warps)
+    static constexpr uint32_t xfree = amb + 8 * kRing;           // [2] mbarriers: exchange buffer of an A team drained
+    static constexpr uint32_t bfull = xfree + 16;                // [kNB] mbarriers: row tile has arrived
+    static constexpr uint32_t bempty = bfull + 24;               // [kNB] mbarriers: ... has been read out (8 B warps)
+    static constexpr uint32_t bgo = bempty + 24;                 // [2] mbarriers: the B team's next row tile is there (thread 0)
+    static constexpr uint32_t total = bgo + 16;
+    static_assert(total + 128 <= 232448, "shared memory of one SM");
 };
 // the stationary tile fits next to everything else only for bands that need 14 of the 16 row-blocks
 template <int NI> __host__ __device__ constexpr bool search_stat() { return NI <= 14; }
@@ -266,27 +286,39 @@ BEGE_D void load_products(uint32_t stream_a, uint32_t stat_a, const ulonglong2* 
     }
 }
 
-// v[4 j + k] *= w[k]
-template <int J> BEGE_D void mul4(c2 (&v)[16], const c2 (&w)[4])
-{
-#pragma unroll
-    for (int k = 0; k < 4; ++k) v[4 * J + k] = cmulw(v[4 * J + k], w[k]);
-}
-// products of two row-block pairs: streaming tile from shared memory, stationary values q[0..3] from tensor memory
-template <int I0, bool SINGLE, int IP> BEGE_D void products2(uint32_t stream_a, const c2 (&q)[4], c2 (&v)[16], c2& acc, bool second = true)
+// products of one row-block pair: streaming tile from shared memory, stationary values q[0..1] from tensor memory
+template <int I0, bool SINGLE, int IP> BEGE_D void products1(uint32_t stream_a, const c2 (&q)[2], c2 (&v)[16], c2& acc)
 {
     c2 s0, s1;
     lds128<IP * 4096>(stream_a, s0, s1);
-    c2 r0 = SINGLE ? cmulc(q[0], s0) : cmulc(s0, q[0]);
-    c2 r1 = SINGLE ? cmulc(q[1], s1) : cmulc(s1, q[1]);
-    v[I0 + 2 * IP] = r0; v[I0 + 2 * IP + 1] = r1;
+    const c2 r0 = SINGLE ? cmulc(q[0], s0) : cmulc(s0, q[0]);
+    const c2 r1 = SINGLE ? cmulc(q[1], s1) : cmulc(s1, q[1]);
+    v[I0 + 2 * IP] = r0; v[(I0 + 2 * IP + 1) & 15] = r1;
     acc = fma2(r0, r0, acc); acc = fma2(r1, r1, acc);
-    if (second) {
-        lds128<(IP + 1) * 4096>(stream_a, s0, s1);
-        r0 = SINGLE ? cmulc(q[2], s0) : cmulc(s0, q[2]);
-        r1 = SINGLE ? cmulc(q[3], s1) : cmulc(s1, q[3]);
-        v[(I0 + 2 * IP + 2) & 15] = r0; v[(I0 + 2 * IP + 3) & 15] = r1;
-        acc = fma2(r0, r0, acc); acc = fma2(r1, r1, acc);
+}
+// v[P0 + 2 j + k] *= table entry (2 j + k), entries streamed from tensor memory two at a time, double buffered;
+// the load of chunk 0 into wa was issued by the caller; chunks [0, NCH)
+template <int P0, int NCH, int J = 0> BEGE_D void tm_twiddle(uint32_t taddr, c2 (&v)[16], c2 (&wa)[2], c2 (&wb)[2])
+{
+    if constexpr (J < NCH) {
+        c2 (&cur)[2] = (J & 1) ? wb : wa;
+        c2 (&nxt)[2] = (J & 1) ? wa : wb;
+        tmem_wait_ld(cur);
+        if constexpr (J + 1 < NCH) tmem_ld4(taddr + 4 * (J + 1), nxt);
+        v[P0 + 2 * J] = cmulw(v[P0 + 2 * J], cur[0]);
+        if constexpr (P0 + 2 * J + 1 < 16) v[P0 + 2 * J + 1] = cmulw(v[P0 + 2 * J + 1], cur[1]);
+        tm_twiddle<P0, NCH, J + 1>(taddr, v, wa, wb);
+    }
+}
+template <int I0, bool SINGLE, int IP = 0> BEGE_D void tm_products(uint32_t stream_a, uint32_t taddr, c2 (&v)[16], c2& acc, c2 (&qa)[2], c2 (&qb)[2])
+{
+    if constexpr (IP < 7) {
+        c2 (&cur)[2] = (IP & 1) ? qb : qa;
+        c2 (&nxt)[2] = (IP & 1) ? qa : qb;
+        tmem_wait_ld(cur);
+        if constexpr (IP + 1 < 7) tmem_ld4(taddr + 4 * (IP + 1), nxt);
+        products1<I0, SINGLE, IP>(stream_a, cur, v, acc);
+        tm_products<I0, SINGLE, IP + 1>(stream_a, taddr, v, acc, qa, qb);
     }
 }
 
@@ -322,6 +354,10 @@ k_search(const __grid_constant__ SearchArgs A)
 
     if (threadIdx.x == 0) {
         mbar_init(sb + SM::bars, 1); mbar_init(sb + SM::bars + 8, 1); mbar_init(sb + SM::bars + 16, 1);
+        for (int i = 0; i < kRing; ++i) mbar_init(sb + SM::amb + 8 * i, 8);
+        mbar_init(sb + SM::xfree, 8); mbar_init(sb + SM::xfree + 8, 8);
+        for (int i = 0; i < SM::kNB; ++i) { mbar_init(sb + SM::bfull + 8 * i, 1); mbar_init(sb + SM::bempty + 8 * i, 8); }
+        mbar_init(sb + SM::bgo, 1); mbar_init(sb + SM::bgo + 8, 1);
         fence_mbar_init();
     }
     if (threadIdx.x < 32) tmem_alloc<kTmemCols>(sb + SM::bars + 24);
@@ -408,6 +444,9 @@ k_search(const __grid_constant__ SearchArgs A)
         const uint32_t xw_a = sb + SM::xch + team * SM::kXch + (g * 17 + c) * 8;       // + p * 2176: element [p][g][c]
         const uint32_t xr_a = sb + SM::xch + team * SM::kXch + (p2 * 272 + c2i) * 8;   // + gg * 136
         const uint32_t ssig_a = sb + SM::ssig + team * 32;
+        const uint32_t stg_w = sb + SM::xch + team * SM::kXch + warp * 4096;            // this warp's staging slice
+        const uint32_t stg_a = sb + SM::xch + team * SM::kXch + (p2 * 256 + c2i) * 8;   // + q * 128: row 16 p + q, column c
+        int prev_slot = -1;                                  // ring slot of this team's previous item
         const int bar_id = 1 + team;
         auto stream_src = [&](uint32_t it) { return SINGLE ? tpl_tile(it) : seg_tile(it % nS); };
         const ulonglong2* statg = nullptr;
@@ -422,7 +461,6 @@ k_search(const __grid_constant__ SearchArgs A)
                 bulk_load(stream_buf, stream_src(team), kTileBytes, bar_stream, SINGLE ? policy_evict_first() : policy_evict_last());
             }
         }
-        int pending = -1;                                    // ring slot whose tile this team has yet to publish
         uint32_t nload = 0;                                  // tiles this team has waited for so far
         uint32_t tj_prev = 0;
         if (STAT && !TM_ST && n_items > 0) mbar_wait(bar_stat, 0, abort_flag);
@@ -434,8 +472,8 @@ k_search(const __grid_constant__ SearchArgs A)
             // acquires it, early, so that the L2 round trip is hidden behind stage 1
             unsigned long long d2v = ~0ull;
             if (!(BEGE_ABL & 1) && t == 32 && it >= (uint32_t)kRing) d2v = counter_load_acquire(d2 + slot);
-            c2 qa[4], qb[4];                                 // TMEM staging (stationary values, then theta powers)
-            if (TM_ST) tmem_ld8(tq_a + kTmStat, qa);
+            c2 qa[2], qb[2];                                 // TMEM staging (stationary values, then theta powers)
+            if (TM_ST) tmem_ld4(tq_a + kTmStat, qa);
 #if !(BEGE_ABL & 2)
             mbar_wait(bar_stream, nload & 1, abort_flag);
 #endif
@@ -449,30 +487,12 @@ k_search(const __grid_constant__ SearchArgs A)
             c2 acc = mk(0.f, 0.f);
 #pragma unroll
             for (int r = 0; r < 16; ++r) if (r < I0 || r >= I0 + NI) v[r] = mk(0.f, 0.f);
-            if (TM_ST) {
-                tmem_wait_ld(qa); tmem_ld8(tq_a + kTmStat + 8, qb);
-                products2<I0, SINGLE, 0>(stream_a, qa, v, acc);
-                tmem_wait_ld(qb); tmem_ld8(tq_a + kTmStat + 16, qa);
-                products2<I0, SINGLE, 2>(stream_a, qb, v, acc);
-                tmem_wait_ld(qa); tmem_ld8(tq_a + kTmStat + 24, qb);
-                products2<I0, SINGLE, 4>(stream_a, qa, v, acc);
-                tmem_wait_ld(qb);
-                if (TM_TH) tmem_ld8(tq_a + kTmTheta, qa);
-                products2<I0, SINGLE, 6>(stream_a, qb, v, acc, false);
-            } else {
-                if (TM_TH) tmem_ld8(tq_a + kTmTheta, qa);
-                load_products<I0, NI, SINGLE, STAT>(stream_a, stat_a, statg, v, acc);
-            }
+            if (TM_ST) tm_products<I0, SINGLE>(stream_a, tq_a + kTmStat, v, acc, qa, qb);
+            else load_products<I0, NI, SINGLE, STAT>(stream_a, stat_a, statg, v, acc);
+            if (TM_TH) tmem_ld4(tq_a + kTmTheta, qa);
             fft16<+1>(v);
             if (TM_TH) {                                     // v[p] *= theta^p, p = 1 .. 15
-                tmem_wait_ld(qa); tmem_ld8(tq_a + kTmTheta + 8, qb);
-                v[1] = cmulw(v[1], qa[0]); v[2] = cmulw(v[2], qa[1]); v[3] = cmulw(v[3], qa[2]); v[4] = cmulw(v[4], qa[3]);
-                tmem_wait_ld(qb); tmem_ld8(tq_a + kTmTheta + 16, qa);
-                v[5] = cmulw(v[5], qb[0]); v[6] = cmulw(v[6], qb[1]); v[7] = cmulw(v[7], qb[2]); v[8] = cmulw(v[8], qb[3]);
-                tmem_wait_ld(qa); tmem_ld8(tq_a + kTmTheta + 24, qb);
-                v[9] = cmulw(v[9], qa[0]); v[10] = cmulw(v[10], qa[1]); v[11] = cmulw(v[11], qa[2]); v[12] = cmulw(v[12], qa[3]);
-                tmem_wait_ld(qb);
-                v[13] = cmulw(v[13], qb[0]); v[14] = cmulw(v[14], qb[1]); v[15] = cmulw(v[15], qb[2]);
+                tm_twiddle<1, 8>(tq_a + kTmTheta, v, qa, qb);
             } else {   // powers by a depth-4 product tree
                 const c2 t2 = cmulw(theta, theta), t3 = cmulw(t2, theta);
                 const c2 t4 = cmulw(t2, t2), t5 = cmulw(t3, t2), t6 = cmulw(t2, t4), t7 = cmulw(t3, t4), t8 = cmulw(t4, t4);
@@ -483,6 +503,20 @@ k_search(const __grid_constant__ SearchArgs A)
                 v[13] = cmulw(v[13], cmulw(t5, t8)); v[14] = cmulw(v[14], cmulw(t6, t8));
                 v[15] = cmulw(v[15], cmulw(t7, t8));
             }
+#if BEGE_TMAST
+            // The exchange buffer doubles as the staging area of the previous item's ring tile, which the TMA engine
+            // drains in the background: every warp waits (lane 0, no blocking in practice: the copy was issued a whole
+            // stage ago) until the engine has read its slice, and the team until all eight slices are read.
+            if (lane == 0) {
+                if (BEGE_X & 1) bulk_wait_read0();
+                else {
+                    bulk_wait0();                            // ... and written it: the tile of prev_slot is in the ring
+                    if (prev_slot >= 0) mbar_arrive(sb + SM::amb + 8 * prev_slot);
+                }
+                mbar_arrive(sb + SM::xfree + 8 * team);
+            }
+            mbar_wait(sb + SM::xfree + 8 * team, (nload - 1) & 1, abort_flag);
+#endif
             sts16<2176>(xw_a, v);
             const float sw = warp_sum32(re(acc) + im(acc));
             if (lane == 0) sts32(ssig_a + 4 * warp, sw);
@@ -518,10 +552,27 @@ k_search(const __grid_constant__ SearchArgs A)
             if (t == 32 && d2v < 16ull * (it / kRing)) counter_wait_ge(d2 + slot, 16ull * (it / kRing), abort_flag);
             __syncwarp();
             bar_named(bar_id, 256);                          // exchange buffer free for the team's next item; slot free
-            // the team's ring stores of its previous item were all issued before the FIRST barrier of this item and
-            // have long landed: the release fence does not wait
-            if (t == 0 && pending >= 0) counter_add_release(d1 + pending, 1ull);
             fft16<+1>(v);
+            // T[n2 = p + 16 q][16 b + c] for this thread's (c, p): a half-warp stores 128 contiguous bytes of row n2.
+#if BEGE_TMAST
+            // variant: staged in the (now free) exchange buffer and written out by ONE bulk copy per warp
+            sts16<128>(stg_a, v);
+            if (t == 64)
+                A.sigpart[((A.j0 + grp + (uint64_t)G * tj) * (uint64_t)A.S + (A.m0 + ml) - A.sig_pair0) * 16 + b] = tot;
+            fence_proxy_async_smem();
+            __syncwarp();
+            if (lane == 0 && !(BEGE_ABL & 4)) {
+                bulk_store(myring + (uint64_t)slot * kN + b * 4096 + warp * 512, stg_w, 4096);
+                bulk_commit();
+                if (BEGE_X & 1) mbar_arrive(sb + SM::amb + 8 * slot);
+            }
+            prev_slot = slot;
+        }
+        if (lane == 0) {
+            bulk_wait0();
+            if (prev_slot >= 0 && !(BEGE_X & 1)) mbar_arrive(sb + SM::amb + 8 * prev_slot);
+        }
+#else
             c2* out = myring + (uint64_t)slot * kN + 16 * b + c2i + p2 * 256;
 #pragma unroll
             for (int q = 0; q < 16; ++q) {
@@ -530,10 +581,14 @@ k_search(const __grid_constant__ SearchArgs A)
             }
             if (t == 64)
                 A.sigpart[((A.j0 + grp + (uint64_t)G * tj) * (uint64_t)A.S + (A.m0 + ml) - A.sig_pair0) * 16 + b] = tot;
-            pending = slot;
+            // this warp's part of the tile is on its way: tell the publisher (thread 0 of the B team of the same parity).
+            // The gpu-scope release fence is NOT executed here: it takes about a microsecond and would make this warp
+            // the laggard of the team's barriers; the B team has slack and a thread that idles in a wait loop anyway.
+            __syncwarp();
+            if (lane == 0) mbar_arrive(sb + SM::amb + 8 * slot);
+            (void)prev_slot; (void)stg_a; (void)stg_w;
         }
-        bar_named(bar_id, 256);
-        if (pending >= 0 && t == 0) counter_add_release(d1 + pending, 1ull);
+#endif
     } else if (team >= 2 && !(BEGE_ABL & 32)) {
         // ================================================================ B: pass 2, items ib = team - 2 (mod 2)
         const int kb = team - 2;
@@ -543,35 +598,123 @@ k_search(const __grid_constant__ SearchArgs A)
         const uint32_t pw_a = priv + a * 136;                // + 8 p:    stage-1 output p of lane a
         const uint32_t pr_a = priv + a * 8;                  // + 136 aa: stage-2 input from lane aa
         const uint32_t tbl_a = sb + SM::tbl + a * 16, w1_a = sb + SM::w1t + a * 16;
+#if BEGE_TMAST
+        const uint64_t row_off = (uint64_t)(16 * hw + b) * 16 + (uint64_t)a;   // ring tile r, row 16 p + q (p = hw, q = b), column a
+        constexpr int kRowStep = 4096;
+#else
         const uint64_t row_off = (uint64_t)n2 * 256 + (uint64_t)a;           // T[n2][k1 = a + 16 r]
+        constexpr int kRowStep = 16;
+#endif
         const int bar_id = 4 + kb;
         int prev_slot = -1;
         unsigned long long d1v = 0;                          // t == 0: last acquired value of the item's counter
+        // BEGE_BTMA: the team's 32 KiB row tile; half-warp hw owns row hw (2 KiB) and, once the row is in registers,
+        // uses the same 2 KiB as its private exchange area (element (a, p) at a * 128 + ((a ^ p) << 3): conflict free
+        // both ways)
+        constexpr uint32_t NB = SM::kNB;                     // item i uses tile buffer i % NB (both teams share the buffers)
+        uint32_t d1v_it = ~0u;                               // item whose counter d1v was read for
+        uint32_t ld_it = kb, nit = 0;                        // next item of this team whose copy is to be issued; items started
+        // Thread 0 is the team's poller AND the publisher of A team kb (same item parity): whenever all 8 warps of that
+        // team have stored their part of an item (mbarrier amb[slot]), it issues ONE fence.acq_rel.gpu and then adds 1
+        // to done1[slot] (and, under the same fence, frees the ring slot this team has just read out: done2).
+        constexpr bool PUB = !(BEGE_ABL & (1 | 16));
+        uint32_t pub_it = kb;                                // next item of A team kb to publish
+        auto publish = [&](int free_slot) {
+            uint32_t n = 0;
+            if (PUB)
+                while (n < 4 && pub_it + 2 * n < n_items &&
+                       mbar_test_wait(sb + SM::amb + 8 * ((pub_it + 2 * n) % kRing), ((pub_it + 2 * n) / kRing) & 1)) ++n;
+            if (n == 0 && free_slot < 0) return;
+            if (!(BEGE_X & 2)) fence_acq_rel_gpu();
+            for (uint32_t i = 0; i < n; ++i) counter_add_relaxed(d1 + (pub_it + 2 * i) % kRing, 1ull);
+            pub_it += 2 * n;
+            if (free_slot >= 0) counter_add_relaxed(d2 + free_slot, 1ull);
+        };
         for (uint32_t ib = kb; ib < n_items; ib += 2) {
             const int slot = (int)(ib % kRing);
             const uint32_t tj = SINGLE ? ib : ib / nS;
             const uint32_t ml = SINGLE ? 0u : (uint32_t)(ib - tj * nS);
             const uint64_t jl = grp + (uint64_t)G * tj;
+            c2 v[16];
+#if BEGE_BTMA
+            // The 16 rows n2 = 16 b .. 16 b + 15 of T are 32 KiB contiguous in the ring: ONE bulk copy (TMA engine) brings
+            // them into the team's tile buffer; no warp issues global loads or waits on the LSU queue behind pass 1's
+            // stores.  Thread 0 is the team's service thread: it publishes A team kb's tiles, waits (acquire) until all
+            // 16 tiles of the item are in the ring, issues the copy, and as soon as the copy has landed frees the ring slot.
+            const uint32_t buf = ib % NB, use = ib / NB;
+            const uint32_t btile = sb + SM::bpriv + buf * 32768, bfull = sb + SM::bfull + 8 * buf, bempty = sb + SM::bempty + 8 * buf;
+            const uint32_t in_a = btile + hw * 2048 + a * 8;     // + 128 r: T[n2][k1 = a + 16 r]
+            const uint32_t xw0 = btile + hw * 2048 + a * 136;    // (xw0 ^ (p << 3)):            element (a, p)
+            const uint32_t xr0 = btile + hw * 2048 + a * 8;      // (xr0 ^ (aa << 3)) + 128 aa:  element (aa, p = a)
+            // copy of item `it` of this team into its tile buffer, if the buffer has been read out (item it - NB, either
+            // team) and all 16 tiles of the item are in the ring (d1, acquired: `ready`); non-blocking
+            auto try_load = [&](uint32_t it, bool ready) {
+                const uint32_t bf = it % NB, us = it / NB;
+                if (us > 0 && !mbar_test_wait(sb + SM::bempty + 8 * bf, (us - 1) & 1)) return;
+                if (!ready) return;
+                if (!(BEGE_ABL & 8)) {
+                    fence_proxy_async_smem();
+                    mbar_arrive_expect_tx(sb + SM::bfull + 8 * bf, 32768);
+                    bulk_load(sb + SM::bpriv + bf * 32768, myring + (uint64_t)(it % kRing) * kN + 4096 * b, 32768,
+                              sb + SM::bfull + 8 * bf, policy_evict_first());
+                }
+                ld_it = it + 2;
+            };
+            if (t == 0) {
+                const unsigned long long target = 16ull * (ib / kRing + 1);
+                const long long t0 = clock64();
+                for (;;) {
+                    if (ld_it == ib) {                       // copy of this item not yet issued
+                        publish(-1);
+                        try_load(ib, (BEGE_ABL & 1) || counter_load_acquire(d1 + slot) >= target);
+                    }
+                    if (ld_it > ib && ((BEGE_ABL & 8) || mbar_test_wait(bfull, use & 1))) break;
+                    if (*(volatile int*)abort_flag) break;
+                    if (clock64() - t0 > kSpinLimit) { *(volatile int*)abort_flag = 1; break; }
+                    __nanosleep(40);
+                }
+                // The other seven warps wait on a per-team barrier, not on the tile's own: the tile buffers are shared
+                // by both teams, and a warp that runs ahead could otherwise mistake an older phase of the same parity.
+                mbar_arrive(sb + SM::bgo + 8 * kb);
+                publish(slot);                               // the rows are in shared memory: the ring slot is free
+                // look at the counter of the team's next item now; the answer is used after the exchange
+                if (!(BEGE_ABL & 1) && ib + 2 < n_items && ld_it == ib + 2) { d1v = counter_load_acquire(d1 + (ib + 2) % kRing); d1v_it = ib + 2; }
+            }
+            __syncwarp();
+            mbar_wait(sb + SM::bgo + 8 * kb, nit & 1, abort_flag);
+            ++nit;
+            lds16<128>(in_a, v);
+            const uint64_t pair = (A.j0 + jl) * (uint64_t)A.S + (A.m0 + ml);
+            const float part = __ldcg(A.sigpart + (pair - A.sig_pair0) * 16 + a);
+#else
 #if !(BEGE_ABL & 1)
-            if (t == 0 && d1v < 16ull * (ib / kRing + 1))    // all 16 tiles are in the ring
-                counter_wait_ge(d1 + slot, 16ull * (ib / kRing + 1), abort_flag);
+            if (t == 0 && d1v < 16ull * (ib / kRing + 1)) {  // wait until all 16 tiles of the item are in the ring
+                const unsigned long long target = 16ull * (ib / kRing + 1);
+                const long long t0 = clock64();
+                for (;;) {
+                    publish(-1);
+                    if (counter_load_acquire(d1 + slot) >= target) break;
+                    if (*(volatile int*)abort_flag) break;
+                    if (clock64() - t0 > kSpinLimit) { *(volatile int*)abort_flag = 1; break; }
+                    __nanosleep(100);
+                }
+            }
 #endif
             __syncwarp();
             bar_named(bar_id, 256);                          // ... and every warp of the team is done with its
-            if (t == 224 && prev_slot >= 0)                  // loads of the team's previous item: free that slot
-                counter_add_release(d2 + prev_slot, 1ull);
+            if (t == 0) publish(prev_slot);                  // loads of the team's previous item: free that slot
             const c2* src = myring + (uint64_t)slot * kN + row_off;
-            c2 v[16];
 #pragma unroll
-            for (int r = 0; r < 16; ++r) v[r] = (BEGE_ABL & 8) ? mk((float)(r + a), (float)ib) : __ldcg(src + 16 * r);
+            for (int r = 0; r < 16; ++r) v[r] = (BEGE_ABL & 8) ? mk((float)(r + a), (float)ib) : __ldcg(src + kRowStep * r);
             const uint64_t pair = (A.j0 + jl) * (uint64_t)A.S + (A.m0 + ml);
             const float part = __ldcg(A.sigpart + (pair - A.sig_pair0) * 16 + a);
             // look at the counter of the team's next item now: the answer is there when the item starts
             d1v = 0;
             if (!(BEGE_ABL & 1) && t == 0 && ib + 2 < n_items) d1v = counter_load_acquire(d1 + (ib + 2) % kRing);
-            c2 wa[4], wb[4];
+#endif
+            c2 wa[2], wb[2];
             if (TM_TW) {
-                tmem_ld8(tq + kTmDelta, wa);
+                tmem_ld4(tq + kTmDelta, wa);
                 // four-step factor wN^(16 b k1), k1 = a + 16 r: its CTA-uniform part w256^(b r) here, the rest in delta_p
 #pragma unroll
                 for (int r = 1; r < 16; ++r) { const float2 w = c_w256[(b * r) & 255]; v[r] = cmulw(v[r], w.x, w.y); }
@@ -580,22 +723,26 @@ k_search(const __grid_constant__ SearchArgs A)
             }
             const float sumR2 = hw_sum16(part);
             fft16<+1>(v);
-            if (TM_TW) {                                     // v[p] *= delta_p = wN^(16 b a) w256^(a p)
-                tmem_wait_ld(wa); tmem_ld8(tq + kTmDelta + 8, wb);
-                mul4<0>(v, wa);
-                tmem_wait_ld(wb); tmem_ld8(tq + kTmDelta + 16, wa);
-                mul4<1>(v, wb);
-                tmem_wait_ld(wa); tmem_ld8(tq + kTmDelta + 24, wb);
-                mul4<2>(v, wa);
-                tmem_wait_ld(wb);
-                mul4<3>(v, wb);
-            } else {
-                twiddle16<true>(w1_a, v);                    // w256^(a p)
-            }
+            if (TM_TW) tm_twiddle<0, 8>(tq + kTmDelta, v, wa, wb);    // v[p] *= delta_p = wN^(16 b a) w256^(a p)
+            else twiddle16<true>(w1_a, v);                            // w256^(a p)
+#if BEGE_BTMA
+            __syncwarp();                                    // every lane of the half-warp has its row in registers
+#pragma unroll
+            for (int p = 0; p < 16; ++p) sts64<0>(xw0 ^ (uint32_t)(p << 3), v[p]);
+            __syncwarp();
+#pragma unroll
+            for (int aa = 0; aa < 16; ++aa) v[aa] = lds64<0>((xr0 ^ (uint32_t)(aa << 3)) + 128 * aa);
+            fence_proxy_async_smem();                        // these generic accesses before the next bulk copy into the tile
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bempty);
+            if (t == 0 && ib + 2 < n_items && ld_it == ib + 2)   // bring in the team's next item while this one is finished
+                try_load(ib + 2, (BEGE_ABL & 1) || (d1v_it == ib + 2 && d1v >= 16ull * ((ib + 2) / kRing + 1)));
+#else
             sts16<8>(pw_a, v);
             __syncwarp();
             lds16<136>(pr_a, v);
             __syncwarp();
+#endif
             fft16<+1>(v);
             // lane a holds Z[n1 = a + 16 q]; lag n = 256 n1 + n2
             const float thr = A.k2 * sumR2;
@@ -674,8 +821,19 @@ k_search(const __grid_constant__ SearchArgs A)
             }
             prev_slot = slot;
         }
+#if BEGE_BTMA
+        prev_slot = -1;                                      // every slot was freed when its copy landed
+#else
         bar_named(bar_id, 256);
-        if (t == 224 && prev_slot >= 0) counter_add_release(d2 + prev_slot, 1ull);
+#endif
+        if (t == 0) {
+            publish(prev_slot);
+            while (PUB && pub_it < n_items) {                // tiles A team kb stores after this team's last item
+                mbar_wait(sb + SM::amb + 8 * (pub_it % kRing), (pub_it / kRing) & 1, abort_flag);
+                if (*(volatile int*)abort_flag) break;
+                publish(-1);
+            }
+        }
     }
     // every warp is done with the tensor memory: give it back
     tmem_fence_before_sync();
@@ -1028,6 +1186,7 @@ extern "C" int bege_segment_load(bege_plan* p, const float* x, uint32_t S)
 static void set_l2_window(bege_plan* p, void* ring)
 {
     if (p->l2_window == ring) return;
+    if (getenv("BEGE_NOL2WIN")) return;
     const size_t bytes = (size_t)p->G * kRing * kN * sizeof(c2);
     if (!p->l2_limit_saved) { cudaDeviceGetLimit(&p->l2_limit_prev, cudaLimitPersistingL2CacheSize); p->l2_limit_saved = true; }
     cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, bytes);
