@@ -31,7 +31,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-from paper_1708_01609_b200 import synth  # noqa: E402
+import bege_synth as synth  # noqa: E402
 
 METRIC = "template correlations/sec at N=2^16 C2C fp32 on 1 B200; % of FFT roofline"   # BASELINE.json, verbatim
 UNIT = "correlations/s"

@@ -157,56 +157,49 @@ k_fwd_cols(const c2* __restrict__ G, c2* __restrict__ out, uint64_t out_stride, 
 // co-resident).  The 16 CTAs of a group share the group's (template, segment) items; item `it` of a group is the
 // pair (template grp + G (it / nS), segment it % nS).  CTA (b, grp) owns columns k1 = 16 b + c in pass 1 and rows
 // n2 = 16 b + r in pass 2.  Four teams of 8 warps, two per pass, team k of a pass taking the items it = k (mod 2).
+//
 //   A teams (pass 1): R = conj(H) X needs one column tile of the template spectrum and one of the segment spectrum.
-//              One of them is STATIONARY in shared memory, the other STREAMS through a per-team buffer by bulk
-//              async copy (mbarrier-tracked, refilled as soon as the team has read it):
+//              One of them is STATIONARY -- it sits in tensor memory, 14 complex numbers per thread -- and the other
+//              STREAMS through a per-team shared-memory buffer by bulk async copy (mbarrier-tracked, refilled as soon
+//              as the team has read it):
 //                single-segment calls (nS = 1): X stationary (loaded once per launch), H streams from HBM;
 //                batched calls (nS >= 2):       H stationary (one load per template, it serves all nS segments --
 //                                               PAPER.md:156 "loaded once per M inverse FFTs"), X streams from L2.
-//              Stage 1: half-warp c, lane g holds rows k2 = g + 16 i of column c: 128-bit loads of both tiles,
-//              conj(H) X, Parseval partial sum, 16-point DFTs, twiddles theta^p generated from one complex number
-//              per thread.  One exchange through shared memory (two named barriers of the team per item).
-//              Stage 2: lane c, p = warp-pair index: 16-point DFTs, and T[n2 = p + 16 q][16 b + c] goes straight
-//              from registers to the ring in L2 (128 B per half-warp and store).
-//   B teams (pass 2): wait for all 16 tiles of an item, half-warp r loads its row of T from the ring,
-//              runs the 256-point row DFT over k1 through a private shared-memory region, thresholds against
-//              k^2 sum|R|^2 and compacts the tails with warp-aggregated atomics.
-// Hand-over (PTX memory model): per group and ring slot two monotone counters.
-//   done1 (tiles in the ring): every A team adds 1 per item with red.release.gpu by ONE thread after a team barrier
-//              that follows all the team's ring stores (release is cumulative over the barrier).  ONE thread of the
-//              B team spins on ld.acquire.gpu until 16 tiles have arrived, then the team barrier releases the other
-//              seven warps, which sleep in hardware meanwhile (no polling instructions).
-//   done2 (ring slot read out): one thread of the B team adds 1 with red.release.gpu after the team barrier of the
-//              team's NEXT item, which every warp reaches only after its loads of this item have returned.  ONE
-//              thread of the A team acquires 16 of them before the barrier that precedes the team's ring stores.
-// The ring holds kRing items per group (G x kRing x 512 KiB) and lives in L2.  Four-step twiddle wN^(k1 n2) with
-// n2 = p + 16 q is split into wN^(k1 p), folded into theta = exp(2 pi i (256 g + k1) / N) of pass 1, and
-// wN^(16 k1 q), applied by pass 2 to its inputs (q = n2 >> 4 is the CTA's tile index there: a 16 x 16 table in
-// shared memory); theta and the tables are rounded once from fp64 angles.
-#ifndef BEGE_BTMA
-#define BEGE_BTMA 1        // 1: pass 2 gets its 16 ring rows by one bulk copy into shared memory (0: global loads)
-#endif
-#ifndef BEGE_TMAST
-#define BEGE_TMAST 0       // 1: ring tiles leave through per-warp bulk copies from the exchange buffer instead of direct stores
-#endif
-#ifndef BEGE_X
-#define BEGE_X 0           // timing experiments only (results invalid): 1 publish before the copy completes, 2 no fences
-#endif
-#ifndef BEGE_RING
-#define BEGE_RING 8
-#endif
-constexpr int kRing = BEGE_RING;
-constexpr int kSearchThreads = 32 * 32;
-
-// Loop-invariant per-thread tables live in tensor memory (read with tcgen05.ld: no L1/LSU wavefronts):
+//              Stage 1: half-warp c, lane g holds rows k2 = g + 16 i of column c: 128-bit loads of the streaming
+//              tile, conj(H) X, Parseval partial sum, 16-point DFTs, twiddles theta^p (tensor memory).  One exchange
+//              through shared memory (two named barriers of the team per item).  Stage 2: lane c, p = warp-pair
+//              index: 16-point DFTs, and T[n2 = p + 16 q][16 b + c] goes straight from registers to the ring in L2
+//              (128 B per half-warp and store).
+//   B teams (pass 2): the 16 rows of T this CTA owns are 32 KiB contiguous in the ring: ONE bulk copy brings them
+//              into a shared-memory tile (3 tiles rotate over the items of both teams, so the next item's copy runs
+//              while this one is computed).  Half-warp r reads its row, applies the four-step factor, runs the
+//              256-point row DFT over k1 with the tile itself as its private exchange area (xor swizzle), thresholds
+//              against k^2 sum|R|^2 and compacts the tails with warp-aggregated atomics.  No warp of pass 2 issues a
+//              global load, so none queues behind the store bursts of pass 1 in the LSU.
+//
+// Tensor memory holds the loop-invariant per-thread tables (read with tcgen05.ld: no L1/LSU wavefronts -- the LSU
+// data pipe was the binding unit of the round-1 kernel at 75 %, see profiles/):
 //   columns [0, 32):    pass 2: delta_p = exp(2 pi i a (b + 16 p) / 4096), p < 16 -- the lane-dependent part of the
-//                       four-step factor wN^(16 b k1) times the inner twiddle w256^(a p); all four lane quadrants
-//   columns [32, 96):   pass 1: the stationary tile, 28 columns per thread (14 complex), 32 per warp of a lane quadrant
-//   columns [96, 160):  pass 1: theta^p, p = 1 .. 15, same arrangement
-// The CTA-uniform part of the four-step factor, w256^(b r), comes from constant memory (uniform loads).
-#ifndef BEGE_TM
-#define BEGE_TM 7          // 1: pass-2 twiddles, 2: stationary tile, 4: theta powers (timing experiments switch them off)
-#endif
+//                       four-step factor wN^(16 b k1), k1 = a + 16 r, times the inner twiddle w256^(a p); 4 quadrants
+//   columns [32, 96):   pass 1: the stationary tile, 28 columns per thread, 32 per warp of a lane quadrant
+//   columns [96, 160):  pass 1: theta^p = exp(2 pi i p (256 g + k1) / N), p = 1 .. 15, same arrangement
+// The CTA-uniform part of the four-step factor, w256^(b r), comes from constant memory (uniform loads).  All table
+// entries are rounded once from fp64 angles.
+//
+// Hand-over between the passes (PTX memory model): per group and ring slot two monotone counters.
+//   done1 (tiles in the ring): each warp of an A team arrives on the CTA's mbarrier amb[slot] after its ring stores.
+//              Thread 0 of the B team of the same item parity -- the team's service thread, which idles in a wait
+//              loop whenever pass 2 is ahead -- sees the phase complete, executes ONE fence.acq_rel.gpu and adds 1 to
+//              done1[slot] (the gpu-scope fence takes about a microsecond while the SM has stores in flight; on a
+//              pass-1 warp it would make that warp the laggard of the team's barriers).
+//              The same thread waits with ld.acquire.gpu until all 16 tiles of its team's item have been added, then
+//              issues the bulk copy of the rows.
+//   done2 (ring slot read out): as soon as that copy has landed (mbarrier), the service thread adds 1 to done2[slot]
+//              under the same kind of fence.  ONE thread of the A team acquires 16 of them, early in the item, before
+//              the barrier that precedes the team's ring stores.
+// The ring holds kRing items per group (G x kRing x 512 KiB) and lives in L2.
+constexpr int kRing = 8;
+constexpr int kSearchThreads = 32 * 32;
 constexpr int kTmemCols = 256;
 constexpr uint32_t kTmDelta = 0, kTmStat = 32, kTmTheta = 96;
 __constant__ float2 c_w256[256];           // exp(2 pi i m / 256), rounded from fp64 (host, bege_plan_create)
@@ -221,31 +214,26 @@ struct SearchArgs {
 };
 
 // shared-memory map of k_search (byte offsets from the 128-byte aligned base)
-template <int NI, bool STAT> struct SearchSmem {
+template <int NI> struct SearchSmem {
     static constexpr uint32_t kTile = NI * 256 * 8;              // one column tile of a spectrum
     static constexpr uint32_t kXch = 16 * 16 * 17 * 8;           // padded pass-1 exchange buffer, [p][g][c]
-    static constexpr uint32_t kPriv = 16 * 17 * 8;               // padded private region of a pass-2 half-warp (BEGE_BTMA = 0)
-    static constexpr int kNB = NI <= 14 ? 3 : 2;                 // 32 KiB row tiles of pass 2 (BEGE_BTMA = 1)
-    static constexpr uint32_t stream = 0;                        // [2]  streaming tile of each A team
-    static constexpr uint32_t xch = stream + 2 * kTile;          // [2]
-    static constexpr uint32_t bpriv = xch + 2 * kXch;            // [32] private regions / [kNB] row tiles
-    static constexpr uint32_t kBBytes = BEGE_BTMA ? kNB * 32768 : 32 * kPriv;
-    static constexpr uint32_t stat = bpriv + kBBytes;            //      stationary tile in shared memory (only if !TMEM)
-    static constexpr uint32_t tbl = stat + ((STAT && !(BEGE_TM & 2)) ? kTile : 0);   // (BEGE_TM & 1) == 0 only
-    static constexpr uint32_t w1t = tbl + ((BEGE_TM & 1) ? 0 : 2048);
-    static constexpr uint32_t ssig = w1t + ((BEGE_TM & 1) ? 0 : 2048);   // [2][8] Parseval partial sums of the A warps
-    static constexpr uint32_t bars = ssig + 64;                  // mbarriers: stream[2], stat; TMEM base address @ +24
+    static constexpr int kNB = NI <= 14 ? 3 : 2;                 // 32 KiB row tiles of pass 2
+    static constexpr uint32_t stream = 0;                        // [2]   streaming tile of each A team
+    static constexpr uint32_t xch = stream + 2 * kTile;          // [2]   exchange buffer of each A team
+    static constexpr uint32_t btile = xch + 2 * kXch;            // [kNB] row tiles of pass 2
+    static constexpr uint32_t ssig = btile + kNB * 32768;        // [2][8] Parseval partial sums of the A warps
+    static constexpr uint32_t bars = ssig + 64;                  // mbarriers: stream[2]; TMEM base address @ +24
     static constexpr uint32_t amb = bars + 32;                   // [kRing] mbarriers: tile of ring slot stored (8 A warps)
-    static constexpr uint32_t xfree = amb + 8 * kRing;           // [2] mbarriers: exchange buffer of an A team drained
-    static constexpr uint32_t bfull = xfree + 16;                // [kNB] mbarriers: row tile has arrived
+    static constexpr uint32_t bfull = amb + 8 * kRing;           // [kNB] mbarriers: row tile has arrived
     static constexpr uint32_t bempty = bfull + 24;               // [kNB] mbarriers: ... has been read out (8 B warps)
     static constexpr uint32_t bgo = bempty + 24;                 // [2] mbarriers: the B team's next row tile is there (thread 0)
     static constexpr uint32_t total = bgo + 16;
     static_assert(total + 128 <= 232448, "shared memory of one SM");
 };
-// the stationary tile fits next to everything else only for bands that need 14 of the 16 row-blocks
-template <int NI> __host__ __device__ constexpr bool search_stat() { return NI <= 14; }
-template <int NI> constexpr int search_smem() { return (int)SearchSmem<NI, search_stat<NI>()>::total + 128; }
+// the stationary tile has its tensor-memory arrangement written out for bands that need 14 of the 16 row-blocks;
+// other bands read it from global memory (L2) -- correct, not tuned
+template <int NI> __host__ __device__ constexpr bool search_stat() { return NI == 14; }
+template <int NI> constexpr int search_smem() { return (int)SearchSmem<NI>::total + 128; }
 
 // 16 values to shared memory at a + p * STRIDE bytes
 template <int STRIDE, int P = 0> BEGE_D void sts16(uint32_t a, const c2 (&v)[16])
@@ -256,45 +244,38 @@ template <int STRIDE, int P = 0> BEGE_D void lds16(uint32_t a, c2 (&v)[16])
 {
     if constexpr (P < 16) { v[P] = lds64<P * STRIDE>(a); lds16<STRIDE, P + 1>(a, v); }
 }
-// v[2 i], v[2 i + 1] *= table entries (2 i, 2 i + 1) at a + i * 256 bytes (one 128-bit load per pair); FIRST: skip entry 0
-template <bool FIRST, int IP = 0> BEGE_D void twiddle16(uint32_t a, c2 (&v)[16])
-{
-    if constexpr (IP < 8) {
-        c2 w0, w1;
-        lds128<IP * 256>(a, w0, w1);
-        if (!(FIRST && IP == 0)) v[2 * IP] = cmulw(v[2 * IP], w0);
-        v[2 * IP + 1] = cmulw(v[2 * IP + 1], w1);
-        twiddle16<FIRST, IP + 1>(a, v);
-    }
-}
-// stage 1 of pass 1: v[I0 + 2 ip], v[I0 + 2 ip + 1] = conj(H) X for the row-block pair ip, acc += |.|^2 (packed)
-template <int I0, int NI, bool SINGLE, bool STAT, int IP = 0>
-BEGE_D void load_products(uint32_t stream_a, uint32_t stat_a, const ulonglong2* __restrict__ statg, c2 (&v)[16], c2& acc)
-{
-    if constexpr (IP < NI / 2) {
-        c2 s0, s1, q0, q1;
-        lds128<IP * 4096>(stream_a, s0, s1);
-        if constexpr (STAT) lds128<IP * 4096>(stat_a, q0, q1);
-        else { const ulonglong2 q = __ldg(statg + IP * 256); q0 = q.x; q1 = q.y; }
-        // SINGLE: the template streams, the segment is stationary; batched: the other way round
-        const c2 r0 = SINGLE ? cmulc(q0, s0) : cmulc(s0, q0);
-        const c2 r1 = SINGLE ? cmulc(q1, s1) : cmulc(s1, q1);
-        v[I0 + 2 * IP] = r0; v[I0 + 2 * IP + 1] = r1;
-        acc = fma2(r0, r0, acc);
-        acc = fma2(r1, r1, acc);
-        load_products<I0, NI, SINGLE, STAT, IP + 1>(stream_a, stat_a, statg, v, acc);
-    }
-}
-
-// products of one row-block pair: streaming tile from shared memory, stationary values q[0..1] from tensor memory
-template <int I0, bool SINGLE, int IP> BEGE_D void products1(uint32_t stream_a, const c2 (&q)[2], c2 (&v)[16], c2& acc)
+// stage 1 of pass 1: v[I0 + 2 ip], v[I0 + 2 ip + 1] = conj(H) X for the row-block pair ip, acc += |.|^2 (packed);
+// q0, q1: the stationary values.  SINGLE: the template streams, the segment is stationary; batched: the other way round
+template <int I0, bool SINGLE, int IP> BEGE_D void products1(uint32_t stream_a, c2 q0, c2 q1, c2 (&v)[16], c2& acc)
 {
     c2 s0, s1;
     lds128<IP * 4096>(stream_a, s0, s1);
-    const c2 r0 = SINGLE ? cmulc(q[0], s0) : cmulc(s0, q[0]);
-    const c2 r1 = SINGLE ? cmulc(q[1], s1) : cmulc(s1, q[1]);
+    const c2 r0 = SINGLE ? cmulc(q0, s0) : cmulc(s0, q0);
+    const c2 r1 = SINGLE ? cmulc(q1, s1) : cmulc(s1, q1);
     v[I0 + 2 * IP] = r0; v[(I0 + 2 * IP + 1) & 15] = r1;
     acc = fma2(r0, r0, acc); acc = fma2(r1, r1, acc);
+}
+// ... stationary values streamed from tensor memory one pair at a time, double buffered (the load of pair 0 into qa
+// was issued by the caller)
+template <int I0, bool SINGLE, int IP = 0> BEGE_D void tm_products(uint32_t stream_a, uint32_t taddr, c2 (&v)[16], c2& acc, c2 (&qa)[2], c2 (&qb)[2])
+{
+    if constexpr (IP < 7) {
+        c2 (&cur)[2] = (IP & 1) ? qb : qa;
+        c2 (&nxt)[2] = (IP & 1) ? qa : qb;
+        tmem_wait_ld(cur);
+        if constexpr (IP + 1 < 7) tmem_ld4(taddr + 4 * (IP + 1), nxt);
+        products1<I0, SINGLE, IP>(stream_a, cur[0], cur[1], v, acc);
+        tm_products<I0, SINGLE, IP + 1>(stream_a, taddr, v, acc, qa, qb);
+    }
+}
+// ... stationary values from global memory (bands that keep all 16 row-blocks)
+template <int I0, int NI, bool SINGLE, int IP = 0> BEGE_D void gl_products(uint32_t stream_a, const ulonglong2* __restrict__ statg, c2 (&v)[16], c2& acc)
+{
+    if constexpr (IP < NI / 2) {
+        const ulonglong2 q = __ldg(statg + IP * 256);
+        products1<I0, SINGLE, IP>(stream_a, q.x, q.y, v, acc);
+        gl_products<I0, NI, SINGLE, IP + 1>(stream_a, statg, v, acc);
+    }
 }
 // v[P0 + 2 j + k] *= table entry (2 j + k), entries streamed from tensor memory two at a time, double buffered;
 // the load of chunk 0 into wa was issued by the caller; chunks [0, NCH)
@@ -310,29 +291,14 @@ template <int P0, int NCH, int J = 0> BEGE_D void tm_twiddle(uint32_t taddr, c2 
         tm_twiddle<P0, NCH, J + 1>(taddr, v, wa, wb);
     }
 }
-template <int I0, bool SINGLE, int IP = 0> BEGE_D void tm_products(uint32_t stream_a, uint32_t taddr, c2 (&v)[16], c2& acc, c2 (&qa)[2], c2 (&qb)[2])
-{
-    if constexpr (IP < 7) {
-        c2 (&cur)[2] = (IP & 1) ? qb : qa;
-        c2 (&nxt)[2] = (IP & 1) ? qa : qb;
-        tmem_wait_ld(cur);
-        if constexpr (IP + 1 < 7) tmem_ld4(taddr + 4 * (IP + 1), nxt);
-        products1<I0, SINGLE, IP>(stream_a, cur, v, acc);
-        tm_products<I0, SINGLE, IP + 1>(stream_a, taddr, v, acc, qa, qb);
-    }
-}
 
 template <int I0, int NI, bool SINGLE, bool DBG>
 __global__ void __launch_bounds__(kSearchThreads, 1)
 k_search(const __grid_constant__ SearchArgs A)
 {
-    constexpr bool STAT = search_stat<NI>();
-    constexpr bool TM_TW = (BEGE_TM & 1) != 0;               // pass-2 twiddles from TMEM + constant memory
-    constexpr bool TM_ST = STAT && (BEGE_TM & 2) != 0;       // stationary tile in TMEM instead of shared memory
-    constexpr bool TM_TH = (BEGE_TM & 4) != 0;               // theta powers from TMEM instead of the product tree
-    using SM = SearchSmem<NI, STAT>;
+    constexpr bool STAT = search_stat<NI>();                 // stationary tile in tensor memory
+    using SM = SearchSmem<NI>;
     static_assert(NI % 2 == 0, "row-blocks are stored in pairs");
-    static_assert(!TM_ST || NI == 14, "TMEM arrangement of the stationary tile is written out for 14 row-blocks");
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const uint32_t sb = smem_u32(smem_raw);
     const int team = threadIdx.x >> 8;                       // 0, 1: A teams; 2, 3: B teams
@@ -353,27 +319,13 @@ k_search(const __grid_constant__ SearchArgs A)
     auto seg_tile = [&](uint32_t ml) { return A.xseg + ((uint64_t)(A.m0 + ml) * 16 + b) * kTile; };
 
     if (threadIdx.x == 0) {
-        mbar_init(sb + SM::bars, 1); mbar_init(sb + SM::bars + 8, 1); mbar_init(sb + SM::bars + 16, 1);
+        mbar_init(sb + SM::bars, 1); mbar_init(sb + SM::bars + 8, 1);
         for (int i = 0; i < kRing; ++i) mbar_init(sb + SM::amb + 8 * i, 8);
-        mbar_init(sb + SM::xfree, 8); mbar_init(sb + SM::xfree + 8, 8);
         for (int i = 0; i < SM::kNB; ++i) { mbar_init(sb + SM::bfull + 8 * i, 1); mbar_init(sb + SM::bempty + 8 * i, 8); }
         mbar_init(sb + SM::bgo, 1); mbar_init(sb + SM::bgo + 8, 1);
         fence_mbar_init();
     }
     if (threadIdx.x < 32) tmem_alloc<kTmemCols>(sb + SM::bars + 24);
-    if (!TM_TW) {
-        if (team == 2) {                                     // tbl: exp(2 pi i 16 b (a + 16 r) / N)
-            const int r = t >> 4, a = t & 15;
-            double sn, cs;
-            sincospi(2.0 * (double)((16 * b * (a + 16 * r)) & (kN - 1)) / (double)kN, &sn, &cs);
-            reinterpret_cast<float2*>(smem_raw + SM::tbl)[((r >> 1) * 16 + a) * 2 + (r & 1)] = make_float2((float)cs, (float)sn);
-        } else if (team == 3) {                              // w1t: exp(2 pi i a p / 256)
-            const int p = t >> 4, a = t & 15;
-            double sn, cs;
-            sincospi(2.0 * (double)((a * p) & 255) / 256.0, &sn, &cs);
-            reinterpret_cast<float2*>(smem_raw + SM::w1t)[((p >> 1) * 16 + a) * 2 + (p & 1)] = make_float2((float)cs, (float)sn);
-        }
-    }
     tmem_fence_before_sync();
     __syncthreads();
     tmem_fence_after_sync();
@@ -392,7 +344,7 @@ k_search(const __grid_constant__ SearchArgs A)
         tmem_wait_st();
     };
     if (team == 0) {
-        if (TM_TW && warp < 4) {                             // delta_p, one copy per lane quadrant
+        if (warp < 4) {                                      // delta_p, one copy per lane quadrant
             const int a = lane & 15;
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
@@ -406,7 +358,7 @@ k_search(const __grid_constant__ SearchArgs A)
                 tmem_st8(tq + kTmDelta + 8 * j, r);
             }
         }
-        if (TM_TH) {                                         // theta^p, p = 1 .. 15 (+ one unused entry)
+        {                                                    // theta^p, p = 1 .. 15 (+ one unused entry)
             const int c = t >> 4, g = t & 15;
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
@@ -421,7 +373,7 @@ k_search(const __grid_constant__ SearchArgs A)
                 tmem_st8(tq_a + kTmTheta + 8 * j, r);
             }
         }
-        if (TM_ST && n_items > 0) stat_to_tmem(SINGLE ? seg_tile(0) : tpl_tile(0));
+        if (STAT && n_items > 0) stat_to_tmem(SINGLE ? seg_tile(0) : tpl_tile(0));
         tmem_wait_st();
     }
     tmem_fence_before_sync();
@@ -432,29 +384,16 @@ k_search(const __grid_constant__ SearchArgs A)
         // ================================================================ A: pass 1, items it = team (mod 2)
         const int c = t >> 4, g = t & 15;                    // stage 1: column of the tile, lane of its half-warp
         const int c2i = t & 15, p2 = t >> 4;                 // stage 2: column, index p of n2 = p + 16 q
-        c2 theta = mk(1.f, 0.f);                             // exp(2 pi i (256 g + k1) / N), k1 = 16 b + c
-        if (!TM_TH) {
-            double sn, cs;
-            sincospi(2.0 * (double)(256 * g + 16 * b + c) / (double)kN, &sn, &cs);
-            theta = mk((float)cs, (float)sn);
-        }
-        const uint32_t bar_stream = sb + SM::bars + 8 * team, bar_stat = sb + SM::bars + 16;
+        const uint32_t bar_stream = sb + SM::bars + 8 * team;
         const uint32_t stream_buf = sb + SM::stream + team * kTileBytes;
-        const uint32_t stream_a = stream_buf + t * 16, stat_a = sb + SM::stat + t * 16;
+        const uint32_t stream_a = stream_buf + t * 16;
         const uint32_t xw_a = sb + SM::xch + team * SM::kXch + (g * 17 + c) * 8;       // + p * 2176: element [p][g][c]
         const uint32_t xr_a = sb + SM::xch + team * SM::kXch + (p2 * 272 + c2i) * 8;   // + gg * 136
         const uint32_t ssig_a = sb + SM::ssig + team * 32;
-        const uint32_t stg_w = sb + SM::xch + team * SM::kXch + warp * 4096;            // this warp's staging slice
-        const uint32_t stg_a = sb + SM::xch + team * SM::kXch + (p2 * 256 + c2i) * 8;   // + q * 128: row 16 p + q, column c
-        int prev_slot = -1;                                  // ring slot of this team's previous item
         const int bar_id = 1 + team;
         auto stream_src = [&](uint32_t it) { return SINGLE ? tpl_tile(it) : seg_tile(it % nS); };
-        const ulonglong2* statg = nullptr;
+        const ulonglong2* statg = nullptr;                   // !STAT: the stationary tile in global memory
         if (n_items > 0) {
-            if (STAT && !TM_ST && team == 0 && t == 0) {     // first stationary tile
-                mbar_arrive_expect_tx(bar_stat, kTileBytes);
-                bulk_load(sb + SM::stat, SINGLE ? seg_tile(0) : tpl_tile(0), kTileBytes, bar_stat, policy_evict_last());
-            }
             if (!STAT) statg = reinterpret_cast<const ulonglong2*>(SINGLE ? seg_tile(0) : tpl_tile(0)) + t;
             if (t == 0 && (uint32_t)team < n_items && !(BEGE_ABL & 2)) {
                 mbar_arrive_expect_tx(bar_stream, kTileBytes);
@@ -463,7 +402,6 @@ k_search(const __grid_constant__ SearchArgs A)
         }
         uint32_t nload = 0;                                  // tiles this team has waited for so far
         uint32_t tj_prev = 0;
-        if (STAT && !TM_ST && n_items > 0) mbar_wait(bar_stat, 0, abort_flag);
         for (uint32_t it = team; it < n_items; it += 2) {
             const uint32_t tj = SINGLE ? it : it / nS;
             const uint32_t ml = SINGLE ? 0u : (uint32_t)(it - tj * nS);
@@ -473,50 +411,22 @@ k_search(const __grid_constant__ SearchArgs A)
             unsigned long long d2v = ~0ull;
             if (!(BEGE_ABL & 1) && t == 32 && it >= (uint32_t)kRing) d2v = counter_load_acquire(d2 + slot);
             c2 qa[2], qb[2];                                 // TMEM staging (stationary values, then theta powers)
-            if (TM_ST) tmem_ld4(tq_a + kTmStat, qa);
+            if (STAT) tmem_ld4(tq_a + kTmStat, qa);
 #if !(BEGE_ABL & 2)
             mbar_wait(bar_stream, nload & 1, abort_flag);
 #endif
             ++nload;
-            if (!SINGLE && tj != tj_prev) {                  // first item of a template for this team (not the first)
-                if (STAT && !TM_ST) mbar_wait(bar_stat, tj & 1, abort_flag);
-                if (!STAT) statg = reinterpret_cast<const ulonglong2*>(tpl_tile(tj)) + t;
-                tj_prev = tj;
-            }
+            if (!SINGLE && !STAT && tj != tj_prev) statg = reinterpret_cast<const ulonglong2*>(tpl_tile(tj)) + t;
+            tj_prev = tj;
             c2 v[16];
             c2 acc = mk(0.f, 0.f);
 #pragma unroll
             for (int r = 0; r < 16; ++r) if (r < I0 || r >= I0 + NI) v[r] = mk(0.f, 0.f);
-            if (TM_ST) tm_products<I0, SINGLE>(stream_a, tq_a + kTmStat, v, acc, qa, qb);
-            else load_products<I0, NI, SINGLE, STAT>(stream_a, stat_a, statg, v, acc);
-            if (TM_TH) tmem_ld4(tq_a + kTmTheta, qa);
+            if constexpr (STAT) tm_products<I0, SINGLE>(stream_a, tq_a + kTmStat, v, acc, qa, qb);
+            else gl_products<I0, NI, SINGLE>(stream_a, statg, v, acc);
+            tmem_ld4(tq_a + kTmTheta, qa);
             fft16<+1>(v);
-            if (TM_TH) {                                     // v[p] *= theta^p, p = 1 .. 15
-                tm_twiddle<1, 8>(tq_a + kTmTheta, v, qa, qb);
-            } else {   // powers by a depth-4 product tree
-                const c2 t2 = cmulw(theta, theta), t3 = cmulw(t2, theta);
-                const c2 t4 = cmulw(t2, t2), t5 = cmulw(t3, t2), t6 = cmulw(t2, t4), t7 = cmulw(t3, t4), t8 = cmulw(t4, t4);
-                v[1] = cmulw(v[1], theta); v[2] = cmulw(v[2], t2); v[3] = cmulw(v[3], t3); v[4] = cmulw(v[4], t4);
-                v[5] = cmulw(v[5], t5); v[6] = cmulw(v[6], t6); v[7] = cmulw(v[7], t7); v[8] = cmulw(v[8], t8);
-                v[9] = cmulw(v[9], cmulw(theta, t8)); v[10] = cmulw(v[10], cmulw(t2, t8));
-                v[11] = cmulw(v[11], cmulw(t3, t8)); v[12] = cmulw(v[12], cmulw(t4, t8));
-                v[13] = cmulw(v[13], cmulw(t5, t8)); v[14] = cmulw(v[14], cmulw(t6, t8));
-                v[15] = cmulw(v[15], cmulw(t7, t8));
-            }
-#if BEGE_TMAST
-            // The exchange buffer doubles as the staging area of the previous item's ring tile, which the TMA engine
-            // drains in the background: every warp waits (lane 0, no blocking in practice: the copy was issued a whole
-            // stage ago) until the engine has read its slice, and the team until all eight slices are read.
-            if (lane == 0) {
-                if (BEGE_X & 1) bulk_wait_read0();
-                else {
-                    bulk_wait0();                            // ... and written it: the tile of prev_slot is in the ring
-                    if (prev_slot >= 0) mbar_arrive(sb + SM::amb + 8 * prev_slot);
-                }
-                mbar_arrive(sb + SM::xfree + 8 * team);
-            }
-            mbar_wait(sb + SM::xfree + 8 * team, (nload - 1) & 1, abort_flag);
-#endif
+            tm_twiddle<1, 8>(tq_a + kTmTheta, v, qa, qb);    // v[p] *= theta^p, p = 1 .. 15
             sts16<2176>(xw_a, v);
             const float sw = warp_sum32(re(acc) + im(acc));
             if (lane == 0) sts32(ssig_a + 4 * warp, sw);
@@ -532,15 +442,10 @@ k_search(const __grid_constant__ SearchArgs A)
             if (!SINGLE && STAT) {                           // last item of this template for this team: once both A
                 if (it + 2 >= (tj + 1) * nS && tj + 1 < nTg) {   // teams are past it, bring in the next template's tile
                     bar_named(3, 512);
-                    if (TM_ST) {
-                        if (team == 0) stat_to_tmem(tpl_tile(tj + 1));
-                        tmem_fence_before_sync();
-                        bar_named(3, 512);
-                        tmem_fence_after_sync();
-                    } else if (team == 0 && t == 0) {
-                        mbar_arrive_expect_tx(bar_stat, kTileBytes);
-                        bulk_load(sb + SM::stat, tpl_tile(tj + 1), kTileBytes, bar_stat, policy_evict_first());
-                    }
+                    if (team == 0) stat_to_tmem(tpl_tile(tj + 1));
+                    tmem_fence_before_sync();
+                    bar_named(3, 512);
+                    tmem_fence_after_sync();
                 }
             }
             lds16<136>(xr_a, v);
@@ -553,26 +458,7 @@ k_search(const __grid_constant__ SearchArgs A)
             __syncwarp();
             bar_named(bar_id, 256);                          // exchange buffer free for the team's next item; slot free
             fft16<+1>(v);
-            // T[n2 = p + 16 q][16 b + c] for this thread's (c, p): a half-warp stores 128 contiguous bytes of row n2.
-#if BEGE_TMAST
-            // variant: staged in the (now free) exchange buffer and written out by ONE bulk copy per warp
-            sts16<128>(stg_a, v);
-            if (t == 64)
-                A.sigpart[((A.j0 + grp + (uint64_t)G * tj) * (uint64_t)A.S + (A.m0 + ml) - A.sig_pair0) * 16 + b] = tot;
-            fence_proxy_async_smem();
-            __syncwarp();
-            if (lane == 0 && !(BEGE_ABL & 4)) {
-                bulk_store(myring + (uint64_t)slot * kN + b * 4096 + warp * 512, stg_w, 4096);
-                bulk_commit();
-                if (BEGE_X & 1) mbar_arrive(sb + SM::amb + 8 * slot);
-            }
-            prev_slot = slot;
-        }
-        if (lane == 0) {
-            bulk_wait0();
-            if (prev_slot >= 0 && !(BEGE_X & 1)) mbar_arrive(sb + SM::amb + 8 * prev_slot);
-        }
-#else
+            // T[n2 = p + 16 q][16 b + c] for this thread's (c, p): a half-warp stores 128 contiguous bytes of row n2
             c2* out = myring + (uint64_t)slot * kN + 16 * b + c2i + p2 * 256;
 #pragma unroll
             for (int q = 0; q < 16; ++q) {
@@ -581,85 +467,61 @@ k_search(const __grid_constant__ SearchArgs A)
             }
             if (t == 64)
                 A.sigpart[((A.j0 + grp + (uint64_t)G * tj) * (uint64_t)A.S + (A.m0 + ml) - A.sig_pair0) * 16 + b] = tot;
-            // this warp's part of the tile is on its way: tell the publisher (thread 0 of the B team of the same parity).
-            // The gpu-scope release fence is NOT executed here: it takes about a microsecond and would make this warp
-            // the laggard of the team's barriers; the B team has slack and a thread that idles in a wait loop anyway.
+            // this warp's part of the tile is on its way: tell the publisher (thread 0 of the B team of the same parity)
             __syncwarp();
             if (lane == 0) mbar_arrive(sb + SM::amb + 8 * slot);
-            (void)prev_slot; (void)stg_a; (void)stg_w;
         }
-#endif
     } else if (team >= 2 && !(BEGE_ABL & 32)) {
         // ================================================================ B: pass 2, items ib = team - 2 (mod 2)
         const int kb = team - 2;
         const int hw = t >> 4, a = t & 15;                   // row of the row tile, lane of its half-warp
         const int n2 = 16 * b + hw;
-        const uint32_t priv = sb + SM::bpriv + (kb * 16 + hw) * SM::kPriv;
-        const uint32_t pw_a = priv + a * 136;                // + 8 p:    stage-1 output p of lane a
-        const uint32_t pr_a = priv + a * 8;                  // + 136 aa: stage-2 input from lane aa
-        const uint32_t tbl_a = sb + SM::tbl + a * 16, w1_a = sb + SM::w1t + a * 16;
-#if BEGE_TMAST
-        const uint64_t row_off = (uint64_t)(16 * hw + b) * 16 + (uint64_t)a;   // ring tile r, row 16 p + q (p = hw, q = b), column a
-        constexpr int kRowStep = 4096;
-#else
-        const uint64_t row_off = (uint64_t)n2 * 256 + (uint64_t)a;           // T[n2][k1 = a + 16 r]
-        constexpr int kRowStep = 16;
-#endif
-        const int bar_id = 4 + kb;
-        int prev_slot = -1;
-        unsigned long long d1v = 0;                          // t == 0: last acquired value of the item's counter
-        // BEGE_BTMA: the team's 32 KiB row tile; half-warp hw owns row hw (2 KiB) and, once the row is in registers,
-        // uses the same 2 KiB as its private exchange area (element (a, p) at a * 128 + ((a ^ p) << 3): conflict free
-        // both ways)
         constexpr uint32_t NB = SM::kNB;                     // item i uses tile buffer i % NB (both teams share the buffers)
-        uint32_t d1v_it = ~0u;                               // item whose counter d1v was read for
-        uint32_t ld_it = kb, nit = 0;                        // next item of this team whose copy is to be issued; items started
-        // Thread 0 is the team's poller AND the publisher of A team kb (same item parity): whenever all 8 warps of that
-        // team have stored their part of an item (mbarrier amb[slot]), it issues ONE fence.acq_rel.gpu and then adds 1
-        // to done1[slot] (and, under the same fence, frees the ring slot this team has just read out: done2).
+        // ---- service thread (t == 0) state
         constexpr bool PUB = !(BEGE_ABL & (1 | 16));
         uint32_t pub_it = kb;                                // next item of A team kb to publish
+        uint32_t ld_it = kb;                                 // next item of this team whose copy is to be issued
+        unsigned long long d1v = 0; uint32_t d1v_it = ~0u;   // last acquired tiles-arrived counter and its item
+        uint32_t nit = 0;                                    // items this team has started
+        // whenever all 8 warps of A team kb have stored their part of an item (mbarrier amb[slot]): ONE
+        // fence.acq_rel.gpu, then done1[slot] += 1 (and, under the same fence, done2[free_slot] += 1)
         auto publish = [&](int free_slot) {
             uint32_t n = 0;
             if (PUB)
                 while (n < 4 && pub_it + 2 * n < n_items &&
                        mbar_test_wait(sb + SM::amb + 8 * ((pub_it + 2 * n) % kRing), ((pub_it + 2 * n) / kRing) & 1)) ++n;
             if (n == 0 && free_slot < 0) return;
-            if (!(BEGE_X & 2)) fence_acq_rel_gpu();
+            fence_acq_rel_gpu();
             for (uint32_t i = 0; i < n; ++i) counter_add_relaxed(d1 + (pub_it + 2 * i) % kRing, 1ull);
             pub_it += 2 * n;
             if (free_slot >= 0) counter_add_relaxed(d2 + free_slot, 1ull);
+        };
+        // copy of item `it` of this team into its tile buffer, if the buffer has been read out (item it - NB, either
+        // team) and all 16 tiles of the item are in the ring (d1, acquired: `ready`); non-blocking
+        auto try_load = [&](uint32_t it, bool ready) {
+            const uint32_t bf = it % NB, us = it / NB;
+            if (us > 0 && !mbar_test_wait(sb + SM::bempty + 8 * bf, (us - 1) & 1)) return;
+            if (!ready) return;
+            if (!(BEGE_ABL & 8)) {
+                fence_proxy_async_smem();
+                mbar_arrive_expect_tx(sb + SM::bfull + 8 * bf, 32768);
+                bulk_load(sb + SM::btile + bf * 32768, myring + (uint64_t)(it % kRing) * kN + 4096 * b, 32768,
+                          sb + SM::bfull + 8 * bf, policy_evict_first());
+            }
+            ld_it = it + 2;
         };
         for (uint32_t ib = kb; ib < n_items; ib += 2) {
             const int slot = (int)(ib % kRing);
             const uint32_t tj = SINGLE ? ib : ib / nS;
             const uint32_t ml = SINGLE ? 0u : (uint32_t)(ib - tj * nS);
             const uint64_t jl = grp + (uint64_t)G * tj;
-            c2 v[16];
-#if BEGE_BTMA
-            // The 16 rows n2 = 16 b .. 16 b + 15 of T are 32 KiB contiguous in the ring: ONE bulk copy (TMA engine) brings
-            // them into the team's tile buffer; no warp issues global loads or waits on the LSU queue behind pass 1's
-            // stores.  Thread 0 is the team's service thread: it publishes A team kb's tiles, waits (acquire) until all
-            // 16 tiles of the item are in the ring, issues the copy, and as soon as the copy has landed frees the ring slot.
             const uint32_t buf = ib % NB, use = ib / NB;
-            const uint32_t btile = sb + SM::bpriv + buf * 32768, bfull = sb + SM::bfull + 8 * buf, bempty = sb + SM::bempty + 8 * buf;
-            const uint32_t in_a = btile + hw * 2048 + a * 8;     // + 128 r: T[n2][k1 = a + 16 r]
-            const uint32_t xw0 = btile + hw * 2048 + a * 136;    // (xw0 ^ (p << 3)):            element (a, p)
-            const uint32_t xr0 = btile + hw * 2048 + a * 8;      // (xr0 ^ (aa << 3)) + 128 aa:  element (aa, p = a)
-            // copy of item `it` of this team into its tile buffer, if the buffer has been read out (item it - NB, either
-            // team) and all 16 tiles of the item are in the ring (d1, acquired: `ready`); non-blocking
-            auto try_load = [&](uint32_t it, bool ready) {
-                const uint32_t bf = it % NB, us = it / NB;
-                if (us > 0 && !mbar_test_wait(sb + SM::bempty + 8 * bf, (us - 1) & 1)) return;
-                if (!ready) return;
-                if (!(BEGE_ABL & 8)) {
-                    fence_proxy_async_smem();
-                    mbar_arrive_expect_tx(sb + SM::bfull + 8 * bf, 32768);
-                    bulk_load(sb + SM::bpriv + bf * 32768, myring + (uint64_t)(it % kRing) * kN + 4096 * b, 32768,
-                              sb + SM::bfull + 8 * bf, policy_evict_first());
-                }
-                ld_it = it + 2;
-            };
+            // half-warp hw owns row hw of the tile (2 KiB) and, once the row is in registers, uses the same 2 KiB as its
+            // private exchange area: element (a, p) at a * 128 + ((a ^ p) << 3), conflict free both ways
+            const uint32_t row = sb + SM::btile + buf * 32768 + hw * 2048;
+            const uint32_t in_a = row + a * 8;               // + 128 r:                     T[n2][k1 = a + 16 r]
+            const uint32_t xw0 = row + a * 136;              // (xw0 ^ (p << 3)):            element (a, p)
+            const uint32_t xr0 = row + a * 8;                // (xr0 ^ (aa << 3)) + 128 aa:  element (aa, p = a)
             if (t == 0) {
                 const unsigned long long target = 16ull * (ib / kRing + 1);
                 const long long t0 = clock64();
@@ -668,7 +530,7 @@ k_search(const __grid_constant__ SearchArgs A)
                         publish(-1);
                         try_load(ib, (BEGE_ABL & 1) || counter_load_acquire(d1 + slot) >= target);
                     }
-                    if (ld_it > ib && ((BEGE_ABL & 8) || mbar_test_wait(bfull, use & 1))) break;
+                    if (ld_it > ib && ((BEGE_ABL & 8) || mbar_test_wait(sb + SM::bfull + 8 * buf, use & 1))) break;
                     if (*(volatile int*)abort_flag) break;
                     if (clock64() - t0 > kSpinLimit) { *(volatile int*)abort_flag = 1; break; }
                     __nanosleep(40);
@@ -683,49 +545,18 @@ k_search(const __grid_constant__ SearchArgs A)
             __syncwarp();
             mbar_wait(sb + SM::bgo + 8 * kb, nit & 1, abort_flag);
             ++nit;
+            c2 v[16];
             lds16<128>(in_a, v);
             const uint64_t pair = (A.j0 + jl) * (uint64_t)A.S + (A.m0 + ml);
             const float part = __ldcg(A.sigpart + (pair - A.sig_pair0) * 16 + a);
-#else
-#if !(BEGE_ABL & 1)
-            if (t == 0 && d1v < 16ull * (ib / kRing + 1)) {  // wait until all 16 tiles of the item are in the ring
-                const unsigned long long target = 16ull * (ib / kRing + 1);
-                const long long t0 = clock64();
-                for (;;) {
-                    publish(-1);
-                    if (counter_load_acquire(d1 + slot) >= target) break;
-                    if (*(volatile int*)abort_flag) break;
-                    if (clock64() - t0 > kSpinLimit) { *(volatile int*)abort_flag = 1; break; }
-                    __nanosleep(100);
-                }
-            }
-#endif
-            __syncwarp();
-            bar_named(bar_id, 256);                          // ... and every warp of the team is done with its
-            if (t == 0) publish(prev_slot);                  // loads of the team's previous item: free that slot
-            const c2* src = myring + (uint64_t)slot * kN + row_off;
-#pragma unroll
-            for (int r = 0; r < 16; ++r) v[r] = (BEGE_ABL & 8) ? mk((float)(r + a), (float)ib) : __ldcg(src + kRowStep * r);
-            const uint64_t pair = (A.j0 + jl) * (uint64_t)A.S + (A.m0 + ml);
-            const float part = __ldcg(A.sigpart + (pair - A.sig_pair0) * 16 + a);
-            // look at the counter of the team's next item now: the answer is there when the item starts
-            d1v = 0;
-            if (!(BEGE_ABL & 1) && t == 0 && ib + 2 < n_items) d1v = counter_load_acquire(d1 + (ib + 2) % kRing);
-#endif
             c2 wa[2], wb[2];
-            if (TM_TW) {
-                tmem_ld4(tq + kTmDelta, wa);
-                // four-step factor wN^(16 b k1), k1 = a + 16 r: its CTA-uniform part w256^(b r) here, the rest in delta_p
+            tmem_ld4(tq + kTmDelta, wa);
+            // four-step factor wN^(16 b k1), k1 = a + 16 r: its CTA-uniform part w256^(b r) here, the rest in delta_p
 #pragma unroll
-                for (int r = 1; r < 16; ++r) { const float2 w = c_w256[(b * r) & 255]; v[r] = cmulw(v[r], w.x, w.y); }
-            } else {
-                twiddle16<false>(tbl_a, v);                  // wN^(16 k1 q), q = b
-            }
+            for (int r = 1; r < 16; ++r) { const float2 w = c_w256[(b * r) & 255]; v[r] = cmulw(v[r], w.x, w.y); }
             const float sumR2 = hw_sum16(part);
             fft16<+1>(v);
-            if (TM_TW) tm_twiddle<0, 8>(tq + kTmDelta, v, wa, wb);    // v[p] *= delta_p = wN^(16 b a) w256^(a p)
-            else twiddle16<true>(w1_a, v);                            // w256^(a p)
-#if BEGE_BTMA
+            tm_twiddle<0, 8>(tq + kTmDelta, v, wa, wb);      // v[p] *= delta_p = wN^(16 b a) w256^(a p)
             __syncwarp();                                    // every lane of the half-warp has its row in registers
 #pragma unroll
             for (int p = 0; p < 16; ++p) sts64<0>(xw0 ^ (uint32_t)(p << 3), v[p]);
@@ -734,15 +565,9 @@ k_search(const __grid_constant__ SearchArgs A)
             for (int aa = 0; aa < 16; ++aa) v[aa] = lds64<0>((xr0 ^ (uint32_t)(aa << 3)) + 128 * aa);
             fence_proxy_async_smem();                        // these generic accesses before the next bulk copy into the tile
             __syncwarp();
-            if (lane == 0) mbar_arrive(bempty);
+            if (lane == 0) mbar_arrive(sb + SM::bempty + 8 * buf);
             if (t == 0 && ib + 2 < n_items && ld_it == ib + 2)   // bring in the team's next item while this one is finished
                 try_load(ib + 2, (BEGE_ABL & 1) || (d1v_it == ib + 2 && d1v >= 16ull * ((ib + 2) / kRing + 1)));
-#else
-            sts16<8>(pw_a, v);
-            __syncwarp();
-            lds16<136>(pr_a, v);
-            __syncwarp();
-#endif
             fft16<+1>(v);
             // lane a holds Z[n1 = a + 16 q]; lag n = 256 n1 + n2
             const float thr = A.k2 * sumR2;
@@ -819,16 +644,10 @@ k_search(const __grid_constant__ SearchArgs A)
                     }
                 }
             }
-            prev_slot = slot;
         }
-#if BEGE_BTMA
-        prev_slot = -1;                                      // every slot was freed when its copy landed
-#else
-        bar_named(bar_id, 256);
-#endif
-        if (t == 0) {
-            publish(prev_slot);
-            while (PUB && pub_it < n_items) {                // tiles A team kb stores after this team's last item
+        if (t == 0) {                                        // tiles A team kb stores after this team's last copy
+            publish(-1);
+            while (PUB && pub_it < n_items) {
                 mbar_wait(sb + SM::amb + 8 * (pub_it % kRing), (pub_it / kRing) & 1, abort_flag);
                 if (*(volatile int*)abort_flag) break;
                 publish(-1);
@@ -1186,7 +1005,6 @@ extern "C" int bege_segment_load(bege_plan* p, const float* x, uint32_t S)
 static void set_l2_window(bege_plan* p, void* ring)
 {
     if (p->l2_window == ring) return;
-    if (getenv("BEGE_NOL2WIN")) return;
     const size_t bytes = (size_t)p->G * kRing * kN * sizeof(c2);
     if (!p->l2_limit_saved) { cudaDeviceGetLimit(&p->l2_limit_prev, cudaLimitPersistingL2CacheSize); p->l2_limit_saved = true; }
     cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, bytes);

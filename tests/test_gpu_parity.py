@@ -6,7 +6,7 @@ identical except for entries within 1e-4*sigma of the threshold; integer fields 
 import numpy as np
 import pytest
 
-from paper_1708_01609_b200 import synth
+import bege_synth as synth
 
 pytestmark = pytest.mark.gpu
 

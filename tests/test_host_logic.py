@@ -9,7 +9,8 @@ import socket
 import numpy as np
 import pytest
 
-from paper_1708_01609_b200 import bege, shard, synth, build
+from paper_1708_01609_b200 import bege, shard, build
+import bege_synth as synth
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 

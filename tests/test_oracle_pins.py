@@ -11,7 +11,7 @@ import numpy as np
 import pytest
 
 from oracle import bege_oracle as bo
-from paper_1708_01609_b200 import synth
+import bege_synth as synth
 
 FS, N, BAND, TAU = synth.FS, synth.N_SEG, synth.BAND, synth.TAU
 GOLD = os.path.join(os.path.dirname(__file__), "golden", "paper_numbers.txt")
