@@ -226,8 +226,8 @@ template <int NI> struct SearchSmem {
     static constexpr uint32_t amb = bars + 32;                   // [kRing] mbarriers: tile of ring slot stored (8 A warps)
     static constexpr uint32_t bfull = amb + 8 * kRing;           // [kNB] mbarriers: row tile has arrived
     static constexpr uint32_t bempty = bfull + 24;               // [kNB] mbarriers: ... has been read out (8 B warps)
-    static constexpr uint32_t bgo = bempty + 24;                 // [2] mbarriers: the B team's next row tile is there (thread 0)
-    static constexpr uint32_t total = bgo + 16;
+    static constexpr uint32_t bgo = bempty + 24;                 // [2][4] mbarriers: row tile of the B team's item is there (thread 0)
+    static constexpr uint32_t total = bgo + 64;
     static_assert(total + 128 <= 232448, "shared memory of one SM");
 };
 // the stationary tile has its tensor-memory arrangement written out for bands that need 14 of the 16 row-blocks;
@@ -322,7 +322,7 @@ k_search(const __grid_constant__ SearchArgs A)
         mbar_init(sb + SM::bars, 1); mbar_init(sb + SM::bars + 8, 1);
         for (int i = 0; i < kRing; ++i) mbar_init(sb + SM::amb + 8 * i, 8);
         for (int i = 0; i < SM::kNB; ++i) { mbar_init(sb + SM::bfull + 8 * i, 1); mbar_init(sb + SM::bempty + 8 * i, 8); }
-        mbar_init(sb + SM::bgo, 1); mbar_init(sb + SM::bgo + 8, 1);
+        for (int i = 0; i < 8; ++i) mbar_init(sb + SM::bgo + 8 * i, 1);
         fence_mbar_init();
     }
     if (threadIdx.x < 32) tmem_alloc<kTmemCols>(sb + SM::bars + 24);
@@ -537,13 +537,16 @@ k_search(const __grid_constant__ SearchArgs A)
                 }
                 // The other seven warps wait on a per-team barrier, not on the tile's own: the tile buffers are shared
                 // by both teams, and a warp that runs ahead could otherwise mistake an older phase of the same parity.
-                mbar_arrive(sb + SM::bgo + 8 * kb);
+                // Four barriers rotate over the team's items: this thread is never more than NB = 3 items ahead of the
+                // team's slowest warp (a buffer is refilled only after all eight warps have read it out), so a waiter
+                // and this thread never meet on a barrier in different uses.
+                mbar_arrive(sb + SM::bgo + 32 * kb + 8 * (nit & 3));
                 publish(slot);                               // the rows are in shared memory: the ring slot is free
                 // look at the counter of the team's next item now; the answer is used after the exchange
                 if (!(BEGE_ABL & 1) && ib + 2 < n_items && ld_it == ib + 2) { d1v = counter_load_acquire(d1 + (ib + 2) % kRing); d1v_it = ib + 2; }
             }
             __syncwarp();
-            mbar_wait(sb + SM::bgo + 8 * kb, nit & 1, abort_flag);
+            mbar_wait(sb + SM::bgo + 32 * kb + 8 * (nit & 3), (nit >> 2) & 1, abort_flag);
             ++nit;
             c2 v[16];
             lds16<128>(in_a, v);

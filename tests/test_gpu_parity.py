@@ -405,3 +405,150 @@ def test_band_threshold_matches_oracle(cfg0, bo):
     t_all, n_all = plan.search(k_lo, cap=1 << 20)
     t_inf, n_inf = plan.search_band(k_lo, float("inf"), cap=1 << 20)
     assert n_inf == n_all and np.array_equal(np.sort(key(t_inf)), np.sort(key(t_all)))
+
+
+# ----------------------------------------------------------------------------- paths the round-1 suite did not reach
+def test_full_row_blocks_batched(bo, bege):
+    """A band that needs all 16 row-blocks AND several segments per call: k_search<0, 16, batched>, whose
+    stationary template tile is read from global memory and whose segment tiles stream through shared memory."""
+    band = (100.0, 1900.0)
+    xs = np.stack([synth.as_segment(synth.band_limit(synth.white_noise(80 + s), FS, *band)) for s in range(3)])
+    f0, fd = synth.bank_grid(2, 3, 200.0, 1600.0, -150.0, 150.0)
+    Xs = np.stack([bo.segment_spectrum(x, FS, *band) for x in xs])
+    k = 2.8
+    lo_tails, _, sigma_o, _ = bo.search(Xs, f0, fd, TAU, FS, k - 1e-3)
+    with bege.Plan(N, FS, band) as plan:
+        plan.bank_generate(f0, fd, TAU)
+        plan.segment_load(xs)
+        tails, n = plan.search(k, cap=1 << 20)
+        must, _ = check_tail_sets(tails, n, lo_tails, k)
+        assert must > 200
+        sg = plan.get_sigma()
+        assert np.max(np.abs(sg - sigma_o) / sigma_o) <= SIGMA_RTOL
+        for (j, m) in ((0, 0), (3, 1), (5, 2)):
+            z, s = bo.correlate(Xs[m], bo.template(f0[j], fd[j], TAU, FS, N))
+            zg, sgj = plan.debug_correlate(j, m)
+            assert rel_l2(zg.astype(np.complex128), z) <= REL_L2 and abs(sgj - s) / s <= SIGMA_RTOL
+
+
+@pytest.mark.parametrize("grid,seed", [(1024, 2), (512, 3)])
+def test_corner_templates_of_the_large_banks(bo, bege, grid, seed):
+    """z and sigma on the four corners of the configs[2] (1024 x 1024) and configs[4] (512 x 512) grids:
+    (350 Hz, -400 Hz/s) ... (2000 Hz, +400 Hz/s).  The corner templates keep only part of their energy in band --
+    the case that needs the fp64 bank transform."""
+    f0, fd = synth.bank_grid(grid, grid, 350.0, 2000.0, -400.0, 400.0)
+    corners = np.array([0, grid - 1, grid * (grid - 1), grid * grid - 1])
+    x = synth.noise_segment(seed)[None, :]
+    X = bo.segment_spectrum(x[0], FS, *BAND)
+    with bege.Plan(N, FS, BAND) as plan:
+        plan.bank_generate(f0[corners], fd[corners], TAU)
+        plan.segment_load(x)
+        for j in range(4):
+            z, s = bo.correlate(X, bo.template(f0[corners[j]], fd[corners[j]], TAU, FS, N))
+            zg, sgj = plan.debug_correlate(j, 0)
+            assert rel_l2(zg.astype(np.complex128), z) <= REL_L2, (corners[j], rel_l2(zg.astype(np.complex128), z))
+            assert abs(sgj - s) / s <= SIGMA_RTOL
+
+
+def test_split_launches_equal_one_launch(bo, bege):
+    """bege_search splits a search whose items per CTA group exceed the kernel's 32-bit count into several launches
+    that share the record buffer; a debug setter lowers the limit so that a small bank reaches that branch."""
+    w = synth.config0()
+    X = bo.segment_spectrum(w.x[0], FS, *BAND)
+    k = 3.0
+    key = lambda tt: np.sort(tt["template_id"].astype(np.uint64) << np.uint64(32) | tt["lag"].astype(np.uint64))
+    with bege.Plan(N, FS, BAND) as plan:
+        plan.bank_generate(w.f0, w.fdot, TAU)
+        plan.segment_load(w.x)
+        one, n_one = plan.search(k, cap=1 << 20)
+        s_one = plan.get_sigma().copy()
+        launches0 = plan.stats()["kernel_launches"]
+        plan.debug_set_max_items(3)                      # 3 items per group and launch: 256 templates -> 10 launches
+        many, n_many = plan.search(k, cap=1 << 20)
+        assert plan.stats()["kernel_launches"] - launches0 >= 10
+        s_many = plan.get_sigma().copy()
+        snr_a, id_a, nh_a = plan.search_maxproj(k)
+        plan.debug_set_max_items((1 << 30) - 1)
+        snr_b, id_b, nh_b = plan.search_maxproj(k)
+    assert n_many == n_one and np.array_equal(key(one), key(many))
+    assert np.array_equal(s_one, s_many)
+    assert nh_a == nh_b and np.array_equal(snr_a, snr_b) and np.array_equal(id_a, id_b)
+    lo_tails, _, _, _ = bo.search(X[None, :], w.f0, w.fdot, TAU, FS, k - 1e-3, cap=1 << 20)
+    check_tail_sets(many, n_many, lo_tails, k)
+
+
+def test_soak_repeated_large_searches(bege):
+    """Twelve searches of a 147,456-template slice of the configs[2] bank (16,384 ring cycles per group each):
+    the hand-over protocol must give bit-identical tail sets and sigma every time."""
+    f0, fd = synth.config2_bank()
+    T, j_lo = 147456, 300_000
+    x = synth.noise_segment(2)[None, :]
+    key = lambda tt: np.sort(tt["template_id"].astype(np.uint64) << np.uint64(32) | tt["lag"].astype(np.uint64))
+    with bege.Plan(N, FS, BAND) as plan:
+        plan.bank_generate(f0[j_lo:j_lo + T], fd[j_lo:j_lo + T], TAU)
+        plan.segment_load(x)
+        ref = sref = None
+        for i in range(12):
+            tails, n = plan.search(3.6, cap=1 << 22)
+            assert n == tails.size and n > 1000
+            kk, sg = key(tails), plan.get_sigma()
+            if ref is None:
+                ref, sref = kk, sg.copy()
+            assert np.array_equal(kk, ref) and np.array_equal(sg, sref), i
+
+
+def test_bench_chunk_sized_launch_sampled(bo, bege):
+    """One search of the size bench.py launches per chunk (366,048 templates of the configs[2] bank, S = 1): sliced
+    into eight launches whose record copies overlap the next slice; sampled templates against the oracle."""
+    import torch
+    f0, fd = synth.config2_bank()
+    free, _ = torch.cuda.mem_get_info()
+    T = int(min(366048, (free * 0.85) // (14 * 32768)))  # bench.py sizes its chunks the same way (366,048 on 180 GB)
+    T -= T % 72
+    j_lo = 366048                                        # the second of bench.py's three chunks
+    x = synth.noise_segment(2)[None, :]
+    k = 4.0
+    X = bo.segment_spectrum(x[0], FS, *BAND)
+    with bege.Plan(N, FS, BAND) as plan:
+        plan.bank_generate(f0[j_lo:j_lo + T], fd[j_lo:j_lo + T], TAU)
+        plan.segment_load(x)
+        tails, n = plan.search(k, cap=1 << 22)
+        sg = plan.get_sigma()[:, 0]
+    assert n == tails.size and n > 100
+    assert tails["template_id"].max() < T and tails["lag"].max() < N and np.all(tails["snr"] > k)
+    assert np.all(np.isfinite(sg)) and np.all(sg > 0)
+    fired = np.unique(tails["template_id"])
+    sample = np.unique(np.concatenate([fired[:: max(1, fired.size // 24)][:24], np.arange(11, T, T // 24), [0, T - 1]]))
+    lo_tails, _, sigma_o, _ = bo.search(X[None, :], f0[j_lo + sample], fd[j_lo + sample], TAU, FS, k - 1e-3)
+    sel = tails[np.isin(tails["template_id"], sample)].copy()
+    sel["template_id"] = np.searchsorted(sample, sel["template_id"]).astype(np.uint32)
+    check_tail_sets(sel, sel.size, lo_tails, k)
+    assert np.max(np.abs(sg[sample] - sigma_o[:, 0]) / sigma_o[:, 0]) <= SIGMA_RTOL
+
+
+def test_config4_full_size_tail_heavy(bo, bege):
+    """configs[4] at full size: 2^18 templates, k = 3, tens of millions of records (hundreds of MB) through the sliced
+    search with overlapped record copies; every record's fields are checked for consistency, the count against the
+    sum over the per-slice properties, and a strided sample of templates against the oracle."""
+    w = synth.config4()
+    T = w.n_templates
+    assert T == 1 << 18
+    k = 3.0
+    cap = 90_000_000
+    X = bo.segment_spectrum(w.x[0], FS, *BAND)
+    with bege.Plan(N, FS, BAND) as plan:
+        plan.bank_generate(w.f0, w.fdot, TAU)
+        plan.segment_load(w.x)
+        tails, n = plan.search(k, cap=cap, copy=False)
+        sg = plan.get_sigma()[:, 0]
+        assert n == tails.size and 20_000_000 < n < cap          # roughly 0.3 % of 1.7e10 outputs (BASELINE.json)
+        assert int(tails["template_id"].max()) < T and int(tails["lag"].max()) < N
+        assert float(tails["snr"].min()) >= k * (1 - 1e-6)        # |z|^2 > k^2 sum|R|^2 in fp32; the reported ratio rounds once more
+        counts = np.bincount(tails["template_id"], minlength=T)
+        sample = np.arange(5, T, T // 48)[:48]
+        lo_tails, _, sigma_o, _ = bo.search(X[None, :], w.f0[sample], w.fdot[sample], TAU, FS, k - 1e-3, cap=1 << 22)
+        sel = tails[np.isin(tails["template_id"], sample)].copy()
+        assert sel.size == int(counts[sample].sum())
+        sel["template_id"] = np.searchsorted(sample, sel["template_id"]).astype(np.uint32)
+        check_tail_sets(sel, sel.size, lo_tails, k)
+        assert np.max(np.abs(sg[sample] - sigma_o[:, 0]) / sigma_o[:, 0]) <= SIGMA_RTOL
