@@ -5,15 +5,22 @@ One "step" = one pass of the whole 2^20-template bank (1024 x 1024 grid, 350-200
 against one 16 s segment of band-limited Gaussian noise (seed 2), k = 6.  The bank (2^20 x 448 KiB of
 in-band spectra) does not fit HBM, so it is processed in chunks: chunk generation (bege_bank_generate) is
 untimed, as BASELINE.json configs[2] states ("template spectra are precomputed once, and the search is
-timed separately from generation"); the timed region of a step is the sum over chunks of bege_search,
-each bracketed by a device synchronize and CUDA events on the plan's stream.
+timed separately from generation") but its time is reported beside the number; the timed region of a step
+is the sum over chunks of bege_search, each bracketed by a device synchronize and CUDA events on the
+plan's stream.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--templates T]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference|cufft] [--templates T]
 
-N > 1 (torchrun): every rank searches its own 2^20-template shard of an N-times finer fdot grid (weak
-scaling, no data-path collective); tail records are gathered on rank 0 after the timed region.
---impl reference times the fp64 CPU oracle (oracle/) on the host cores, on a bounded sample.
---impl cufft times the same steps built from library kernels (torch + cuFFT): a reference point for context only.
+The same JSON line also carries two more workloads of BASELINE.json: `segment_batched`
+(configs[3]: 64 segments x 2^16 templates) and `tail_heavy` (configs[4]: 2^18 templates at k = 3, tens of
+millions of records crossing PCIe while the search goes on).
+
+--gpus N > 1 without a torchrun environment: bench.py starts N ranks itself (torch.distributed.run,
+127.0.0.1).  Every rank searches its own 2^20-template shard of an N-times finer fdot grid (weak scaling,
+no data-path collective); after the timed region the tail records of all ranks are gathered on rank 0
+(shard.gather_tails).  --impl reference times the fp64 CPU oracle (oracle/) on the host cores, on a
+bounded sample.  --impl cufft times the same steps built from library kernels (torch + cuFFT): a
+reference point for context only.
 """
 from __future__ import annotations
 
@@ -37,9 +44,11 @@ METRIC = "template correlations/sec at N=2^16 C2C fp32 on 1 B200; % of FFT roofl
 UNIT = "correlations/s"
 FFT_FLOP = 5.0 * 65536 * 16                       # PAPER.md:134 eq.(10): 5 N log2 N
 ALG_BYTES_PER_CORR = 52802 * 8                    # two-sided in-band template spectrum, S = 1
-# dram__bytes_read.sum + dram__bytes_write.sum of k_search per correlation, from the ncu --set full capture summarised
-# in profiles/r1g_search_kernel_final.md (36,864-template launch: 16.914 GB read + 0.365 GB written)
-NCU_DRAM_BYTES_PER_CORR = (16.913879e9 + 0.365349e9) / 36864
+# dram__bytes_read.sum + dram__bytes_write.sum of k_search per correlation: an OFFLINE constant, taken from the
+# `ncu --set full` capture of the kernel as committed (profiles/r2_search_kernel.md: 36,864-template launch,
+# 16.914 GB read + 0.005 GB written); it does not follow later kernel changes by itself.
+NCU_DRAM_BYTES_PER_CORR = (16.914e9 + 0.005e9) / 36864
+NCU_SOURCE = "profiles/r2_search_kernel.md"
 FP32_PEAK = 148 * 128 * 2 * 1.965e9               # SMs x fp32 lanes x 2 flop x max SM clock
 
 
@@ -94,7 +103,7 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------ oracle arm
-def oracle_rate(f0, fdot, x, k_sigma, sample: int, seconds_hint: float = 0.0):
+def oracle_rate(f0, fdot, x, k_sigma, sample: int):
     """Correlations/s of the fp64 CPU oracle, as it stands, on a strided sample of the bank."""
     from oracle import bege_oracle as bo
     X = np.stack([bo.segment_spectrum(xm, synth.FS, *synth.BAND) for xm in x])
@@ -190,14 +199,117 @@ def run_cufft(args, rank, local_rank):
           flush=True)
 
 
+# ------------------------------------------------------------------------------------------ launch self-test stand-in
+class _LaunchSelfTestPlan:
+    """NOT a search.  `--selftest-launch` exercises bench.py's own multi-rank plumbing (spawn, rendezvous, barrier,
+    max-over-ranks timing, gather of tail records on rank 0) on a box without GPUs; it stands in for bege.Plan with
+    the same method names, produces a few fixed records per chunk and never runs under any other flag.  The JSON
+    line of such a run carries "selftest_launch": true and value null."""
+
+    def __init__(self, rank):
+        self.rank, self.n, self.launches = rank, 0, 0
+
+    def stats(self):
+        return {"hbm_bytes_per_template": 14 * 32768, "kernel_launches": self.launches, "fused_kernel_ms": 1.0,
+                "fused_kernel_launches": 1}
+
+    def alloc_workspace(self, *a):
+        return 0
+
+    def bank_generate(self, f0, fdot, tau):
+        self.n = len(f0)
+
+    def segment_load(self, x):
+        self.launches += 2
+
+    def search(self, k, cap=0, copy=True):
+        from paper_1708_01609_b200 import bege
+        self.launches += 1
+        t = np.zeros(3, dtype=bege.TAIL_DTYPE)
+        t["template_id"] = [0, self.n // 2, self.n - 1]
+        t["lag"] = 100 + self.rank
+        t["snr"] = 7.0
+        time.sleep(0.01)
+        return t, 3
+
+    def set_profiling(self, on): pass
+    def reset_stats(self): pass
+    def close(self): pass
+
+
 # ------------------------------------------------------------------------------------------ our arm
+def _extra_workloads(args, dev, local_rank):
+    """configs[3] (segment-batched) and configs[4] (tail-heavy), measured like the headline: CUDA events around
+    bege_search, wall clock around segment_load + search for the end-to-end figure.  Rank 0, N = 1 only."""
+    import torch
+    from paper_1708_01609_b200 import bege
+    out = {}
+
+    def timed(plan, x_host, k, cap, reps):
+        rates, e2e, n = [], [], 0
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for i in range(reps + 1):
+            torch.cuda.synchronize(dev)
+            t0 = time.perf_counter()
+            plan.segment_load(x_host)
+            e0.record()
+            _t, n = plan.search(k, cap=cap, copy=False)
+            e1.record()
+            torch.cuda.synchronize(dev)
+            t1 = time.perf_counter()
+            if i:                                                    # first pass warms up
+                rates.append(plan.n_templates * plan.n_segments / (e0.elapsed_time(e1) * 1e-3))
+                e2e.append(plan.n_templates * plan.n_segments / (t1 - t0))
+        return float(np.median(rates)), float(np.median(e2e)), int(n)
+
+    def kernel_rate(plan, k, cap):
+        plan.set_profiling(True); plan.reset_stats()
+        plan.search(k, cap=cap, copy=False)
+        st = plan.stats(); plan.set_profiling(False)
+        return plan.n_templates * plan.n_segments / (st["fused_kernel_ms"] * 1e-3)
+
+    # ---- configs[3]: 64 segments x 2^16 templates (the paper's M^2 block structure, PAPER.md:158-160)
+    w = synth.config3(args.batched_segments)
+    x_host = torch.from_numpy(w.x).pin_memory()
+    with bege.Plan(synth.N_SEG, synth.FS, synth.BAND, device=local_rank) as plan:
+        t0 = time.perf_counter(); plan.bank_generate(w.f0, w.fdot, synth.TAU); gen_s = time.perf_counter() - t0
+        rate, e2e, n = timed(plan, x_host, w.k_sigma, 1 << 20, args.extra_reps)
+        krate = kernel_rate(plan, w.k_sigma, 1 << 20)
+    out["segment_batched"] = {
+        "workload": f"configs[3]: {w.x.shape[0]} segments x {w.n_templates} templates, k = {w.k_sigma}",
+        "S": int(w.x.shape[0]), "T": int(w.n_templates), "corr_per_s": rate, "kernel_corr_per_s": krate,
+        "frac": rate * FFT_FLOP / FP32_PEAK, "e2e_corr_per_s": e2e, "n_tails": n,
+        "h2d_bytes": int(w.x.size * 8), "d2h_bytes": 8 + 12 * n, "bank_generate_ms": 1e3 * gen_s}
+    del x_host
+    torch.cuda.empty_cache()
+
+    # ---- configs[4]: 2^18 templates, k = 3: ~6e7 records (0.7 GB) must cross PCIe without holding up the search
+    w = synth.config4()
+    x_host = torch.from_numpy(w.x).pin_memory()
+    cap = args.tail_cap
+    with bege.Plan(synth.N_SEG, synth.FS, synth.BAND, device=local_rank) as plan:
+        t0 = time.perf_counter(); plan.bank_generate(w.f0, w.fdot, synth.TAU); gen_s = time.perf_counter() - t0
+        rate, e2e, n = timed(plan, x_host, w.k_sigma, cap, args.extra_reps)
+        krate = kernel_rate(plan, w.k_sigma, cap)
+    out["tail_heavy"] = {
+        "workload": f"configs[4]: 1 segment + 40 glitches x {w.n_templates} templates, k = {w.k_sigma}",
+        "T": int(w.n_templates), "k": w.k_sigma, "corr_per_s": rate, "kernel_corr_per_s": krate,
+        "frac": rate * FFT_FLOP / FP32_PEAK, "e2e_corr_per_s": e2e, "n_tails": n, "cap": cap,
+        "d2h_bytes": 8 + 12 * min(n, cap), "d2h_note": "records of search slice i are copied on a side stream "
+        "while slice i+1 is searched (8 slices); corr_per_s includes those copies", "bank_generate_ms": 1e3 * gen_s}
+    return out
+
+
 def run_ours(args, rank, world, local_rank):
     import torch
     import torch.distributed as dist
     from paper_1708_01609_b200 import bege, shard
 
-    torch.cuda.set_device(local_rank)
-    dev = torch.device("cuda", local_rank)
+    selftest = args.selftest_launch
+    dev = None
+    if not selftest:
+        torch.cuda.set_device(local_rank)
+        dev = torch.device("cuda", local_rank)
     T_total = args.templates
     # weak scaling: rank r owns templates [r*T, (r+1)*T) of an N-times finer fdot grid
     if world == 1 and T_total == 1 << 20:
@@ -209,53 +321,74 @@ def run_ours(args, rank, world, local_rank):
         else:
             f0a, fda = synth.bank_grid(1, T_total * world, 1100.0, 1100.0, -400.0, 400.0)
         f0, fdot = f0a[rank::world].copy(), fda[rank::world].copy()
-    x_host = torch.from_numpy(synth.noise_segment(2)[None, :]).pin_memory()
+    x_np = synth.noise_segment(2)[None, :]
+    x_host = torch.from_numpy(x_np) if selftest else torch.from_numpy(x_np).pin_memory()
     k_sigma, cap = 6.0, 1 << 16
 
-    plan = bege.Plan(synth.N_SEG, synth.FS, synth.BAND, device=local_rank)
+    if selftest:
+        plan = _LaunchSelfTestPlan(rank)
+        chunk = args.chunk or T_total
+    else:
+        plan = bege.Plan(synth.N_SEG, synth.FS, synth.BAND, device=local_rank)
+        tpl_bytes = plan.stats()["hbm_bytes_per_template"]
+        free, _total = torch.cuda.mem_get_info(dev)
+        chunk = args.chunk or int(min(T_total, (free * 0.88) // tpl_bytes))
+        chunk = max(72, chunk - chunk % 72) if chunk < T_total else T_total
+        plan.alloc_workspace(chunk, 1, cap)
     tpl_bytes = plan.stats()["hbm_bytes_per_template"]
-    free, _total = torch.cuda.mem_get_info(dev)
-    chunk = args.chunk or int(min(T_total, (free * 0.88) // tpl_bytes))
-    chunk = max(72, chunk - chunk % 72) if chunk < T_total else T_total
-    plan.alloc_workspace(chunk, 1, cap)
     chunks = shard.chunk_ranges(0, T_total, chunk)
     plan.segment_load(x_host)
 
     sampler = ClockSampler(local_rank)
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in chunks]
+    ev = None if selftest else [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in chunks]
 
     def barrier():
-        torch.cuda.synchronize(dev)
+        if not selftest:
+            torch.cuda.synchronize(dev)
         if world > 1:
             dist.barrier()
 
+    last_tails = []
+
     def one_step(timed: bool, windows, acc):
         """generation untimed; per chunk: [segment_load from pinned host + search] = e2e, [search] = value."""
-        n_tails = 0
+        n_tails, search_ms = 0, 0.0
+        last_tails.clear()
         for ci, (a, b) in enumerate(chunks):
-            plan.bank_generate(f0[a:b], fdot[a:b], synth.TAU)              # untimed (configs[2])
+            g0 = time.perf_counter()
+            plan.bank_generate(f0[a:b], fdot[a:b], synth.TAU)              # untimed (configs[2]); synchronous
+            g1 = time.perf_counter()
             barrier()
             l0 = plan.stats()["kernel_launches"]
             t0 = time.perf_counter()
             plan.segment_load(x_host)                                        # H2D of the segment + forward FFT
             t1 = time.perf_counter()
-            ev[ci][0].record()
-            _tails, n = plan.search(k_sigma, cap=cap, copy=False)            # D2H of count + records inside
-            ev[ci][1].record()
-            torch.cuda.synchronize(dev)
+            if ev:
+                ev[ci][0].record()
+            tails, n = plan.search(k_sigma, cap=cap, copy=False)             # D2H of count + records inside
+            if ev:
+                ev[ci][1].record()
+                torch.cuda.synchronize(dev)
             t2 = time.perf_counter()
             n_tails += n
+            last_tails.append(shard.globalize(np.array(tails, copy=True), a + rank * T_total))
+            ms = ev[ci][0].elapsed_time(ev[ci][1]) if ev else 1e3 * (t2 - t1)
+            search_ms += ms
             if timed:
                 windows.append((t1, t2))
-                acc["search_ms"] += ev[ci][0].elapsed_time(ev[ci][1])
+                acc["search_ms"] += ms
                 acc["e2e_s"] += t2 - t0
+                acc["gen_s"] += g1 - g0
+                acc["load_s"] += t1 - t0
                 acc["d2h"] += 8 + 12 * min(n, cap)
                 acc["h2d"] += x_host.numel() * 8
                 acc["launches"] += plan.stats()["kernel_launches"] - l0
+        if timed:
+            acc["step_ms"].append(search_ms)
         return n_tails
 
     sampler.start()
-    acc = {"search_ms": 0.0, "e2e_s": 0.0, "d2h": 0, "h2d": 0, "launches": 0}
+    acc = {"search_ms": 0.0, "e2e_s": 0.0, "gen_s": 0.0, "load_s": 0.0, "d2h": 0, "h2d": 0, "launches": 0, "step_ms": []}
     windows = []
     for _ in range(args.warmup):
         one_step(False, windows, acc)
@@ -268,7 +401,7 @@ def run_ours(args, rank, world, local_rank):
     st = plan.stats()
     sampler.stop()
 
-    # dominant kernels (pass 1 + pass 2 of the search), timed alone with CUDA events on the plan's stream
+    # dominant kernel, timed alone with CUDA events on the plan's stream (each launch bracketed, synchronised)
     plan.set_profiling(True)
     plan.reset_stats()
     a, b = chunks[-1]
@@ -278,15 +411,29 @@ def run_ours(args, rank, world, local_rank):
     kern_s = pst["fused_kernel_ms"] * 1e-3
     kern_corr = b - a
 
-    search_s = torch.tensor([acc["search_ms"] * 1e-3, acc["e2e_s"]], dtype=torch.float64, device=dev)
+    times = torch.tensor([acc["search_ms"] * 1e-3, acc["e2e_s"]], dtype=torch.float64, device=dev if dev else "cpu")
+    gathered = None
     if world > 1:
-        dist.all_reduce(search_s, op=dist.ReduceOp.MAX)
-    t_search, t_e2e = float(search_s[0]), float(search_s[1])
+        dist.all_reduce(times, op=dist.ReduceOp.MAX)
+        # the only exchange of the path: the (rare) tail records of every rank's last pass, concatenated on rank 0
+        mine = np.concatenate(last_tails) if last_tails else np.zeros(0, dtype=bege.TAIL_DTYPE)
+        gathered = shard.gather_tails(mine)
+    t_search, t_e2e = float(times[0]), float(times[1])
     total_corr = T_total * world * args.steps
     value = total_corr / t_search
     e2e = total_corr / t_e2e
+    plan.close()
     if rank != 0:
-        plan.close()
+        return
+
+    if selftest:
+        print(json.dumps({"selftest_launch": True, "metric": METRIC, "value": None, "unit": UNIT, "n_gpus": world,
+                          "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_search / max(args.steps, 1),
+                          "gathered_tails": int(gathered.size) if gathered is not None else None,
+                          "gathered_ids_ok": bool(gathered is None or np.array_equal(
+                              np.sort(np.unique(gathered["template_id"] // T_total)), np.arange(world))),
+                          "config": {"workload": f"launch self-test, {T_total} templates per rank, {len(chunks)} chunks"}}),
+              flush=True)
         return
 
     peaks = {}
@@ -298,9 +445,15 @@ def run_ours(args, rank, world, local_rank):
     rate_kernel = kern_corr / kern_s
     hbm_achieved = rate_kernel * ALG_BYTES_PER_CORR * 1e-9
     alu_achieved = rate_kernel * FFT_FLOP * 1e-12
+    step_ms = np.asarray(acc["step_ms"])
+    extras = {}
+    if world == 1 and not args.no_extras:
+        del x_host
+        torch.cuda.empty_cache()
+        extras = _extra_workloads(args, dev, local_rank)
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
-        v, used, dt, _ = oracle_rate(f0, fdot, x_host.numpy(), k_sigma, args.cpu_sample)
+        v, used, dt, _ = oracle_rate(f0, fdot, x_np, k_sigma, args.cpu_sample)
         cpu = {"value": v, "unit": UNIT, "cores": used, "kind": "oracle",
                "sample": f"{args.cpu_sample} templates strided over the 2^20 bank x 1 segment ({dt:.1f} s)"}
     line = {
@@ -313,18 +466,27 @@ def run_ours(args, rank, world, local_rank):
                    "timed": "sum over chunks of bege_search (incl. D2H of tails); chunk generation untimed",
                    "l2": f"inputs larger than L2 (each chunk streams {chunk * tpl_bytes / 2**30:.1f} GiB of spectra)",
                    "tails_per_step": n_tails},
+        "median": {"ms_per_step": float(np.median(step_ms)), "value": T_total / (float(np.median(step_ms)) * 1e-3),
+                   "ms_per_step_min": float(step_ms.min()), "ms_per_step_max": float(step_ms.max())},
+        "bank_generate_ms_per_step": 1e3 * acc["gen_s"] / args.steps,
+        "segment_load_ms_per_step": 1e3 * acc["load_s"] / args.steps,
+        "untimed_note": "bank_generate (fp64, once per chunk and pass because the 2^20-template bank exceeds HBM) is not "
+                        "part of value; segment_load (H2D + forward FFT of the segment) is part of e2e only",
         "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": acc["h2d"] // args.steps,
                 "d2h_bytes_per_step": acc["d2h"] // args.steps,
                 "what": "per chunk: bege_segment_load from pinned host memory + bege_search into pinned host memory"},
         "gpu_launches": int(acc["launches"]),
-        "gpu_launches_note": "kernels of libbege.so launched inside the timed calls (per chunk: 2 segment-load kernels + 1 persistent search kernel); the untimed bank generation launched %d more" % (int(st["kernel_launches"]) - int(acc["launches"])),
+        "gpu_launches_note": "kernels of libbege.so launched inside the timed calls (per chunk: 2 segment-load kernels + "
+                             "the persistent search kernel, up to 8 launches = slices); the untimed bank generation "
+                             "launched %d more" % (int(st["kernel_launches"]) - int(acc["launches"])),
         "clocks": sampler.summary(windows),
         "gflops_equiv": value * FFT_FLOP * 1e-9,
         "roofline": {"bound": "alu", "achieved": alu_achieved, "peak": FP32_PEAK * 1e-12, "unit": "TFLOP/s",
                      "frac": alu_achieved / (FP32_PEAK * 1e-12), "traffic": NCU_DRAM_BYTES_PER_CORR * kern_corr,
-                     "traffic_note": "bytes per launch = ncu dram bytes per correlation (profiles/r1g_search_kernel_final.md) x correlations of the timed launch",
-                     "kernel": "k_search (persistent warp-specialised search kernel, one launch per bank chunk), CUDA events on the plan's stream, "
-                               f"{pst['fused_kernel_launches']} launch over {kern_corr} correlations",
+                     "traffic_source": "offline", "traffic_note": "bytes per launch group = ncu dram bytes per correlation "
+                     f"({NCU_SOURCE}) x correlations of the timed search; not re-measured in this run",
+                     "kernel": "k_search (persistent warp-specialised search kernel), CUDA events on the plan's stream, "
+                               f"{pst['fused_kernel_launches']} launches (slices of one search) over {kern_corr} correlations",
                      "peak_source": "derived: 148 SM x 128 fp32 lanes x 2 x 1.965 GHz (DESIGN.md); "
                                     "flops = 5 N log2 N per correlation (PAPER.md:134)",
                      "hbm": {"achieved": hbm_achieved, "peak": hbm_peak, "unit": "GB/s",
@@ -333,14 +495,27 @@ def run_ours(args, rank, world, local_rank):
         "cpu_baseline": cpu,
         "context": {"paper": "~8e4 correlations/s per GPU, ~1e6 on ~12 GPUs, ~65% of clFFT (AMD, OpenCL; PAPER.md:211)"},
     }
+    line.update(extras)
+    if gathered is not None:
+        line["gathered_tails"] = int(gathered.size)
     print(json.dumps(line), flush=True)
-    plan.close()
+
+
+def spawn_ranks(args):
+    """`python bench.py --gpus N` with no torchrun environment: start the N ranks here (one per GPU, 127.0.0.1)."""
+    import socket
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "WARN")
+    return subprocess.call(cmd, env=env)
 
 
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference", "cufft"])
     ap.add_argument("--templates", type=int, default=1 << 20, help="templates per GPU (default: configs[2])")
@@ -348,8 +523,16 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=24576)
     ap.add_argument("--ref-sample", type=int, default=8192)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the configs[3] / configs[4] blocks")
+    ap.add_argument("--batched-segments", type=int, default=64)
+    ap.add_argument("--extra-reps", type=int, default=2)
+    ap.add_argument("--tail-cap", type=int, default=80_000_000)
     ap.add_argument("--cufft-batch", type=int, default=2048, help="templates per step of the --impl cufft reference point")
+    ap.add_argument("--selftest-launch", action="store_true",
+                    help="exercise the multi-rank plumbing only (gloo, no GPU, no search): see _LaunchSelfTestPlan")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "ours":
+        sys.exit(spawn_ranks(args))
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -362,7 +545,7 @@ def main():
     if world > 1:
         import torch.distributed as dist
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl")
+        dist.init_process_group("gloo" if args.selftest_launch else "nccl")
     try:
         run_ours(args, rank, world, local_rank)
     finally:

@@ -5,6 +5,7 @@ import ctypes
 import os
 import re
 import socket
+import sys
 
 import numpy as np
 import pytest
@@ -144,3 +145,24 @@ def test_two_rank_bank_sharding_over_gloo():
         p.join(120)
         assert p.exitcode == 0
     assert q.get(timeout=5) is True
+
+
+def test_bench_starts_its_own_ranks_and_gathers_tails():
+    """`python bench.py --gpus 2` with no torchrun environment must start two ranks by itself, rendezvous on
+    127.0.0.1, time with max-over-ranks and gather the tail records on rank 0.  No GPU here: --selftest-launch
+    swaps the plan for a stand-in that produces three fixed records per chunk (gloo backend); everything else is
+    bench.py's real launch path."""
+    import json
+    import subprocess
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "1", "--warmup", "0",
+                          "--selftest-launch", "--templates", "1000", "--chunk", "400"],
+                         capture_output=True, text=True, timeout=300, env=env)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1, out.stdout                      # rank 0 alone prints
+    line = json.loads(lines[0])
+    assert line["selftest_launch"] is True and line["value"] is None
+    assert line["n_gpus"] == 2
+    assert line["gathered_tails"] == 2 * 3 * 3              # 2 ranks x 3 chunks x 3 records
+    assert line["gathered_ids_ok"] is True                  # ids were made global: both ranks' shards are present
