@@ -4,8 +4,7 @@
 // keep only a small part of their energy inside the analysis band.  An fp32 transform of the unit-norm template has
 // an absolute error of ~1e-7 per bin, i.e. a relative error of up to 1e-3 on such in-band bins, and the correlation
 // then misses the 2e-5 parity bound (measured: 4.5e-4).  The bank is generated once, off the timed path, so the
-// transform runs in fp64 (own radix-16 kernels below, same index maps as the fp32 kernels in bege.cu) and every
-// stored bin carries one fp32 rounding.
+// transform runs in fp64 (own radix-16 kernel below) and every stored bin carries one fp32 rounding.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -54,90 +53,107 @@ BEGE_DD void dfft16f(d2 (&a)[16])
         for (int k1 = k0 + 1; k1 < 4; ++k1) { const d2 t = a[4 * k0 + k1]; a[4 * k0 + k1] = a[4 * k1 + k0]; a[4 * k1 + k0] = t; }
 }
 
-// step A: chirp synthesis (fp64 phase) + pruned row DFTs.  grid (16, templates in batch), 256 threads.
-// Same index map as k_fwd_rows_data (bege.cu): CTA (ia, jl) owns the rows nl = ga + 16 ia; only nh < 16 inputs are
-// non-zero (L <= 4096); output G[k1 = p + 16 q][nl] times wN^(-nl k1), tile layout, fp64.
-// tw256d[m] = exp(2 pi i m / 256), twNd[m] = exp(2 pi i m / N) (host-built double tables).
-__global__ void __launch_bounds__(256)
-k_bank_rows64(const double* __restrict__ f0, const double* __restrict__ fdot, uint64_t j0, double fs, uint32_t L,
-              double inv_norm, const d2* __restrict__ tw256d, const d2* __restrict__ twNd, d2* __restrict__ G)
-{
-    __shared__ d2 samp[16][16];          // [nh][ga]
-    const int t = threadIdx.x, ia = blockIdx.x;
-    const uint64_t jl = blockIdx.y;
-    {
-        const int ga = t & 15, nh = t >> 4;
-        const uint32_t n = ga + 16 * ia + 256 * nh;
-        d2 s = dmk(0.0, 0.0);
-        if (n < L) {
-            const double tt = (double)n / fs;
-            const double cyc = f0[j0 + jl] * tt + 0.5 * fdot[j0 + jl] * tt * tt;
-            const double fr = cyc - floor(cyc);
-            double sn, cs;
-            sincospi(2.0 * fr, &sn, &cs);
-            const double w = (0.5 - 0.5 * cospi(2.0 * (double)n / (double)(L - 1))) * inv_norm;
-            s = dmk(w * cs, w * sn);
-        }
-        samp[nh][ga] = s;
-    }
-    __syncthreads();
-    const int ga = t >> 4, p = t & 15;
-    const int nl = ga + 16 * ia;
-    d2 v[16];
-#pragma unroll
-    for (int nh = 0; nh < 16; ++nh) {
-        const d2 w = tw256d[(p * nh) & 255];                    // exp(+2 pi i nh p / 256)
-        v[nh] = dmul(samp[nh][ga], w.x, -w.y);
-    }
-    dfft16f(v);
-    d2* out = G + jl * (uint64_t)65536;
-#pragma unroll
-    for (int q = 0; q < 16; ++q) {
-        const int k1 = p + 16 * q;
-        const d2 w = twNd[(nl * k1) & 65535];                   // exp(+2 pi i nl k1 / N)
-        out[((q * 16 + ia) * 16 + p) * 16 + ga] = dmul(v[q], w.x, -w.y);
-    }
-}
+// One kernel, no global scratch: H[16 m + r] = sum_n (h[n] e^(-2 pi i r n / N)) e^(-2 pi i m n / 4096), n < 4096 -- the
+// N = 65536-point spectrum of a template of at most 4096 samples is 16 interleaved 4096-point transforms of the template
+// times a slow modulation (r = k mod 16).  A CTA of 256 threads owns a template: it synthesises the 4096 samples once
+// (fp64 phase: three sincospi per thread, the rest by the exact recurrences of a quadratic phase) and runs the 16
+// transforms one after the other in shared memory (16 x 16 x 16, two exchanges, xor-swizzled), so the only global
+// traffic is the 448 KiB of fp32 spectrum it stores, in 256-byte runs.  grid = persistent CTAs over the templates.
+//   4096-point index maps:  n = nl + 256 nh,  nl = l0 + 16 l1;   m = m1 + 16 (q0 + 16 q1)
+//     S1: thread nl:        over nh -> m1, input twiddle w256^(-r nh) (the modulation), output twiddle wN^(-nl (r + 16 m1))
+//     S2: thread (m1, l0):  over l1 -> q0, twiddle w256^(-l0 q0)
+//     S3: thread (m1, q0):  over l0 -> q1
+//   bin k = 16 m + r = (16 m1 + r) + 256 (q0 + 16 q1): tile b = m1, column c = r, lane g = q0, row-block i = q1.
+// hann: L window values times 1 / ||h|| (host, fp64).  tw256d[m] = exp(2 pi i m / 256).
+constexpr int kBankSmem = 3 * 4096 * 16;   // samples + two exchange buffers, fp64 complex
 
-// step B: 256-point column DFTs over nl in fp64, stores the kept row-blocks [I0, I0 + NI) as fp32 in tile layout.
-// grid (16 tiles, batch), 256 threads, 64 KiB dynamic shared memory ([16 half-warps][256] d2, xor swizzled).
-__global__ void __launch_bounds__(256)
-k_bank_cols64(const d2* __restrict__ G, float2* __restrict__ out, uint64_t out_stride, int I0, int NI,
-              const d2* __restrict__ tw256d)
+__global__ void __launch_bounds__(256, 1)
+k_bank_gen64(const double* __restrict__ f0, const double* __restrict__ fdot, uint64_t T, double fs, uint32_t L,
+             const double* __restrict__ hann, const d2* __restrict__ tw256d, float2* __restrict__ out,
+             uint64_t out_stride, int I0, int NI)
 {
     extern __shared__ __align__(16) unsigned char bank64_smem[];
-    d2* sm = reinterpret_cast<d2*>(bank64_smem);
-    const int t = threadIdx.x, b = blockIdx.x;
-    const uint64_t jl = blockIdx.y;
-    const int c = t >> 4, g = t & 15;
-    const d2* in = G + jl * (uint64_t)65536 + (uint64_t)b * 4096;
-    d2 v[16];
-#pragma unroll
-    for (int i = 0; i < 16; ++i) v[i] = in[(i * 16 + c) * 16 + g];
-    dfft16f(v);
-    d2* priv = sm + c * 256;
-#pragma unroll
-    for (int p = 0; p < 16; ++p) {
-        const d2 w = tw256d[(g * p) & 255];
-        priv[(g << 4) + (p ^ g)] = dmul(v[p], w.x, -w.y);
+    d2* base = reinterpret_cast<d2*>(bank64_smem);          // [nh][nl]
+    d2* bufA = base + 4096;                                  // [m1][l0][l1 ^ l0]
+    d2* bufB = bufA + 4096;                                  // [m1][l0][q0 ^ l0]
+    const int t = threadIdx.x;
+    const int l0 = t & 15, l1 = t >> 4;                      // S1: nl = t = l0 + 16 l1
+    const int m1 = t >> 4;                                   // S2: (m1, l0);  S3: (m1, q0 = l0)
+    // exp(-2 pi i nl / N) and its 16th power: the thread's S1 output twiddle is rho^(r + 16 m1)
+    d2 rho, rho16;
+    {
+        double sn, cs;
+        sincospi(2.0 * (double)t / 65536.0, &sn, &cs); rho = dmk(cs, -sn);
+        sincospi(2.0 * (double)(16 * t) / 65536.0, &sn, &cs); rho16 = dmk(cs, -sn);
     }
-    __syncwarp();
+    for (uint64_t j = blockIdx.x; j < T; j += gridDim.x) {
+        {   // samples n = t + 256 nh: z_nh = exp(2 pi i c(n)), c(n) = f0 n/fs + fdot (n/fs)^2 / 2 cycles;
+            // z_(nh+1) = z_nh D_nh, D_(nh+1) = D_nh C (second differences of a quadratic are constant)
+            const double f = f0[j], fd = fdot[j], tt = (double)t / fs, dt = 256.0 / fs;
+            auto expc = [](double cyc) { double sn, cs; sincospi(2.0 * (cyc - floor(cyc)), &sn, &cs); return dmk(cs, sn); };
+            d2 z = expc(f * tt + 0.5 * fd * tt * tt);
+            d2 D = expc(f * dt + 0.5 * fd * (2.0 * tt * dt + dt * dt));
+            const d2 C = expc(fd * dt * dt);
 #pragma unroll
-    for (int a = 0; a < 16; ++a) v[a] = priv[(a << 4) + (g ^ a)];
-    __syncwarp();
-    dfft16f(v);
-    // lane p = g holds k2 = p + 16 q; stored layout: row-blocks in pairs, one 16-byte word per thread and pair
-    float4* o = reinterpret_cast<float4*>(out + jl * out_stride + (uint64_t)b * NI * 256) + t;
-#pragma unroll
-    for (int ip = 0; ip < 8; ++ip) {
-        if (2 * ip < NI) {
-            float4 w;
-            if (I0 == 1) { w = make_float4((float)v[(2 * ip + 1) & 15].x, (float)v[(2 * ip + 1) & 15].y,
-                                           (float)v[(2 * ip + 2) & 15].x, (float)v[(2 * ip + 2) & 15].y); }
-            else         { w = make_float4((float)v[2 * ip].x, (float)v[2 * ip].y,
-                                           (float)v[(2 * ip + 1) & 15].x, (float)v[(2 * ip + 1) & 15].y); }
-            o[ip * 256] = w;
+            for (int nh = 0; nh < 16; ++nh) {
+                const uint32_t n = (uint32_t)t + 256u * nh;
+                const double w = n < L ? hann[n] : 0.0;
+                base[nh * 256 + t] = dmk(w * z.x, w * z.y);
+                z = dmul(z, D.x, D.y);
+                D = dmul(D, C.x, C.y);
+            }
         }
+        __syncthreads();
+        d2 rho_r = dmk(1.0, 0.0);                            // rho^r
+        float4* o = reinterpret_cast<float4*>(out + j * out_stride);
+        for (int r = 0; r < 16; ++r) {
+            d2 v[16];
+            // ---- S1
+#pragma unroll
+            for (int nh = 0; nh < 16; ++nh) {
+                const d2 w = tw256d[(r * nh) & 255];
+                v[nh] = dmul(base[nh * 256 + t], w.x, -w.y);
+            }
+            dfft16f(v);
+            {
+                d2 w = rho_r;
+#pragma unroll
+                for (int mm = 0; mm < 16; ++mm) {
+                    bufA[mm * 256 + l0 * 16 + (l1 ^ l0)] = dmul(v[mm], w.x, w.y);
+                    w = dmul(w, rho16.x, rho16.y);
+                }
+            }
+            rho_r = dmul(rho_r, rho.x, rho.y);
+            __syncthreads();
+            // ---- S2: thread (m1, l0)
+#pragma unroll
+            for (int k = 0; k < 16; ++k) v[k] = bufA[m1 * 256 + l0 * 16 + (k ^ l0)];
+            dfft16f(v);
+#pragma unroll
+            for (int q0 = 0; q0 < 16; ++q0) {
+                const d2 w = tw256d[(l0 * q0) & 255];
+                bufB[m1 * 256 + l0 * 16 + (q0 ^ l0)] = dmul(v[q0], w.x, -w.y);
+            }
+            __syncthreads();
+            // ---- S3: thread (m1, q0 = l0)
+#pragma unroll
+            for (int k = 0; k < 16; ++k) v[k] = bufB[m1 * 256 + k * 16 + (l0 ^ k)];
+            dfft16f(v);
+            // v[q1] = H[k], k = (16 m1 + r) + 256 (q0 + 16 q1): tile m1, thread 16 r + q0, row-block q1 (stored in pairs)
+            float4* ot = o + (size_t)m1 * (NI / 2) * 256 + 16 * r + l0;
+#pragma unroll
+            for (int ip = 0; ip < 8; ++ip) {
+                if (2 * ip < NI) {
+                    float4 w;
+                    if (I0 == 1) w = make_float4((float)v[(2 * ip + 1) & 15].x, (float)v[(2 * ip + 1) & 15].y,
+                                                 (float)v[(2 * ip + 2) & 15].x, (float)v[(2 * ip + 2) & 15].y);
+                    else         w = make_float4((float)v[2 * ip].x, (float)v[2 * ip].y,
+                                                 (float)v[(2 * ip + 1) & 15].x, (float)v[(2 * ip + 1) & 15].y);
+                    ot[ip * 256] = w;
+                }
+            }
+        }
+        // the next template's samples overwrite `base` only after every thread has passed the barriers of r = 15
     }
 }
 

@@ -41,7 +41,7 @@
 namespace bege {
 
 constexpr int kN = 65536;
-constexpr int kBatch = 72;                 // spectra per launch of the forward transforms (fp64 bank staging: 75 MB)
+constexpr int kBatch = 72;                 // segments per launch of the forward transforms (fp32 staging: 38 MB)
 constexpr int kMaxGroups = 32;             // search: persistent CTA groups of 16 tiles (9 on a 148-SM B200)
 constexpr uint64_t kMiscHdr = 4096;        // counter @0, abort flag @8, hits @16, done1 @256, done2 @2048 (per group and ring slot)
 constexpr int kMaxSlices = 8;              // launches per search whose record copies overlap the next launch
@@ -696,8 +696,9 @@ struct bege_plan {
     uint32_t klo = 0, khi = 0;
     int I0 = 0, NI = 16;
     int G = 0;                      // search groups (16 CTAs each), all co-resident
+    int n_sm = 0;
     float2 *tw256 = nullptr, *twN = nullptr;
-    d2 *tw256d = nullptr, *twNd = nullptr;   // exp(2 pi i m / 256), exp(2 pi i m / N) in fp64 (bank generation)
+    d2* tw256d = nullptr;           // exp(2 pi i m / 256) in fp64 (bank generation)
     // workspace
     unsigned char* ws = nullptr; uint64_t ws_bytes = 0, bump = 0; bool user_ws = false;
     Slot s_bank, s_x, s_scratch, s_sig, s_rec, s_misc, s_par, s_tmp;
@@ -806,6 +807,7 @@ extern "C" int bege_plan_create(bege_plan** out, uint32_t N, double fs, double l
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return bail(BEGE_ECUDA);
     if (prop.major < 10) return bail(BEGE_ECUDA);              // sm_100a code only
+    p->n_sm = prop.multiProcessorCount;
     // a caller on the legacy default stream passes cudaStreamLegacy (handle 0 would be indistinguishable from NULL)
     if (stream) p->stream = (cudaStream_t)stream;
     else { if (cudaStreamCreateWithFlags(&p->stream, cudaStreamNonBlocking) != cudaSuccess) return bail(BEGE_ECUDA); p->own_stream = true; }
@@ -842,13 +844,11 @@ extern "C" int bege_plan_create(bege_plan** out, uint32_t N, double fs, double l
             wN[(size_t)n2 * 256 + k1] = make_float2((float)cos(a), (float)sin(a));
         }
     {
-        std::vector<d2> t256(256), tN(N);
+        std::vector<d2> t256(256);
         for (int m = 0; m < 256; ++m) { t256[m].x = cos(2.0 * M_PI * m / 256.0); t256[m].y = sin(2.0 * M_PI * m / 256.0); }
-        for (uint32_t m = 0; m < N; ++m) { tN[m].x = cos(2.0 * M_PI * m / (double)N); tN[m].y = sin(2.0 * M_PI * m / (double)N); }
-        if (cudaMalloc(&p->tw256d, 256 * sizeof(d2)) != cudaSuccess || cudaMalloc(&p->twNd, N * sizeof(d2)) != cudaSuccess) return bail(BEGE_ENOMEM);
-        if (cudaMemcpy(p->tw256d, t256.data(), 256 * sizeof(d2), cudaMemcpyHostToDevice) != cudaSuccess ||
-            cudaMemcpy(p->twNd, tN.data(), N * sizeof(d2), cudaMemcpyHostToDevice) != cudaSuccess) return bail(BEGE_ECUDA);
-        if (cudaFuncSetAttribute(k_bank_cols64, cudaFuncAttributeMaxDynamicSharedMemorySize, 16 * 256 * (int)sizeof(d2)) != cudaSuccess) return bail(BEGE_ECUDA);
+        if (cudaMalloc(&p->tw256d, 256 * sizeof(d2)) != cudaSuccess) return bail(BEGE_ENOMEM);
+        if (cudaMemcpy(p->tw256d, t256.data(), 256 * sizeof(d2), cudaMemcpyHostToDevice) != cudaSuccess) return bail(BEGE_ECUDA);
+        if (cudaFuncSetAttribute(k_bank_gen64, cudaFuncAttributeMaxDynamicSharedMemorySize, kBankSmem) != cudaSuccess) return bail(BEGE_ECUDA);
     }
     {   // exp(2 pi i m / 256) for the search kernel's CTA-uniform twiddles (constant memory of this device's context)
         std::vector<float2> lin(256);
@@ -891,7 +891,6 @@ extern "C" void bege_plan_destroy(bege_plan* p)
     if (p->tw256) cudaFree(p->tw256);
     if (p->twN) cudaFree(p->twN);
     if (p->tw256d) cudaFree(p->tw256d);
-    if (p->twNd) cudaFree(p->twNd);
     if (p->h_count) cudaFreeHost(p->h_count);
     if (p->ev_a) cudaEventDestroy(p->ev_a);
     if (p->ev_b) cudaEventDestroy(p->ev_b);
@@ -900,11 +899,11 @@ extern "C" void bege_plan_destroy(bege_plan* p)
     delete p;
 }
 
-// one region serves the fp64 staging of the bank generation (kBatch spectra of 16-byte elements), the fp32 staging of
-// the segment transform and the search ring (G groups x kRing items)
+// one region serves the fp32 staging of the segment transform (kBatch segments), the window table of the bank
+// generation and the search ring (G groups x kRing items)
 static uint64_t scratch_bytes(const bege_plan* p)
 {
-    return std::max<uint64_t>((uint64_t)kBatch * kN * sizeof(d2), (uint64_t)p->G * kRing * kN * sizeof(c2));
+    return std::max<uint64_t>((uint64_t)kBatch * kN * sizeof(c2), (uint64_t)p->G * kRing * kN * sizeof(c2));
 }
 
 extern "C" int bege_plan_workspace_bytes(const bege_plan* p, uint64_t T, uint32_t S, uint64_t cap, uint64_t* bytes)
@@ -953,19 +952,21 @@ extern "C" int bege_bank_generate(bege_plan* p, const double* f0, const double* 
     double* d_f0 = (double*)par; double* d_fd = d_f0 + T;
     CU(p, cudaMemcpyAsync(d_f0, f0, T * sizeof(double), cudaMemcpyHostToDevice, p->stream));
     CU(p, cudaMemcpyAsync(d_fd, fdot, T * sizeof(double), cudaMemcpyHostToDevice, p->stream));
-    // unit L2 norm: ||h||^2 = sum_n hann_L[n]^2 (the phase factor has modulus 1)
+    // unit L2 norm: ||h||^2 = sum_n hann_L[n]^2 (the phase factor has modulus 1); the window goes to the device
+    // already divided by the norm
     const uint32_t L = (uint32_t)Ll;
+    std::vector<double> hann(L);
     double n2 = 0;
-    for (uint32_t n = 0; n < L; ++n) { const double w = 0.5 - 0.5 * cos(2.0 * M_PI * n / (double)(L - 1)); n2 += w * w; }
+    for (uint32_t n = 0; n < L; ++n) { hann[n] = 0.5 - 0.5 * cos(2.0 * M_PI * n / (double)(L - 1)); n2 += hann[n] * hann[n]; }
     const double inv_norm = 1.0 / sqrt(n2);
+    for (uint32_t n = 0; n < L; ++n) hann[n] *= inv_norm;
+    double* d_hann = (double*)scr;                           // the scratch region is free outside a search
+    CU(p, cudaMemcpyAsync(d_hann, hann.data(), L * sizeof(double), cudaMemcpyHostToDevice, p->stream));
     const uint64_t stride = tpl_bytes(p) / sizeof(c2);
-    for (uint64_t j0 = 0; j0 < T; j0 += kBatch) {
-        const unsigned nb = (unsigned)std::min<uint64_t>(kBatch, T - j0);
-        k_bank_rows64<<<dim3(16, nb), 256, 0, p->stream>>>(d_f0, d_fd, j0, p->fs, L, inv_norm, p->tw256d, p->twNd, (d2*)scr);
-        k_bank_cols64<<<dim3(16, nb), 256, 16 * 256 * sizeof(d2), p->stream>>>((const d2*)scr, (float2*)bank + j0 * stride, stride,
-                                                                            p->I0, p->NI, p->tw256d);
-        count_launch(p, 2);
-    }
+    const unsigned ctas = (unsigned)std::min<uint64_t>(T, (uint64_t)p->n_sm);
+    k_bank_gen64<<<ctas, 256, kBankSmem, p->stream>>>(d_f0, d_fd, T, p->fs, L, d_hann, p->tw256d, (float2*)bank, stride, p->I0, p->NI);
+    count_launch(p);
+    CU(p, cudaStreamSynchronize(p->stream));                 // `hann` (pageable) must outlive its copy
     CU(p, cudaGetLastError());
     CU(p, cudaStreamSynchronize(p->stream));
     p->T = T; p->tau = tau; p->L = L;
