@@ -353,6 +353,140 @@ uint64_t bo_search_band(const double* Xs, uint32_t S, const double* f0, const do
     return count;
 }
 
+/* ------------------------------------------------------------ dual stream -- */
+/*
+ * The paper's own setting, PAPER.md:155 step (i): "FFT is applied to arrays of complex numbers, merging pairs of real
+ * H1 and L1 data", x = H1 + i L1, filtered with REAL chirp templates, so that one complex correlation
+ * holds both detectors' outputs:  z[n] = sum_s w[s] x[(n+s) mod N]  =>  rho_1 = Re z (H1),  rho_2 = Im z (L1).
+ *
+ * Real template (reading 23): the real part of BASELINE.json's waveform,
+ *   w_n = hann_L[n] cos(2 pi c_n),  c_n = f0 t_n + fdot t_n^2 / 2,  n < L;  w <- w / ||w||_2;  zero padded to N.
+ */
+int bo_template_real(double f0, double fdot, double tau, double fs, uint32_t N, double* h)
+{
+    long Ll = lround(tau * fs);
+    if (Ll < 2 || (uint64_t)Ll > N) return 1;
+    uint32_t L = (uint32_t)Ll;
+    memset(h, 0, sizeof(double) * 2 * (size_t)N);
+    double norm2 = 0.0;
+    for (uint32_t n = 0; n < L; ++n) {
+        double t = (double)n / fs;
+        double wn = 0.5 - 0.5 * cos(2.0 * BO_PI * (double)n / (double)(L - 1));
+        double c = f0 * t + 0.5 * fdot * t * t;
+        c -= floor(c);
+        h[2 * n] = wn * cos(2.0 * BO_PI * c);
+        norm2 += h[2 * n] * h[2 * n];
+    }
+    double inv = 1.0 / sqrt(norm2);
+    for (uint32_t n = 0; n < L; ++n) h[2 * n] *= inv;
+    return 0;
+}
+
+/*
+ * One (real template, packed segment) pair.  z as in bo_correlate_spectra (eq.5); per detector
+ * stream the standard deviation of its REAL output by the definition PAPER.md:96 eq.(6):
+ *   sigma_1^2 = N^-1 sum_n (Re z[n])^2,   sigma_2^2 = N^-1 sum_n (Im z[n])^2.
+ * Hs: template spectrum.  z may be NULL.
+ */
+int bo_correlate_dual(const double* X, const double* Hs, uint32_t N, double* z, double* sigma1, double* sigma2)
+{
+    double* zz = z ? z : (double*)malloc(sizeof(double) * 2 * (size_t)N);
+    if (!zz) return 2;
+    for (uint32_t k = 0; k < N; ++k) {                    /* R = conj(H) X */
+        double hr = Hs[2 * k], hi = Hs[2 * k + 1], xr = X[2 * k], xi = X[2 * k + 1];
+        zz[2 * k]     = hr * xr + hi * xi;
+        zz[2 * k + 1] = hr * xi - hi * xr;
+    }
+    int rc = bo_fft(zz, N, +1);
+    double s1 = 0.0, s2 = 0.0, inv = 1.0 / (double)N;
+    for (uint32_t n = 0; n < N; ++n) {
+        zz[2 * n] *= inv; zz[2 * n + 1] *= inv;
+        s1 += zz[2 * n] * zz[2 * n];
+        s2 += zz[2 * n + 1] * zz[2 * n + 1];
+    }
+    *sigma1 = sqrt(s1 * inv);
+    *sigma2 = sqrt(s2 * inv);
+    if (!z) free(zz);
+    return rc;
+}
+
+/*
+ * The same two standard deviations from the SPECTRUM, eq.(7) (Parseval for a real series, whose Fourier
+ * coefficients are Hermitian: the sum over half the spectrum, times sqrt 2).  The coefficients of Re z and Im z are
+ * the Hermitian and anti-Hermitian parts of R:  A[k] = (R[k] + conj(R[N-k]))/2,  B[k] = (R[k] - conj(R[N-k]))/(2i);
+ * sigma_1 = (sqrt 2 / N) sqrt( sum_{k=1}^{N/2-1} |A[k]|^2 + (|A[0]|^2 + |A[N/2]|^2)/2 ), likewise sigma_2 with B (the
+ * paper drops the DC and Nyquist terms, which vanish for band-limited data).  Used by the pins only.
+ */
+void bo_sigma_dual_parseval(const double* X, const double* Hs, uint32_t N, double* sigma1, double* sigma2)
+{
+    double sa = 0.0, sb = 0.0;
+    for (uint32_t k = 0; k <= N / 2; ++k) {
+        uint32_t km = (N - k) % N;
+        double r1r = Hs[2 * k] * X[2 * k] + Hs[2 * k + 1] * X[2 * k + 1];           /* R[k]     */
+        double r1i = Hs[2 * k] * X[2 * k + 1] - Hs[2 * k + 1] * X[2 * k];
+        double r2r = Hs[2 * km] * X[2 * km] + Hs[2 * km + 1] * X[2 * km + 1];       /* R[N-k]   */
+        double r2i = Hs[2 * km] * X[2 * km + 1] - Hs[2 * km + 1] * X[2 * km];
+        double ar = 0.5 * (r1r + r2r), ai = 0.5 * (r1i - r2i);                       /* (R[k] + conj R[N-k]) / 2 */
+        double br = 0.5 * (r1i + r2i), bi = -0.5 * (r1r - r2r);                      /* (R[k] - conj R[N-k]) / 2i */
+        double w = (k == 0 || k == N / 2) ? 0.5 : 1.0;
+        sa += w * (ar * ar + ai * ai);
+        sb += w * (br * br + bi * bi);
+    }
+    *sigma1 = sqrt(2.0) / (double)N * sqrt(sa);
+    *sigma2 = sqrt(2.0) / (double)N * sqrt(sb);
+}
+
+/*
+ * Dual-stream search in the paper's output form, Table 3 ("sample offset i, rho_1, f_1, rho_2, f_2 ...
+ * Zeros represent no hit"): per sample offset m*N + n and per detector stream d the largest |rho_d|/sigma_d over the
+ * bank among the hits |rho_d[n]| > k sigma_d (eq.9 on each real stream, two-sided), with its template
+ * ("we select data with maximal rho values"); 0 / UINT32_MAX where no template hits; ties go to the
+ * smaller template id.  sigma_out (may be NULL): T*S*2 values, [j][m][stream].  Plain serial loops.
+ */
+int bo_search_dual(const double* Xs, uint32_t S, const double* f0, const double* fdot, uint64_t T,
+                   double tau, double fs, uint32_t N, double k_sigma,
+                   double* snr1, uint32_t* id1, double* snr2, uint32_t* id2, double* sigma_out)
+{
+    double* Hs = (double*)malloc(sizeof(double) * 2 * (size_t)N);
+    double* z  = (double*)malloc(sizeof(double) * 2 * (size_t)N);
+    if (!Hs || !z) { free(Hs); free(z); return 2; }
+    for (size_t i = 0; i < (size_t)S * N; ++i) { snr1[i] = snr2[i] = 0.0; id1[i] = id2[i] = UINT32_MAX; }
+    for (uint64_t j = 0; j < T; ++j) {
+        if (bo_template_real(f0[j], fdot[j], tau, fs, N, Hs) || bo_fft(Hs, N, -1)) { free(Hs); free(z); return 1; }
+        for (uint32_t m = 0; m < S; ++m) {
+            double s1 = 0.0, s2 = 0.0;
+            bo_correlate_dual(Xs + 2 * (size_t)m * N, Hs, N, z, &s1, &s2);
+            if (sigma_out) { sigma_out[((size_t)j * S + m) * 2] = s1; sigma_out[((size_t)j * S + m) * 2 + 1] = s2; }
+            for (uint32_t n = 0; n < N; ++n) {
+                size_t i = (size_t)m * N + n;
+                double a1 = fabs(z[2 * n]), a2 = fabs(z[2 * n + 1]);
+                if (s1 > 0.0 && a1 > k_sigma * s1 && a1 / s1 > snr1[i]) { snr1[i] = a1 / s1; id1[i] = (uint32_t)j; }
+                if (s2 > 0.0 && a2 > k_sigma * s2 && a2 / s2 > snr2[i]) { snr2[i] = a2 / s2; id2[i] = (uint32_t)j; }
+            }
+        }
+    }
+    free(Hs); free(z);
+    return 0;
+}
+
+/*
+ * H1-L1 coincidences of a dual-stream output, PAPER.md:219 ("simultaneous hits with frequency pairs (f_1, f_2) of H1
+ * and L1 that are relatively close, |f_1 - f_2| < Delta"): offsets where both streams hold a hit, and among those the
+ * ones whose templates' start frequencies differ by less than delta_hz.
+ */
+void bo_dual_coincidences(const uint32_t* id1, const uint32_t* id2, uint64_t n, const double* f0, double delta_hz,
+                          uint64_t* n_simultaneous, uint64_t* n_coincident)
+{
+    uint64_t a = 0, b = 0;
+    for (uint64_t i = 0; i < n; ++i) {
+        if (id1[i] != UINT32_MAX && id2[i] != UINT32_MAX) {
+            ++a;
+            if (fabs(f0[id1[i]] - f0[id2[i]]) < delta_hz) ++b;
+        }
+    }
+    *n_simultaneous = a; *n_coincident = b;
+}
+
 /* PAPER.md:134 eq.(10), :160: nominal flops of one FFT_N. */
 double bo_fft_flops(uint32_t N)
 {

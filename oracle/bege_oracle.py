@@ -68,6 +68,18 @@ def lib():
         L.bo_search_maxproj.restype = ctypes.c_int
         L.bo_search_band.argtypes = [dp, u32, dp, dp, u64, dbl, dbl, u32, dbl, dbl, ctypes.POINTER(_Tail), u64]
         L.bo_search_band.restype = u64
+        L.bo_template_real.argtypes = [dbl, dbl, dbl, dbl, u32, dp]
+        L.bo_template_real.restype = ctypes.c_int
+        L.bo_correlate_dual.argtypes = [dp, dp, u32, dp, dp, dp]
+        L.bo_correlate_dual.restype = ctypes.c_int
+        L.bo_sigma_dual_parseval.argtypes = [dp, dp, u32, dp, dp]
+        L.bo_sigma_dual_parseval.restype = None
+        L.bo_search_dual.argtypes = [dp, u32, dp, dp, u64, dbl, dbl, u32, dbl, dp, ctypes.POINTER(u32), dp,
+                                     ctypes.POINTER(u32), dp]
+        L.bo_search_dual.restype = ctypes.c_int
+        L.bo_dual_coincidences.argtypes = [ctypes.POINTER(u32), ctypes.POINTER(u32), u64, dp, dbl,
+                                           ctypes.POINTER(u64), ctypes.POINTER(u64)]
+        L.bo_dual_coincidences.restype = None
         L.bo_fft_flops.argtypes = [u32]
         L.bo_fft_flops.restype = dbl
         _lib = L
@@ -195,6 +207,66 @@ def search_band(Xs, f0, fdot, tau: float, fs: float, k_lo: float, k_hi: float, c
         raise RuntimeError("bo_search_band failed")
     tails = tails[: min(n, cap)]
     return tails[np.lexsort((tails["lag"], tails["template_id"]))], int(n)
+
+
+def template_real(f0: float, fdot: float, tau: float, fs: float, N: int) -> np.ndarray:
+    """Real chirp template of the dual-stream search (bo_template_real), as a complex128 array with zero imaginary part."""
+    h = np.zeros(N, dtype=np.complex128)
+    if lib().bo_template_real(float(f0), float(fdot), float(tau), float(fs), N, _dp(h.view(np.float64))):
+        raise ValueError("bo_template_real: bad arguments")
+    return h
+
+
+def correlate_dual(X, h):
+    """(z, sigma_1, sigma_2) for a packed segment spectrum X and a real template h (time domain)."""
+    X = _c128(X)
+    N = X.size
+    Hs = fft(h, -1)
+    z = np.zeros(N, dtype=np.complex128)
+    s1, s2 = ctypes.c_double(), ctypes.c_double()
+    if lib().bo_correlate_dual(_dp(X.view(np.float64)), _dp(Hs.view(np.float64)), N, _dp(z.view(np.float64)),
+                               ctypes.byref(s1), ctypes.byref(s2)):
+        raise RuntimeError("bo_correlate_dual failed")
+    return z, s1.value, s2.value
+
+
+def sigma_dual_parseval(X, h):
+    """(sigma_1, sigma_2) from the product spectrum alone, eq.(7)."""
+    X = _c128(X)
+    Hs = fft(h, -1)
+    s1, s2 = ctypes.c_double(), ctypes.c_double()
+    lib().bo_sigma_dual_parseval(_dp(X.view(np.float64)), _dp(Hs.view(np.float64)), X.size, ctypes.byref(s1), ctypes.byref(s2))
+    return s1.value, s2.value
+
+
+def search_dual(Xs, f0, fdot, tau: float, fs: float, k_sigma: float):
+    """Dual-stream search (bo_search_dual): (snr1[S, N], id1[S, N], snr2[S, N], id2[S, N], sigma[T, S, 2])."""
+    Xs = np.atleast_2d(_c128(Xs))
+    S, N = Xs.shape
+    f0 = np.ascontiguousarray(np.asarray(f0, dtype=np.float64))
+    fdot = np.ascontiguousarray(np.asarray(fdot, dtype=np.float64))
+    snr1, snr2 = np.zeros((S, N)), np.zeros((S, N))
+    id1, id2 = np.zeros((S, N), dtype=np.uint32), np.zeros((S, N), dtype=np.uint32)
+    sig = np.zeros((f0.size, S, 2))
+    u32p = ctypes.POINTER(ctypes.c_uint32)
+    rc = lib().bo_search_dual(_dp(Xs.view(np.float64)), S, _dp(f0), _dp(fdot), f0.size, float(tau), float(fs), N,
+                              float(k_sigma), _dp(snr1), id1.ctypes.data_as(u32p), _dp(snr2), id2.ctypes.data_as(u32p),
+                              _dp(sig))
+    if rc:
+        raise RuntimeError(f"bo_search_dual rc={rc}")
+    return snr1, id1, snr2, id2, sig
+
+
+def dual_coincidences(id1, id2, f0, delta_hz: float):
+    """(offsets with a hit in both streams, those with |f_1 - f_2| < delta_hz)."""
+    id1 = np.ascontiguousarray(id1, dtype=np.uint32).ravel()
+    id2 = np.ascontiguousarray(id2, dtype=np.uint32).ravel()
+    f0 = np.ascontiguousarray(np.asarray(f0, dtype=np.float64))
+    a, b = ctypes.c_uint64(), ctypes.c_uint64()
+    u32p = ctypes.POINTER(ctypes.c_uint32)
+    lib().bo_dual_coincidences(id1.ctypes.data_as(u32p), id2.ctypes.data_as(u32p), id1.size, _dp(f0), float(delta_hz),
+                               ctypes.byref(a), ctypes.byref(b))
+    return int(a.value), int(b.value)
 
 
 def fft_flops(N: int) -> float:

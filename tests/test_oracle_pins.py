@@ -389,3 +389,120 @@ def test_band_threshold_is_the_extended_output_minus_its_top():
     assert n_same == n_full and np.array_equal(same["lag"], full["lag"])
     _, n_none = bo.search_band(X[None, :], w.f0[ids], w.fdot[ids], TAU, FS, 3.0, 3.0)
     assert n_none == 0
+
+
+# ------------------------------------------------------------------ dual-stream search (PAPER.md:155, :70, :100 eq.7, :221 Table 3)
+def _packed_noise(seed_h1, seed_l1):
+    """x = H1 + i L1: two independent band-limited Gaussian streams packed into one complex segment."""
+    h1 = synth.band_limit(synth.white_noise(seed_h1))
+    l1 = synth.band_limit(synth.white_noise(seed_l1))
+    return h1, l1, (h1 + 1j * l1)
+
+
+def test_real_template_is_the_normalised_real_part():
+    """bo_template_real: w_n = hann cos(2 pi c_n), unit norm, no imaginary part -- written out here with numpy."""
+    f0, fd = 777.0, -123.0
+    w = bo.template_real(f0, fd, TAU, FS, N)
+    L = int(round(TAU * FS))
+    n = np.arange(L)
+    ref = np.hanning(L) * np.cos(2 * np.pi * (f0 * n / FS + 0.5 * fd * (n / FS) ** 2))
+    ref /= np.linalg.norm(ref)
+    assert np.all(w.imag == 0) and np.all(w[L:] == 0)
+    assert abs(np.linalg.norm(w) - 1) < 1e-14
+    assert np.max(np.abs(w.real[:L] - ref)) < 1e-12
+    # and it is proportional to the real part of the complex template of the single-stream search
+    h = bo.template(f0, fd, TAU, FS, N)
+    c = np.vdot(h.real, w.real) / np.vdot(h.real, h.real)
+    assert np.max(np.abs(w.real - c * h.real)) < 1e-12
+
+
+def test_dual_sigma_is_eq6_and_eq7():
+    """sigma per detector stream: the definition (eq.6, rms of the real output) against an independent numpy
+    evaluation, and against Parseval's half-spectrum form for a real series (eq.7), which is the
+    form the paper prints (sqrt 2 / N sqrt(sum over half the spectrum))."""
+    h1, l1, x = _packed_noise(21, 22)
+    X = bo.segment_spectrum(x, FS, *BAND)
+    for (f0, fd) in ((500.0, 120.0), (1500.0, -350.0), (1990.0, 400.0)):
+        w = bo.template_real(f0, fd, TAU, FS, N)
+        z, s1, s2 = bo.correlate_dual(X, w)
+        zn = np.fft.ifft(np.conj(np.fft.fft(w)) * X)                    # the library's transform, eq.(5)
+        assert np.linalg.norm(z - zn) < 1e-12 * np.linalg.norm(zn)
+        assert abs(s1 - np.sqrt(np.mean(zn.real ** 2))) < 1e-13 * s1   # eq.(6) on the H1 output
+        assert abs(s2 - np.sqrt(np.mean(zn.imag ** 2))) < 1e-13 * s2   # eq.(6) on the L1 output
+        p1, p2 = bo.sigma_dual_parseval(X, w)                           # eq.(7)
+        assert abs(p1 - s1) < 1e-12 * s1 and abs(p2 - s2) < 1e-12 * s2
+
+
+def test_dual_packing_equals_two_separate_real_searches():
+    """Packing is exact: Re z of (H1 + i L1) is the correlation of H1 alone, Im z that of L1 alone (linearity of
+    eq.3 with a real template) -- checked against the single-stream functions, which are pinned on their own, and
+    against the direct time-domain sum of eq.(3) on sampled lags."""
+    h1, l1, x = _packed_noise(23, 24)
+    X = bo.segment_spectrum(x, FS, *BAND)
+    X1 = bo.segment_spectrum(h1.astype(np.complex128), FS, *BAND)
+    X2 = bo.segment_spectrum(l1.astype(np.complex128), FS, *BAND)
+    w = bo.template_real(900.0, 200.0, TAU, FS, N)
+    z, s1, s2 = bo.correlate_dual(X, w)
+    z1, _ = bo.correlate(X1, w)
+    z2, _ = bo.correlate(X2, w)
+    assert np.max(np.abs(z1.imag)) < 1e-12 and np.max(np.abs(z2.imag)) < 1e-12
+    assert np.max(np.abs(z.real - z1.real)) < 1e-12 and np.max(np.abs(z.imag - z2.real)) < 1e-12
+    assert abs(s1 - np.sqrt(np.mean(z1.real ** 2))) < 1e-13 and abs(s2 - np.sqrt(np.mean(z2.real ** 2))) < 1e-13
+    lags = np.array([0, 1, 4095, 30000, N - 4096, N - 1], dtype=np.uint32)
+    L = int(round(TAU * FS))
+    for stream, part in ((h1, z.real), (l1, z.imag)):
+        xhat = bo.fft(bo.band_mask(bo.fft(stream.astype(np.complex128), -1), FS, *BAND), +1) / N
+        d = bo.correlate_direct(xhat, w, L, lags)
+        assert np.max(np.abs(d.real - part[lags])) < 1e-11
+
+
+def test_dual_tail_counts_follow_the_real_two_sided_law():
+    """Each stream's output is real and near-Gaussian: P(|rho| > k sigma) = erfc(k / sqrt 2)."""
+    h1, l1, x = _packed_noise(25, 26)
+    X = bo.segment_spectrum(x, FS, *BAND)
+    f0, fd = synth.bank_grid(6, 4, 500.0, 1800.0, -150.0, 150.0)
+    k = 3.0
+    c1 = c2 = 0
+    for a, b in zip(f0, fd):
+        z, s1, s2 = bo.correlate_dual(X, bo.template_real(a, b, TAU, FS, N))
+        c1 += int(np.sum(np.abs(z.real) > k * s1))
+        c2 += int(np.sum(np.abs(z.imag) > k * s2))
+    expect = f0.size * N * math.erfc(k / math.sqrt(2.0))                # 4247
+    for c in (c1, c2):
+        assert abs(c - expect) < 0.12 * expect, (c, expect)            # outputs are correlated over ~10 lags: several x Poisson
+
+
+def test_search_dual_against_brute_force_and_injection_in_one_stream():
+    """bo_search_dual (Table 3 form) rebuilt offset by offset from bo_correlate_dual; a chirp injected into H1 only is
+    found in stream 1 at its template and lag, and not in stream 2; simultaneous / coincident counts by hand."""
+    h1, l1, _ = _packed_noise(27, 28)
+    h1, n0 = synth.inject_chirp(h1, 1000.0, 50.0, 5.0, 12.0)
+    x = h1 + 1j * l1
+    X = bo.segment_spectrum(x, FS, *BAND)
+    f0 = np.array([600.0, 1000.0, 1000.0, 1400.0])                        # entries 1 and 2 identical: a planted tie
+    fd = np.array([-100.0, 50.0, 50.0, 200.0])
+    k = 3.2
+    snr1, id1, snr2, id2, sig = bo.search_dual(X[None, :], f0, fd, TAU, FS, k)
+    none = np.iinfo(np.uint32).max
+    b1, b2 = np.zeros(N), np.zeros(N)
+    j1, j2 = np.full(N, none, dtype=np.uint32), np.full(N, none, dtype=np.uint32)
+    for j in range(f0.size):
+        z, s1, s2 = bo.correlate_dual(X, bo.template_real(f0[j], fd[j], TAU, FS, N))
+        assert abs(sig[j, 0, 0] - s1) < 1e-15 and abs(sig[j, 0, 1] - s2) < 1e-15
+        r1, r2 = np.abs(z.real) / s1, np.abs(z.imag) / s2
+        u1, u2 = (r1 > k) & (r1 > b1), (r2 > k) & (r2 > b2)
+        b1[u1], j1[u1] = r1[u1], j
+        b2[u2], j2[u2] = r2[u2], j
+    assert np.array_equal(snr1[0], b1) and np.array_equal(id1[0], j1)
+    assert np.array_equal(snr2[0], b2) and np.array_equal(id2[0], j2)
+    assert not np.any(id1 == 2) or np.all(snr1[id1 == 2] > 0)             # ties keep the smaller id ...
+    assert not np.any((id1 == 2))                                          # ... so the duplicate never wins
+    peak = int(np.argmax(snr1[0]))
+    # a real correlation output oscillates at the carrier (4 samples per cycle at 1 kHz): the largest |rho| may sit a
+    # cycle or two off the envelope maximum at n0
+    assert id1[0, peak] == 1 and abs(peak - n0) <= 8 and snr1[0, peak] > 8.0
+    assert snr2[0, max(0, n0 - 50): n0 + 50].max() < 5.0                  # nothing in the other detector there
+    both = (id1[0] != none) & (id2[0] != none)
+    n_sim, n_coi = bo.dual_coincidences(id1, id2, f0, 50.0)
+    assert n_sim == int(both.sum())
+    assert n_coi == int(np.sum(np.abs(f0[id1[0][both]] - f0[id2[0][both]]) < 50.0))
