@@ -132,6 +132,26 @@ int bege_search_band(bege_plan*, float k_lo, float k_hi, bege_tail* tails_out, u
  */
 int bege_search_maxproj(bege_plan*, float k_sigma, float* snr_out, uint32_t* id_out, uint64_t* n_hits);
 
+/*
+ * NEXT row of the scope table -- the paper's own input and output form (PAPER.md:155 step i: "FFT is applied to arrays
+ * of complex numbers, merging pairs of real H1 and L1 data"; real chirp templates; Table 3).
+ * bege_bank_generate_real: as bege_bank_generate with the REAL template w_n = hann_L[n] cos(2 pi (f0 t_n + fdot t_n^2/2)),
+ *   unit L2 norm.  bege_search works on such a bank too; bege_search_dual requires it.
+ * bege_search_dual: the loaded segments are read as x = H1 + i L1, so Re z and Im z of the one complex correlation are the
+ *   two detectors' filter outputs.  Per stream d, sigma_d = rms of its real output, predicted from the product spectrum
+ *   by Parseval's theorem for a real series (eq.7, Hermitian split of R); a hit is |rho_d[n]| > k_sigma
+ *   sigma_d (eq.9, two-sided).  For every offset i = m*N + n: snrD_out[i] = the largest |rho_d|/sigma_d over
+ *   the bank among the hits (0 if none), idD_out[i] = its template (UINT32_MAX if none; equal values go to the smaller
+ *   id).  *n_simultaneous (may be NULL): offsets with a hit in both streams; *n_coincident (may be NULL): those whose two
+ *   templates' start frequencies differ by less than delta_hz (|f_1 - f_2| < Delta).
+ *   Host arrays of n_segments*N entries each.  The band must lie inside bins [4096, 61440) (BEGE_EINVAL otherwise).
+ * bege_get_sigma_dual: sigma_1, sigma_2 of the last bege_search_dual, n_templates*n_segments floats each, template-major.
+ */
+int bege_bank_generate_real(bege_plan*, const double* f0_hz, const double* fdot_hz_s, uint64_t n_templates, double tau_s);
+int bege_search_dual(bege_plan*, float k_sigma, float* snr1_out, uint32_t* id1_out, float* snr2_out, uint32_t* id2_out,
+                     double delta_hz, uint64_t* n_simultaneous, uint64_t* n_coincident);
+int bege_get_sigma_dual(bege_plan*, float* sigma1_out, float* sigma2_out);
+
 /* sigma_jm of the last bege_search, host array of n_templates*n_segments floats, template-major. */
 int bege_get_sigma(bege_plan*, float* sigma_out);
 

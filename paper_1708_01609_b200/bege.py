@@ -25,6 +25,7 @@ _STATUS = {0: "BEGE_OK", 1: "BEGE_EINVAL", 2: "BEGE_ESTATE", 3: "BEGE_ENOMEM", 4
 SYMBOLS = [
     "bege_plan_create", "bege_plan_workspace_bytes", "bege_plan_set_workspace", "bege_bank_generate",
     "bege_segment_load", "bege_search", "bege_search_band", "bege_search_maxproj", "bege_get_sigma", "bege_debug_correlate",
+    "bege_bank_generate_real", "bege_search_dual", "bege_get_sigma_dual",
     "bege_debug_template_spectrum", "bege_debug_segment_spectrum", "bege_debug_set_max_items", "bege_plan_set_profiling",
     "bege_plan_get_stats", "bege_plan_reset_stats", "bege_last_error", "bege_plan_destroy", "bege_version",
 ]
@@ -64,6 +65,9 @@ def load_library() -> ctypes.CDLL:
     L.bege_search_band.argtypes = [vp, ctypes.c_float, ctypes.c_float, vp, u64, ctypes.POINTER(u64)]
     L.bege_search_maxproj.argtypes = [vp, ctypes.c_float, vp, vp, ctypes.POINTER(u64)]
     L.bege_get_sigma.argtypes = [vp, vp]
+    L.bege_bank_generate_real.argtypes = [vp, vp, vp, u64, dbl]
+    L.bege_search_dual.argtypes = [vp, ctypes.c_float, vp, vp, vp, vp, dbl, ctypes.POINTER(u64), ctypes.POINTER(u64)]
+    L.bege_get_sigma_dual.argtypes = [vp, vp, vp]
     L.bege_debug_correlate.argtypes = [vp, u64, u32, vp, ctypes.POINTER(ctypes.c_float)]
     L.bege_debug_template_spectrum.argtypes = [vp, u64, vp]
     L.bege_debug_segment_spectrum.argtypes = [vp, u32, vp]
@@ -167,6 +171,14 @@ class Plan:
         self._check(self._L.bege_bank_generate(self._h, f0.ctypes.data, fdot.ctypes.data, f0.size, float(tau)))
         self.n_templates = int(f0.size)
 
+    def bank_generate_real(self, f0, fdot, tau: float = 1.0):
+        """Bank of real templates (dual-stream search)."""
+        f0 = np.ascontiguousarray(np.asarray(f0, dtype=np.float64))
+        fdot = np.ascontiguousarray(np.asarray(fdot, dtype=np.float64))
+        assert f0.ndim == 1 and f0.shape == fdot.shape
+        self._check(self._L.bege_bank_generate_real(self._h, f0.ctypes.data, fdot.ctypes.data, f0.size, float(tau)))
+        self.n_templates = int(f0.size)
+
     def segment_load(self, x):
         """x: (S, N) complex64 -- numpy array, or torch tensor (CPU, pinned or CUDA)."""
         if isinstance(x, np.ndarray):
@@ -221,6 +233,23 @@ class Plan:
         self._check(self._L.bege_search_maxproj(self._h, ctypes.c_float(k_sigma), snr.ctypes.data, ids.ctypes.data,
                                                 ctypes.byref(n)))
         return snr, ids, int(n.value)
+
+    def search_dual(self, k_sigma: float, delta_hz: float = 50.0):
+        """Dual-stream search (x = H1 + i L1): (snr1, id1, snr2, id2) of shape (S, N), n_simultaneous, n_coincident."""
+        shape = (self.n_segments, self.N)
+        snr1, snr2 = np.empty(shape, dtype=np.float32), np.empty(shape, dtype=np.float32)
+        id1, id2 = np.empty(shape, dtype=np.uint32), np.empty(shape, dtype=np.uint32)
+        ns, nc = ctypes.c_uint64(), ctypes.c_uint64()
+        self._check(self._L.bege_search_dual(self._h, ctypes.c_float(k_sigma), snr1.ctypes.data, id1.ctypes.data,
+                                             snr2.ctypes.data, id2.ctypes.data, float(delta_hz),
+                                             ctypes.byref(ns), ctypes.byref(nc)))
+        return snr1, id1, snr2, id2, int(ns.value), int(nc.value)
+
+    def get_sigma_dual(self):
+        s1 = np.empty((self.n_templates, self.n_segments), dtype=np.float32)
+        s2 = np.empty((self.n_templates, self.n_segments), dtype=np.float32)
+        self._check(self._L.bege_get_sigma_dual(self._h, s1.ctypes.data, s2.ctypes.data))
+        return s1, s2
 
     def get_sigma(self) -> np.ndarray:
         out = np.empty((self.n_templates, self.n_segments), dtype=np.float32)

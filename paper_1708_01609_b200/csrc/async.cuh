@@ -149,6 +149,20 @@ BEGE_DA void tmem_wait_ld(unsigned long long (&w)[2])
     asm volatile("tcgen05.wait::ld.sync.aligned;" : "+l"(w[0]), "+l"(w[1]) :: "memory");
 }
 
+// two columns (dual-stream search: two real table entries), and the wait that covers a complex and a real staging array
+BEGE_DA void tmem_ld2f(uint32_t taddr, float (&w)[2])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];" : "=f"(w[0]), "=f"(w[1]) : "r"(taddr));
+}
+BEGE_DA void tmem_st2(uint32_t taddr, uint32_t r0, uint32_t r1)
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" :: "r"(taddr), "r"(r0), "r"(r1) : "memory");
+}
+BEGE_DA void tmem_wait_ld(unsigned long long (&w)[2], float (&f)[2])
+{
+    asm volatile("tcgen05.wait::ld.sync.aligned;" : "+l"(w[0]), "+l"(w[1]), "+f"(f[0]), "+f"(f[1]) :: "memory");
+}
+
 // ---- named barrier of `nthreads` threads
 BEGE_DA void bar_named(int id, int nthreads) { asm volatile("bar.sync %0, %1;" :: "r"(id), "r"(nthreads) : "memory"); }
 

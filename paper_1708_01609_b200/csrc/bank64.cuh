@@ -67,11 +67,14 @@ BEGE_DD void dfft16f(d2 (&a)[16])
 // hann: L window values times 1 / ||h|| (host, fp64).  tw256d[m] = exp(2 pi i m / 256).
 constexpr int kBankSmem = 3 * 4096 * 16;   // samples + two exchange buffers, fp64 complex
 
+// real_tpl: the real template of the dual-stream search, w_n = hann_n cos(2 pi c_n) / ||.||; its
+// norm depends on the template and is formed here (fp64 block sum).
 __global__ void __launch_bounds__(256, 1)
 k_bank_gen64(const double* __restrict__ f0, const double* __restrict__ fdot, uint64_t T, double fs, uint32_t L,
              const double* __restrict__ hann, const d2* __restrict__ tw256d, float2* __restrict__ out,
-             uint64_t out_stride, int I0, int NI)
+             uint64_t out_stride, int I0, int NI, int real_tpl)
 {
+    __shared__ double red[8];
     extern __shared__ __align__(16) unsigned char bank64_smem[];
     d2* base = reinterpret_cast<d2*>(bank64_smem);          // [nh][nl]
     d2* bufA = base + 4096;                                  // [m1][l0][l1 ^ l0]
@@ -94,13 +97,27 @@ k_bank_gen64(const double* __restrict__ f0, const double* __restrict__ fdot, uin
             d2 z = expc(f * tt + 0.5 * fd * tt * tt);
             d2 D = expc(f * dt + 0.5 * fd * (2.0 * tt * dt + dt * dt));
             const d2 C = expc(fd * dt * dt);
+            double n2 = 0.0;
 #pragma unroll
             for (int nh = 0; nh < 16; ++nh) {
                 const uint32_t n = (uint32_t)t + 256u * nh;
                 const double w = n < L ? hann[n] : 0.0;
-                base[nh * 256 + t] = dmk(w * z.x, w * z.y);
+                base[nh * 256 + t] = dmk(w * z.x, real_tpl ? 0.0 : w * z.y);
+                n2 += (w * z.x) * (w * z.x);
                 z = dmul(z, D.x, D.y);
                 D = dmul(D, C.x, C.y);
+            }
+            if (real_tpl) {                                  // unit L2 norm of the real template
+#pragma unroll
+                for (int d = 16; d >= 1; d >>= 1) n2 += __shfl_xor_sync(0xffffffffu, n2, d);
+                if ((t & 31) == 0) red[t >> 5] = n2;
+                __syncthreads();
+                double tot = 0.0;
+#pragma unroll
+                for (int w8 = 0; w8 < 8; ++w8) tot += red[w8];
+                const double inv = 1.0 / sqrt(tot);
+#pragma unroll
+                for (int nh = 0; nh < 16; ++nh) base[nh * 256 + t].x *= inv;
             }
         }
         __syncthreads();

@@ -183,6 +183,7 @@ k_fwd_cols(const c2* __restrict__ G, c2* __restrict__ out, uint64_t out_stride, 
 //                       four-step factor wN^(16 b k1), k1 = a + 16 r, times the inner twiddle w256^(a p); 4 quadrants
 //   columns [32, 96):   pass 1: the stationary tile, 28 columns per thread, 32 per warp of a lane quadrant
 //   columns [96, 160):  pass 1: theta^p = exp(2 pi i p (256 g + k1) / N), p = 1 .. 15, same arrangement
+//   columns [160, 192): pass 1, dual-stream search only: Re(X[k] X[N-k]) of the segment, 14 columns per thread
 // The CTA-uniform part of the four-step factor, w256^(b r), comes from constant memory (uniform loads).  All table
 // entries are rounded once from fp64 angles.
 //
@@ -201,11 +202,11 @@ k_fwd_cols(const c2* __restrict__ G, c2* __restrict__ out, uint64_t out_stride, 
 constexpr int kRing = 8;
 constexpr int kSearchThreads = 32 * 32;
 constexpr int kTmemCols = 256;
-constexpr uint32_t kTmDelta = 0, kTmStat = 32, kTmTheta = 96;
+constexpr uint32_t kTmDelta = 0, kTmStat = 32, kTmTheta = 96, kTmQ = 160;   // kTmQ: 16 columns per warp of a quadrant
 __constant__ float2 c_w256[256];           // exp(2 pi i m / 256), rounded from fp64 (host, bege_plan_create)
 
 struct SearchArgs {
-    const c2* bank; const c2* xseg; c2* ring; float* sigpart; bege_tail* rec; c2* zdbg;
+    const c2* bank; const c2* xseg; const float* qseg; c2* ring; float* sigpart; bege_tail* rec; c2* zdbg;
     unsigned long long cap; unsigned long long* counter; unsigned long long* done1; unsigned long long* done2;
     int* abort_flag;
     uint64_t j0, nT, sig_pair0;
@@ -221,8 +222,8 @@ template <int NI> struct SearchSmem {
     static constexpr uint32_t stream = 0;                        // [2]   streaming tile of each A team
     static constexpr uint32_t xch = stream + 2 * kTile;          // [2]   exchange buffer of each A team
     static constexpr uint32_t btile = xch + 2 * kXch;            // [kNB] row tiles of pass 2
-    static constexpr uint32_t ssig = btile + kNB * 32768;        // [2][8] Parseval partial sums of the A warps
-    static constexpr uint32_t bars = ssig + 64;                  // mbarriers: stream[2]; TMEM base address @ +24
+    static constexpr uint32_t ssig = btile + kNB * 32768;        // [2][2][8] Parseval partial sums of the A warps (sum|R|^2, dual: P)
+    static constexpr uint32_t bars = ssig + 128;                 // mbarriers: stream[2]; TMEM base address @ +24
     static constexpr uint32_t amb = bars + 32;                   // [kRing] mbarriers: tile of ring slot stored (8 A warps)
     static constexpr uint32_t bfull = amb + 8 * kRing;           // [kNB] mbarriers: row tile has arrived
     static constexpr uint32_t bempty = bfull + 24;               // [kNB] mbarriers: ... has been read out (8 B warps)
@@ -268,6 +269,28 @@ template <int I0, bool SINGLE, int IP = 0> BEGE_D void tm_products(uint32_t stre
         tm_products<I0, SINGLE, IP + 1>(stream_a, taddr, v, acc, qa, qb);
     }
 }
+// ... dual-stream search (SINGLE only): besides R = conj(W) X and sum |R|^2 also P = sum_k |W[k]|^2 Re(X[k] X[N-k]), which
+// splits sum |R|^2 into the two detector streams (see k_search); Re(X[k] X[N-k]) comes from tensor memory as well
+template <int I0, int IP = 0> BEGE_D void tm_products_dual(uint32_t stream_a, uint32_t tx, uint32_t tqr, c2 (&v)[16], c2& acc, float& pacc,
+                                                           c2 (&qa)[2], c2 (&qb)[2], float (&ra)[2], float (&rb)[2])
+{
+    if constexpr (IP < 7) {
+        c2 (&cur)[2] = (IP & 1) ? qb : qa;
+        c2 (&nxt)[2] = (IP & 1) ? qa : qb;
+        float (&rcur)[2] = (IP & 1) ? rb : ra;
+        float (&rnxt)[2] = (IP & 1) ? ra : rb;
+        tmem_wait_ld(cur, rcur);
+        if constexpr (IP + 1 < 7) { tmem_ld4(tx + 4 * (IP + 1), nxt); tmem_ld2f(tqr + 2 * (IP + 1), rnxt); }
+        c2 s0, s1;
+        lds128<IP * 4096>(stream_a, s0, s1);
+        const c2 r0 = cmulc(cur[0], s0), r1 = cmulc(cur[1], s1);
+        v[I0 + 2 * IP] = r0; v[(I0 + 2 * IP + 1) & 15] = r1;
+        acc = fma2(r0, r0, acc); acc = fma2(r1, r1, acc);
+        pacc = fmaf(fmaf(im(s0), im(s0), re(s0) * re(s0)), rcur[0], pacc);
+        pacc = fmaf(fmaf(im(s1), im(s1), re(s1) * re(s1)), rcur[1], pacc);
+        tm_products_dual<I0, IP + 1>(stream_a, tx, tqr, v, acc, pacc, qa, qb, ra, rb);
+    }
+}
 // ... stationary values from global memory (bands that keep all 16 row-blocks)
 template <int I0, int NI, bool SINGLE, int IP = 0> BEGE_D void gl_products(uint32_t stream_a, const ulonglong2* __restrict__ statg, c2 (&v)[16], c2& acc)
 {
@@ -292,11 +315,18 @@ template <int P0, int NCH, int J = 0> BEGE_D void tm_twiddle(uint32_t taddr, c2 
     }
 }
 
-template <int I0, int NI, bool SINGLE, bool DBG>
+// DUAL (single-segment calls, 14 row-blocks): the dual-stream search of PAPER.md:155 -- x = H1 + i L1, REAL templates, so
+// Re z and Im z are the two detectors' outputs.  Their variances are the Hermitian split of the product spectrum
+// (eq.7): N^2 sigma_1^2 = (S + P)/2, N^2 sigma_2^2 = (S - P)/2 with S = sum|R|^2 and
+// P = Re sum_k R[k] R[N-k] = sum_k |W[k]|^2 Re(X[k] X[N-k]) (W Hermitian) -- a second per-tile partial sum next to S,
+// no pairing of bins across tiles.  Output: per sample offset and stream the largest |rho|/sigma and its template
+// (Table 3), by 64-bit atomicMax as in the max projection.
+template <int I0, int NI, bool SINGLE, bool DBG, bool DUAL>
 __global__ void __launch_bounds__(kSearchThreads, 1)
 k_search(const __grid_constant__ SearchArgs A)
 {
     constexpr bool STAT = search_stat<NI>();                 // stationary tile in tensor memory
+    static_assert(!DUAL || (SINGLE && STAT && !DBG), "dual-stream search: single-segment calls on 14 row-blocks");
     using SM = SearchSmem<NI>;
     static_assert(NI % 2 == 0, "row-blocks are stored in pairs");
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -374,6 +404,14 @@ k_search(const __grid_constant__ SearchArgs A)
             }
         }
         if (STAT && n_items > 0) stat_to_tmem(SINGLE ? seg_tile(0) : tpl_tile(0));
+        if (DUAL && n_items > 0) {                           // Re(X[k] X[N-k]) of this thread's 14 bins
+            const float2* src = reinterpret_cast<const float2*>(A.qseg + ((uint64_t)A.m0 * 16 + b) * (uint64_t)(NI * 256)) + t;
+#pragma unroll
+            for (int ip = 0; ip < NI / 2; ++ip) {
+                const float2 q = __ldcg(src + ip * 256);
+                tmem_st2(tq + kTmQ + 16u * (uint32_t)(warp >> 2) + 2 * ip, __float_as_uint(q.x), __float_as_uint(q.y));
+            }
+        }
         tmem_wait_st();
     }
     tmem_fence_before_sync();
@@ -389,7 +427,7 @@ k_search(const __grid_constant__ SearchArgs A)
         const uint32_t stream_a = stream_buf + t * 16;
         const uint32_t xw_a = sb + SM::xch + team * SM::kXch + (g * 17 + c) * 8;       // + p * 2176: element [p][g][c]
         const uint32_t xr_a = sb + SM::xch + team * SM::kXch + (p2 * 272 + c2i) * 8;   // + gg * 136
-        const uint32_t ssig_a = sb + SM::ssig + team * 32;
+        const uint32_t ssig_a = sb + SM::ssig + team * 32;     // + 64: the dual-stream search's second sum
         const int bar_id = 1 + team;
         auto stream_src = [&](uint32_t it) { return SINGLE ? tpl_tile(it) : seg_tile(it % nS); };
         const ulonglong2* statg = nullptr;                   // !STAT: the stationary tile in global memory
@@ -411,7 +449,9 @@ k_search(const __grid_constant__ SearchArgs A)
             unsigned long long d2v = ~0ull;
             if (!(BEGE_ABL & 1) && t == 32 && it >= (uint32_t)kRing) d2v = counter_load_acquire(d2 + slot);
             c2 qa[2], qb[2];                                 // TMEM staging (stationary values, then theta powers)
+            float ra[2], rb[2], pacc = 0.f;                  // dual-stream search: staging of Re(X[k] X[N-k]), P
             if (STAT) tmem_ld4(tq_a + kTmStat, qa);
+            if (DUAL) tmem_ld2f(tq + kTmQ + 16u * (uint32_t)(warp >> 2), ra);
 #if !(BEGE_ABL & 2)
             mbar_wait(bar_stream, nload & 1, abort_flag);
 #endif
@@ -422,7 +462,8 @@ k_search(const __grid_constant__ SearchArgs A)
             c2 acc = mk(0.f, 0.f);
 #pragma unroll
             for (int r = 0; r < 16; ++r) if (r < I0 || r >= I0 + NI) v[r] = mk(0.f, 0.f);
-            if constexpr (STAT) tm_products<I0, SINGLE>(stream_a, tq_a + kTmStat, v, acc, qa, qb);
+            if constexpr (DUAL) tm_products_dual<I0>(stream_a, tq_a + kTmStat, tq + kTmQ + 16u * (uint32_t)(warp >> 2), v, acc, pacc, qa, qb, ra, rb);
+            else if constexpr (STAT) tm_products<I0, SINGLE>(stream_a, tq_a + kTmStat, v, acc, qa, qb);
             else gl_products<I0, NI, SINGLE>(stream_a, statg, v, acc);
             tmem_ld4(tq_a + kTmTheta, qa);
             fft16<+1>(v);
@@ -430,6 +471,7 @@ k_search(const __grid_constant__ SearchArgs A)
             sts16<2176>(xw_a, v);
             const float sw = warp_sum32(re(acc) + im(acc));
             if (lane == 0) sts32(ssig_a + 4 * warp, sw);
+            if (DUAL) { const float pw = warp_sum32(pacc); if (lane == 0) sts32(ssig_a + 64 + 4 * warp, pw); }
             bar_named(bar_id, 256);                          // exchange buffer complete, both tiles read out
             if (t == 0 && !(BEGE_ABL & 2)) {                 // order the streaming tile of this team's next item
                 const uint32_t it2 = it + 2;
@@ -449,10 +491,14 @@ k_search(const __grid_constant__ SearchArgs A)
                 }
             }
             lds16<136>(xr_a, v);
-            float tot = 0.f;
+            float tot = 0.f, ptot = 0.f;
             if (t == 64) {
 #pragma unroll
                 for (int w = 0; w < 8; ++w) tot += lds32(ssig_a + 4 * w);
+                if (DUAL) {
+#pragma unroll
+                    for (int w = 0; w < 8; ++w) ptot += lds32(ssig_a + 64 + 4 * w);
+                }
             }
             if (t == 32 && d2v < 16ull * (it / kRing)) counter_wait_ge(d2 + slot, 16ull * (it / kRing), abort_flag);
             __syncwarp();
@@ -465,8 +511,11 @@ k_search(const __grid_constant__ SearchArgs A)
                 const c2 o = v[q];
                 if (!(BEGE_ABL & 4) || re(o) == 1.2345e-30f) out[q * 4096] = o;
             }
-            if (t == 64)
-                A.sigpart[((A.j0 + grp + (uint64_t)G * tj) * (uint64_t)A.S + (A.m0 + ml) - A.sig_pair0) * 16 + b] = tot;
+            if (t == 64) {
+                const uint64_t pr = (A.j0 + grp + (uint64_t)G * tj) * (uint64_t)A.S + (A.m0 + ml) - A.sig_pair0;
+                A.sigpart[pr * (DUAL ? 32 : 16) + b] = tot;
+                if (DUAL) A.sigpart[pr * 32 + 16 + b] = ptot;
+            }
             // this warp's part of the tile is on its way: tell the publisher (thread 0 of the B team of the same parity)
             __syncwarp();
             if (lane == 0) mbar_arrive(sb + SM::amb + 8 * slot);
@@ -551,13 +600,15 @@ k_search(const __grid_constant__ SearchArgs A)
             c2 v[16];
             lds16<128>(in_a, v);
             const uint64_t pair = (A.j0 + jl) * (uint64_t)A.S + (A.m0 + ml);
-            const float part = __ldcg(A.sigpart + (pair - A.sig_pair0) * 16 + a);
+            const float part = __ldcg(A.sigpart + (pair - A.sig_pair0) * (DUAL ? 32 : 16) + a);
+            const float ppart = DUAL ? __ldcg(A.sigpart + (pair - A.sig_pair0) * 32 + 16 + a) : 0.f;
             c2 wa[2], wb[2];
             tmem_ld4(tq + kTmDelta, wa);
             // four-step factor wN^(16 b k1), k1 = a + 16 r: its CTA-uniform part w256^(b r) here, the rest in delta_p
 #pragma unroll
             for (int r = 1; r < 16; ++r) { const float2 w = c_w256[(b * r) & 255]; v[r] = cmulw(v[r], w.x, w.y); }
             const float sumR2 = hw_sum16(part);
+            const float sumP = DUAL ? hw_sum16(ppart) : 0.f;
             fft16<+1>(v);
             tm_twiddle<0, 8>(tq + kTmDelta, v, wa, wb);      // v[p] *= delta_p = wN^(16 b a) w256^(a p)
             __syncwarp();                                    // every lane of the half-warp has its row in registers
@@ -574,11 +625,15 @@ k_search(const __grid_constant__ SearchArgs A)
             fft16<+1>(v);
             // lane a holds Z[n1 = a + 16 q]; lag n = 256 n1 + n2
             const float thr = A.k2 * sumR2;
+            // dual-stream search: N^2 sigma_1^2 = (S + P)/2 for Re z (H1), N^2 sigma_2^2 = (S - P)/2 for Im z (L1)
+            const float var1 = 0.5f * (sumR2 + sumP), var2 = 0.5f * (sumR2 - sumP);
+            const float thr1 = A.k2 * var1, thr2 = A.k2 * var2;
             bool any = false;
 #pragma unroll
             for (int q = 0; q < 16; ++q) {
                 const float zr = re(v[q]), zi = im(v[q]);
-                any |= fmaf(zi, zi, zr * zr) > thr;
+                if (DUAL) any |= (zr * zr > thr1) | (zi * zi > thr2);
+                else any |= fmaf(zi, zi, zr * zr) > thr;
             }
             if (DBG) {
                 const float invN = 1.0f / (float)kN;
@@ -589,6 +644,23 @@ k_search(const __grid_constant__ SearchArgs A)
 #if BEGE_ABL
             if (thr == -1.f)                                 // timing experiment only: never emit
 #endif
+            if (DUAL) {
+                if (__any_sync(0xffffffffu, any)) {
+                    // PAPER.md:221 Table 3: per sample offset and stream the largest |rho|/sigma and its template
+                    unsigned long long* proj1 = reinterpret_cast<unsigned long long*>(A.rec);
+                    unsigned long long* proj2 = proj1 + (uint64_t)A.S * kN;
+                    const uint32_t lag0 = (uint32_t)(A.m0 + ml) * (uint32_t)kN + (uint32_t)(a * 256 + n2);
+                    const unsigned long long idkey = (unsigned long long)(0xffffffffu - (uint32_t)(A.j0 + jl));
+#pragma unroll
+                    for (int q = 0; q < 16; ++q) {
+                        const float zr = re(v[q]), zi = im(v[q]);
+                        if (zr * zr > thr1 && var1 > 0.f)
+                            atomicMax(proj1 + lag0 + 4096u * q, ((unsigned long long)__float_as_uint(sqrtf(zr * zr / var1)) << 32) | idkey);
+                        if (zi * zi > thr2 && var2 > 0.f)
+                            atomicMax(proj2 + lag0 + 4096u * q, ((unsigned long long)__float_as_uint(sqrtf(zi * zi / var2)) << 32) | idkey);
+                    }
+                }
+            } else
             if (__any_sync(0xffffffffu, any)) {
                 unsigned hits = 0;
                 float mag[16];
@@ -678,6 +750,62 @@ __global__ void k_sigma(const float* __restrict__ sigpart, float* __restrict__ s
     sigma[i] = sqrtf(s) / (float)kN;
 }
 
+// dual-stream search: Q[k] = Re(X[k] X[N-k]) of a stored segment spectrum, same tile layout (one float per bin).
+// grid (16 tiles, segments), 256 threads.
+__global__ void __launch_bounds__(256)
+k_dual_q(const c2* __restrict__ xs, float* __restrict__ q, int I0, int NI)
+{
+    const int t = threadIdx.x, b = blockIdx.x;
+    const uint64_t m = blockIdx.y;
+    const int c = t >> 4, g = t & 15;
+    const c2* X = xs + m * (uint64_t)(16 * NI * 256);
+    float* Q = q + m * (uint64_t)(16 * NI * 256);
+    for (int ii = 0; ii < NI; ++ii) {
+        const uint32_t k = (uint32_t)(16 * b + c) + 256u * (uint32_t)(g + 16 * (ii + I0));
+        const uint32_t km = ((uint32_t)kN - k) & (uint32_t)(kN - 1);
+        const int bm = (int)((km & 255u) >> 4), cm = (int)(km & 15u), gm = (int)((km >> 8) & 15u), im_ = (int)(km >> 12) - I0;
+        const size_t idx = (((size_t)b * (NI / 2) + ii / 2) * 256 + t) * 2 + (ii & 1);
+        float val = 0.f;
+        if (im_ >= 0 && im_ < NI) {
+            const c2 a = X[idx], d = X[(((size_t)bm * (NI / 2) + im_ / 2) * 256 + 16 * cm + gm) * 2 + (im_ & 1)];
+            val = re(a) * re(d) - im(a) * im(d);
+        }
+        Q[idx] = val;
+    }
+}
+
+// dual-stream search: sigma_1 = sqrt((S + P)/2)/N, sigma_2 = sqrt((S - P)/2)/N from the 2 x 16 tile partial sums of a pair
+__global__ void k_sigma_dual(const float* __restrict__ sigpart, float* __restrict__ s1, float* __restrict__ s2, uint64_t n)
+{
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float v[16], w[16];
+    for (int a = 0; a < 16; ++a) { v[a] = sigpart[i * 32 + a]; w[a] = sigpart[i * 32 + 16 + a]; }
+    for (int d = 8; d >= 1; d >>= 1)
+        for (int a = 0; a < d; ++a) { v[a] = v[a] + v[a + d]; w[a] = w[a] + w[a + d]; }     // the order of hw_sum16
+    s1[i] = sqrtf(fmaxf(0.5f * (v[0] + w[0]), 0.f)) / (float)kN;
+    s2[i] = sqrtf(fmaxf(0.5f * (v[0] - w[0]), 0.f)) / (float)kN;
+}
+
+// dual-stream search: offsets with a hit in both streams, and those whose templates' start frequencies differ by less
+// than delta
+__global__ void k_dual_coinc(const uint32_t* __restrict__ id1, const uint32_t* __restrict__ id2, const double* __restrict__ f0,
+                             double delta, uint64_t n, unsigned long long* __restrict__ out)
+{
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    bool sim = false, coi = false;
+    if (i < n) {
+        const uint32_t a = id1[i], b = id2[i];
+        sim = a != 0xffffffffu && b != 0xffffffffu;
+        coi = sim && fabs(f0[a] - f0[b]) < delta;
+    }
+    const unsigned ms = __ballot_sync(0xffffffffu, sim), mc = __ballot_sync(0xffffffffu, coi);
+    if ((threadIdx.x & 31) == 0) {
+        if (ms) atomicAdd(out, (unsigned long long)__popc(ms));
+        if (mc) atomicAdd(out + 1, (unsigned long long)__popc(mc));
+    }
+}
+
 }  // namespace bege
 
 // =================================================================================================
@@ -701,7 +829,8 @@ struct bege_plan {
     d2* tw256d = nullptr;           // exp(2 pi i m / 256) in fp64 (bank generation)
     // workspace
     unsigned char* ws = nullptr; uint64_t ws_bytes = 0, bump = 0; bool user_ws = false;
-    Slot s_bank, s_x, s_scratch, s_sig, s_rec, s_misc, s_par, s_tmp;
+    Slot s_bank, s_x, s_q, s_scratch, s_sig, s_rec, s_misc, s_par, s_tmp;
+    bool bank_real = false, have_sigma_dual = false;
     std::vector<cudaEvent_t> ev_slice;
     uint64_t T = 0; uint32_t S = 0; double tau = 0; uint32_t L = 0;
     bool have_sigma = false;
@@ -779,15 +908,17 @@ static uint64_t tpl_bytes(const bege_plan* p) { return (uint64_t)p->NI * 16 * 25
 
 static void count_launch(bege_plan* p, uint64_t n = 1) { p->stats.kernel_launches += n; }
 
-// the eight instantiations of the search kernel: row-blocks kept (14 / 16), single-segment or batched, debug z output
-static const void* search_variant(int NI, bool single, bool dbg)
+// the instantiations of the search kernel: row-blocks kept (14 / 16), single-segment or batched, debug z output;
+// plus the dual-stream variant (single-segment, 14 row-blocks)
+static const void* search_variant(int NI, bool single, bool dbg, bool dual = false)
 {
+    if (dual) return (const void*)k_search<1, 14, true, false, true>;
     if (NI == 14) {
-        if (single) return dbg ? (const void*)k_search<1, 14, true, true> : (const void*)k_search<1, 14, true, false>;
-        return dbg ? (const void*)k_search<1, 14, false, true> : (const void*)k_search<1, 14, false, false>;
+        if (single) return dbg ? (const void*)k_search<1, 14, true, true, false> : (const void*)k_search<1, 14, true, false, false>;
+        return dbg ? (const void*)k_search<1, 14, false, true, false> : (const void*)k_search<1, 14, false, false, false>;
     }
-    if (single) return dbg ? (const void*)k_search<0, 16, true, true> : (const void*)k_search<0, 16, true, false>;
-    return dbg ? (const void*)k_search<0, 16, false, true> : (const void*)k_search<0, 16, false, false>;
+    if (single) return dbg ? (const void*)k_search<0, 16, true, true, false> : (const void*)k_search<0, 16, true, false, false>;
+    return dbg ? (const void*)k_search<0, 16, false, true, false> : (const void*)k_search<0, 16, false, false, false>;
 }
 
 extern "C" const char* bege_version(void) { return "bege 0.2 (sm_100a)"; }
@@ -862,9 +993,9 @@ extern "C" int bege_plan_create(bege_plan** out, uint32_t N, double fs, double l
 
     // the search kernel needs all its CTAs co-resident (groups hand over through global counters)
     int occ = 0;
-    for (int i = 0; i < 8; ++i) {
-        const void* f = search_variant(i >> 2 ? 16 : 14, (i >> 1) & 1, i & 1);
-        const int sm = (i >> 2) ? search_smem<16>() : search_smem<14>();
+    for (int i = 0; i < 9; ++i) {
+        const void* f = i == 8 ? search_variant(14, true, false, true) : search_variant(i >> 2 ? 16 : 14, (i >> 1) & 1, i & 1);
+        const int sm = (i < 8 && (i >> 2)) ? search_smem<16>() : search_smem<14>();
         if (cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, sm) != cudaSuccess) return bail(BEGE_ECUDA);
         int o = 0;
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, f, kSearchThreads, sm) != cudaSuccess) return bail(BEGE_ECUDA);
@@ -887,7 +1018,7 @@ extern "C" void bege_plan_destroy(bege_plan* p)
     drop_l2_window(p);
     if (p->side) { cudaStreamSynchronize(p->side); cudaStreamDestroy(p->side); }
     if (p->own_stream && p->stream) cudaStreamDestroy(p->stream);
-    for (Slot* s : {&p->s_bank, &p->s_x, &p->s_scratch, &p->s_sig, &p->s_rec, &p->s_misc, &p->s_par, &p->s_tmp}) slot_free(*s);
+    for (Slot* s : {&p->s_bank, &p->s_x, &p->s_q, &p->s_scratch, &p->s_sig, &p->s_rec, &p->s_misc, &p->s_par, &p->s_tmp}) slot_free(*s);
     if (p->tw256) cudaFree(p->tw256);
     if (p->twN) cudaFree(p->twN);
     if (p->tw256d) cudaFree(p->tw256d);
@@ -914,11 +1045,12 @@ extern "C" int bege_plan_workspace_bytes(const bege_plan* p, uint64_t T, uint32_
     b += al(T * tpl_bytes(p));                         // bank
     b += al(T * 16);                                   // template parameters (f0, fdot)
     b += al((uint64_t)S * tpl_bytes(p));               // segment spectra
+    b += al((uint64_t)S * tpl_bytes(p) / 2);           // Re(X[k] X[N-k]) (dual-stream search)
     b += al(scratch_bytes(p));                          // four-step staging (stays in L2)
-    b += al(T * S * 16 * sizeof(float));               // Parseval partial sums
-    b += al(std::max<uint64_t>(cap * sizeof(bege_tail), (uint64_t)S * kN * 8));   // records / max-projection array
+    b += al(T * S * 32 * sizeof(float));               // Parseval partial sums (two per tile in the dual-stream search)
+    b += al(std::max<uint64_t>(cap * sizeof(bege_tail), (uint64_t)S * kN * 16));  // records / max-projection array(s)
     b += al(kMiscHdr + (uint64_t)S * kN * sizeof(c2)); // counters + raw segment staging
-    b += al(std::max<uint64_t>(std::max<uint64_t>(T * S * sizeof(float), (uint64_t)S * kN * 8), kN * sizeof(c2) + 256));   // sigma / projection / debug output
+    b += al(std::max<uint64_t>(std::max<uint64_t>(2 * T * S * sizeof(float), (uint64_t)S * kN * 16), kN * sizeof(c2) + 256));   // sigma / projection / debug output
     *bytes = b + 4096;
     return BEGE_OK;
 }
@@ -930,13 +1062,25 @@ extern "C" int bege_plan_set_workspace(bege_plan* p, void* dev_ptr, uint64_t byt
     CU(p, cudaSetDevice(p->device));
     CU(p, cudaStreamSynchronize(p->stream));
     drop_l2_window(p);
-    for (Slot* s : {&p->s_bank, &p->s_x, &p->s_scratch, &p->s_sig, &p->s_rec, &p->s_misc, &p->s_par, &p->s_tmp}) slot_free(*s);
+    for (Slot* s : {&p->s_bank, &p->s_x, &p->s_q, &p->s_scratch, &p->s_sig, &p->s_rec, &p->s_misc, &p->s_par, &p->s_tmp}) slot_free(*s);
     p->ws = (unsigned char*)dev_ptr; p->ws_bytes = dev_ptr ? bytes : 0; p->bump = 0; p->user_ws = dev_ptr != nullptr;
     p->T = 0; p->S = 0; p->have_sigma = false;
     return BEGE_OK;
 }
 
+static int bank_generate_impl(bege_plan* p, const double* f0, const double* fdot, uint64_t T, double tau, bool real_tpl);
+
 extern "C" int bege_bank_generate(bege_plan* p, const double* f0, const double* fdot, uint64_t T, double tau)
+{
+    return bank_generate_impl(p, f0, fdot, T, tau, false);
+}
+
+extern "C" int bege_bank_generate_real(bege_plan* p, const double* f0, const double* fdot, uint64_t T, double tau)
+{
+    return bank_generate_impl(p, f0, fdot, T, tau, true);
+}
+
+static int bank_generate_impl(bege_plan* p, const double* f0, const double* fdot, uint64_t T, double tau, bool real_tpl)
 {
     if (!p) return BEGE_EINVAL;
     if (!f0 || !fdot || T == 0 || T > 0xffffffffull) return fail(p, BEGE_EINVAL, "bad bank arguments");
@@ -948,7 +1092,7 @@ extern "C" int bege_bank_generate(bege_plan* p, const double* f0, const double* 
     if ((rc = slot_get(p, p->s_bank, T * tpl_bytes(p), &bank))) return rc;
     if ((rc = slot_get(p, p->s_par, T * 16, &par))) return rc;
     if ((rc = slot_get(p, p->s_scratch, scratch_bytes(p), &scr))) return rc;
-    p->T = 0; p->have_sigma = false;
+    p->T = 0; p->have_sigma = false; p->have_sigma_dual = false;
     double* d_f0 = (double*)par; double* d_fd = d_f0 + T;
     CU(p, cudaMemcpyAsync(d_f0, f0, T * sizeof(double), cudaMemcpyHostToDevice, p->stream));
     CU(p, cudaMemcpyAsync(d_fd, fdot, T * sizeof(double), cudaMemcpyHostToDevice, p->stream));
@@ -964,12 +1108,12 @@ extern "C" int bege_bank_generate(bege_plan* p, const double* f0, const double* 
     CU(p, cudaMemcpyAsync(d_hann, hann.data(), L * sizeof(double), cudaMemcpyHostToDevice, p->stream));
     const uint64_t stride = tpl_bytes(p) / sizeof(c2);
     const unsigned ctas = (unsigned)std::min<uint64_t>(T, (uint64_t)p->n_sm);
-    k_bank_gen64<<<ctas, 256, kBankSmem, p->stream>>>(d_f0, d_fd, T, p->fs, L, d_hann, p->tw256d, (float2*)bank, stride, p->I0, p->NI);
+    k_bank_gen64<<<ctas, 256, kBankSmem, p->stream>>>(d_f0, d_fd, T, p->fs, L, d_hann, p->tw256d, (float2*)bank, stride, p->I0, p->NI, real_tpl ? 1 : 0);
     count_launch(p);
     CU(p, cudaStreamSynchronize(p->stream));                 // `hann` (pageable) must outlive its copy
     CU(p, cudaGetLastError());
     CU(p, cudaStreamSynchronize(p->stream));
-    p->T = T; p->tau = tau; p->L = L;
+    p->T = T; p->tau = tau; p->L = L; p->bank_real = real_tpl;
     return BEGE_OK;
 }
 
@@ -983,7 +1127,7 @@ extern "C" int bege_segment_load(bege_plan* p, const float* x, uint32_t S)
     if ((rc = slot_get(p, p->s_x, (uint64_t)S * tpl_bytes(p), &xs))) return rc;
     if ((rc = slot_get(p, p->s_misc, kMiscHdr + (uint64_t)S * kN * sizeof(c2), &misc))) return rc;
     if ((rc = slot_get(p, p->s_scratch, scratch_bytes(p), &scr))) return rc;
-    p->S = 0; p->have_sigma = false;
+    p->S = 0; p->have_sigma = false; p->have_sigma_dual = false;
     c2* raw = (c2*)((unsigned char*)misc + kMiscHdr);
     cudaPointerAttributes at;
     cudaError_t e = cudaPointerGetAttributes(&at, x);
@@ -996,6 +1140,12 @@ extern "C" int bege_segment_load(bege_plan* p, const float* x, uint32_t S)
         k_fwd_rows_data<<<dim3(16, nb), 256, 0, p->stream>>>(raw + (uint64_t)m0 * kN, p->tw256, p->twN, (c2*)scr);
         k_fwd_cols<true><<<dim3(16, nb), 256, 0, p->stream>>>((const c2*)scr, (c2*)xs + m0 * stride, stride, p->I0, p->NI, p->tw256, p->klo, p->khi);
         count_launch(p, 2);
+    }
+    {   // Re(X[k] X[N-k]) for the dual-stream search: one float per stored bin, same layout
+        void* q;
+        if ((rc = slot_get(p, p->s_q, (uint64_t)S * tpl_bytes(p) / 2, &q))) return rc;
+        k_dual_q<<<dim3(16, S), 256, 0, p->stream>>>((const c2*)xs, (float*)q, p->I0, p->NI);
+        count_launch(p);
     }
     CU(p, cudaGetLastError());
     CU(p, cudaStreamSynchronize(p->stream));
@@ -1026,20 +1176,21 @@ static void set_l2_window(bege_plan* p, void* ring)
 // one cooperative launch of the persistent search kernel over templates [j0, j0 + nT) x segments [m0, m0 + nS)
 static int launch_search(bege_plan* p, const c2* bank, const c2* xs, c2* ring, float* sig, uint64_t sig_pair0, float k2, float k2hi,
                          bege_tail* rec, uint64_t cap, unsigned char* misc, c2* zdbg, uint64_t j0, uint64_t nT, uint32_t m0,
-                         uint32_t nS, bool first = true)
+                         uint32_t nS, bool first = true, const float* qseg = nullptr)
 {
+    const bool dual = qseg != nullptr;
     // the first launch of a search also clears the record counter and the abort flag (first 16 bytes)
     CU(p, cudaMemsetAsync(misc + (first ? 0 : 16), 0, kMiscHdr - (first ? 0 : 16), p->stream));
     const int G = (int)std::min<uint64_t>((uint64_t)p->G, nT);
     const dim3 grid(16, G);
     set_l2_window(p, (void*)ring);
     SearchArgs a{};
-    a.bank = bank; a.xseg = xs; a.ring = ring; a.sigpart = sig; a.rec = rec; a.zdbg = zdbg;
+    a.bank = bank; a.xseg = xs; a.qseg = qseg; a.ring = ring; a.sigpart = sig; a.rec = rec; a.zdbg = zdbg;
     a.cap = cap; a.counter = (unsigned long long*)misc; a.abort_flag = (int*)(misc + 8);
     a.done1 = (unsigned long long*)(misc + 256); a.done2 = (unsigned long long*)(misc + 2048);
     a.j0 = j0; a.nT = nT; a.sig_pair0 = sig_pair0; a.m0 = m0; a.nS = nS; a.S = p->S; a.k2 = k2; a.k2hi = k2hi;
     void* args[] = {&a};
-    const void* f = search_variant(p->NI, nS == 1, zdbg != nullptr);
+    const void* f = search_variant(p->NI, nS == 1, zdbg != nullptr, dual);
     const int smem = p->NI == 14 ? search_smem<14>() : search_smem<16>();
     if (p->profiling) cudaEventRecord(p->ev_a, p->stream);
     CU(p, cudaLaunchCooperativeKernel(f, grid, dim3(kSearchThreads), args, smem, p->stream));
@@ -1084,7 +1235,7 @@ static int search_impl(bege_plan* p, float k_sigma, float k_hi, bege_tail* tails
     CU(p, cudaSetDevice(p->device));
     void *sig, *rec, *misc, *scr, *bank, *xs;
     int rc;
-    if ((rc = slot_get(p, p->s_sig, p->T * p->S * 16 * sizeof(float), &sig))) return rc;
+    if ((rc = slot_get(p, p->s_sig, p->T * p->S * 32 * sizeof(float), &sig))) return rc;
     if ((rc = slot_get(p, p->s_rec, cap * sizeof(bege_tail), &rec))) return rc;
     if ((rc = slot_get(p, p->s_misc, kMiscHdr, &misc))) return rc;
     if ((rc = slot_get(p, p->s_scratch, scratch_bytes(p), &scr))) return rc;
@@ -1136,7 +1287,7 @@ static int search_impl(bege_plan* p, float k_sigma, float k_hi, bege_tail* tails
                               cudaMemcpyDeviceToHost, p->side));
     CU(p, cudaStreamSynchronize(p->side));
     p->stats.correlations += p->T * p->S;
-    p->have_sigma = true;
+    p->have_sigma = true; p->have_sigma_dual = false;
     *n_tails = total;
     if (total > cap) return fail(p, BEGE_EOVERFLOW, "%llu tails exceed cap %llu", (unsigned long long)total, (unsigned long long)cap);
     return BEGE_OK;
@@ -1178,7 +1329,7 @@ extern "C" int bege_search_maxproj(bege_plan* p, float k_sigma, float* snr_out, 
     void *sig, *proj, *misc, *scr, *bank, *xs, *tmp;
     int rc;
     const uint64_t n = (uint64_t)p->S * kN;
-    if ((rc = slot_get(p, p->s_sig, p->T * p->S * 16 * sizeof(float), &sig))) return rc;
+    if ((rc = slot_get(p, p->s_sig, p->T * p->S * 32 * sizeof(float), &sig))) return rc;
     if ((rc = slot_get(p, p->s_rec, n * sizeof(unsigned long long), &proj))) return rc;
     if ((rc = slot_get(p, p->s_misc, kMiscHdr, &misc))) return rc;
     if ((rc = slot_get(p, p->s_scratch, scratch_bytes(p), &scr))) return rc;
@@ -1205,8 +1356,84 @@ extern "C" int bege_search_maxproj(bege_plan* p, float k_sigma, float* snr_out, 
     drop_l2_window(p);
     if (rc) return rc;
     p->stats.correlations += p->T * p->S;
-    p->have_sigma = true;
+    p->have_sigma = true; p->have_sigma_dual = false;
     if (n_hits) *n_hits = *p->h_count;
+    return BEGE_OK;
+}
+
+extern "C" int bege_search_dual(bege_plan* p, float k_sigma, float* snr1, uint32_t* id1, float* snr2, uint32_t* id2,
+                                double delta_hz, uint64_t* n_simultaneous, uint64_t* n_coincident)
+{
+    if (!p) return BEGE_EINVAL;
+    if (!snr1 || !id1 || !snr2 || !id2 || !(k_sigma >= 0.f)) return fail(p, BEGE_EINVAL, "bad search arguments");
+    if (!p->T || !p->S) return fail(p, BEGE_ESTATE, "bege_search_dual needs a generated bank and loaded segments");
+    if (!p->bank_real) return fail(p, BEGE_ESTATE, "bege_search_dual needs a bank of real templates (bege_bank_generate_real)");
+    if (p->NI != 14) return fail(p, BEGE_EINVAL, "bege_search_dual supports bands inside bins [4096, 61440) only");
+    CU(p, cudaSetDevice(p->device));
+    void *sig, *proj, *misc, *scr, *bank, *xs, *q, *tmp, *par;
+    int rc;
+    const uint64_t n = (uint64_t)p->S * kN;
+    if ((rc = slot_get(p, p->s_sig, p->T * p->S * 32 * sizeof(float), &sig))) return rc;
+    if ((rc = slot_get(p, p->s_rec, 2 * n * sizeof(unsigned long long), &proj))) return rc;
+    if ((rc = slot_get(p, p->s_misc, kMiscHdr, &misc))) return rc;
+    if ((rc = slot_get(p, p->s_scratch, scratch_bytes(p), &scr))) return rc;
+    if ((rc = slot_get(p, p->s_tmp, 2 * n * 8, &tmp))) return rc;
+    if ((rc = slot_get(p, p->s_bank, 0, &bank))) return rc;
+    if ((rc = slot_get(p, p->s_x, 0, &xs))) return rc;
+    if ((rc = slot_get(p, p->s_q, 0, &q))) return rc;
+    if ((rc = slot_get(p, p->s_par, 0, &par))) return rc;
+    p->have_sigma = false; p->have_sigma_dual = false;
+    CU(p, cudaMemsetAsync(proj, 0, 2 * n * sizeof(unsigned long long), p->stream));
+    const uint64_t maxT = std::max<uint64_t>(1, p->max_items) * (uint64_t)p->G;
+    bool first = true;
+    // the stationary operand of a single-segment launch is the segment (and its Q): one launch (group) per segment
+    for (uint32_t m = 0; m < p->S; ++m)
+        for (uint64_t jj = 0; jj < p->T; jj += maxT) {
+            if ((rc = launch_search(p, (const c2*)bank, (const c2*)xs, (c2*)scr, (float*)sig, 0, k_sigma * k_sigma, INFINITY,
+                                    (bege_tail*)proj, ~0ull, (unsigned char*)misc, nullptr, jj, std::min(maxT, p->T - jj), m, 1,
+                                    first, (const float*)q))) { drop_l2_window(p); return rc; }
+            first = false;
+        }
+    CU(p, cudaGetLastError());
+    float* d_snr1 = (float*)tmp; uint32_t* d_id1 = (uint32_t*)(d_snr1 + n);
+    float* d_snr2 = (float*)(d_id1 + n); uint32_t* d_id2 = (uint32_t*)(d_snr2 + n);
+    unsigned long long* d_cnt = (unsigned long long*)((unsigned char*)misc + 16);      // hits1, hits2, simultaneous, coincident
+    CU(p, cudaMemsetAsync(d_cnt, 0, 4 * sizeof(unsigned long long), p->stream));
+    const unsigned nb = (unsigned)((n + 255) / 256);
+    k_proj_decode<<<nb, 256, 0, p->stream>>>((const unsigned long long*)proj, d_snr1, d_id1, d_cnt, n);
+    k_proj_decode<<<nb, 256, 0, p->stream>>>((const unsigned long long*)proj + n, d_snr2, d_id2, d_cnt + 1, n);
+    k_dual_coinc<<<nb, 256, 0, p->stream>>>(d_id1, d_id2, (const double*)par, delta_hz, n, d_cnt + 2);
+    count_launch(p, 3);
+    CU(p, cudaMemcpyAsync(snr1, d_snr1, n * sizeof(float), cudaMemcpyDeviceToHost, p->stream));
+    CU(p, cudaMemcpyAsync(id1, d_id1, n * sizeof(uint32_t), cudaMemcpyDeviceToHost, p->stream));
+    CU(p, cudaMemcpyAsync(snr2, d_snr2, n * sizeof(float), cudaMemcpyDeviceToHost, p->stream));
+    CU(p, cudaMemcpyAsync(id2, d_id2, n * sizeof(uint32_t), cudaMemcpyDeviceToHost, p->stream));
+    CU(p, cudaMemcpyAsync(p->h_count + 2, d_cnt, 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, p->stream));
+    rc = check_abort(p, (unsigned char*)misc);      // synchronises the stream
+    drop_l2_window(p);
+    if (rc) return rc;
+    p->stats.correlations += p->T * p->S;
+    p->have_sigma_dual = true;
+    if (n_simultaneous) *n_simultaneous = p->h_count[4];
+    if (n_coincident) *n_coincident = p->h_count[5];
+    return BEGE_OK;
+}
+
+extern "C" int bege_get_sigma_dual(bege_plan* p, float* sigma1_out, float* sigma2_out)
+{
+    if (!p || !sigma1_out || !sigma2_out) return BEGE_EINVAL;
+    if (!p->have_sigma_dual) return fail(p, BEGE_ESTATE, "bege_get_sigma_dual needs a completed bege_search_dual");
+    CU(p, cudaSetDevice(p->device));
+    const uint64_t n = p->T * p->S;
+    void *sig, *tmp;
+    int rc;
+    if ((rc = slot_get(p, p->s_sig, 0, &sig))) return rc;
+    if ((rc = slot_get(p, p->s_tmp, 2 * n * sizeof(float), &tmp))) return rc;
+    k_sigma_dual<<<(unsigned)((n + 255) / 256), 256, 0, p->stream>>>((const float*)sig, (float*)tmp, (float*)tmp + n, n);
+    count_launch(p);
+    CU(p, cudaMemcpyAsync(sigma1_out, tmp, n * sizeof(float), cudaMemcpyDeviceToHost, p->stream));
+    CU(p, cudaMemcpyAsync(sigma2_out, (float*)tmp + n, n * sizeof(float), cudaMemcpyDeviceToHost, p->stream));
+    CU(p, cudaStreamSynchronize(p->stream));
     return BEGE_OK;
 }
 

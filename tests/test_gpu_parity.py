@@ -552,3 +552,62 @@ def test_config4_full_size_tail_heavy(bo, bege):
         sel["template_id"] = np.searchsorted(sample, sel["template_id"]).astype(np.uint32)
         check_tail_sets(sel, sel.size, lo_tails, k)
         assert np.max(np.abs(sg[sample] - sigma_o[:, 0]) / sigma_o[:, 0]) <= SIGMA_RTOL
+
+
+# ----------------------------------------------------------------------------- dual-stream search
+def test_dual_stream_search_matches_oracle(bo, bege):
+    """x = H1 + i L1 with real templates: per stream sigma (Hermitian split of the product spectrum, eq.7), the
+    Table-3 output (largest |rho|/sigma and its template per offset and stream), simultaneous / coincident counts.
+    A chirp is injected into H1 of segment 1 only."""
+    xs = []
+    n0 = None
+    for m in range(2):
+        h1 = synth.band_limit(synth.white_noise(60 + 2 * m))
+        l1 = synth.band_limit(synth.white_noise(61 + 2 * m))
+        if m == 1:
+            h1, n0 = synth.inject_chirp(h1, 1000.0, 50.0, 5.0, 12.0)
+        xs.append((h1 + 1j * l1).astype(np.complex64))
+    xs = np.stack(xs)
+    Xs = np.stack([bo.segment_spectrum(x, FS, *BAND) for x in xs])
+    w = synth.config0()
+    f0 = np.concatenate([w.f0[::5], [1000.0, 1000.0]])        # 54 templates, the last two identical (a planted tie)
+    fd = np.concatenate([w.fdot[::5], [50.0, 50.0]])
+    k, delta = 3.0, 300.0
+    o1, oi1, o2, oi2, sig_o = bo.search_dual(Xs, f0, fd, TAU, FS, k - 1e-3)
+    with bege.Plan(N, FS, BAND) as plan:
+        plan.bank_generate_real(f0, fd, TAU)
+        plan.segment_load(xs)
+        g1, gi1, g2, gi2, n_sim, n_coi = plan.search_dual(k, delta)
+        s1, s2 = plan.get_sigma_dual()
+        # the real bank under the plain search: z against the oracle's dual correlation
+        for (j, m) in ((0, 0), (53, 1), (20, 1)):
+            z, _, _ = bo.correlate_dual(Xs[m], bo.template_real(f0[j], fd[j], TAU, FS, N))
+            zg, _ = plan.debug_correlate(j, m)
+            assert rel_l2(zg.astype(np.complex128), z) <= REL_L2
+    assert np.max(np.abs(s1 - sig_o[:, :, 0]) / sig_o[:, :, 0]) <= SIGMA_RTOL
+    assert np.max(np.abs(s2 - sig_o[:, :, 1]) / sig_o[:, :, 1]) <= SIGMA_RTOL
+    none = np.iinfo(np.uint32).max
+    n_checked = 0
+    for g, gi, o, oi, stream in ((g1, gi1, o1, oi1, 0), (g2, gi2, o2, oi2, 1)):
+        assert np.all((g == 0) == (gi == none))
+        must, may = o > k + GUARD, o > k - GUARD
+        assert not np.any(must & (g == 0)), "oracle offsets missing on the GPU"
+        assert not np.any((g > 0) & ~may), "GPU offsets the oracle does not have"
+        both = must & (g > 0)
+        assert np.max(np.abs(g[both] - o[both]) / o[both]) < 2e-5
+        diff = both & (gi != oi)                                # near-ties: the other template must be as good
+        for m, n in zip(*np.nonzero(diff)):
+            z, t1, t2 = bo.correlate_dual(Xs[m], bo.template_real(f0[gi[m, n]], fd[gi[m, n]], TAU, FS, N))
+            val = abs(z[n].real) / t1 if stream == 0 else abs(z[n].imag) / t2
+            assert abs(val - o[m, n]) / o[m, n] < 2e-6
+        assert not np.any(gi == 53)                             # equal values go to the smaller template id
+        n_checked += int(both.sum())
+    assert n_checked > 10000
+    peak = np.unravel_index(np.argmax(g1), g1.shape)
+    assert peak[0] == 1 and gi1[peak] == 52 and abs(int(peak[1]) - n0) <= 8 and g1[peak] > 8.0
+    assert g2[1, n0 - 50: n0 + 50].max() < 5.0                  # nothing in the other detector
+    sim = (gi1 != none) & (gi2 != none)
+    assert n_sim == int(sim.sum())
+    assert n_coi == int(np.sum(np.abs(f0[gi1[sim]] - f0[gi2[sim]]) < delta))
+    os_, oc = bo.dual_coincidences(oi1, oi2, f0, delta)        # the oracle's counts at its own (slightly lower) threshold
+    assert abs(n_sim - os_) <= 0.02 * os_ + 5 and abs(n_coi - oc) <= 0.02 * oc + 5
