@@ -201,6 +201,9 @@ k_fwd_cols(const c2* __restrict__ G, c2* __restrict__ out, uint64_t out_stride, 
 // The ring holds kRing items per group (G x kRing x 512 KiB) and lives in L2.
 constexpr int kRing = 8;
 constexpr int kSearchThreads = 32 * 32;
+#ifndef BEGE_STATS
+#define BEGE_STATS 0       // 1: one CTA prints wait statistics of its service threads at the end (experiments only)
+#endif
 constexpr int kTmemCols = 256;
 constexpr uint32_t kTmDelta = 0, kTmStat = 32, kTmTheta = 96, kTmQ = 160;   // kTmQ: 16 columns per warp of a quadrant
 __constant__ float2 c_w256[256];           // exp(2 pi i m / 256), rounded from fp64 (host, bege_plan_create)
@@ -228,7 +231,8 @@ template <int NI> struct SearchSmem {
     static constexpr uint32_t bfull = amb + 8 * kRing;           // [kNB] mbarriers: row tile has arrived
     static constexpr uint32_t bempty = bfull + 24;               // [kNB] mbarriers: ... has been read out (8 B warps)
     static constexpr uint32_t bgo = bempty + 24;                 // [2][4] mbarriers: row tile of the B team's item is there (thread 0)
-    static constexpr uint32_t total = bgo + 64;
+    static constexpr uint32_t pubit = bgo + 64;                  // [2] u32: next item of A team k to publish (claimed by atomicCAS)
+    static constexpr uint32_t total = pubit + 8;
     static_assert(total + 128 <= 232448, "shared memory of one SM");
 };
 // the stationary tile has its tensor-memory arrangement written out for bands that need 14 of the 16 row-blocks;
@@ -353,6 +357,8 @@ k_search(const __grid_constant__ SearchArgs A)
         for (int i = 0; i < kRing; ++i) mbar_init(sb + SM::amb + 8 * i, 8);
         for (int i = 0; i < SM::kNB; ++i) { mbar_init(sb + SM::bfull + 8 * i, 1); mbar_init(sb + SM::bempty + 8 * i, 8); }
         for (int i = 0; i < 8; ++i) mbar_init(sb + SM::bgo + 8 * i, 1);
+        reinterpret_cast<volatile uint32_t*>(smem_raw + SM::pubit)[0] = 0;
+        reinterpret_cast<volatile uint32_t*>(smem_raw + SM::pubit)[1] = 1;
         fence_mbar_init();
     }
     if (threadIdx.x < 32) tmem_alloc<kTmemCols>(sb + SM::bars + 24);
@@ -440,6 +446,7 @@ k_search(const __grid_constant__ SearchArgs A)
         }
         uint32_t nload = 0;                                  // tiles this team has waited for so far
         uint32_t tj_prev = 0;
+        long long st_d2 = 0, st_tma = 0; unsigned st_nd2 = 0;
         for (uint32_t it = team; it < n_items; it += 2) {
             const uint32_t tj = SINGLE ? it : it / nS;
             const uint32_t ml = SINGLE ? 0u : (uint32_t)(it - tj * nS);
@@ -453,7 +460,7 @@ k_search(const __grid_constant__ SearchArgs A)
             if (STAT) tmem_ld4(tq_a + kTmStat, qa);
             if (DUAL) tmem_ld2f(tq + kTmQ + 16u * (uint32_t)(warp >> 2), ra);
 #if !(BEGE_ABL & 2)
-            mbar_wait(bar_stream, nload & 1, abort_flag);
+            { const long long c0 = BEGE_STATS ? clock64() : 0; mbar_wait(bar_stream, nload & 1, abort_flag); if (BEGE_STATS) st_tma += clock64() - c0; }
 #endif
             ++nload;
             if (!SINGLE && !STAT && tj != tj_prev) statg = reinterpret_cast<const ulonglong2*>(tpl_tile(tj)) + t;
@@ -500,7 +507,11 @@ k_search(const __grid_constant__ SearchArgs A)
                     for (int w = 0; w < 8; ++w) ptot += lds32(ssig_a + 64 + 4 * w);
                 }
             }
-            if (t == 32 && d2v < 16ull * (it / kRing)) counter_wait_ge(d2 + slot, 16ull * (it / kRing), abort_flag);
+            if (t == 32 && d2v < 16ull * (it / kRing)) {
+                const long long c0 = BEGE_STATS ? clock64() : 0;
+                counter_wait_ge(d2 + slot, 16ull * (it / kRing), abort_flag);
+                if (BEGE_STATS) { st_d2 += clock64() - c0; ++st_nd2; }
+            }
             __syncwarp();
             bar_named(bar_id, 256);                          // exchange buffer free for the team's next item; slot free
             fft16<+1>(v);
@@ -520,29 +531,39 @@ k_search(const __grid_constant__ SearchArgs A)
             __syncwarp();
             if (lane == 0) mbar_arrive(sb + SM::amb + 8 * slot);
         }
+        if (BEGE_STATS && b == 3 && grp == 1 && (t == 32 || t == 0))
+            printf("A team %d t %d: items %u, d2 waits %u, d2 wait cycles/item %lld, stream-tile wait cycles/item %lld\n", team, t, nload,
+                   st_nd2, st_d2 / (long long)max(nload, 1u), st_tma / (long long)max(nload, 1u));
     } else if (team >= 2 && !(BEGE_ABL & 32)) {
         // ================================================================ B: pass 2, items ib = team - 2 (mod 2)
         const int kb = team - 2;
         const int hw = t >> 4, a = t & 15;                   // row of the row tile, lane of its half-warp
         const int n2 = 16 * b + hw;
         constexpr uint32_t NB = SM::kNB;                     // item i uses tile buffer i % NB (both teams share the buffers)
-        // ---- service thread (t == 0) state
+        // ---- service state.  Thread 0 polls done1 (acquire) and issues the bulk copies; the gpu-scope fences -- about a
+        // microsecond each while the SM has stores in flight -- are kept off its warp, whose progress paces the team: the
+        // warp (1 + item mod 7) of the team takes them at the top of each item (once per seven items and warp).  Thread 0
+        // takes them only inside its wait loop, when pass 2 is ahead of pass 1 and the team idles anyway (somebody must
+        // publish then, or the group would stall).  The publication cursor lives in shared memory and is claimed by CAS.
         constexpr bool PUB = !(BEGE_ABL & (1 | 16));
-        uint32_t pub_it = kb;                                // next item of A team kb to publish
+        uint32_t* const pub_it = reinterpret_cast<uint32_t*>(smem_raw + SM::pubit) + kb;   // next item of A team kb to publish
         uint32_t ld_it = kb;                                 // next item of this team whose copy is to be issued
         unsigned long long d1v = 0; uint32_t d1v_it = ~0u;   // last acquired tiles-arrived counter and its item
         uint32_t nit = 0;                                    // items this team has started
+        long long st_top = 0; unsigned st_ntop = 0, st_nmid = 0, st_spin = 0;
         // whenever all 8 warps of A team kb have stored their part of an item (mbarrier amb[slot]): ONE
         // fence.acq_rel.gpu, then done1[slot] += 1 (and, under the same fence, done2[free_slot] += 1)
         auto publish = [&](int free_slot) {
             uint32_t n = 0;
-            if (PUB)
-                while (n < 4 && pub_it + 2 * n < n_items &&
-                       mbar_test_wait(sb + SM::amb + 8 * ((pub_it + 2 * n) % kRing), ((pub_it + 2 * n) / kRing) & 1)) ++n;
+            const uint32_t first = *(volatile uint32_t*)pub_it;
+            if (PUB) {
+                while (n < 4 && first + 2 * n < n_items &&
+                       mbar_test_wait(sb + SM::amb + 8 * ((first + 2 * n) % kRing), ((first + 2 * n) / kRing) & 1)) ++n;
+                if (n && atomicCAS(pub_it, first, first + 2 * n) != first) n = 0;      // another thread of the team has them
+            }
             if (n == 0 && free_slot < 0) return;
             fence_acq_rel_gpu();
-            for (uint32_t i = 0; i < n; ++i) counter_add_relaxed(d1 + (pub_it + 2 * i) % kRing, 1ull);
-            pub_it += 2 * n;
+            for (uint32_t i = 0; i < n; ++i) counter_add_relaxed(d1 + (first + 2 * i) % kRing, 1ull);
             if (free_slot >= 0) counter_add_relaxed(d2 + free_slot, 1ull);
         };
         // copy of item `it` of this team into its tile buffer, if the buffer has been read out (item it - NB, either
@@ -574,7 +595,9 @@ k_search(const __grid_constant__ SearchArgs A)
             if (t == 0) {
                 const unsigned long long target = 16ull * (ib / kRing + 1);
                 const long long t0 = clock64();
+                if (BEGE_STATS) { if (ld_it == ib) ++st_ntop; else ++st_nmid; }
                 for (;;) {
+                    if (BEGE_STATS) ++st_spin;
                     if (ld_it == ib) {                       // copy of this item not yet issued
                         publish(-1);
                         try_load(ib, (BEGE_ABL & 1) || counter_load_acquire(d1 + slot) >= target);
@@ -589,13 +612,15 @@ k_search(const __grid_constant__ SearchArgs A)
                 // Four barriers rotate over the team's items: this thread is never more than NB = 3 items ahead of the
                 // team's slowest warp (a buffer is refilled only after all eight warps have read it out), so a waiter
                 // and this thread never meet on a barrier in different uses.
+                if (BEGE_STATS) st_top += clock64() - t0;
                 mbar_arrive(sb + SM::bgo + 32 * kb + 8 * (nit & 3));
-                publish(slot);                               // the rows are in shared memory: the ring slot is free
                 // look at the counter of the team's next item now; the answer is used after the exchange
                 if (!(BEGE_ABL & 1) && ib + 2 < n_items && ld_it == ib + 2) { d1v = counter_load_acquire(d1 + (ib + 2) % kRing); d1v_it = ib + 2; }
             }
             __syncwarp();
             mbar_wait(sb + SM::bgo + 32 * kb + 8 * (nit & 3), (nit >> 2) & 1, abort_flag);
+            // the rows are in shared memory: the ring slot is free.  This item's fence duty: warp 1 + (nit mod 7)
+            if (warp == 1 + (int)(nit % 7) && lane == 0) publish(slot);
             ++nit;
             c2 v[16];
             lds16<128>(in_a, v);
@@ -720,10 +745,15 @@ k_search(const __grid_constant__ SearchArgs A)
                 }
             }
         }
+        if (BEGE_STATS && b == 3 && grp == 1 && t == 0)
+            printf("B team %d: items %u, copies issued at the item top %u / ahead %u, top-loop cycles/item %lld, spins/item %u\n", kb, nit,
+                   st_ntop, st_nmid, st_top / (long long)max(nit, 1u), st_spin / max(nit, 1u));
         if (t == 0) {                                        // tiles A team kb stores after this team's last copy
             publish(-1);
-            while (PUB && pub_it < n_items) {
-                mbar_wait(sb + SM::amb + 8 * (pub_it % kRing), (pub_it / kRing) & 1, abort_flag);
+            for (;;) {
+                const uint32_t nx = *(volatile uint32_t*)pub_it;
+                if (!PUB || nx >= n_items) break;
+                mbar_wait(sb + SM::amb + 8 * (nx % kRing), (nx / kRing) & 1, abort_flag);
                 if (*(volatile int*)abort_flag) break;
                 publish(-1);
             }
