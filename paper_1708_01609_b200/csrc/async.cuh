@@ -72,7 +72,9 @@ BEGE_DA void mbar_wait(uint32_t bar, uint32_t parity, int* abort_flag)
     const long long t0 = clock64();
     while (!mbar_try_wait(bar, parity)) {
         if (*(volatile int*)abort_flag) return;
-        if (clock64() - t0 > kSpinLimit) { *(volatile int*)abort_flag = 1; return; }
+        if (clock64() - t0 > kSpinLimit) {
+            *(volatile int*)abort_flag = 1; return;
+        }
     }
 }
 
@@ -166,6 +168,18 @@ BEGE_DA void tmem_wait_ld(unsigned long long (&w)[2], float (&f)[2])
 // ---- named barrier of `nthreads` threads
 BEGE_DA void bar_named(int id, int nthreads) { asm volatile("bar.sync %0, %1;" :: "r"(id), "r"(nthreads) : "memory"); }
 
+// ---- cta-scope monotone counter in shared memory (where a parity wait could be more than one phase away)
+BEGE_DA void smem_counter_add_release(uint32_t addr, uint32_t v)
+{
+    asm volatile("red.release.cta.shared::cta.add.u32 [%0], %1;" :: "r"(addr), "r"(v) : "memory");
+}
+BEGE_DA uint32_t smem_counter_load_acquire(uint32_t addr)
+{
+    uint32_t v;
+    asm volatile("ld.acquire.cta.shared::cta.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+    return v;
+}
+
 // ---- gpu-scope counters
 BEGE_DA void counter_add_release(unsigned long long* ctr, unsigned long long v)
 {
@@ -192,7 +206,9 @@ BEGE_DA void counter_wait_ge(const unsigned long long* ctr, unsigned long long t
         __nanosleep(100);
         if (counter_load_acquire(ctr) >= target) return;
         if (*(volatile int*)abort_flag) return;
-        if (clock64() - t0 > kSpinLimit) { *(volatile int*)abort_flag = 1; return; }
+        if (clock64() - t0 > kSpinLimit) {
+            *(volatile int*)abort_flag = 1; return;
+        }
     }
 }
 

@@ -199,7 +199,10 @@ k_fwd_cols(const c2* __restrict__ G, c2* __restrict__ out, uint64_t out_stride, 
 //              under the same kind of fence.  ONE thread of the A team acquires 16 of them, early in the item, before
 //              the barrier that precedes the team's ring stores.
 // The ring holds kRing items per group (G x kRing x 512 KiB) and lives in L2.
-constexpr int kRing = 8;
+#ifndef BEGE_RING
+#define BEGE_RING 16
+#endif
+constexpr int kRing = BEGE_RING;
 constexpr int kSearchThreads = 32 * 32;
 #ifndef BEGE_STATS
 #define BEGE_STATS 0       // 1: one CTA prints wait statistics of its service threads at the end (experiments only)
@@ -229,7 +232,7 @@ template <int NI> struct SearchSmem {
     static constexpr uint32_t bars = ssig + 128;                 // mbarriers: stream[2]; TMEM base address @ +24
     static constexpr uint32_t amb = bars + 32;                   // [kRing] mbarriers: tile of ring slot stored (8 A warps)
     static constexpr uint32_t bfull = amb + 8 * kRing;           // [kNB] mbarriers: row tile has arrived
-    static constexpr uint32_t bempty = bfull + 24;               // [kNB] mbarriers: ... has been read out (8 B warps)
+    static constexpr uint32_t bempty = bfull + 24;               // [kNB] u32 counters (8-byte pitch): warps that have read a tile out
     static constexpr uint32_t bgo = bempty + 24;                 // [2][4] mbarriers: row tile of the B team's item is there (thread 0)
     static constexpr uint32_t pubit = bgo + 64;                  // [2] u32: next item of A team k to publish (claimed by atomicCAS)
     static constexpr uint32_t total = pubit + 8;
@@ -355,7 +358,10 @@ k_search(const __grid_constant__ SearchArgs A)
     if (threadIdx.x == 0) {
         mbar_init(sb + SM::bars, 1); mbar_init(sb + SM::bars + 8, 1);
         for (int i = 0; i < kRing; ++i) mbar_init(sb + SM::amb + 8 * i, 8);
-        for (int i = 0; i < SM::kNB; ++i) { mbar_init(sb + SM::bfull + 8 * i, 1); mbar_init(sb + SM::bempty + 8 * i, 8); }
+        for (int i = 0; i < SM::kNB; ++i) {
+            mbar_init(sb + SM::bfull + 8 * i, 1);
+            *reinterpret_cast<volatile uint32_t*>(smem_raw + SM::bempty + 8 * i) = 0;
+        }
         for (int i = 0; i < 8; ++i) mbar_init(sb + SM::bgo + 8 * i, 1);
         reinterpret_cast<volatile uint32_t*>(smem_raw + SM::pubit)[0] = 0;
         reinterpret_cast<volatile uint32_t*>(smem_raw + SM::pubit)[1] = 1;
@@ -567,10 +573,12 @@ k_search(const __grid_constant__ SearchArgs A)
             if (free_slot >= 0) counter_add_relaxed(d2 + free_slot, 1ull);
         };
         // copy of item `it` of this team into its tile buffer, if the buffer has been read out (item it - NB, either
-        // team) and all 16 tiles of the item are in the ring (d1, acquired: `ready`); non-blocking
+        // team) and all 16 tiles of the item are in the ring (d1, acquired: `ready`); non-blocking.  "Read out" is a
+        // monotone count of warps (8 per use), not an mbarrier: this thread may look at a buffer whose use before last
+        // (by a slow warp of its own team) is still going on, two phases away, where a parity test cannot tell.
         auto try_load = [&](uint32_t it, bool ready) {
             const uint32_t bf = it % NB, us = it / NB;
-            if (us > 0 && !mbar_test_wait(sb + SM::bempty + 8 * bf, (us - 1) & 1)) return;
+            if (us > 0 && smem_counter_load_acquire(sb + SM::bempty + 8 * bf) < 8 * us) return;
             if (!ready) return;
             if (!(BEGE_ABL & 8)) {
                 fence_proxy_async_smem();
@@ -604,7 +612,9 @@ k_search(const __grid_constant__ SearchArgs A)
                     }
                     if (ld_it > ib && ((BEGE_ABL & 8) || mbar_test_wait(sb + SM::bfull + 8 * buf, use & 1))) break;
                     if (*(volatile int*)abort_flag) break;
-                    if (clock64() - t0 > kSpinLimit) { *(volatile int*)abort_flag = 1; break; }
+                    if (clock64() - t0 > kSpinLimit) {
+                        *(volatile int*)abort_flag = 1; break;
+                    }
                     __nanosleep(40);
                 }
                 // The other seven warps wait on a per-team barrier, not on the tile's own: the tile buffers are shared
@@ -635,6 +645,8 @@ k_search(const __grid_constant__ SearchArgs A)
             const float sumR2 = hw_sum16(part);
             const float sumP = DUAL ? hw_sum16(ppart) : 0.f;
             fft16<+1>(v);
+            if (t == 0 && ib + 2 < n_items && ld_it == ib + 2)   // first chance to bring in the team's next item
+                try_load(ib + 2, (BEGE_ABL & 1) || (d1v_it == ib + 2 && d1v >= 16ull * ((ib + 2) / kRing + 1)));
             tm_twiddle<0, 8>(tq + kTmDelta, v, wa, wb);      // v[p] *= delta_p = wN^(16 b a) w256^(a p)
             __syncwarp();                                    // every lane of the half-warp has its row in registers
 #pragma unroll
@@ -644,7 +656,7 @@ k_search(const __grid_constant__ SearchArgs A)
             for (int aa = 0; aa < 16; ++aa) v[aa] = lds64<0>((xr0 ^ (uint32_t)(aa << 3)) + 128 * aa);
             fence_proxy_async_smem();                        // these generic accesses before the next bulk copy into the tile
             __syncwarp();
-            if (lane == 0) mbar_arrive(sb + SM::bempty + 8 * buf);
+            if (lane == 0) smem_counter_add_release(sb + SM::bempty + 8 * buf, 1);
             if (t == 0 && ib + 2 < n_items && ld_it == ib + 2)   // bring in the team's next item while this one is finished
                 try_load(ib + 2, (BEGE_ABL & 1) || (d1v_it == ib + 2 && d1v >= 16ull * ((ib + 2) / kRing + 1)));
             fft16<+1>(v);
