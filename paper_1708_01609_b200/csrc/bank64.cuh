@@ -8,6 +8,7 @@
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
+#include "cplx.cuh"
 
 namespace bege {
 
@@ -157,7 +158,7 @@ k_bank_gen64(const double* __restrict__ f0, const double* __restrict__ fdot, uin
             for (int k = 0; k < 16; ++k) v[k] = bufB[m1 * 256 + k * 16 + (l0 ^ k)];
             dfft16f(v);
             // v[q1] = H[k], k = (16 m1 + r) + 256 (q0 + 16 q1): tile m1, thread 16 r + q0, row-block q1 (stored in pairs)
-            float4* ot = o + (size_t)m1 * (NI / 2) * 256 + 16 * r + l0;
+            float4* ot = o + tile_word(NI, m1, 0, 16 * r + l0);       // + 32 ip
 #pragma unroll
             for (int ip = 0; ip < 8; ++ip) {
                 if (2 * ip < NI) {
@@ -166,7 +167,7 @@ k_bank_gen64(const double* __restrict__ f0, const double* __restrict__ fdot, uin
                                                  (float)v[(2 * ip + 2) & 15].x, (float)v[(2 * ip + 2) & 15].y);
                     else         w = make_float4((float)v[2 * ip].x, (float)v[2 * ip].y,
                                                  (float)v[(2 * ip + 1) & 15].x, (float)v[(2 * ip + 1) & 15].y);
-                    ot[ip * 256] = w;
+                    ot[ip * 32] = w;
                 }
             }
         }

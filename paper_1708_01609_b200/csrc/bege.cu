@@ -11,11 +11,10 @@
 //     step A (k_fwd_rows_*): DFT over nh + twiddle -> scratch G (tile layout), step B (k_fwd_cols): DFT over nl
 //   every 256-point DFT is 16 x 16: a half-warp owns one DFT, each lane 16 points in registers.
 //
-// "Tile layout" of a stored spectrum (bank, segments): for tile b (columns k1 = 16 b + c), kept row-block i
-// (rows k2 = g + 16 i, i in [I0, I0 + NI)), thread t = 16 c + g of a pass-1 team, element index
-// ((b*NI/2 + (i - I0)/2)*256 + t)*2 + ((i - I0) & 1): a thread's two row-blocks of a pair are one 16-byte word, a
-// team reads 4 KiB per 128-bit load, conflict free.  The forward scratch G keeps the plain order
-// ((b*16 + i)*16 + c)*16 + g over all 16 row-blocks.
+// "Tile layout" of a stored spectrum (bank, segments): see tile_word() in cplx.cuh -- per tile b (columns k1 = 16 b + c)
+// only the kept row-blocks i in [I0, I0 + NI) (rows k2 = g + 16 i), two row-blocks per 16-byte word, the words of one
+// warp of a pass-1 team contiguous (NI * 256 bytes: one bulk copy per warp and item).  The forward scratch G keeps the
+// plain order ((b*16 + i)*16 + c)*16 + g over all 16 row-blocks.
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -24,6 +23,7 @@
 #include <string>
 #include <vector>
 
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include "../../include/bege.h"
@@ -43,7 +43,11 @@ namespace bege {
 constexpr int kN = 65536;
 constexpr int kBatch = 72;                 // segments per launch of the forward transforms (fp32 staging: 38 MB)
 constexpr int kMaxGroups = 32;             // search: persistent CTA groups of 16 tiles (9 on a 148-SM B200)
-constexpr uint64_t kMiscHdr = 4096;        // counter @0, abort flag @8, hits @16, done1 @256, done2 @2048 (per group and ring slot)
+// counter block of a search, each hot word on its own 128-byte line (the record counter takes an atomic per warp with
+// tails; a poll of the abort flag on the same line would queue behind them): record counter, abort flag, hit counters,
+// done1 / done2 (per group and ring slot: kMaxGroups x kRing x 8 bytes each)
+constexpr uint64_t kOffCounter = 0, kOffAbort = 128, kOffHits = 256, kOffDone1 = 1024, kOffDone2 = 8192, kMiscHdr = 16384;
+static_assert(kOffDone1 + (uint64_t)kMaxGroups * 16 * 8 <= kOffDone2 && kOffDone2 + (uint64_t)kMaxGroups * 16 * 8 <= kMiscHdr, "counter block");
 constexpr int kMaxSlices = 8;              // launches per search whose record copies overlap the next launch
 constexpr uint64_t kSliceMinCorr = 32768;  // do not slice below this many correlations per slice
 
@@ -129,7 +133,7 @@ k_fwd_cols(const c2* __restrict__ G, c2* __restrict__ out, uint64_t out_stride, 
     for (int i = 0; i < 16; ++i) v[i] = in[(i * 16 + c) * 16 + g];
     hw_fft256<-1>(v, w1, sm[c], g);
     // lane p = g holds k2 = p + 16 q; row-blocks are stored in pairs (one 16-byte word per thread and pair)
-    ulonglong2* o = reinterpret_cast<ulonglong2*>(out + jl * out_stride + (uint64_t)b * NI * 256) + t;
+    ulonglong2* o = reinterpret_cast<ulonglong2*>(out + jl * out_stride) + tile_word(NI, b, 0, t);   // + 32 ip
     const uint32_t k1 = 16 * b + c;
 #pragma unroll
     for (int q = 0; q < 16; ++q) {
@@ -146,7 +150,7 @@ k_fwd_cols(const c2* __restrict__ G, c2* __restrict__ out, uint64_t out_stride, 
             // (I0, NI) is (1, 14) or (0, 16): both spelled out so that v is indexed with compile-time constants
             if (I0 == 1) { w.x = v[(2 * ip + 1) & 15]; w.y = v[(2 * ip + 2) & 15]; }
             else         { w.x = v[2 * ip]; w.y = v[(2 * ip + 1) & 15]; }
-            o[ip * 256] = w;
+            o[ip * 32] = w;
         }
     }
 }
@@ -158,32 +162,41 @@ k_fwd_cols(const c2* __restrict__ G, c2* __restrict__ out, uint64_t out_stride, 
 // pair (template grp + G (it / nS), segment it % nS).  CTA (b, grp) owns columns k1 = 16 b + c in pass 1 and rows
 // n2 = 16 b + r in pass 2.  Four teams of 8 warps, two per pass, team k of a pass taking the items it = k (mod 2).
 //
-//   A teams (pass 1): R = conj(H) X needs one column tile of the template spectrum and one of the segment spectrum.
-//              One of them is STATIONARY -- it sits in tensor memory, 14 complex numbers per thread -- and the other
-//              STREAMS through a per-team shared-memory buffer by bulk async copy (mbarrier-tracked, refilled as soon
-//              as the team has read it):
+//   A teams (pass 1): every WARP is autonomous -- it owns two columns of the tile (half-warp = column c, lane g holds
+//              rows k2 = g + 16 i), and nothing in its item needs another warp: no CTA or team barrier in the loop
+//              (the team barriers of the earlier version cost pass 1 a quarter of its time, profiles/r2a_*).
+//              R = conj(H) X needs one column tile of the template spectrum and one of the segment spectrum.  One of
+//              them is STATIONARY -- it sits in tensor memory, 14 complex numbers per thread -- and the other STREAMS
+//              through a per-warp shared-memory buffer: the warp's words of a tile are contiguous (tile_word), ONE
+//              bulk async copy per warp and item, tracked by the warp's own mbarrier, issued as soon as the warp has
+//              read the previous one:
 //                single-segment calls (nS = 1): X stationary (loaded once per launch), H streams from HBM;
 //                batched calls (nS >= 2):       H stationary (one load per template, it serves all nS segments --
 //                                               PAPER.md:156 "loaded once per M inverse FFTs"), X streams from L2.
-//              Stage 1: half-warp c, lane g holds rows k2 = g + 16 i of column c: 128-bit loads of the streaming
-//              tile, conj(H) X, Parseval partial sum, 16-point DFTs, twiddles theta^p (tensor memory).  One exchange
-//              through shared memory (two named barriers of the team per item).  Stage 2: lane c, p = warp-pair
-//              index: 16-point DFTs, and T[n2 = p + 16 q][16 b + c] goes straight from registers to the ring in L2
-//              (128 B per half-warp and store).
-//   B teams (pass 2): the 16 rows of T this CTA owns are 32 KiB contiguous in the ring: ONE bulk copy brings them
-//              into a shared-memory tile (3 tiles rotate over the items of both teams, so the next item's copy runs
-//              while this one is computed).  Half-warp r reads its row, applies the four-step factor, runs the
-//              256-point row DFT over k1 with the tile itself as its private exchange area (xor swizzle), thresholds
-//              against k^2 sum|R|^2 and compacts the tails with warp-aggregated atomics.  No warp of pass 2 issues a
-//              global load, so none queues behind the store bursts of pass 1 in the LSU.
+//              Stage 1: 128-bit loads of the streaming tile, conj(H) X, Parseval partial sum, 16-point DFTs, twiddles
+//              theta^p (tensor memory).  The 256-point column DFT is finished inside the half-warp: one exchange
+//              through a private padded shared-memory region (__syncwarp only), 16-point DFTs, and lane p holds
+//              T[n2 = p + 16 q][k1] in v[q].  The ring keeps an item as T'[k1][n2] (column-major): the 16 lanes of a
+//              half-warp store 128 contiguous bytes per q, a warp fills 4 KiB contiguous per item.
+//   B teams (pass 2): the 16 rows n2 of T this CTA owns are a 256 x 16 box of T' (256 lines of 128 bytes): ONE tensor
+//              copy (TMA, 128-byte swizzle) brings it into a 32 KiB shared-memory tile (3 tiles rotate over the items
+//              of both teams, so the next item's copy runs while this one is computed).  The 16 lanes that own row r
+//              read its 256 values (conflict free thanks to the swizzle and to the lane map below), apply the four-step
+//              factor, run the 256-point row DFT over k1 with their own 256 slots of the tile as the exchange area,
+//              threshold against k^2 sum|R|^2 and compact the tails with warp-aggregated atomics.  No warp of pass 2
+//              issues a global load of ring data, so none queues behind the store bursts of pass 1 in the LSU.
+//              Lane map of a B warp w: row r = 2 w + ((lane >> 3) & 1), a = (lane & 7) | ((lane >> 4) << 3), so that
+//              each hardware half-warp covers 8 values of a x 2 rows = 16 distinct 8-byte bank pairs.
 //
 // Tensor memory holds the loop-invariant per-thread tables (read with tcgen05.ld: no L1/LSU wavefronts -- the LSU
 // data pipe was the binding unit of the round-1 kernel at 75 %, see profiles/):
 //   columns [0, 32):    pass 2: delta_p = exp(2 pi i a (b + 16 p) / 4096), p < 16 -- the lane-dependent part of the
 //                       four-step factor wN^(16 b k1), k1 = a + 16 r, times the inner twiddle w256^(a p); 4 quadrants
-//   columns [32, 96):   pass 1: the stationary tile, 28 columns per thread, 32 per warp of a lane quadrant
+//   columns [32, 96):   pass 1, team 0: the stationary tile, 28 columns per thread, 32 per warp of a lane quadrant
 //   columns [96, 160):  pass 1: theta^p = exp(2 pi i p (256 g + k1) / N), p = 1 .. 15, same arrangement
 //   columns [160, 192): pass 1, dual-stream search only: Re(X[k] X[N-k]) of the segment, 14 columns per thread
+//   columns [192, 256): pass 1, team 1: its copy of the stationary tile (batched calls: the teams change template
+//                       at different times)
 // The CTA-uniform part of the four-step factor, w256^(b r), comes from constant memory (uniform loads).  All table
 // entries are rounded once from fp64 angles.
 //
@@ -192,26 +205,34 @@ k_fwd_cols(const c2* __restrict__ G, c2* __restrict__ out, uint64_t out_stride, 
 //              Thread 0 of the B team of the same item parity -- the team's service thread, which idles in a wait
 //              loop whenever pass 2 is ahead -- sees the phase complete, executes ONE fence.acq_rel.gpu and adds 1 to
 //              done1[slot] (the gpu-scope fence takes about a microsecond while the SM has stores in flight; on a
-//              pass-1 warp it would make that warp the laggard of the team's barriers).
+//              pass-1 warp it would stall that warp's item).
 //              The same thread waits with ld.acquire.gpu until all 16 tiles of its team's item have been added, then
-//              issues the bulk copy of the rows.
-//   done2 (ring slot read out): as soon as that copy has landed (mbarrier), the service thread adds 1 to done2[slot]
-//              under the same kind of fence.  ONE thread of the A team acquires 16 of them, early in the item, before
-//              the barrier that precedes the team's ring stores.
+//              issues the tensor copy of the rows.
+//   done2 (ring slot read out): as soon as that copy has landed (mbarrier), a thread of the B team adds 1 to
+//              done2[slot] under the same kind of fence.  Lane 0 of every A warp acquires 16 of them (load issued at
+//              the top of the item, looked at just before the warp's ring stores, __syncwarp in between).
 // The ring holds kRing items per group (G x kRing x 512 KiB) and lives in L2.
 #ifndef BEGE_RING
 #define BEGE_RING 16
 #endif
 constexpr int kRing = BEGE_RING;
 constexpr int kSearchThreads = 32 * 32;
+#ifndef BEGE_FWD
+#define BEGE_FWD 0
+#endif
+#ifndef BEGE_BGO
+#define BEGE_BGO 1
+#endif
 #ifndef BEGE_STATS
 #define BEGE_STATS 0       // 1: one CTA prints wait statistics of its service threads at the end (experiments only)
 #endif
 constexpr int kTmemCols = 256;
-constexpr uint32_t kTmDelta = 0, kTmStat = 32, kTmTheta = 96, kTmQ = 160;   // kTmQ: 16 columns per warp of a quadrant
+constexpr uint32_t kTmDelta = 0, kTmStat = 32, kTmTheta = 96, kTmQ = 160, kTmStat1 = 192;   // kTmQ: 16 columns per warp of a quadrant
 __constant__ float2 c_w256[256];           // exp(2 pi i m / 256), rounded from fp64 (host, bege_plan_create)
+constexpr int kSigPart = 128;              // Parseval partial sums per pair: 16 tiles x 8 warps (dual-stream search: two sets)
 
 struct SearchArgs {
+    CUtensorMap ring_map;                  // T' of all groups and ring slots as a 2-D fp32 tensor: (512, G * kRing * 256)
     const c2* bank; const c2* xseg; const float* qseg; c2* ring; float* sigpart; bege_tail* rec; c2* zdbg;
     unsigned long long cap; unsigned long long* counter; unsigned long long* done1; unsigned long long* done2;
     int* abort_flag;
@@ -220,28 +241,30 @@ struct SearchArgs {
     float k2, k2hi;
 };
 
-// shared-memory map of k_search (byte offsets from the 128-byte aligned base)
+// shared-memory map of k_search (byte offsets from the 2048-byte aligned base)
 template <int NI> struct SearchSmem {
     static constexpr uint32_t kTile = NI * 256 * 8;              // one column tile of a spectrum
-    static constexpr uint32_t kXch = 16 * 16 * 17 * 8;           // padded pass-1 exchange buffer, [p][g][c]
+    static constexpr uint32_t kWarpTile = kTile / 8;             // ... the words of one warp
+    static constexpr uint32_t kXch = 16 * 17 * 8;                // padded private exchange region of a half-warp, [g][17]
     static constexpr int kNB = NI <= 14 ? 3 : 2;                 // 32 KiB row tiles of pass 2
-    static constexpr uint32_t stream = 0;                        // [2]   streaming tile of each A team
-    static constexpr uint32_t xch = stream + 2 * kTile;          // [2]   exchange buffer of each A team
-    static constexpr uint32_t btile = xch + 2 * kXch;            // [kNB] row tiles of pass 2
-    static constexpr uint32_t ssig = btile + kNB * 32768;        // [2][2][8] Parseval partial sums of the A warps (sum|R|^2, dual: P)
-    static constexpr uint32_t bars = ssig + 128;                 // mbarriers: stream[2]; TMEM base address @ +24
-    static constexpr uint32_t amb = bars + 32;                   // [kRing] mbarriers: tile of ring slot stored (8 A warps)
+    static constexpr uint32_t btile = 0;                         // [kNB] row tiles of pass 2 (swizzled: 1024-byte aligned)
+    static constexpr uint32_t stream = btile + kNB * 32768;      // [2][8] streaming tile part of each A warp
+    static constexpr uint32_t xch = stream + 2 * kTile;          // [2][16] exchange region of each A half-warp
+    static constexpr uint32_t abar = xch + 32 * kXch;            // [16] mbarriers: streaming tile part of an A warp has arrived
+    static constexpr uint32_t amb = abar + 128;                  // [kRing] mbarriers: tile of ring slot stored (8 A warps)
     static constexpr uint32_t bfull = amb + 8 * kRing;           // [kNB] mbarriers: row tile has arrived
     static constexpr uint32_t bempty = bfull + 24;               // [kNB] u32 counters (8-byte pitch): warps that have read a tile out
-    static constexpr uint32_t bgo = bempty + 24;                 // [2][4] mbarriers: row tile of the B team's item is there (thread 0)
-    static constexpr uint32_t pubit = bgo + 64;                  // [2] u32: next item of A team k to publish (claimed by atomicCAS)
-    static constexpr uint32_t total = pubit + 8;
-    static_assert(total + 128 <= 232448, "shared memory of one SM");
+    static constexpr uint32_t bgo = bempty + 24;                 // [2][4] mbarriers (experiment BEGE_BGO)
+    static constexpr uint32_t pubit = bgo + 64;                 // [2] u32: next item of A team k to publish (claimed by atomicCAS)
+    static constexpr uint32_t freed = pubit + 8;                 // [2] u32: items of A team k whose ring slots all 16 CTAs have read out
+    static constexpr uint32_t tmem = freed + 8;                  // TMEM base address
+    static constexpr uint32_t total = tmem + 8;
+    static_assert(total + 2048 <= 232448, "shared memory of one SM");
 };
 // the stationary tile has its tensor-memory arrangement written out for bands that need 14 of the 16 row-blocks;
 // other bands read it from global memory (L2) -- correct, not tuned
 template <int NI> __host__ __device__ constexpr bool search_stat() { return NI == 14; }
-template <int NI> constexpr int search_smem() { return (int)SearchSmem<NI>::total + 128; }
+template <int NI> constexpr int search_smem() { return (int)SearchSmem<NI>::total + 2048; }
 
 // 16 values to shared memory at a + p * STRIDE bytes
 template <int STRIDE, int P = 0> BEGE_D void sts16(uint32_t a, const c2 (&v)[16])
@@ -257,7 +280,7 @@ template <int STRIDE, int P = 0> BEGE_D void lds16(uint32_t a, c2 (&v)[16])
 template <int I0, bool SINGLE, int IP> BEGE_D void products1(uint32_t stream_a, c2 q0, c2 q1, c2 (&v)[16], c2& acc)
 {
     c2 s0, s1;
-    lds128<IP * 4096>(stream_a, s0, s1);
+    lds128<IP * 512>(stream_a, s0, s1);
     const c2 r0 = SINGLE ? cmulc(q0, s0) : cmulc(s0, q0);
     const c2 r1 = SINGLE ? cmulc(q1, s1) : cmulc(s1, q1);
     v[I0 + 2 * IP] = r0; v[(I0 + 2 * IP + 1) & 15] = r1;
@@ -289,7 +312,7 @@ template <int I0, int IP = 0> BEGE_D void tm_products_dual(uint32_t stream_a, ui
         tmem_wait_ld(cur, rcur);
         if constexpr (IP + 1 < 7) { tmem_ld4(tx + 4 * (IP + 1), nxt); tmem_ld2f(tqr + 2 * (IP + 1), rnxt); }
         c2 s0, s1;
-        lds128<IP * 4096>(stream_a, s0, s1);
+        lds128<IP * 512>(stream_a, s0, s1);
         const c2 r0 = cmulc(cur[0], s0), r1 = cmulc(cur[1], s1);
         v[I0 + 2 * IP] = r0; v[(I0 + 2 * IP + 1) & 15] = r1;
         acc = fma2(r0, r0, acc); acc = fma2(r1, r1, acc);
@@ -302,7 +325,7 @@ template <int I0, int IP = 0> BEGE_D void tm_products_dual(uint32_t stream_a, ui
 template <int I0, int NI, bool SINGLE, int IP = 0> BEGE_D void gl_products(uint32_t stream_a, const ulonglong2* __restrict__ statg, c2 (&v)[16], c2& acc)
 {
     if constexpr (IP < NI / 2) {
-        const ulonglong2 q = __ldg(statg + IP * 256);
+        const ulonglong2 q = __ldg(statg + IP * 32);
         products1<I0, SINGLE, IP>(stream_a, q.x, q.y, v, acc);
         gl_products<I0, NI, SINGLE, IP + 1>(stream_a, statg, v, acc);
     }
@@ -336,12 +359,13 @@ k_search(const __grid_constant__ SearchArgs A)
     static_assert(!DUAL || (SINGLE && STAT && !DBG), "dual-stream search: single-segment calls on 14 row-blocks");
     using SM = SearchSmem<NI>;
     static_assert(NI % 2 == 0, "row-blocks are stored in pairs");
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    const uint32_t sb = smem_u32(smem_raw);
+    extern __shared__ __align__(1024) unsigned char smem_dyn[];
+    // the row tiles of pass 2 are addressed with xor arithmetic on bits 4 .. 10: 2048-byte aligned base
+    const uint32_t sb = (smem_u32(smem_dyn) + 2047u) & ~2047u;
+    unsigned char* const smem_raw = smem_dyn + (sb - smem_u32(smem_dyn));
     const int team = threadIdx.x >> 8;                       // 0, 1: A teams; 2, 3: B teams
     const int t = threadIdx.x & 255, warp = t >> 5, lane = t & 31;   // within the team
     const int b = blockIdx.x, grp = blockIdx.y, G = gridDim.y;
-    constexpr uint32_t kTileBytes = SM::kTile;
     constexpr uint64_t kTile = (uint64_t)NI * 256;           // elements
     int* const abort_flag = A.abort_flag;
 
@@ -356,7 +380,7 @@ k_search(const __grid_constant__ SearchArgs A)
     auto seg_tile = [&](uint32_t ml) { return A.xseg + ((uint64_t)(A.m0 + ml) * 16 + b) * kTile; };
 
     if (threadIdx.x == 0) {
-        mbar_init(sb + SM::bars, 1); mbar_init(sb + SM::bars + 8, 1);
+        for (int i = 0; i < 16; ++i) mbar_init(sb + SM::abar + 8 * i, 1);
         for (int i = 0; i < kRing; ++i) mbar_init(sb + SM::amb + 8 * i, 8);
         for (int i = 0; i < SM::kNB; ++i) {
             mbar_init(sb + SM::bfull + 8 * i, 1);
@@ -365,29 +389,32 @@ k_search(const __grid_constant__ SearchArgs A)
         for (int i = 0; i < 8; ++i) mbar_init(sb + SM::bgo + 8 * i, 1);
         reinterpret_cast<volatile uint32_t*>(smem_raw + SM::pubit)[0] = 0;
         reinterpret_cast<volatile uint32_t*>(smem_raw + SM::pubit)[1] = 1;
+        reinterpret_cast<volatile uint32_t*>(smem_raw + SM::freed)[0] = 0;
+        reinterpret_cast<volatile uint32_t*>(smem_raw + SM::freed)[1] = 0;
         fence_mbar_init();
     }
-    if (threadIdx.x < 32) tmem_alloc<kTmemCols>(sb + SM::bars + 24);
+    if (threadIdx.x < 32) tmem_alloc<kTmemCols>(sb + SM::tmem);
     tmem_fence_before_sync();
     __syncthreads();
     tmem_fence_after_sync();
     // this warp's lane quadrant of the tensor memory (lane field = bits 16 and up)
-    const uint32_t tq = *reinterpret_cast<volatile uint32_t*>(smem_raw + SM::bars + 24) + ((uint32_t)(warp & 3) << 21);
+    const uint32_t tq = *reinterpret_cast<volatile uint32_t*>(smem_raw + SM::tmem) + ((uint32_t)(warp & 3) << 21);
     const uint32_t tq_a = tq + 32u * (uint32_t)(warp >> 2);  // pass 1: column block of this warp inside a table
-    // the stationary tile of pass 1 goes from global memory to this thread's TMEM columns (team 0 does it for both)
+    const uint32_t tq_s = tq_a + (team == 1 ? kTmStat1 : kTmStat);   // pass 1: this team's stationary tile
+    // the stationary tile of pass 1 goes from global memory to this thread's TMEM columns (every A warp its own part)
     auto stat_to_tmem = [&](const c2* tile) {
-        const ulonglong2* src = reinterpret_cast<const ulonglong2*>(tile) + t;
+        const ulonglong2* src = reinterpret_cast<const ulonglong2*>(tile) + tile_word(NI, 0, 0, t);
 #pragma unroll
         for (int ip = 0; ip < NI / 2; ++ip) {
-            const ulonglong2 q = __ldcg(src + ip * 256);
+            const ulonglong2 q = __ldcg(src + ip * 32);
             const uint32_t r[4] = {(uint32_t)q.x, (uint32_t)(q.x >> 32), (uint32_t)q.y, (uint32_t)(q.y >> 32)};
-            tmem_st4(tq_a + kTmStat + 4 * ip, r);
+            tmem_st4(tq_s + 4 * ip, r);
         }
         tmem_wait_st();
     };
     if (team == 0) {
-        if (warp < 4) {                                      // delta_p, one copy per lane quadrant
-            const int a = lane & 15;
+        if (warp < 4) {                                      // delta_p, one copy per lane quadrant, B lane map
+            const int a = (lane & 7) | ((lane >> 4) << 3);
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 uint32_t r[8];
@@ -415,138 +442,141 @@ k_search(const __grid_constant__ SearchArgs A)
                 tmem_st8(tq_a + kTmTheta + 8 * j, r);
             }
         }
-        if (STAT && n_items > 0) stat_to_tmem(SINGLE ? seg_tile(0) : tpl_tile(0));
         if (DUAL && n_items > 0) {                           // Re(X[k] X[N-k]) of this thread's 14 bins
-            const float2* src = reinterpret_cast<const float2*>(A.qseg + ((uint64_t)A.m0 * 16 + b) * (uint64_t)(NI * 256)) + t;
+            const float2* src = reinterpret_cast<const float2*>(A.qseg + ((uint64_t)A.m0 * 16 + b) * (uint64_t)(NI * 256)) + tile_word(NI, 0, 0, t);
 #pragma unroll
             for (int ip = 0; ip < NI / 2; ++ip) {
-                const float2 q = __ldcg(src + ip * 256);
+                const float2 q = __ldcg(src + ip * 32);
                 tmem_st2(tq + kTmQ + 16u * (uint32_t)(warp >> 2) + 2 * ip, __float_as_uint(q.x), __float_as_uint(q.y));
             }
         }
         tmem_wait_st();
     }
+    if (team < 2 && STAT && SINGLE && n_items > 0) stat_to_tmem(seg_tile(0));
     tmem_fence_before_sync();
     __syncthreads();
     tmem_fence_after_sync();
 
     if (team < 2 && !(BEGE_ABL & 16)) {
         // ================================================================ A: pass 1, items it = team (mod 2)
-        const int c = t >> 4, g = t & 15;                    // stage 1: column of the tile, lane of its half-warp
-        const int c2i = t & 15, p2 = t >> 4;                 // stage 2: column, index p of n2 = p + 16 q
-        const uint32_t bar_stream = sb + SM::bars + 8 * team;
-        const uint32_t stream_buf = sb + SM::stream + team * kTileBytes;
-        const uint32_t stream_a = stream_buf + t * 16;
-        const uint32_t xw_a = sb + SM::xch + team * SM::kXch + (g * 17 + c) * 8;       // + p * 2176: element [p][g][c]
-        const uint32_t xr_a = sb + SM::xch + team * SM::kXch + (p2 * 272 + c2i) * 8;   // + gg * 136
-        const uint32_t ssig_a = sb + SM::ssig + team * 32;     // + 64: the dual-stream search's second sum
-        const int bar_id = 1 + team;
-        auto stream_src = [&](uint32_t it) { return SINGLE ? tpl_tile(it) : seg_tile(it % nS); };
+        const int c = t >> 4, g = t & 15;                    // column of the tile, lane of its half-warp (stage 2: g = p)
+        const int aw = team * 8 + warp;                      // A warp of the CTA
+        const uint32_t bar_w = sb + SM::abar + 8 * aw;
+        const uint32_t wbuf = sb + SM::stream + aw * SM::kWarpTile;
+        const uint32_t stream_a = wbuf + lane * 16;
+        const uint32_t xa = sb + SM::xch + (uint32_t)(aw * 2 + (lane >> 4)) * SM::kXch;
+        const uint32_t xw_a = xa + g * 136;                  // + 8 p:    element (g, p) of the half-warp's region
+        const uint32_t xr_a = xa + g * 8;                    // + 136 gg: element (gg, p = g)
+        const uint32_t freed_a = sb + SM::freed + 4 * team;
+        constexpr uint32_t kWarpElems = SM::kWarpTile / 8;
+        // streaming tile part of this warp: template `it` (single-segment calls) / segment ml (batched calls)
+        auto stream_src = [&](uint32_t it, uint32_t ml) { return (SINGLE ? tpl_tile(it) : seg_tile(ml)) + (uint32_t)warp * kWarpElems; };
         const ulonglong2* statg = nullptr;                   // !STAT: the stationary tile in global memory
         if (n_items > 0) {
-            if (!STAT) statg = reinterpret_cast<const ulonglong2*>(SINGLE ? seg_tile(0) : tpl_tile(0)) + t;
-            if (t == 0 && (uint32_t)team < n_items && !(BEGE_ABL & 2)) {
-                mbar_arrive_expect_tx(bar_stream, kTileBytes);
-                bulk_load(stream_buf, stream_src(team), kTileBytes, bar_stream, SINGLE ? policy_evict_first() : policy_evict_last());
+            if (!STAT && SINGLE) statg = reinterpret_cast<const ulonglong2*>(seg_tile(0)) + tile_word(NI, 0, 0, t);
+            if (lane == 0 && (uint32_t)team < n_items && !(BEGE_ABL & 2)) {
+                mbar_arrive_expect_tx(bar_w, SM::kWarpTile);
+                bulk_load(wbuf, stream_src(team, (uint32_t)team % nS), SM::kWarpTile, bar_w, SINGLE ? policy_evict_first() : policy_evict_last());
             }
         }
-        uint32_t nload = 0;                                  // tiles this team has waited for so far
-        uint32_t tj_prev = 0;
-        long long st_d2 = 0, st_tma = 0; unsigned st_nd2 = 0;
+        uint32_t nload = 0;                                  // tiles this warp has waited for so far
+        uint32_t tj_prev = ~0u;
+        // (template, segment) of the item, stepped without a division per item: batched calls have nS >= 2
+        uint32_t tj_c = SINGLE ? 0u : (uint32_t)team / nS, ml_c = SINGLE ? 0u : (uint32_t)team % nS;
         for (uint32_t it = team; it < n_items; it += 2) {
-            const uint32_t tj = SINGLE ? it : it / nS;
-            const uint32_t ml = SINGLE ? 0u : (uint32_t)(it - tj * nS);
+            const uint32_t tj = SINGLE ? it : tj_c;
+            const uint32_t ml = SINGLE ? 0u : ml_c;
+            uint32_t ml_next = ml + 2;                       // segment of the team's next item
+            if (!SINGLE && ml_next >= nS) { ml_next -= nS; ++tj_c; }
+            ml_c = ml_next;
             const int slot = (int)(it % kRing);
-            // slot-free counter (ring slot read out by pass 2 of item it - kRing, all 16 CTAs of the group): ONE thread
-            // acquires it, early, so that the L2 round trip is hidden behind stage 1
-            unsigned long long d2v = ~0ull;
-            if (!(BEGE_ABL & 1) && t == 32 && it >= (uint32_t)kRing) d2v = counter_load_acquire(d2 + slot);
+            if (!SINGLE && tj != tj_prev) {                  // batched calls: this warp's part of the next template
+                if (STAT) stat_to_tmem(tpl_tile(tj));
+                else statg = reinterpret_cast<const ulonglong2*>(tpl_tile(tj)) + tile_word(NI, 0, 0, t);
+                tj_prev = tj;
+            }
             c2 qa[2], qb[2];                                 // TMEM staging (stationary values, then theta powers)
             float ra[2], rb[2], pacc = 0.f;                  // dual-stream search: staging of Re(X[k] X[N-k]), P
-            if (STAT) tmem_ld4(tq_a + kTmStat, qa);
+            if (STAT) tmem_ld4(tq_s, qa);
             if (DUAL) tmem_ld2f(tq + kTmQ + 16u * (uint32_t)(warp >> 2), ra);
 #if !(BEGE_ABL & 2)
-            { const long long c0 = BEGE_STATS ? clock64() : 0; mbar_wait(bar_stream, nload & 1, abort_flag); if (BEGE_STATS) st_tma += clock64() - c0; }
+            mbar_wait(bar_w, nload & 1, abort_flag);
 #endif
             ++nload;
-            if (!SINGLE && !STAT && tj != tj_prev) statg = reinterpret_cast<const ulonglong2*>(tpl_tile(tj)) + t;
-            tj_prev = tj;
             c2 v[16];
             c2 acc = mk(0.f, 0.f);
 #pragma unroll
             for (int r = 0; r < 16; ++r) if (r < I0 || r >= I0 + NI) v[r] = mk(0.f, 0.f);
-            if constexpr (DUAL) tm_products_dual<I0>(stream_a, tq_a + kTmStat, tq + kTmQ + 16u * (uint32_t)(warp >> 2), v, acc, pacc, qa, qb, ra, rb);
-            else if constexpr (STAT) tm_products<I0, SINGLE>(stream_a, tq_a + kTmStat, v, acc, qa, qb);
+            if constexpr (DUAL) tm_products_dual<I0>(stream_a, tq_s, tq + kTmQ + 16u * (uint32_t)(warp >> 2), v, acc, pacc, qa, qb, ra, rb);
+            else if constexpr (STAT) tm_products<I0, SINGLE>(stream_a, tq_s, v, acc, qa, qb);
             else gl_products<I0, NI, SINGLE>(stream_a, statg, v, acc);
             tmem_ld4(tq_a + kTmTheta, qa);
-            fft16<+1>(v);
-            tm_twiddle<1, 8>(tq_a + kTmTheta, v, qa, qb);    // v[p] *= theta^p, p = 1 .. 15
-            sts16<2176>(xw_a, v);
-            const float sw = warp_sum32(re(acc) + im(acc));
-            if (lane == 0) sts32(ssig_a + 4 * warp, sw);
-            if (DUAL) { const float pw = warp_sum32(pacc); if (lane == 0) sts32(ssig_a + 64 + 4 * warp, pw); }
-            bar_named(bar_id, 256);                          // exchange buffer complete, both tiles read out
-            if (t == 0 && !(BEGE_ABL & 2)) {                 // order the streaming tile of this team's next item
+            __syncwarp();                                    // the warp has read its part of the streaming tile:
+            if (lane == 0 && !(BEGE_ABL & 2)) {              // order the part of this team's next item
                 const uint32_t it2 = it + 2;
                 if (it2 < n_items) {
-                    mbar_arrive_expect_tx(bar_stream, kTileBytes);
-                    bulk_load(stream_buf, stream_src(it2), kTileBytes, bar_stream,
-                              SINGLE ? policy_evict_first() : policy_evict_last());
+                    mbar_arrive_expect_tx(bar_w, SM::kWarpTile);
+                    bulk_load(wbuf, stream_src(it2, ml_next), SM::kWarpTile, bar_w, SINGLE ? policy_evict_first() : policy_evict_last());
                 }
             }
-            if (!SINGLE && STAT) {                           // last item of this template for this team: once both A
-                if (it + 2 >= (tj + 1) * nS && tj + 1 < nTg) {   // teams are past it, bring in the next template's tile
-                    bar_named(3, 512);
-                    if (team == 0) stat_to_tmem(tpl_tile(tj + 1));
-                    tmem_fence_before_sync();
-                    bar_named(3, 512);
-                    tmem_fence_after_sync();
-                }
-            }
-            lds16<136>(xr_a, v);
-            float tot = 0.f, ptot = 0.f;
-            if (t == 64) {
-#pragma unroll
-                for (int w = 0; w < 8; ++w) tot += lds32(ssig_a + 4 * w);
-                if (DUAL) {
-#pragma unroll
-                    for (int w = 0; w < 8; ++w) ptot += lds32(ssig_a + 64 + 4 * w);
-                }
-            }
-            if (t == 32 && d2v < 16ull * (it / kRing)) {
-                const long long c0 = BEGE_STATS ? clock64() : 0;
-                counter_wait_ge(d2 + slot, 16ull * (it / kRing), abort_flag);
-                if (BEGE_STATS) { st_d2 += clock64() - c0; ++st_nd2; }
-            }
-            __syncwarp();
-            bar_named(bar_id, 256);                          // exchange buffer free for the team's next item; slot free
             fft16<+1>(v);
-            // T[n2 = p + 16 q][16 b + c] for this thread's (c, p): a half-warp stores 128 contiguous bytes of row n2
-            c2* out = myring + (uint64_t)slot * kN + 16 * b + c2i + p2 * 256;
+            tm_twiddle<1, 8>(tq_a + kTmTheta, v, qa, qb);    // v[p] *= theta^p, p = 1 .. 15
+            sts16<8>(xw_a, v);
+            const float sw = warp_sum32(re(acc) + im(acc));  // (includes the __syncwarp the exchange needs)
+            const float pw = DUAL ? warp_sum32(pacc) : 0.f;
+            __syncwarp();
+            lds16<136>(xr_a, v);
+            if (lane == 0) {
+                const uint64_t pr = (A.j0 + grp + (uint64_t)G * tj) * (uint64_t)A.S + (A.m0 + ml) - A.sig_pair0;
+                float* sp = A.sigpart + pr * (DUAL ? 2 * kSigPart : kSigPart) + b * 8 + warp;
+                sp[0] = sw;
+                if (DUAL) sp[kSigPart] = pw;
+            }
+            // Ring slot free?  Item it - kRing = item (it >> 1) - kRing / 2 of this team must have been read out by all
+            // 16 CTAs of the group: the B team of the same parity watches the global counter done2 and forwards it as a
+            // CTA-local count (one global poller per team instead of eight warps on one L2 line; warp-uniform here).
+            if (!BEGE_FWD && !(BEGE_ABL & 1) && it >= (uint32_t)kRing) {
+                const unsigned long long need = 16ull * (it / kRing);
+                if (counter_load_acquire(d2 + slot) < need) counter_wait_ge(d2 + slot, need, abort_flag);
+            }
+            if (BEGE_FWD && !(BEGE_ABL & 1) && it >= (uint32_t)kRing) {
+                const uint32_t need = (it >> 1) - (uint32_t)(kRing / 2) + 1u;
+                if (smem_counter_load_acquire(freed_a) < need) {
+                    const long long t0 = clock64();
+                    while (smem_counter_load_acquire(freed_a) < need) {
+                        __nanosleep(200);
+                        if (*(volatile int*)abort_flag) break;
+                        if (clock64() - t0 > kSpinLimit) { *(volatile int*)abort_flag = 1; break; }
+                    }
+                }
+            }
+            __syncwarp();                                    // exchange region free for the next item; ring slot free
+            fft16<+1>(v);
+            // T'[k1 = 16 b + c][n2 = p + 16 q], p = g: a half-warp stores 128 contiguous bytes per q
+            c2* out = myring + (uint64_t)slot * kN + (uint32_t)(16 * b + c) * 256u + g;
 #pragma unroll
             for (int q = 0; q < 16; ++q) {
                 const c2 o = v[q];
-                if (!(BEGE_ABL & 4) || re(o) == 1.2345e-30f) out[q * 4096] = o;
-            }
-            if (t == 64) {
-                const uint64_t pr = (A.j0 + grp + (uint64_t)G * tj) * (uint64_t)A.S + (A.m0 + ml) - A.sig_pair0;
-                A.sigpart[pr * (DUAL ? 32 : 16) + b] = tot;
-                if (DUAL) A.sigpart[pr * 32 + 16 + b] = ptot;
+                if (!(BEGE_ABL & 4) || re(o) == 1.2345e-30f) out[q * 16] = o;
             }
             // this warp's part of the tile is on its way: tell the publisher (thread 0 of the B team of the same parity)
             __syncwarp();
             if (lane == 0) mbar_arrive(sb + SM::amb + 8 * slot);
         }
-        if (BEGE_STATS && b == 3 && grp == 1 && (t == 32 || t == 0))
-            printf("A team %d t %d: items %u, d2 waits %u, d2 wait cycles/item %lld, stream-tile wait cycles/item %lld\n", team, t, nload,
-                   st_nd2, st_d2 / (long long)max(nload, 1u), st_tma / (long long)max(nload, 1u));
     } else if (team >= 2 && !(BEGE_ABL & 32)) {
         // ================================================================ B: pass 2, items ib = team - 2 (mod 2)
         const int kb = team - 2;
-        const int hw = t >> 4, a = t & 15;                   // row of the row tile, lane of its half-warp
+        // lane map: 8 values of a x 2 rows per hardware half-warp (conflict-free 64-bit accesses of the swizzled tile)
+        const int a = (lane & 7) | ((lane >> 4) << 3);       // lane of the row's 256-point DFT
+        const int rbit = (lane >> 3) & 1;
+        const int hw = 2 * warp + rbit;                      // row of the row tile
         const int n2 = 16 * b + hw;
         constexpr uint32_t NB = SM::kNB;                     // item i uses tile buffer i % NB (both teams share the buffers)
-        // ---- service state.  Thread 0 polls done1 (acquire) and issues the bulk copies; the gpu-scope fences -- about a
+        // The tile is T'[k1][16 rows] as the tensor copy leaves it: line k1 at 128 k1, its 16-byte chunk j at position
+        // j ^ (k1 & 7) (128-byte swizzle).  Row hw owns slot (k1) = 128 k1 + 16 ((hw >> 1) ^ (k1 & 7)) + 8 (hw & 1) of
+        // every line; after the loads the same 256 slots are the row's private exchange area.
+        const uint32_t base_a = (uint32_t)a * 128u + ((uint32_t)(((hw >> 1) ^ a) & 7) << 4) + 8u * (uint32_t)(hw & 1);
+        // ---- service state.  Thread 0 polls done1 (acquire) and issues the tensor copies; the gpu-scope fences -- about a
         // microsecond each while the SM has stores in flight -- are kept off its warp, whose progress paces the team: the
         // warp (1 + item mod 7) of the team takes them at the top of each item (once per seven items and warp).  Thread 0
         // takes them only inside its wait loop, when pass 2 is ahead of pass 1 and the team idles anyway (somebody must
@@ -572,6 +602,20 @@ k_search(const __grid_constant__ SearchArgs A)
             for (uint32_t i = 0; i < n; ++i) counter_add_relaxed(d1 + (first + 2 * i) % kRing, 1ull);
             if (free_slot >= 0) counter_add_relaxed(d2 + free_slot, 1ull);
         };
+        // items kb, kb + 2, ... whose ring slots have been read out by ALL 16 CTAs of the group (done2, acquired) are
+        // counted in shared memory for A team kb.  Called by one thread of the team at a time (the duty lane after the
+        // team barrier of an item, thread 0 inside its wait loop before it).
+        const uint32_t freed_b = sb + SM::freed + 4 * kb;
+        auto advance_freed = [&]() {
+            const uint32_t c0 = *reinterpret_cast<volatile uint32_t*>(smem_raw + SM::freed + 4 * kb);
+            uint32_t c = c0;
+            while (c < c0 + 2) {
+                const uint32_t itc = kb + 2 * c;
+                if (itc >= n_items || counter_load_acquire(d2 + itc % kRing) < 16ull * (itc / kRing + 1)) break;
+                ++c;
+            }
+            if (c != c0) smem_counter_add_release(freed_b, c - c0);
+        };
         // copy of item `it` of this team into its tile buffer, if the buffer has been read out (item it - NB, either
         // team) and all 16 tiles of the item are in the ring (d1, acquired: `ready`); non-blocking.  "Read out" is a
         // monotone count of warps (8 per use), not an mbarrier: this thread may look at a buffer whose use before last
@@ -581,28 +625,30 @@ k_search(const __grid_constant__ SearchArgs A)
             if (us > 0 && smem_counter_load_acquire(sb + SM::bempty + 8 * bf) < 8 * us) return;
             if (!ready) return;
             if (!(BEGE_ABL & 8)) {
-                fence_proxy_async_smem();
+                fence_proxy_async_all();                     // the tile's generic reads and the acquired ring stores first
                 mbar_arrive_expect_tx(sb + SM::bfull + 8 * bf, 32768);
-                bulk_load(sb + SM::btile + bf * 32768, myring + (uint64_t)(it % kRing) * kN + 4096 * b, 32768,
-                          sb + SM::bfull + 8 * bf, policy_evict_first());
+                // box (32 floats = this CTA's 16 rows, 256 lines k1) of item (grp, slot)
+                tma_load_2d(sb + SM::btile + bf * 32768, &A.ring_map, 32 * b, (int)(((uint32_t)grp * kRing + it % kRing) * 256u),
+                            sb + SM::bfull + 8 * bf, policy_evict_first());
             }
             ld_it = it + 2;
         };
+        uint32_t tj_c = SINGLE ? 0u : (uint32_t)kb / nS, ml_c = SINGLE ? 0u : (uint32_t)kb % nS;
         for (uint32_t ib = kb; ib < n_items; ib += 2) {
             const int slot = (int)(ib % kRing);
-            const uint32_t tj = SINGLE ? ib : ib / nS;
-            const uint32_t ml = SINGLE ? 0u : (uint32_t)(ib - tj * nS);
+            const uint32_t tj = SINGLE ? ib : tj_c;
+            const uint32_t ml = SINGLE ? 0u : ml_c;
+            if (!SINGLE) { ml_c += 2; if (ml_c >= nS) { ml_c -= nS; ++tj_c; } }
             const uint64_t jl = grp + (uint64_t)G * tj;
             const uint32_t buf = ib % NB, use = ib / NB;
-            // half-warp hw owns row hw of the tile (2 KiB) and, once the row is in registers, uses the same 2 KiB as its
-            // private exchange area: element (a, p) at a * 128 + ((a ^ p) << 3), conflict free both ways
-            const uint32_t row = sb + SM::btile + buf * 32768 + hw * 2048;
-            const uint32_t in_a = row + a * 8;               // + 128 r:                     T[n2][k1 = a + 16 r]
-            const uint32_t xw0 = row + a * 136;              // (xw0 ^ (p << 3)):            element (a, p)
-            const uint32_t xr0 = row + a * 8;                // (xr0 ^ (aa << 3)) + 128 aa:  element (aa, p = a)
+            const uint32_t w0 = sb + SM::btile + buf * 32768 + base_a;   // + 2048 i: T[n2][k1 = a + 16 i]
+            //   (w0 ^ cx(p)) + 2048 p:  exchange slot of element (a, p), slot index 16 p + (a ^ p)
+            //   (w0 + 2048 a) ^ cx(aa): element (aa, p = a), with cx(j) = 128 j + 16 (j & 7)
+            const uint32_t r0 = w0 + 2048u * (uint32_t)a;
             if (t == 0) {
                 const unsigned long long target = 16ull * (ib / kRing + 1);
                 const long long t0 = clock64();
+                uint32_t spin = 0;
                 if (BEGE_STATS) { if (ld_it == ib) ++st_ntop; else ++st_nmid; }
                 for (;;) {
                     if (BEGE_STATS) ++st_spin;
@@ -615,46 +661,54 @@ k_search(const __grid_constant__ SearchArgs A)
                     if (clock64() - t0 > kSpinLimit) {
                         *(volatile int*)abort_flag = 1; break;
                     }
+                    if (BEGE_FWD && !(BEGE_ABL & 1) && (++spin & 7u) == 0u) advance_freed();   // A may be waiting for exactly this
                     __nanosleep(40);
                 }
-                // The other seven warps wait on a per-team barrier, not on the tile's own: the tile buffers are shared
-                // by both teams, and a warp that runs ahead could otherwise mistake an older phase of the same parity.
-                // Four barriers rotate over the team's items: this thread is never more than NB = 3 items ahead of the
-                // team's slowest warp (a buffer is refilled only after all eight warps have read it out), so a waiter
-                // and this thread never meet on a barrier in different uses.
+                // The other seven warps wait for this thread at the team's named barrier below: blocked in hardware, they
+                // take no issue slots from the working warps (a try_wait loop on the tile's mbarrier cost more
+                // instructions per item than the item's arithmetic, profiles/r2b_*).
                 if (BEGE_STATS) st_top += clock64() - t0;
-                mbar_arrive(sb + SM::bgo + 32 * kb + 8 * (nit & 3));
+                if (BEGE_BGO) mbar_arrive(sb + SM::bgo + 32 * kb + 8 * (nit & 3));
                 // look at the counter of the team's next item now; the answer is used after the exchange
                 if (!(BEGE_ABL & 1) && ib + 2 < n_items && ld_it == ib + 2) { d1v = counter_load_acquire(d1 + (ib + 2) % kRing); d1v_it = ib + 2; }
             }
             __syncwarp();
-            mbar_wait(sb + SM::bgo + 32 * kb + 8 * (nit & 3), (nit >> 2) & 1, abort_flag);
+            if (BEGE_BGO) mbar_wait_lean(sb + SM::bgo + 32 * kb + 8 * (nit & 3), (nit >> 2) & 1, abort_flag);
+            else bar_named(1 + kb, 256);                     // the other seven warps block here in hardware (no spinning)
             // the rows are in shared memory: the ring slot is free.  This item's fence duty: warp 1 + (nit mod 7)
             if (warp == 1 + (int)(nit % 7) && lane == 0) publish(slot);
+            if (BEGE_FWD && !(BEGE_ABL & 1) && warp == 1 + (int)((nit + 3) % 7) && lane == 0) advance_freed();
             ++nit;
             c2 v[16];
-            lds16<128>(in_a, v);
+            lds16<2048>(w0, v);
             const uint64_t pair = (A.j0 + jl) * (uint64_t)A.S + (A.m0 + ml);
-            const float part = __ldcg(A.sigpart + (pair - A.sig_pair0) * (DUAL ? 32 : 16) + a);
-            const float ppart = DUAL ? __ldcg(A.sigpart + (pair - A.sig_pair0) * 32 + 16 + a) : 0.f;
+            // Parseval partial sums of tile a: 8 warps, fixed order
+            const float4* sp = reinterpret_cast<const float4*>(A.sigpart + (pair - A.sig_pair0) * (DUAL ? 2 * kSigPart : kSigPart) + 8 * a);
+            const float4 s0 = __ldcg(sp), s1 = __ldcg(sp + 1);
+            const float part = ((s0.x + s0.y) + (s0.z + s0.w)) + ((s1.x + s1.y) + (s1.z + s1.w));
+            float ppart = 0.f;
+            if (DUAL) {
+                const float4 p0 = __ldcg(sp + kSigPart / 4), p1 = __ldcg(sp + kSigPart / 4 + 1);
+                ppart = ((p0.x + p0.y) + (p0.z + p0.w)) + ((p1.x + p1.y) + (p1.z + p1.w));
+            }
             c2 wa[2], wb[2];
             tmem_ld4(tq + kTmDelta, wa);
             // four-step factor wN^(16 b k1), k1 = a + 16 r: its CTA-uniform part w256^(b r) here, the rest in delta_p
 #pragma unroll
             for (int r = 1; r < 16; ++r) { const float2 w = c_w256[(b * r) & 255]; v[r] = cmulw(v[r], w.x, w.y); }
-            const float sumR2 = hw_sum16(part);
-            const float sumP = DUAL ? hw_sum16(ppart) : 0.f;
+            const float sumR2 = row_sum16(part);
+            const float sumP = DUAL ? row_sum16(ppart) : 0.f;
             fft16<+1>(v);
             if (t == 0 && ib + 2 < n_items && ld_it == ib + 2)   // first chance to bring in the team's next item
                 try_load(ib + 2, (BEGE_ABL & 1) || (d1v_it == ib + 2 && d1v >= 16ull * ((ib + 2) / kRing + 1)));
             tm_twiddle<0, 8>(tq + kTmDelta, v, wa, wb);      // v[p] *= delta_p = wN^(16 b a) w256^(a p)
-            __syncwarp();                                    // every lane of the half-warp has its row in registers
+            __syncwarp();                                    // every lane of the row has its values in registers
 #pragma unroll
-            for (int p = 0; p < 16; ++p) sts64<0>(xw0 ^ (uint32_t)(p << 3), v[p]);
+            for (int p = 0; p < 16; ++p) sts64<0>((w0 ^ (uint32_t)(128 * p + 16 * (p & 7))) + 2048u * p, v[p]);
             __syncwarp();
 #pragma unroll
-            for (int aa = 0; aa < 16; ++aa) v[aa] = lds64<0>((xr0 ^ (uint32_t)(aa << 3)) + 128 * aa);
-            fence_proxy_async_smem();                        // these generic accesses before the next bulk copy into the tile
+            for (int aa = 0; aa < 16; ++aa) v[aa] = lds64<0>(r0 ^ (uint32_t)(128 * aa + 16 * (aa & 7)));
+            fence_proxy_async_smem();                        // these generic accesses before the next tensor copy into the tile
             __syncwarp();
             if (lane == 0) smem_counter_add_release(sb + SM::bempty + 8 * buf, 1);
             if (t == 0 && ib + 2 < n_items && ld_it == ib + 2)   // bring in the team's next item while this one is finished
@@ -777,19 +831,23 @@ k_search(const __grid_constant__ SearchArgs A)
     if (threadIdx.x < 32) tmem_dealloc<kTmemCols>(tq);
 }
 
-// sigma_jm = sqrt(sum of the 16 tile partial sums) / N
+// sum of the 8 warp partial sums of a tile, in the order pass 2 uses
+__host__ __device__ inline float tile_sum8(const float* w)
+{
+    return ((w[0] + w[1]) + (w[2] + w[3])) + ((w[4] + w[5]) + (w[6] + w[7]));
+}
+
+// sigma_jm = sqrt(sum of the 16 x 8 partial sums) / N
 __global__ void k_sigma(const float* __restrict__ sigpart, float* __restrict__ sigma, uint64_t n)
 {
     const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    float s = 0.f;
-    // same pairwise order as hw_sum16 (xor 8, 4, 2, 1) so that sigma matches the search bit for bit
+    // same order as pass 2 (tile_sum8, then row_sum16: xor 8, 4, 2, 1) so that sigma matches the search bit for bit
     float v[16];
-    for (int a = 0; a < 16; ++a) v[a] = sigpart[i * 16 + a];
+    for (int a = 0; a < 16; ++a) v[a] = tile_sum8(sigpart + i * kSigPart + 8 * a);
     for (int d = 8; d >= 1; d >>= 1)
         for (int a = 0; a < d; ++a) v[a] = v[a] + v[a + d];
-    s = v[0];
-    sigma[i] = sqrtf(s) / (float)kN;
+    sigma[i] = sqrtf(v[0]) / (float)kN;
 }
 
 // dual-stream search: Q[k] = Re(X[k] X[N-k]) of a stored segment spectrum, same tile layout (one float per bin).
@@ -806,25 +864,25 @@ k_dual_q(const c2* __restrict__ xs, float* __restrict__ q, int I0, int NI)
         const uint32_t k = (uint32_t)(16 * b + c) + 256u * (uint32_t)(g + 16 * (ii + I0));
         const uint32_t km = ((uint32_t)kN - k) & (uint32_t)(kN - 1);
         const int bm = (int)((km & 255u) >> 4), cm = (int)(km & 15u), gm = (int)((km >> 8) & 15u), im_ = (int)(km >> 12) - I0;
-        const size_t idx = (((size_t)b * (NI / 2) + ii / 2) * 256 + t) * 2 + (ii & 1);
+        const size_t idx = (size_t)tile_word(NI, b, ii / 2, t) * 2 + (ii & 1);
         float val = 0.f;
         if (im_ >= 0 && im_ < NI) {
-            const c2 a = X[idx], d = X[(((size_t)bm * (NI / 2) + im_ / 2) * 256 + 16 * cm + gm) * 2 + (im_ & 1)];
+            const c2 a = X[idx], d = X[(size_t)tile_word(NI, bm, im_ / 2, 16 * cm + gm) * 2 + (im_ & 1)];
             val = re(a) * re(d) - im(a) * im(d);
         }
         Q[idx] = val;
     }
 }
 
-// dual-stream search: sigma_1 = sqrt((S + P)/2)/N, sigma_2 = sqrt((S - P)/2)/N from the 2 x 16 tile partial sums of a pair
+// dual-stream search: sigma_1 = sqrt((S + P)/2)/N, sigma_2 = sqrt((S - P)/2)/N from the 2 x 128 partial sums of a pair
 __global__ void k_sigma_dual(const float* __restrict__ sigpart, float* __restrict__ s1, float* __restrict__ s2, uint64_t n)
 {
     const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     float v[16], w[16];
-    for (int a = 0; a < 16; ++a) { v[a] = sigpart[i * 32 + a]; w[a] = sigpart[i * 32 + 16 + a]; }
+    for (int a = 0; a < 16; ++a) { v[a] = tile_sum8(sigpart + i * 2 * kSigPart + 8 * a); w[a] = tile_sum8(sigpart + i * 2 * kSigPart + kSigPart + 8 * a); }
     for (int d = 8; d >= 1; d >>= 1)
-        for (int a = 0; a < d; ++a) { v[a] = v[a] + v[a + d]; w[a] = w[a] + w[a + d]; }     // the order of hw_sum16
+        for (int a = 0; a < d; ++a) { v[a] = v[a] + v[a + d]; w[a] = w[a] + w[a + d]; }     // the order of row_sum16
     s1[i] = sqrtf(fmaxf(0.5f * (v[0] + w[0]), 0.f)) / (float)kN;
     s2[i] = sqrtf(fmaxf(0.5f * (v[0] - w[0]), 0.f)) / (float)kN;
 }
@@ -880,6 +938,8 @@ struct bege_plan {
     unsigned long long* h_count = nullptr;
     cudaEvent_t ev_a = nullptr, ev_b = nullptr, ev_done = nullptr;
     bool profiling = false;
+    CUtensorMap ring_map{};          // the ring as a 2-D tensor (pass 2 fetches its row tiles with one tensor copy)
+    void* ring_map_for = nullptr;   // ring address the map was encoded for
     void* l2_window = nullptr;      // ring region currently marked persisting in L2 (access policy window of the stream)
     size_t l2_limit_prev = 0; bool l2_limit_saved = false;   // device limit found before the first search
     uint64_t max_items = ((1ull << 31) - 1) / 2;   // per group and launch (the kernel counts items in 32 bits)
@@ -1089,10 +1149,10 @@ extern "C" int bege_plan_workspace_bytes(const bege_plan* p, uint64_t T, uint32_
     b += al((uint64_t)S * tpl_bytes(p));               // segment spectra
     b += al((uint64_t)S * tpl_bytes(p) / 2);           // Re(X[k] X[N-k]) (dual-stream search)
     b += al(scratch_bytes(p));                          // four-step staging (stays in L2)
-    b += al(T * S * 32 * sizeof(float));               // Parseval partial sums (two per tile in the dual-stream search)
+    b += al(T * S * 2 * kSigPart * sizeof(float));     // Parseval partial sums (two sets in the dual-stream search)
     b += al(std::max<uint64_t>(cap * sizeof(bege_tail), (uint64_t)S * kN * 16));  // records / max-projection array(s)
     b += al(kMiscHdr + (uint64_t)S * kN * sizeof(c2)); // counters + raw segment staging
-    b += al(std::max<uint64_t>(std::max<uint64_t>(2 * T * S * sizeof(float), (uint64_t)S * kN * 16), kN * sizeof(c2) + 256));   // sigma / projection / debug output
+    b += al(std::max<uint64_t>(std::max<uint64_t>(2 * T * S * sizeof(float), (uint64_t)S * kN * 16), kN * sizeof(c2) + 512));   // sigma / projection / debug output
     *bytes = b + 4096;
     return BEGE_OK;
 }
@@ -1215,21 +1275,52 @@ static void set_l2_window(bege_plan* p, void* ring)
     p->l2_window = ring;
 }
 
+// The ring as pass 2 sees it: a 2-D fp32 tensor, inner dimension the 256 complex n2 of a line (512 floats), outer
+// dimension the lines k1 of all groups and ring slots; box = this CTA's 16 rows (32 floats = 128 bytes) x 256 lines,
+// 128-byte swizzle.  Encoded by the driver (cuTensorMapEncodeTiled, looked up at run time: no link to libcuda).
+static int make_ring_map(bege_plan* p, void* ring)
+{
+    if (p->ring_map_for == ring) return BEGE_OK;
+    typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static encode_fn encode = nullptr;
+    if (!encode) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess || !fn ||
+            qr != cudaDriverEntryPointSuccess) { cudaGetLastError(); return fail(p, BEGE_ECUDA, "cuTensorMapEncodeTiled not available"); }
+        encode = (encode_fn)fn;
+    }
+    const cuuint64_t gdim[2] = {512, (cuuint64_t)p->G * kRing * 256};
+    const cuuint64_t gstride[1] = {2048};                    // bytes between lines
+    const cuuint32_t box[2] = {32, 256};
+    const cuuint32_t estride[2] = {1, 1};
+    const CUresult r = encode(&p->ring_map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, ring, gdim, gstride, box, estride,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(p, BEGE_ECUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
+    p->ring_map_for = ring;
+    return BEGE_OK;
+}
+
 // one cooperative launch of the persistent search kernel over templates [j0, j0 + nT) x segments [m0, m0 + nS)
 static int launch_search(bege_plan* p, const c2* bank, const c2* xs, c2* ring, float* sig, uint64_t sig_pair0, float k2, float k2hi,
                          bege_tail* rec, uint64_t cap, unsigned char* misc, c2* zdbg, uint64_t j0, uint64_t nT, uint32_t m0,
                          uint32_t nS, bool first = true, const float* qseg = nullptr)
 {
     const bool dual = qseg != nullptr;
-    // the first launch of a search also clears the record counter and the abort flag (first 16 bytes)
-    CU(p, cudaMemsetAsync(misc + (first ? 0 : 16), 0, kMiscHdr - (first ? 0 : 16), p->stream));
+    // the first launch of a search also clears the record counter, the abort flag and the hit counters
+    CU(p, cudaMemsetAsync(misc + (first ? 0 : kOffDone1), 0, kMiscHdr - (first ? 0 : kOffDone1), p->stream));
     const int G = (int)std::min<uint64_t>((uint64_t)p->G, nT);
     const dim3 grid(16, G);
     set_l2_window(p, (void*)ring);
+    { const int rc = make_ring_map(p, (void*)ring); if (rc) return rc; }
     SearchArgs a{};
+    a.ring_map = p->ring_map;
     a.bank = bank; a.xseg = xs; a.qseg = qseg; a.ring = ring; a.sigpart = sig; a.rec = rec; a.zdbg = zdbg;
-    a.cap = cap; a.counter = (unsigned long long*)misc; a.abort_flag = (int*)(misc + 8);
-    a.done1 = (unsigned long long*)(misc + 256); a.done2 = (unsigned long long*)(misc + 2048);
+    a.cap = cap; a.counter = (unsigned long long*)(misc + kOffCounter); a.abort_flag = (int*)(misc + kOffAbort);
+    a.done1 = (unsigned long long*)(misc + kOffDone1); a.done2 = (unsigned long long*)(misc + kOffDone2);
     a.j0 = j0; a.nT = nT; a.sig_pair0 = sig_pair0; a.m0 = m0; a.nS = nS; a.S = p->S; a.k2 = k2; a.k2hi = k2hi;
     void* args[] = {&a};
     const void* f = search_variant(p->NI, nS == 1, zdbg != nullptr, dual);
@@ -1249,7 +1340,7 @@ static int launch_search(bege_plan* p, const c2* bank, const c2* xs, c2* ring, f
 static int check_abort(bege_plan* p, unsigned char* misc)
 {
     int flag = 0;
-    CU(p, cudaMemcpyAsync(&flag, misc + 8, sizeof flag, cudaMemcpyDeviceToHost, p->stream));
+    CU(p, cudaMemcpyAsync(&flag, misc + kOffAbort, sizeof flag, cudaMemcpyDeviceToHost, p->stream));
     CU(p, cudaStreamSynchronize(p->stream));
     if (flag) return fail(p, BEGE_ECUDA, "search pipeline timed out waiting on a group counter");
     return BEGE_OK;
@@ -1277,7 +1368,7 @@ static int search_impl(bege_plan* p, float k_sigma, float k_hi, bege_tail* tails
     CU(p, cudaSetDevice(p->device));
     void *sig, *rec, *misc, *scr, *bank, *xs;
     int rc;
-    if ((rc = slot_get(p, p->s_sig, p->T * p->S * 32 * sizeof(float), &sig))) return rc;
+    if ((rc = slot_get(p, p->s_sig, p->T * p->S * 2 * kSigPart * sizeof(float), &sig))) return rc;
     if ((rc = slot_get(p, p->s_rec, cap * sizeof(bege_tail), &rec))) return rc;
     if ((rc = slot_get(p, p->s_misc, kMiscHdr, &misc))) return rc;
     if ((rc = slot_get(p, p->s_scratch, scratch_bytes(p), &scr))) return rc;
@@ -1304,7 +1395,7 @@ static int search_impl(bege_plan* p, float k_sigma, float k_hi, bege_tail* tails
     }
     CU(p, cudaGetLastError());
     CU(p, cudaMemcpyAsync(p->h_count, counter, sizeof(unsigned long long), cudaMemcpyDeviceToHost, p->stream));
-    CU(p, cudaMemcpyAsync(p->h_count + 1, (unsigned char*)misc + 8, sizeof(int), cudaMemcpyDeviceToHost, p->stream));
+    CU(p, cudaMemcpyAsync(p->h_count + 1, (unsigned char*)misc + kOffAbort, sizeof(int), cudaMemcpyDeviceToHost, p->stream));
     // only the tails cross PCIe: the records of slice i are complete once slice i has finished, and are
     // copied on the side stream while the main stream searches slice i + 1
     uint64_t copied = 0;
@@ -1371,7 +1462,7 @@ extern "C" int bege_search_maxproj(bege_plan* p, float k_sigma, float* snr_out, 
     void *sig, *proj, *misc, *scr, *bank, *xs, *tmp;
     int rc;
     const uint64_t n = (uint64_t)p->S * kN;
-    if ((rc = slot_get(p, p->s_sig, p->T * p->S * 32 * sizeof(float), &sig))) return rc;
+    if ((rc = slot_get(p, p->s_sig, p->T * p->S * 2 * kSigPart * sizeof(float), &sig))) return rc;
     if ((rc = slot_get(p, p->s_rec, n * sizeof(unsigned long long), &proj))) return rc;
     if ((rc = slot_get(p, p->s_misc, kMiscHdr, &misc))) return rc;
     if ((rc = slot_get(p, p->s_scratch, scratch_bytes(p), &scr))) return rc;
@@ -1388,7 +1479,7 @@ extern "C" int bege_search_maxproj(bege_plan* p, float k_sigma, float* snr_out, 
     }
     CU(p, cudaGetLastError());
     float* d_snr = (float*)tmp; uint32_t* d_id = (uint32_t*)(d_snr + n);
-    unsigned long long* d_hits = (unsigned long long*)((unsigned char*)misc + 16);      // cleared by the first launch
+    unsigned long long* d_hits = (unsigned long long*)((unsigned char*)misc + kOffHits);      // cleared by the first launch
     k_proj_decode<<<(unsigned)((n + 255) / 256), 256, 0, p->stream>>>((const unsigned long long*)proj, d_snr, d_id, d_hits, n);
     count_launch(p);
     CU(p, cudaMemcpyAsync(snr_out, d_snr, n * sizeof(float), cudaMemcpyDeviceToHost, p->stream));
@@ -1415,7 +1506,7 @@ extern "C" int bege_search_dual(bege_plan* p, float k_sigma, float* snr1, uint32
     void *sig, *proj, *misc, *scr, *bank, *xs, *q, *tmp, *par;
     int rc;
     const uint64_t n = (uint64_t)p->S * kN;
-    if ((rc = slot_get(p, p->s_sig, p->T * p->S * 32 * sizeof(float), &sig))) return rc;
+    if ((rc = slot_get(p, p->s_sig, p->T * p->S * 2 * kSigPart * sizeof(float), &sig))) return rc;
     if ((rc = slot_get(p, p->s_rec, 2 * n * sizeof(unsigned long long), &proj))) return rc;
     if ((rc = slot_get(p, p->s_misc, kMiscHdr, &misc))) return rc;
     if ((rc = slot_get(p, p->s_scratch, scratch_bytes(p), &scr))) return rc;
@@ -1439,7 +1530,7 @@ extern "C" int bege_search_dual(bege_plan* p, float k_sigma, float* snr1, uint32
     CU(p, cudaGetLastError());
     float* d_snr1 = (float*)tmp; uint32_t* d_id1 = (uint32_t*)(d_snr1 + n);
     float* d_snr2 = (float*)(d_id1 + n); uint32_t* d_id2 = (uint32_t*)(d_snr2 + n);
-    unsigned long long* d_cnt = (unsigned long long*)((unsigned char*)misc + 16);      // hits1, hits2, simultaneous, coincident
+    unsigned long long* d_cnt = (unsigned long long*)((unsigned char*)misc + kOffHits);      // hits1, hits2, simultaneous, coincident
     CU(p, cudaMemsetAsync(d_cnt, 0, 4 * sizeof(unsigned long long), p->stream));
     const unsigned nb = (unsigned)((n + 255) / 256);
     k_proj_decode<<<nb, 256, 0, p->stream>>>((const unsigned long long*)proj, d_snr1, d_id1, d_cnt, n);
@@ -1506,26 +1597,26 @@ extern "C" int bege_debug_correlate(bege_plan* p, uint64_t j, uint32_t m, float*
     int rc;
     if ((rc = slot_get(p, p->s_scratch, scratch_bytes(p), &scr))) return rc;
     if ((rc = slot_get(p, p->s_misc, kMiscHdr, &misc))) return rc;
-    if ((rc = slot_get(p, p->s_tmp, kN * sizeof(c2) + 256, &tmp))) return rc;
+    if ((rc = slot_get(p, p->s_tmp, kN * sizeof(c2) + 512, &tmp))) return rc;
     if ((rc = slot_get(p, p->s_bank, 0, &bank))) return rc;
     if ((rc = slot_get(p, p->s_x, 0, &xs))) return rc;
     c2* zd = (c2*)tmp;
     float* sg = (float*)((unsigned char*)tmp + kN * sizeof(c2));     // private partial sums of this one pair
     const bool prof = p->profiling; p->profiling = false;
-    // sig_pair0 = this pair's index, so that its partial sums land on sg[0..15]
+    // sig_pair0 = this pair's index, so that its partial sums land on sg[0..127]
     rc = launch_search(p, (const c2*)bank, (const c2*)xs, (c2*)scr, sg, j * p->S + m, 1e30f, INFINITY, nullptr, 0,
                        (unsigned char*)misc, zd, j, 1, m, 1);
     p->profiling = prof;
     if (!rc) rc = check_abort(p, (unsigned char*)misc);
     drop_l2_window(p);
     if (rc) return rc;
-    float part[16];
+    float part[kSigPart];
     CU(p, cudaMemcpyAsync(z_out, zd, kN * sizeof(c2), cudaMemcpyDeviceToHost, p->stream));
     CU(p, cudaMemcpyAsync(part, sg, sizeof part, cudaMemcpyDeviceToHost, p->stream));
     CU(p, cudaStreamSynchronize(p->stream));
     if (sigma_out) {
         float v[16];
-        for (int a = 0; a < 16; ++a) v[a] = part[a];
+        for (int a = 0; a < 16; ++a) v[a] = tile_sum8(part + 8 * a);
         for (int d = 8; d >= 1; d >>= 1) for (int a = 0; a < d; ++a) v[a] = v[a] + v[a + d];
         *sigma_out = sqrtf(v[0]) / (float)kN;
     }
@@ -1548,7 +1639,7 @@ static void untile(const bege_plan* p, const std::vector<float2>& tile, float* o
         for (int ii = 0; ii < p->NI; ++ii)
             for (int c = 0; c < 16; ++c)
                 for (int g = 0; g < 16; ++g) {
-                    const float2 v = tile[((((size_t)b * (p->NI / 2) + ii / 2) * 256) + 16 * c + g) * 2 + (ii & 1)];
+                    const float2 v = tile[(size_t)tile_word(p->NI, b, ii / 2, 16 * c + g) * 2 + (ii & 1)];
                     const size_t k = (size_t)(16 * b + c) + 256 * (size_t)(g + 16 * (ii + p->I0));
                     out[2 * k] = v.x; out[2 * k + 1] = v.y;
                 }

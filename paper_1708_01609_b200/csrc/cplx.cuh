@@ -116,9 +116,26 @@ BEGE_D float hw_sum16(float v) {
     v += __shfl_xor_sync(0xffffffffu, v, 1);
     return v;
 }
+// sum over the 16 lanes of a pass-2 row (lane map a = (lane & 7) | ((lane >> 4) << 3): xor 16 is a ^ 8), same tree
+BEGE_D float row_sum16(float v) {
+    v += __shfl_xor_sync(0xffffffffu, v, 16);
+    v += __shfl_xor_sync(0xffffffffu, v, 4);
+    v += __shfl_xor_sync(0xffffffffu, v, 2);
+    v += __shfl_xor_sync(0xffffffffu, v, 1);
+    return v;
+}
 BEGE_D float warp_sum32(float v) {
     v += __shfl_xor_sync(0xffffffffu, v, 16);
     return hw_sum16(v);
+}
+
+// "Tile layout" of a stored spectrum (bank, segments).  Tile b holds the columns k1 = 16 b + c; thread t = 16 c + g of a
+// pass-1 team owns rows k2 = g + 16 i of column c.  Its kept row-blocks are stored in pairs (one 16-byte word per pair
+// ip), and the words of one WARP (32 threads x NI/2 pairs) are contiguous: NI * 256 bytes that the warp brings in with
+// one bulk copy and reads back with conflict-free 128-bit loads.  Index of the 16-byte word of (tile b, pair ip, thread t):
+__host__ __device__ __forceinline__ uint32_t tile_word(int NI, int b, int ip, int t)
+{
+    return ((uint32_t)(b * 8 + (t >> 5)) * (uint32_t)(NI / 2) + (uint32_t)ip) * 32u + (uint32_t)(t & 31);
 }
 
 }  // namespace bege
