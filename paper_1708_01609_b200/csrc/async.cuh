@@ -66,18 +66,6 @@ BEGE_DA bool mbar_try_wait(uint32_t bar, uint32_t parity)
 // abort flag (checked by the host after the launch) and lets the caller run on with whatever it has
 constexpr long long kSpinLimit = 1000000000ll;
 
-#ifndef BEGE_WAIT_HINT
-#define BEGE_WAIT_HINT 2000u
-#endif
-// try_wait with a suspend-time hint (ns): the thread sleeps in hardware until the phase completes or the hint runs out
-BEGE_DA bool mbar_try_wait_hint(uint32_t bar, uint32_t parity, uint32_t ns)
-{
-    uint32_t ok;
-    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                 : "=r"(ok) : "r"(bar), "r"(parity), "r"(ns) : "memory");
-    return ok != 0;
-}
-
 // The wait loop is kept short (a waiting warp shares its scheduler with working ones): the abort flag and the clock are
 // looked at once per 64 probes only.
 BEGE_DA void mbar_wait(uint32_t bar, uint32_t parity, int* abort_flag)
@@ -85,7 +73,7 @@ BEGE_DA void mbar_wait(uint32_t bar, uint32_t parity, int* abort_flag)
     if (mbar_try_wait(bar, parity)) return;
     uint32_t spins = 0;
     long long t0 = 0;
-    while (!(BEGE_WAIT_HINT ? mbar_try_wait_hint(bar, parity, BEGE_WAIT_HINT) : mbar_try_wait(bar, parity))) {
+    while (!mbar_try_wait(bar, parity)) {
         if ((++spins & 63u) == 0u) {
             if (*(volatile int*)abort_flag) return;
             const long long now = clock64();
@@ -93,21 +81,6 @@ BEGE_DA void mbar_wait(uint32_t bar, uint32_t parity, int* abort_flag)
             if (now - t0 > kSpinLimit) {
                 *(volatile int*)abort_flag = 1; return;
             }
-        }
-    }
-}
-
-// two-instruction probe loop; the clock and the abort flag once per 4096 probes
-BEGE_DA void mbar_wait_lean(uint32_t bar, uint32_t parity, int* abort_flag)
-{
-    uint32_t spins = 0;
-    long long t0 = 0;
-    while (!mbar_try_wait(bar, parity)) {
-        if ((++spins & 4095u) == 0u) {
-            if (*(volatile int*)abort_flag) return;
-            const long long now = clock64();
-            if (t0 == 0) t0 = now;
-            if (now - t0 > kSpinLimit) { *(volatile int*)abort_flag = 1; return; }
         }
     }
 }
@@ -141,14 +114,6 @@ BEGE_DA void tma_load_2d(uint32_t smem_dst, const void* tmap, int c0, int c1, ui
                  :: "r"(smem_dst), "l"(tmap), "r"(c0), "r"(c1), "r"(bar), "l"(policy) : "memory");
 }
 
-// shared -> global, joins the issuing thread's current bulk async-group (the TMA engine drains it in the background)
-BEGE_DA void bulk_store(void* gmem_dst, uint32_t smem_src, uint32_t bytes)
-{
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" :: "l"(gmem_dst), "r"(smem_src), "r"(bytes) : "memory");
-}
-BEGE_DA void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
-BEGE_DA void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }   // sources reusable
-BEGE_DA void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }             // writes performed
 // generic-proxy writes to shared memory -> visible to the async proxy (TMA) of this CTA
 BEGE_DA void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 // generic-proxy accesses (of this thread, and what it has acquired) before async-proxy accesses, all state spaces
@@ -224,10 +189,6 @@ BEGE_DA uint32_t smem_counter_load_acquire(uint32_t addr)
 }
 
 // ---- gpu-scope counters
-BEGE_DA void counter_add_release(unsigned long long* ctr, unsigned long long v)
-{
-    asm volatile("red.release.gpu.global.add.u64 [%0], %1;" :: "l"(ctr), "l"(v) : "memory");
-}
 BEGE_DA void fence_acq_rel_gpu() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
 BEGE_DA void counter_add_relaxed(unsigned long long* ctr, unsigned long long v)
 {
@@ -241,15 +202,12 @@ BEGE_DA unsigned long long counter_load_acquire(const unsigned long long* ctr)
 }
 // ONE thread spins until *ctr >= target; every probe is an acquire load, so whatever the thread (and, after a
 // CTA barrier, its team) reads afterwards is ordered after the producers' released writes.
-#ifndef BEGE_POLL_NS
-#define BEGE_POLL_NS 2000
-#endif
 BEGE_DA void counter_wait_ge(const unsigned long long* ctr, unsigned long long target, int* abort_flag)
 {
     if (counter_load_acquire(ctr) >= target) return;
     long long t0 = 0;
     for (uint32_t spins = 1;; ++spins) {
-        __nanosleep(BEGE_POLL_NS);
+        __nanosleep(2000);
         if (counter_load_acquire(ctr) >= target) return;
         if ((spins & 63u) == 0u) {                           // the abort flag and the clock: rarely
             if (*(volatile int*)abort_flag) return;

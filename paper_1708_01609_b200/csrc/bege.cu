@@ -209,20 +209,14 @@ k_fwd_cols(const c2* __restrict__ G, c2* __restrict__ out, uint64_t out_stride, 
 //              The same thread waits with ld.acquire.gpu until all 16 tiles of its team's item have been added, then
 //              issues the tensor copy of the rows.
 //   done2 (ring slot read out): as soon as that copy has landed (mbarrier), a thread of the B team adds 1 to
-//              done2[slot] under the same kind of fence.  Lane 0 of every A warp acquires 16 of them (load issued at
-//              the top of the item, looked at just before the warp's ring stores, __syncwarp in between).
+//              done2[slot] under the same kind of fence.  Every A warp acquires 16 of them just before its ring stores
+//              (all lanes load the one counter, so the warp stays converged; 2 us between probes while waiting).
 // The ring holds kRing items per group (G x kRing x 512 KiB) and lives in L2.
 #ifndef BEGE_RING
 #define BEGE_RING 16
 #endif
 constexpr int kRing = BEGE_RING;
 constexpr int kSearchThreads = 32 * 32;
-#ifndef BEGE_FWD
-#define BEGE_FWD 0
-#endif
-#ifndef BEGE_BGO
-#define BEGE_BGO 1
-#endif
 #ifndef BEGE_STATS
 #define BEGE_STATS 0       // 1: one CTA prints wait statistics of its service threads at the end (experiments only)
 #endif
@@ -254,10 +248,8 @@ template <int NI> struct SearchSmem {
     static constexpr uint32_t amb = abar + 128;                  // [kRing] mbarriers: tile of ring slot stored (8 A warps)
     static constexpr uint32_t bfull = amb + 8 * kRing;           // [kNB] mbarriers: row tile has arrived
     static constexpr uint32_t bempty = bfull + 24;               // [kNB] u32 counters (8-byte pitch): warps that have read a tile out
-    static constexpr uint32_t bgo = bempty + 24;                 // [2][4] mbarriers (experiment BEGE_BGO)
-    static constexpr uint32_t pubit = bgo + 64;                 // [2] u32: next item of A team k to publish (claimed by atomicCAS)
-    static constexpr uint32_t freed = pubit + 8;                 // [2] u32: items of A team k whose ring slots all 16 CTAs have read out
-    static constexpr uint32_t tmem = freed + 8;                  // TMEM base address
+    static constexpr uint32_t pubit = bempty + 24;                               // [2] u32: next item of A team k to publish (claimed by atomicCAS)
+    static constexpr uint32_t tmem = pubit + 8;                  // TMEM base address
     static constexpr uint32_t total = tmem + 8;
     static_assert(total + 2048 <= 232448, "shared memory of one SM");
 };
@@ -386,11 +378,8 @@ k_search(const __grid_constant__ SearchArgs A)
             mbar_init(sb + SM::bfull + 8 * i, 1);
             *reinterpret_cast<volatile uint32_t*>(smem_raw + SM::bempty + 8 * i) = 0;
         }
-        for (int i = 0; i < 8; ++i) mbar_init(sb + SM::bgo + 8 * i, 1);
         reinterpret_cast<volatile uint32_t*>(smem_raw + SM::pubit)[0] = 0;
         reinterpret_cast<volatile uint32_t*>(smem_raw + SM::pubit)[1] = 1;
-        reinterpret_cast<volatile uint32_t*>(smem_raw + SM::freed)[0] = 0;
-        reinterpret_cast<volatile uint32_t*>(smem_raw + SM::freed)[1] = 0;
         fence_mbar_init();
     }
     if (threadIdx.x < 32) tmem_alloc<kTmemCols>(sb + SM::tmem);
@@ -467,7 +456,6 @@ k_search(const __grid_constant__ SearchArgs A)
         const uint32_t xa = sb + SM::xch + (uint32_t)(aw * 2 + (lane >> 4)) * SM::kXch;
         const uint32_t xw_a = xa + g * 136;                  // + 8 p:    element (g, p) of the half-warp's region
         const uint32_t xr_a = xa + g * 8;                    // + 136 gg: element (gg, p = g)
-        const uint32_t freed_a = sb + SM::freed + 4 * team;
         constexpr uint32_t kWarpElems = SM::kWarpTile / 8;
         // streaming tile part of this warp: template `it` (single-segment calls) / segment ml (batched calls)
         auto stream_src = [&](uint32_t it, uint32_t ml) { return (SINGLE ? tpl_tile(it) : seg_tile(ml)) + (uint32_t)warp * kWarpElems; };
@@ -532,23 +520,13 @@ k_search(const __grid_constant__ SearchArgs A)
                 sp[0] = sw;
                 if (DUAL) sp[kSigPart] = pw;
             }
-            // Ring slot free?  Item it - kRing = item (it >> 1) - kRing / 2 of this team must have been read out by all
-            // 16 CTAs of the group: the B team of the same parity watches the global counter done2 and forwards it as a
-            // CTA-local count (one global poller per team instead of eight warps on one L2 line; warp-uniform here).
-            if (!BEGE_FWD && !(BEGE_ABL & 1) && it >= (uint32_t)kRing) {
+            // Ring slot free?  Item it - kRing must have been read out by pass 2 of all 16 CTAs of the group (done2).
+            // All lanes load the one counter (a warp-uniform value keeps the warp converged through the wait; a wait
+            // taken by lane 0 alone left the warp split in two for the rest of the item, profiles/r2b_*); waiting warps
+            // sleep 2 us between probes -- the ring is 16 items deep, and frequent probes of one L2 line slow its reds.
+            if (!(BEGE_ABL & 1) && it >= (uint32_t)kRing) {
                 const unsigned long long need = 16ull * (it / kRing);
                 if (counter_load_acquire(d2 + slot) < need) counter_wait_ge(d2 + slot, need, abort_flag);
-            }
-            if (BEGE_FWD && !(BEGE_ABL & 1) && it >= (uint32_t)kRing) {
-                const uint32_t need = (it >> 1) - (uint32_t)(kRing / 2) + 1u;
-                if (smem_counter_load_acquire(freed_a) < need) {
-                    const long long t0 = clock64();
-                    while (smem_counter_load_acquire(freed_a) < need) {
-                        __nanosleep(200);
-                        if (*(volatile int*)abort_flag) break;
-                        if (clock64() - t0 > kSpinLimit) { *(volatile int*)abort_flag = 1; break; }
-                    }
-                }
             }
             __syncwarp();                                    // exchange region free for the next item; ring slot free
             fft16<+1>(v);
@@ -602,20 +580,6 @@ k_search(const __grid_constant__ SearchArgs A)
             for (uint32_t i = 0; i < n; ++i) counter_add_relaxed(d1 + (first + 2 * i) % kRing, 1ull);
             if (free_slot >= 0) counter_add_relaxed(d2 + free_slot, 1ull);
         };
-        // items kb, kb + 2, ... whose ring slots have been read out by ALL 16 CTAs of the group (done2, acquired) are
-        // counted in shared memory for A team kb.  Called by one thread of the team at a time (the duty lane after the
-        // team barrier of an item, thread 0 inside its wait loop before it).
-        const uint32_t freed_b = sb + SM::freed + 4 * kb;
-        auto advance_freed = [&]() {
-            const uint32_t c0 = *reinterpret_cast<volatile uint32_t*>(smem_raw + SM::freed + 4 * kb);
-            uint32_t c = c0;
-            while (c < c0 + 2) {
-                const uint32_t itc = kb + 2 * c;
-                if (itc >= n_items || counter_load_acquire(d2 + itc % kRing) < 16ull * (itc / kRing + 1)) break;
-                ++c;
-            }
-            if (c != c0) smem_counter_add_release(freed_b, c - c0);
-        };
         // copy of item `it` of this team into its tile buffer, if the buffer has been read out (item it - NB, either
         // team) and all 16 tiles of the item are in the ring (d1, acquired: `ready`); non-blocking.  "Read out" is a
         // monotone count of warps (8 per use), not an mbarrier: this thread may look at a buffer whose use before last
@@ -648,7 +612,6 @@ k_search(const __grid_constant__ SearchArgs A)
             if (t == 0) {
                 const unsigned long long target = 16ull * (ib / kRing + 1);
                 const long long t0 = clock64();
-                uint32_t spin = 0;
                 if (BEGE_STATS) { if (ld_it == ib) ++st_ntop; else ++st_nmid; }
                 for (;;) {
                     if (BEGE_STATS) ++st_spin;
@@ -661,23 +624,19 @@ k_search(const __grid_constant__ SearchArgs A)
                     if (clock64() - t0 > kSpinLimit) {
                         *(volatile int*)abort_flag = 1; break;
                     }
-                    if (BEGE_FWD && !(BEGE_ABL & 1) && (++spin & 7u) == 0u) advance_freed();   // A may be waiting for exactly this
                     __nanosleep(40);
                 }
                 // The other seven warps wait for this thread at the team's named barrier below: blocked in hardware, they
                 // take no issue slots from the working warps (a try_wait loop on the tile's mbarrier cost more
                 // instructions per item than the item's arithmetic, profiles/r2b_*).
                 if (BEGE_STATS) st_top += clock64() - t0;
-                if (BEGE_BGO) mbar_arrive(sb + SM::bgo + 32 * kb + 8 * (nit & 3));
                 // look at the counter of the team's next item now; the answer is used after the exchange
                 if (!(BEGE_ABL & 1) && ib + 2 < n_items && ld_it == ib + 2) { d1v = counter_load_acquire(d1 + (ib + 2) % kRing); d1v_it = ib + 2; }
             }
             __syncwarp();
-            if (BEGE_BGO) mbar_wait_lean(sb + SM::bgo + 32 * kb + 8 * (nit & 3), (nit >> 2) & 1, abort_flag);
-            else bar_named(1 + kb, 256);                     // the other seven warps block here in hardware (no spinning)
+            bar_named(1 + kb, 256);                          // the other seven warps block here in hardware (no spinning)
             // the rows are in shared memory: the ring slot is free.  This item's fence duty: warp 1 + (nit mod 7)
             if (warp == 1 + (int)(nit % 7) && lane == 0) publish(slot);
-            if (BEGE_FWD && !(BEGE_ABL & 1) && warp == 1 + (int)((nit + 3) % 7) && lane == 0) advance_freed();
             ++nit;
             c2 v[16];
             lds16<2048>(w0, v);
