@@ -46,8 +46,8 @@ FFT_FLOP = 5.0 * 65536 * 16                       # PAPER.md:134 eq.(10): 5 N lo
 ALG_BYTES_PER_CORR = 52802 * 8                    # two-sided in-band template spectrum, S = 1
 # dram__bytes_read.sum + dram__bytes_write.sum of k_search per correlation: an OFFLINE constant, taken from the
 # `ncu --set full` capture of the kernel as committed (profiles/r2_search_kernel.md: 36,864-template launch,
-# 16.914 GB read + 0.005 GB written); it does not follow later kernel changes by itself.
-NCU_DRAM_BYTES_PER_CORR = (16.914e9 + 0.005e9) / 36864
+# 16.917 GB read + 0.024 GB written); it does not follow later kernel changes by itself.
+NCU_DRAM_BYTES_PER_CORR = (16.917e9 + 0.024e9) / 36864
 NCU_SOURCE = "profiles/r2_search_kernel.md"
 FP32_PEAK = 148 * 128 * 2 * 1.965e9               # SMs x fp32 lanes x 2 flop x max SM clock
 
@@ -275,7 +275,12 @@ def _extra_workloads(args, dev, local_rank):
         t0 = time.perf_counter(); plan.bank_generate(w.f0, w.fdot, synth.TAU); gen_s = time.perf_counter() - t0
         rate, e2e, n = timed(plan, x_host, w.k_sigma, 1 << 20, args.extra_reps)
         krate = kernel_rate(plan, w.k_sigma, 1 << 20)
+        # the same bank against ONE of the segments, right after (same clocks, same thermal state): like for like
+        plan.segment_load(x_host[:1])
+        kernel_rate(plan, w.k_sigma, 1 << 20)
+        krate1 = kernel_rate(plan, w.k_sigma, 1 << 20)
     out["segment_batched"] = {
+        "kernel_corr_per_s_single_segment_same_bank": krate1,
         "workload": f"configs[3]: {w.x.shape[0]} segments x {w.n_templates} templates, k = {w.k_sigma}",
         "S": int(w.x.shape[0]), "T": int(w.n_templates), "corr_per_s": rate, "kernel_corr_per_s": krate,
         "frac": rate * FFT_FLOP / FP32_PEAK, "e2e_corr_per_s": e2e, "n_tails": n,
