@@ -199,6 +199,26 @@ def run_cufft(args, rank, local_rank):
           flush=True)
 
 
+# ------------------------------------------------------------------------------------------ overlap-save bake-off
+def run_ovs_probe(args, rank, local_rank):
+    """the overlap-save variant's fused kernel (six 16384-point block correlations per template,
+    one CTA per SM, everything in shared memory), timed on synthetic resident spectra.  A measurement for the keep-or-kill
+    decision in DESIGN.md, not the product; sigma and the compaction of records are not in it (both small)."""
+    if rank != 0:
+        return
+    from paper_1708_01609_b200 import bege
+    T = args.ovs_templates
+    ms, hits, _ = bege.ovs_probe(T, 6, reps=max(args.steps, 1), device=local_rank)
+    value = T / (ms * 1e-3)
+    print(json.dumps({"impl": "ovs_probe", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+                      "ms_per_step": ms, "higher_is_better": True, "dtype": "f32", "data": "synthetic",
+                      "config": {"workload": f"{T} resident 16384-point template spectra (128 KiB each) x 6 overlapping blocks "
+                                 "of one segment; multiply + inverse transform in shared memory + threshold per block"},
+                      "gflops_equiv": value * FFT_FLOP * 1e-9, "frac_of_fp32_bound": value * FFT_FLOP / FP32_PEAK,
+                      "bank_bytes_2p20_templates": (1 << 20) * 16384 * 8,
+                      "note": "bake-off probe (SURVEY 8(f)4); correlations/s = templates/s, six blocks each"}), flush=True)
+
+
 # ------------------------------------------------------------------------------------------ launch self-test stand-in
 class _LaunchSelfTestPlan:
     """NOT a search.  `--selftest-launch` exercises bench.py's own multi-rank plumbing (spawn, rendezvous, barrier,
@@ -522,7 +542,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference", "cufft"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference", "cufft", "ovs_probe"])
     ap.add_argument("--templates", type=int, default=1 << 20, help="templates per GPU (default: configs[2])")
     ap.add_argument("--chunk", type=int, default=0, help="bank chunk size (default: what fits HBM)")
     ap.add_argument("--cpu-sample", type=int, default=24576)
@@ -533,6 +553,7 @@ def main():
     ap.add_argument("--extra-reps", type=int, default=2)
     ap.add_argument("--tail-cap", type=int, default=80_000_000)
     ap.add_argument("--cufft-batch", type=int, default=2048, help="templates per step of the --impl cufft reference point")
+    ap.add_argument("--ovs-templates", type=int, default=147456, help="templates of the --impl ovs_probe measurement")
     ap.add_argument("--selftest-launch", action="store_true",
                     help="exercise the multi-rank plumbing only (gloo, no GPU, no search): see _LaunchSelfTestPlan")
     args = ap.parse_args()
@@ -546,6 +567,9 @@ def main():
         return
     if args.impl == "cufft":
         run_cufft(args, rank, local_rank)
+        return
+    if args.impl == "ovs_probe":
+        run_ovs_probe(args, rank, local_rank)
         return
     if world > 1:
         import torch.distributed as dist

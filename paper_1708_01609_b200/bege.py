@@ -27,7 +27,7 @@ SYMBOLS = [
     "bege_segment_load", "bege_search", "bege_search_band", "bege_search_maxproj", "bege_get_sigma", "bege_debug_correlate",
     "bege_bank_generate_real", "bege_search_dual", "bege_get_sigma_dual",
     "bege_debug_template_spectrum", "bege_debug_segment_spectrum", "bege_debug_set_max_items", "bege_plan_set_profiling",
-    "bege_plan_get_stats", "bege_plan_reset_stats", "bege_last_error", "bege_plan_destroy", "bege_version",
+    "bege_plan_get_stats", "bege_plan_reset_stats", "bege_last_error", "bege_plan_destroy", "bege_version", "bege_ovs_probe",
 ]
 
 
@@ -72,6 +72,7 @@ def load_library() -> ctypes.CDLL:
     L.bege_debug_template_spectrum.argtypes = [vp, u64, vp]
     L.bege_debug_segment_spectrum.argtypes = [vp, u32, vp]
     L.bege_debug_set_max_items.argtypes = [vp, u64]
+    L.bege_ovs_probe.argtypes = [i32, u64, u32, u32, ctypes.c_float, vp, vp, vp, u64, ctypes.POINTER(dbl), ctypes.POINTER(u64)]
     L.bege_plan_set_profiling.argtypes = [vp, i32]
     L.bege_plan_get_stats.argtypes = [vp, ctypes.POINTER(Stats)]
     L.bege_plan_reset_stats.argtypes = [vp]
@@ -286,6 +287,26 @@ class Plan:
 
     def reset_stats(self):
         self._check(self._L.bege_plan_reset_stats(self._h))
+
+
+def ovs_probe(n_templates: int, n_blocks: int = 6, reps: int = 3, thr2: float = 3.0e38, h16=None, x16=None,
+              want_z: bool = False, dbg_j: int = 0, device: int = 0):
+    """bege_ovs_probe (include/bege.h): the overlap-save bake-off probe.  Returns (ms per pass, hits, z or None)."""
+    L = load_library()
+    ms, hits = ctypes.c_double(0.0), ctypes.c_uint64(0)
+    z = np.empty((n_blocks, 16384), dtype=np.complex64) if want_z else None
+    if h16 is not None:
+        h16 = np.ascontiguousarray(h16, dtype=np.complex64)
+        assert h16.shape == (n_templates, 16384)
+    if x16 is not None:
+        x16 = np.ascontiguousarray(x16, dtype=np.complex64)
+        assert x16.shape == (n_blocks, 16384)
+    rc = L.bege_ovs_probe(device, n_templates, n_blocks, reps, ctypes.c_float(thr2),
+                          h16.ctypes.data if h16 is not None else None, x16.ctypes.data if x16 is not None else None,
+                          z.ctypes.data if z is not None else None, dbg_j, ctypes.byref(ms), ctypes.byref(hits))
+    if rc != OK:
+        raise BegeError(rc, "bege_ovs_probe failed")
+    return ms.value, hits.value, z
 
 
 def version() -> str:

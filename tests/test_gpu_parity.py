@@ -611,3 +611,28 @@ def test_dual_stream_search_matches_oracle(bo, bege):
     assert n_coi == int(np.sum(np.abs(f0[gi1[sim]] - f0[gi2[sim]]) < delta))
     os_, oc = bo.dual_coincidences(oi1, oi2, f0, delta)        # the oracle's counts at its own (slightly lower) threshold
     assert abs(n_sim - os_) <= 0.02 * os_ + 5 and abs(n_coi - oc) <= 0.02 * oc + 5
+
+
+# ----------------------------------------------------------------------------- overlap-save bake-off probe
+def test_overlap_save_probe_matches_oracle(bo, bege):
+    """six 16384-point block correlations reproduce the oracle's circular correlation on every lag.
+    The block inputs are prepared here from the oracle's own transforms (fp64, rounded once to complex64)."""
+    w = synth.config0()
+    P, STEP, NB = 16384, 12288, 6
+    X = bo.segment_spectrum(w.x[0], FS, *BAND)
+    xhat = bo.fft(X, +1) / N                                   # the band-limited segment
+    x16 = np.stack([bo.fft(xhat[(STEP * i + np.arange(P)) % N], -1) for i in range(NB)]).astype(np.complex64)
+    ids = [0, 37, 119, 255]                                    # an edge template, interior ones, the other corner
+    hs = [bo.template(w.f0[j], w.fdot[j], TAU, FS, N) for j in ids]
+    h16 = np.stack([bo.fft(h[:P], -1) for h in hs]).astype(np.complex64)
+    for d, (j, h) in enumerate(zip(ids, hs)):
+        z, s = bo.correlate(X, h)
+        ms, hits, zb = bege.ovs_probe(len(ids), NB, reps=1, thr2=float((3.0 * s * P) ** 2), h16=h16, x16=x16,
+                                      want_z=True, dbg_j=d)
+        got = np.empty(N, dtype=np.complex128)
+        for i in range(NB):
+            lags = STEP * i + np.arange(STEP)
+            keep = lags < N
+            got[lags[keep]] = zb[i, :STEP][keep]
+        assert rel_l2(got, z) <= REL_L2, (j, rel_l2(got, z))
+        assert ms > 0
