@@ -32,7 +32,7 @@
 #include "bank64.cuh"
 
 #ifndef BEGE_ABL
-// Ablation switches for timing experiments (profiles/r1e_search_kernel.md); never set in the product build, results
+// Ablation switches for timing experiments (profiles/r2_search_kernel.md); never set in the product build, results
 // are garbage when any is set: 1 no cross-CTA waits, 2 no template tile loads, 4 no ring stores, 8 no ring loads,
 // 16 pass-1 teams off, 32 pass-2 teams off.
 #define BEGE_ABL 0
@@ -164,7 +164,7 @@ k_fwd_cols(const c2* __restrict__ G, c2* __restrict__ out, uint64_t out_stride, 
 //
 //   A teams (pass 1): every WARP is autonomous -- it owns two columns of the tile (half-warp = column c, lane g holds
 //              rows k2 = g + 16 i), and nothing in its item needs another warp: no CTA or team barrier in the loop
-//              (the team barriers of the earlier version cost pass 1 a quarter of its time, profiles/r2a_*).
+//              (the team barriers of the earlier version cost pass 1 a quarter of its time, profiles/r2_search_kernel.md).
 //              R = conj(H) X needs one column tile of the template spectrum and one of the segment spectrum.  One of
 //              them is STATIONARY -- it sits in tensor memory, 14 complex numbers per thread -- and the other STREAMS
 //              through a per-warp shared-memory buffer: the warp's words of a tile are contiguous (tile_word), ONE
@@ -526,7 +526,7 @@ k_search(const __grid_constant__ SearchArgs A)
             }
             // Ring slot free?  Item it - kRing must have been read out by pass 2 of all 16 CTAs of the group (done2).
             // All lanes load the one counter (a warp-uniform value keeps the warp converged through the wait; a wait
-            // taken by lane 0 alone left the warp split in two for the rest of the item, profiles/r2b_*); waiting warps
+            // taken by lane 0 alone left the warp split in two for the rest of the item, profiles/r2_search_kernel.md); waiting warps
             // sleep 2 us between probes -- the ring is 16 items deep, and frequent probes of one L2 line slow its reds.
             if (!(BEGE_ABL & 1) && it >= (uint32_t)kRing) {
                 const unsigned long long need = 16ull * (it / kRing);
@@ -632,7 +632,7 @@ k_search(const __grid_constant__ SearchArgs A)
                 }
                 // The other seven warps wait for this thread at the team's named barrier below: blocked in hardware, they
                 // take no issue slots from the working warps (a try_wait loop on the tile's mbarrier cost more
-                // instructions per item than the item's arithmetic, profiles/r2b_*).
+                // instructions per item than the item's arithmetic, profiles/r2_search_kernel.md).
                 if (BEGE_STATS) st_top += clock64() - t0;
                 // look at the counter of the team's next item now; the answer is used after the exchange
                 if (!(BEGE_ABL & 1) && ib + 2 < n_items && ld_it == ib + 2) { d1v = counter_load_acquire(d1 + (ib + 2) % kRing); d1v_it = ib + 2; }
