@@ -197,7 +197,7 @@ k_fwd_cols(const c2* __restrict__ G, c2* __restrict__ out, uint64_t out_stride, 
 //   columns [160, 192): pass 1, dual-stream search only: Re(X[k] X[N-k]) of the segment, 14 columns per thread
 //   columns [192, 256): pass 1, team 1: its copy of the stationary tile (batched calls: the teams change template
 //                       at different times)
-// The CTA-uniform part of the four-step factor, w256^(b r), comes from constant memory (uniform loads).  All table
+// The CTA-uniform part of the four-step factor, w256^(b r), comes from constant memory (uniform loads, one row per CTA).  All table
 // entries are rounded once from fp64 angles.
 //
 // Hand-over between the passes (PTX memory model): per group and ring slot two monotone counters.
@@ -222,7 +222,8 @@ constexpr int kSearchThreads = 32 * 32;
 #endif
 constexpr int kTmemCols = 256;
 constexpr uint32_t kTmDelta = 0, kTmStat = 32, kTmTheta = 96, kTmQ = 160, kTmStat1 = 192;   // kTmQ: 16 columns per warp of a quadrant
-__constant__ float2 c_w256[256];           // exp(2 pi i m / 256), rounded from fp64 (host, bege_plan_create)
+__constant__ float2 c_wb[16][16];          // exp(2 pi i b r / 256): row b = the CTA-uniform part of pass 2's four-step factor;
+                                           // rounded from fp64 (host, bege_plan_create)
 constexpr int kSigPart = 128;              // Parseval partial sums per pair: 16 tiles x 8 warps (dual-stream search: two sets)
 
 struct SearchArgs {
@@ -473,6 +474,12 @@ k_search(const __grid_constant__ SearchArgs A)
         }
         uint32_t nload = 0;                                  // tiles this warp has waited for so far
         uint32_t tj_prev = ~0u;
+        // single-segment calls: item it + 2 is template tj + 2 of the group -- the streaming source and the slot of the
+        // Parseval partial sums advance by constant strides (running pointers instead of 64-bit index arithmetic per item)
+        const c2* src_run = stream_src(team + 2, 0);
+        const uint64_t src_step = (uint64_t)G * 2 * 16 * kTile;
+        float* sp_run = A.sigpart + ((A.j0 + grp + (uint64_t)G * team) * (uint64_t)A.S + A.m0 - A.sig_pair0) * (DUAL ? 2 * kSigPart : kSigPart) + b * 8 + warp;
+        const uint64_t sp_step = (uint64_t)G * 2 * A.S * (DUAL ? 2 * kSigPart : kSigPart);
         // (template, segment) of the item, stepped without a division per item: batched calls have nS >= 2
         uint32_t tj_c = SINGLE ? 0u : (uint32_t)team / nS, ml_c = SINGLE ? 0u : (uint32_t)team % nS;
         for (uint32_t it = team; it < n_items; it += 2) {
@@ -508,9 +515,10 @@ k_search(const __grid_constant__ SearchArgs A)
                 const uint32_t it2 = it + 2;
                 if (it2 < n_items) {
                     mbar_arrive_expect_tx(bar_w, SM::kWarpTile);
-                    bulk_load(wbuf, stream_src(it2, ml_next), SM::kWarpTile, bar_w, SINGLE ? policy_evict_first() : policy_evict_last());
+                    bulk_load(wbuf, SINGLE ? src_run : stream_src(it2, ml_next), SM::kWarpTile, bar_w, SINGLE ? policy_evict_first() : policy_evict_last());
                 }
             }
+            if (SINGLE) src_run += src_step;
             fft16<+1>(v);
             tm_twiddle<1, 8>(tq_a + kTmTheta, v, qa, qb);    // v[p] *= theta^p, p = 1 .. 15
             sts16<8>(xw_a, v);
@@ -519,11 +527,15 @@ k_search(const __grid_constant__ SearchArgs A)
             __syncwarp();
             lds16<136>(xr_a, v);
             if (lane == 0) {
-                const uint64_t pr = (A.j0 + grp + (uint64_t)G * tj) * (uint64_t)A.S + (A.m0 + ml) - A.sig_pair0;
-                float* sp = A.sigpart + pr * (DUAL ? 2 * kSigPart : kSigPart) + b * 8 + warp;
+                float* sp = sp_run;
+                if (!SINGLE) {
+                    const uint64_t pr = (A.j0 + grp + (uint64_t)G * tj) * (uint64_t)A.S + (A.m0 + ml) - A.sig_pair0;
+                    sp = A.sigpart + pr * (DUAL ? 2 * kSigPart : kSigPart) + b * 8 + warp;
+                }
                 sp[0] = sw;
                 if (DUAL) sp[kSigPart] = pw;
             }
+            if (SINGLE) sp_run += sp_step;
             // Ring slot free?  Item it - kRing must have been read out by pass 2 of all 16 CTAs of the group (done2).
             // All lanes load the one counter (a warp-uniform value keeps the warp converged through the wait; a wait
             // taken by lane 0 alone left the warp split in two for the rest of the item, profiles/r2_search_kernel.md); waiting warps
@@ -602,6 +614,8 @@ k_search(const __grid_constant__ SearchArgs A)
             ld_it = it + 2;
         };
         uint32_t tj_c = SINGLE ? 0u : (uint32_t)kb / nS, ml_c = SINGLE ? 0u : (uint32_t)kb % nS;
+        const float* sp_run = A.sigpart + ((A.j0 + grp + (uint64_t)G * kb) * (uint64_t)A.S + A.m0 - A.sig_pair0) * (DUAL ? 2 * kSigPart : kSigPart) + 8 * a;
+        const uint64_t sp_step = (uint64_t)G * 2 * A.S * (DUAL ? 2 * kSigPart : kSigPart);
         for (uint32_t ib = kb; ib < n_items; ib += 2) {
             const int slot = (int)(ib % kRing);
             const uint32_t tj = SINGLE ? ib : tj_c;
@@ -646,7 +660,8 @@ k_search(const __grid_constant__ SearchArgs A)
             lds16<2048>(w0, v);
             const uint64_t pair = (A.j0 + jl) * (uint64_t)A.S + (A.m0 + ml);
             // Parseval partial sums of tile a: 8 warps, fixed order
-            const float4* sp = reinterpret_cast<const float4*>(A.sigpart + (pair - A.sig_pair0) * (DUAL ? 2 * kSigPart : kSigPart) + 8 * a);
+            const float4* sp = reinterpret_cast<const float4*>(SINGLE ? sp_run : A.sigpart + (pair - A.sig_pair0) * (DUAL ? 2 * kSigPart : kSigPart) + 8 * a);
+            if (SINGLE) sp_run += sp_step;
             const float4 s0 = __ldcg(sp), s1 = __ldcg(sp + 1);
             const float part = ((s0.x + s0.y) + (s0.z + s0.w)) + ((s1.x + s1.y) + (s1.z + s1.w));
             float ppart = 0.f;
@@ -658,7 +673,7 @@ k_search(const __grid_constant__ SearchArgs A)
             tmem_ld4(tq + kTmDelta, wa);
             // four-step factor wN^(16 b k1), k1 = a + 16 r: its CTA-uniform part w256^(b r) here, the rest in delta_p
 #pragma unroll
-            for (int r = 1; r < 16; ++r) { const float2 w = c_w256[(b * r) & 255]; v[r] = cmulw(v[r], w.x, w.y); }
+            for (int r = 1; r < 16; ++r) { const float2 w = c_wb[b][r]; v[r] = cmulw(v[r], w.x, w.y); }
             const float sumR2 = row_sum16(part);
             const float sumP = DUAL ? row_sum16(ppart) : 0.f;
             fft16<+1>(v);
@@ -1046,10 +1061,14 @@ extern "C" int bege_plan_create(bege_plan** out, uint32_t N, double fs, double l
         if (cudaMemcpy(p->tw256d, t256.data(), 256 * sizeof(d2), cudaMemcpyHostToDevice) != cudaSuccess) return bail(BEGE_ECUDA);
         if (cudaFuncSetAttribute(k_bank_gen64, cudaFuncAttributeMaxDynamicSharedMemorySize, kBankSmem) != cudaSuccess) return bail(BEGE_ECUDA);
     }
-    {   // exp(2 pi i m / 256) for the search kernel's CTA-uniform twiddles (constant memory of this device's context)
-        std::vector<float2> lin(256);
-        for (int m = 0; m < 256; ++m) lin[m] = make_float2((float)cos(2.0 * M_PI * m / 256.0), (float)sin(2.0 * M_PI * m / 256.0));
-        if (cudaMemcpyToSymbol(c_w256, lin.data(), sizeof(float2) * 256) != cudaSuccess) return bail(BEGE_ECUDA);
+    {   // exp(2 pi i b r / 256) for the search kernel's CTA-uniform twiddles (constant memory of this device's context)
+        std::vector<float2> tb(256);
+        for (int bb = 0; bb < 16; ++bb)
+            for (int r = 0; r < 16; ++r) {
+                const double a = 2.0 * M_PI * (double)((bb * r) & 255) / 256.0;
+                tb[bb * 16 + r] = make_float2((float)cos(a), (float)sin(a));
+            }
+        if (cudaMemcpyToSymbol(c_wb, tb.data(), sizeof(float2) * 256) != cudaSuccess) return bail(BEGE_ECUDA);
     }
     if (cudaMalloc(&p->tw256, w256.size() * sizeof(float2)) != cudaSuccess ||
         cudaMalloc(&p->twN, wN.size() * sizeof(float2)) != cudaSuccess) return bail(BEGE_ENOMEM);
