@@ -50,6 +50,7 @@ ALG_BYTES_PER_CORR = 52802 * 8                    # two-sided in-ba
 NCU_DRAM_BYTES_PER_CORR = (16.913e9 + 0.024e9) / 36864
 NCU_SOURCE = "profiles/r2_search_kernel.md"
 FP32_PEAK = 148 * 128 * 2 * 1.965e9               # SMs x fp32 lanes x 2 flop x max SM clock
+FMA_PIPE_CEILING = 8.6e6                          # what the FMA pipe allows for k_search's instruction mix
 
 
 # ------------------------------------------------------------------------------------------ clocks
@@ -514,6 +515,9 @@ def run_ours(args, rank, world, local_rank):
                                f"{pst['fused_kernel_launches']} launches (slices of one search) over {kern_corr} correlations",
                      "peak_source": "derived: 148 SM x 128 fp32 lanes x 2 x 1.965 GHz (DESIGN.md); "
                                     "flops = 5 N log2 N per correlation (PAPER.md:134)",
+                     "fma_pipe": {"ceiling_corr_per_s": FMA_PIPE_CEILING, "frac": rate_kernel / FMA_PIPE_CEILING,
+                                  "note": "context: ~1,000 FMA-pipe cycles per 32 lags x 16 row pairs of this radix-16 arithmetic "
+                                          "(packed f32x2 = 2 cycles; profiles/r2_search_kernel.md); not the roofline denominator"},
                      "hbm": {"achieved": hbm_achieved, "peak": hbm_peak, "unit": "GB/s",
                              "frac": hbm_achieved / hbm_peak, "of": "measured" if peaks else "fallback",
                              "stored_bytes_per_template": tpl_bytes}},
