@@ -309,6 +309,39 @@ def _extra_workloads(args, dev, local_rank):
     del x_host
     torch.cuda.empty_cache()
 
+    # ---- the paper's own output forms on the configs[1]-sized bank: max projection over the
+    # bank, and the dual-stream search (x = H1 + i L1, real templates: two detector correlations per complex one)
+    f0g, fdg = synth.bank_grid(256, 256, 350.0, 2000.0, -400.0, 400.0)
+    xd = (synth.band_limit(synth.white_noise(200)) + 1j * synth.band_limit(synth.white_noise(201))).astype(np.complex64)[None, :]
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def timed_call(fn, reps):
+        ms = []
+        for i in range(reps + 1):
+            torch.cuda.synchronize(dev)
+            ev0.record(); r = fn(); ev1.record()
+            torch.cuda.synchronize(dev)
+            if i:
+                ms.append(ev0.elapsed_time(ev1))
+        return float(np.median(ms)), r
+
+    with bege.Plan(synth.N_SEG, synth.FS, synth.BAND, device=local_rank) as plan:
+        plan.bank_generate(f0g, fdg, synth.TAU)
+        plan.segment_load(np.ascontiguousarray(xd.real.astype(np.complex64)))
+        ms, r = timed_call(lambda: plan.search_maxproj(3.5), args.extra_reps)
+        out["max_projection"] = {"workload": "256x256 bank x 1 segment, k = 3.5: per sample offset the largest |z|/sigma over the "
+                                 "bank and its template (PAPER.md:166-191)", "T": int(f0g.size), "corr_per_s": f0g.size / (ms * 1e-3),
+                                 "n_offsets_hit": int(r[2]), "d2h_bytes": int(synth.N_SEG * 8),
+                                 "note": "events around bege_search_maxproj, including the D2H of the two N-entry arrays"}
+        plan.bank_generate_real(f0g, fdg, synth.TAU)
+        plan.segment_load(xd)
+        ms, r = timed_call(lambda: plan.search_dual(5.0, 50.0), args.extra_reps)
+        out["dual_stream"] = {"workload": "256x256 bank of REAL templates x 1 segment H1 + i L1, k = 5 (PAPER.md:155, :221)",
+                              "T": int(f0g.size), "corr_per_s": f0g.size / (ms * 1e-3),
+                              "detector_correlations_per_s": 2 * f0g.size / (ms * 1e-3),
+                              "n_simultaneous": int(r[4]), "n_coincident": int(r[5]), "d2h_bytes": int(2 * synth.N_SEG * 8),
+                              "note": "events around bege_search_dual, including the D2H of the four N-entry arrays"}
+
     # ---- configs[4]: 2^18 templates, k = 3: ~6e7 records (0.7 GB) must cross PCIe without holding up the search
     w = synth.config4()
     x_host = torch.from_numpy(w.x).pin_memory()
