@@ -202,12 +202,13 @@ k_fwd_cols(const c2* __restrict__ G, c2* __restrict__ out, uint64_t out_stride, 
 //
 // Hand-over between the passes (PTX memory model): per group and ring slot two monotone counters.
 //   done1 (tiles in the ring): each warp of an A team arrives on the CTA's mbarrier amb[slot] after its ring stores.
-//              Thread 0 of the B team of the same item parity -- the team's service thread, which idles in a wait
-//              loop whenever pass 2 is ahead -- sees the phase complete, executes ONE fence.acq_rel.gpu and adds 1 to
-//              done1[slot] (the gpu-scope fence takes about a microsecond while the SM has stores in flight; on a
-//              pass-1 warp it would stall that warp's item).
-//              The same thread waits with ld.acquire.gpu until all 16 tiles of its team's item have been added, then
-//              issues the tensor copy of the rows.
+//              The warp whose arrival completes the phase (it sees so with a test_wait right after) executes ONE
+//              fence.acq_rel.gpu and adds 1 to done1[slot] -- pass 1 has the time for the microsecond the gpu-scope
+//              fence takes, it is the side that waits for ring slots; a publication cursor in shared memory, claimed by
+//              CAS, keeps every tile published exactly once (thread 0 of the B team of the same item parity publishes
+//              whatever it finds unpublished in its wait loop and after its last item).
+//              That B thread -- the team's service thread -- waits with ld.acquire.gpu until all 16 tiles of its team's
+//              item have been added, then issues the tensor copy of the rows.
 //   done2 (ring slot read out): as soon as that copy has landed (mbarrier), a thread of the B team adds 1 to
 //              done2[slot] under the same kind of fence.  Every A warp acquires 16 of them just before its ring stores
 //              (all lanes load the one counter, so the warp stays converged; 2 us between probes while waiting).
@@ -555,7 +556,23 @@ k_search(const __grid_constant__ SearchArgs A)
             }
             // this warp's part of the tile is on its way: tell the publisher (thread 0 of the B team of the same parity)
             __syncwarp();
-            if (lane == 0) mbar_arrive(sb + SM::amb + 8 * slot);
+            if (lane == 0) {
+                mbar_arrive(sb + SM::amb + 8 * slot);
+                // the warp that completes the tile publishes it right away (pass 1 has the time: it is the one that waits
+                // for ring slots; left to pass 2's service thread the publication sat for microseconds, and the ring's
+                // round trip -- not the arithmetic -- set the pace)
+                if (!(BEGE_ABL & (1 | 16)) && mbar_test_wait(sb + SM::amb + 8 * slot, (it / kRing) & 1)) {
+                    uint32_t* const pub_it = reinterpret_cast<uint32_t*>(smem_raw + SM::pubit) + team;
+                    const uint32_t first = *(volatile uint32_t*)pub_it;
+                    uint32_t n = 0;
+                    while (n < 4 && first + 2 * n < n_items &&
+                           mbar_test_wait(sb + SM::amb + 8 * ((first + 2 * n) % kRing), ((first + 2 * n) / kRing) & 1)) ++n;
+                    if (n && atomicCAS(pub_it, first, first + 2 * n) == first) {
+                        fence_acq_rel_gpu();
+                        for (uint32_t i = 0; i < n; ++i) counter_add_relaxed(d1 + (first + 2 * i) % kRing, 1ull);
+                    }
+                }
+            }
         }
     } else if (team >= 2 && !(BEGE_ABL & 32)) {
         // ================================================================ B: pass 2, items ib = team - 2 (mod 2)
