@@ -46,8 +46,8 @@ FFT_FLOP = 5.0 * 65536 * 16                       # PAPER.md:134 eq.(10): 5 N lo
 ALG_BYTES_PER_CORR = 52802 * 8                    # two-sided in-band template spectrum, S = 1
 # dram__bytes_read.sum + dram__bytes_write.sum of k_search per correlation: an OFFLINE constant, taken from the
 # `ncu --set full` capture of the kernel as committed (profiles/r2_search_kernel.md: 36,864-template launch,
-# 16.913 GB read + 0.024 GB written); it does not follow later kernel changes by itself.
-NCU_DRAM_BYTES_PER_CORR = (16.913e9 + 0.024e9) / 36864
+# 16.914 GB read + 0.024 GB written); it does not follow later kernel changes by itself.
+NCU_DRAM_BYTES_PER_CORR = (16.914e9 + 0.024e9) / 36864
 NCU_SOURCE = "profiles/r2_search_kernel.md"
 FP32_PEAK = 148 * 128 * 2 * 1.965e9               # SMs x fp32 lanes x 2 flop x max SM clock
 FMA_PIPE_CEILING = 8.6e6                          # what the FMA pipe allows for k_search's instruction mix
