@@ -78,8 +78,8 @@ k_bank_gen64(const double* __restrict__ f0, const double* __restrict__ fdot, uin
     __shared__ double red[8];
     extern __shared__ __align__(16) unsigned char bank64_smem[];
     d2* base = reinterpret_cast<d2*>(bank64_smem);          // [nh][nl]
-    d2* bufA = base + 4096;                                  // [m1][l0][l1 ^ l0]
-    d2* bufB = bufA + 4096;                                  // [m1][l0][q0 ^ l0]
+    // two exchange buffers alternate over r ([m1][l0][l1 ^ l0] after S1); S2 rewrites its own row in place ([m1][l0][q0 ^ l0])
+    d2* const buf0 = base + 4096;
     const int t = threadIdx.x;
     const int l0 = t & 15, l1 = t >> 4;                      // S1: nl = t = l0 + 16 l1
     const int m1 = t >> 4;                                   // S2: (m1, l0);  S3: (m1, q0 = l0)
@@ -125,6 +125,7 @@ k_bank_gen64(const double* __restrict__ f0, const double* __restrict__ fdot, uin
         d2 rho_r = dmk(1.0, 0.0);                            // rho^r
         float4* o = reinterpret_cast<float4*>(out + j * out_stride);
         for (int r = 0; r < 16; ++r) {
+            d2* const buf = buf0 + 4096 * (r & 1);
             d2 v[16];
             // ---- S1
 #pragma unroll
@@ -137,25 +138,29 @@ k_bank_gen64(const double* __restrict__ f0, const double* __restrict__ fdot, uin
                 d2 w = rho_r;
 #pragma unroll
                 for (int mm = 0; mm < 16; ++mm) {
-                    bufA[mm * 256 + l0 * 16 + (l1 ^ l0)] = dmul(v[mm], w.x, w.y);
+                    buf[mm * 256 + l0 * 16 + (l1 ^ l0)] = dmul(v[mm], w.x, w.y);
                     w = dmul(w, rho16.x, rho16.y);
                 }
             }
             rho_r = dmul(rho_r, rho.x, rho.y);
             __syncthreads();
-            // ---- S2: thread (m1, l0)
+            // ---- S2: thread (m1, l0), in place on the row it has read
 #pragma unroll
-            for (int k = 0; k < 16; ++k) v[k] = bufA[m1 * 256 + l0 * 16 + (k ^ l0)];
+            for (int k = 0; k < 16; ++k) v[k] = buf[m1 * 256 + l0 * 16 + (k ^ l0)];
             dfft16f(v);
 #pragma unroll
             for (int q0 = 0; q0 < 16; ++q0) {
                 const d2 w = tw256d[(l0 * q0) & 255];
-                bufB[m1 * 256 + l0 * 16 + (q0 ^ l0)] = dmul(v[q0], w.x, -w.y);
+                buf[m1 * 256 + l0 * 16 + (q0 ^ l0)] = dmul(v[q0], w.x, -w.y);
             }
-            __syncthreads();
+            // S3 of thread (m1, q0) reads what the 16 threads (m1, .) -- its own half-warp -- have written: no CTA barrier.
+            // The buffer of r is written again by S1 of r + 2, after the barrier of r + 1, which every warp reaches only
+            // after its S3 of r: one CTA barrier per transform, and the warps are free to drift between them (fp64
+            // arithmetic and shared-memory exchanges of different warps then overlap).
+            __syncwarp();
             // ---- S3: thread (m1, q0 = l0)
 #pragma unroll
-            for (int k = 0; k < 16; ++k) v[k] = bufB[m1 * 256 + k * 16 + (l0 ^ k)];
+            for (int k = 0; k < 16; ++k) v[k] = buf[m1 * 256 + k * 16 + (l0 ^ k)];
             dfft16f(v);
             // v[q1] = H[k], k = (16 m1 + r) + 256 (q0 + 16 q1): tile m1, thread 16 r + q0, row-block q1 (stored in pairs)
             float4* ot = o + tile_word(NI, m1, 0, 16 * r + l0);       // + 32 ip
