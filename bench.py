@@ -535,7 +535,7 @@ def run_ours(args, rank, world, local_rank):
                 "d2h_bytes_per_step": acc["d2h"] // args.steps,
                 "what": "per chunk: bege_segment_load from pinned host memory + bege_search into pinned host memory"},
         "gpu_launches": int(acc["launches"]),
-        "gpu_launches_note": "kernels of libbege.so launched inside the timed calls (per chunk: 2 segment-load kernels + "
+        "gpu_launches_note": "kernels of libbege.so launched inside the timed calls (per chunk: 3 segment-load kernels + "
                              "the persistent search kernel, up to 8 launches = slices); the untimed bank generation "
                              "launched %d more" % (int(st["kernel_launches"]) - int(acc["launches"])),
         "clocks": sampler.summary(windows),
