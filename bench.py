@@ -58,7 +58,7 @@ class ClockSampler:
     """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
-         "clocks_event_reasons.sw_power_cap")
+         "clocks_event_reasons.sw_power_cap,clocks.mem")
 
     def __init__(self, index: int):
         self.index, self.rows, self.proc, self.thr = index, [], None, None
@@ -86,7 +86,7 @@ class ClockSampler:
                 self.proc.kill()
 
     def summary(self, windows):
-        sm, smax, reasons, power = [], 0.0, set(), 0.0
+        sm, smax, reasons, power, mem = [], 0.0, set(), 0.0, []
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for ts, line in self.rows:
             if not any(a <= ts <= b for a, b in windows):
@@ -99,8 +99,13 @@ class ClockSampler:
             for nm, v in zip(names, f[3:7]):
                 if v.lower().startswith("active"):
                     reasons.add(nm)
+            try:
+                mem.append(float(f[7]))
+            except (ValueError, IndexError):
+                pass
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": smax or None,
-                "reasons": sorted(reasons), "samples": len(sm), "power_w_max": power or None}
+                "reasons": sorted(reasons), "samples": len(sm), "power_w_max": power or None,
+                "mem_mhz": float(np.median(mem)) if mem else None}
 
 
 # ------------------------------------------------------------------------------------------ oracle arm
