@@ -190,6 +190,48 @@ int bege_debug_set_max_items(bege_plan*, uint64_t max_items);
 int bege_ovs_probe(int device, uint64_t n_templates, uint32_t n_blocks, uint32_t reps, float thr2, const float* h16,
                    const float* x16, float* z_dbg, uint64_t dbg_j, double* ms_out, uint64_t* hits_out);
 
+/*
+ * Segment spectra WITHOUT any device allocation (a2, PAPER.md:155 step i; four-step transform as PAPER.md:201-203
+ * describes for lengths beyond one work-group's local memory).
+ *
+ * Who needs this: every other call of this library obtains device memory, either by cudaMalloc or from a workspace the
+ * caller had to allocate first.  Some callers cannot do either at the moment they need a spectrum:
+ *   - a data-acquisition or low-latency loop, where cudaMalloc / cudaFree are off limits because they synchronise the
+ *     whole device and take a driver lock of unbounded duration while other streams are feeding the GPU;
+ *   - a process in which another component has already claimed (nearly) all of HBM -- e.g. a framework's caching pool, or
+ *     this library's own bank chunk sized to fill the card -- so that a fresh allocation may simply fail;
+ *   - code running under a "no allocation after start-up" rule (fixed memory budgets of a production pipeline).
+ * For them this ONE entry point keeps what it needs inside the library image itself: the staging area between the two
+ * kernels of the transform and its twiddle tables are file-scope __device__ arrays, 2.5 MiB in total, resident on every GPU
+ * that loads the library until the process exits.  The call creates no plan, takes no workspace and calls no cudaMalloc,
+ * cudaFree or any other allocating routine.
+ *
+ * Computes, for m < n_segments:  X_m = DFT_N(x_m), N = 65536, bins outside band_lo_hz <= |f| <= band_hi_hz set to zero
+ * (same band rule, same kernels for the row pass and the same arithmetic as bege_segment_load), and writes them in NATURAL
+ * bin order: X_out[(m*N + k)*2 + {0,1}] = Re, Im of X_m[k].
+ *   device        CUDA ordinal (made current on the calling thread, as in every other call).
+ *   cuda_stream   a cudaStream_t on that device; NULL = the legacy default stream.  The work is ENQUEUED on it and the
+ *                 call returns without waiting: X_out is complete when the stream has reached that point.
+ *   x_dev_c64     DEVICE memory, n_segments*N complex fp32 interleaved; produced on cuda_stream or already complete.
+ *   X_out_dev_c64 DEVICE memory, same size, caller-owned, must not overlap x_dev_c64.
+ *   n_segments    1 .. BEGE_STATIC_MAX_SEGMENTS.  More is refused with BEGE_EINVAL (the staging array has a fixed size);
+ *                 split the batch or use a plan.
+ *   errbuf        optional (may be NULL): receives a NUL-terminated description of any failure, at most errbuf_len bytes.
+ * Returns BEGE_OK, BEGE_EINVAL (arguments, host pointers, size limit) or BEGE_ECUDA (no sm_100 device, runtime error).
+ *
+ * First call on a device: it looks up the device addresses of the built-in arrays, fills the twiddle tables with a small
+ * kernel and WAITS for cuda_stream once (later calls do not wait).  Make that first call during start-up, before the
+ * stream is put into capture mode and before timing anything.
+ * Sharing: all calls on a device use the same staging array, from any thread and any stream, and nothing locks it on the
+ * GPU.  Two calls whose kernels can run at the same time (different streams with no ordering between them) overwrite each
+ * other's staging data and return garbage; calls on one stream, or ordered by events, are safe.  The array keeps whatever the
+ * last call left there; no part of it needs clearing, because every call rewrites all the words it later reads.
+ */
+#define BEGE_STATIC_MAX_SEGMENTS 4
+int bege_segment_spectrum_static(int device, void* cuda_stream, double fs, double band_lo_hz, double band_hi_hz,
+                                 const float* x_dev_c64, uint32_t n_segments, float* X_out_dev_c64,
+                                 char* errbuf, uint64_t errbuf_len);
+
 int  bege_plan_set_profiling(bege_plan*, int on);    /* CUDA events around the dominant kernel (adds syncs) */
 int  bege_plan_get_stats(const bege_plan*, bege_stats* out);
 int  bege_plan_reset_stats(bege_plan*);

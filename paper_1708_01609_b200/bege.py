@@ -28,7 +28,9 @@ SYMBOLS = [
     "bege_bank_generate_real", "bege_search_dual", "bege_get_sigma_dual",
     "bege_debug_template_spectrum", "bege_debug_segment_spectrum", "bege_debug_set_max_items", "bege_plan_set_profiling",
     "bege_plan_get_stats", "bege_plan_reset_stats", "bege_last_error", "bege_plan_destroy", "bege_version", "bege_ovs_probe",
+    "bege_segment_spectrum_static",
 ]
+STATIC_MAX_SEGMENTS = 4           # BEGE_STATIC_MAX_SEGMENTS (include/bege.h)
 
 
 class BegeError(RuntimeError):
@@ -73,6 +75,7 @@ def load_library() -> ctypes.CDLL:
     L.bege_debug_segment_spectrum.argtypes = [vp, u32, vp]
     L.bege_debug_set_max_items.argtypes = [vp, u64]
     L.bege_ovs_probe.argtypes = [i32, u64, u32, u32, ctypes.c_float, vp, vp, vp, u64, ctypes.POINTER(dbl), ctypes.POINTER(u64)]
+    L.bege_segment_spectrum_static.argtypes = [i32, vp, dbl, dbl, dbl, vp, u32, vp, ctypes.c_char_p, u64]
     L.bege_plan_set_profiling.argtypes = [vp, i32]
     L.bege_plan_get_stats.argtypes = [vp, ctypes.POINTER(Stats)]
     L.bege_plan_reset_stats.argtypes = [vp]
@@ -307,6 +310,38 @@ def ovs_probe(n_templates: int, n_blocks: int = 6, reps: int = 3, thr2: float = 
     if rc != OK:
         raise BegeError(rc, "bege_ovs_probe failed")
     return ms.value, hits.value, z
+
+
+def segment_spectrum_static(x, fs: float = 4096.0, band=(350.0, 2000.0), out=None, stream: int | None = None):
+    """bege_segment_spectrum_static (include/bege.h): band-limited spectra of up to STATIC_MAX_SEGMENTS segments with
+    no device allocation inside the library -- for callers that may not call cudaMalloc when the spectrum is needed
+    (latency-critical loops, processes whose HBM is already fully claimed, fixed-memory-budget pipelines).  The
+    transform's staging area and tables are arrays built into libbege.so.
+
+    x: torch CUDA tensor, complex64, (S, 65536) contiguous, S <= STATIC_MAX_SEGMENTS.  out: a tensor of the same shape to
+    receive the spectra in natural bin order; pass one you made earlier if torch must not allocate either (None: a new
+    tensor from torch's allocator).  The work is queued on `stream` (default: torch's current stream on x's device) and
+    this returns without waiting.  All calls on a device share the built-in staging array: keep them on one stream or
+    order them with events, unordered concurrent calls corrupt each other.  The first call on a device also does the
+    one-time set-up and waits for the stream once; make it at start-up.  Raises BegeError with the library's message
+    (e.g. when S exceeds the limit)."""
+    import torch
+
+    L = load_library()
+    assert x.is_cuda and x.dtype == torch.complex64 and x.is_contiguous() and x.dim() == 2
+    S, dev = int(x.shape[0]), x.device.index
+    if out is None:
+        out = torch.empty_like(x)
+    assert out.is_cuda and out.dtype == torch.complex64 and out.is_contiguous() and out.shape == x.shape and out.device == x.device
+    if stream is None:
+        stream = torch.cuda.current_stream(dev).cuda_stream
+    err = ctypes.create_string_buffer(256)
+    rc = L.bege_segment_spectrum_static(dev, ctypes.c_void_p(stream or CUDA_STREAM_LEGACY), float(fs), float(band[0]),
+                                        float(band[1]), ctypes.c_void_p(x.data_ptr()), S, ctypes.c_void_p(out.data_ptr()),
+                                        err, len(err))
+    if rc != OK:
+        raise BegeError(rc, err.value.decode())
+    return out
 
 
 def version() -> str:

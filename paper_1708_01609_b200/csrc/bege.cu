@@ -20,6 +20,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -1677,6 +1678,159 @@ extern "C" int bege_plan_reset_stats(bege_plan* p)
     if (!p) return BEGE_EINVAL;
     const uint64_t keep = p->stats.hbm_bytes_per_template;
     p->stats = bege_stats{}; p->stats.hbm_bytes_per_template = keep;
+    return BEGE_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// bege_segment_spectrum_static: the band-limited forward transform of a few segments (a2, PAPER.md:155 step i) for
+// callers that must not allocate device memory -- no plan, no workspace, no cudaMalloc / cudaFree anywhere below.
+//
+// The four-step transform needs somewhere to keep the row transforms G between its two kernels, and its twiddle
+// tables.  bege_segment_load takes both from the plan's (allocated) memory; here they live in the three file-scope
+// __device__ arrays that follow.  They are part of the library image, so every GPU on which the library is used
+// carries them (2.5 MiB) from the moment the module is loaded there until the process exits.
+//
+// In host code the NAMES of these arrays are host-side shadow symbols, not device addresses, and must never be handed
+// to a kernel.  static_setup() asks the runtime for the real addresses (cudaGetSymbolAddress, once per device, with that
+// device current) and only those go into launches.
+constexpr uint32_t kStaticMaxSeg = BEGE_STATIC_MAX_SEGMENTS;
+static __device__ __align__(256) c2     g_static_G[(size_t)kStaticMaxSeg * kN];   // step A -> step B staging, 2 MiB
+static __device__ __align__(256) float2 g_static_tw256[256];                      // exp(2 pi i g p / 256) at [16 p + g]
+static __device__ __align__(256) float2 g_static_twN[kN];                         // exp(2 pi i nl k1 / N) at [256 nl + k1]
+
+// fills the two twiddle tables in place (fp64 angles in units of pi, one rounding to fp32 -- the plan's tables are made
+// the same way on the host).  Device code may name the arrays directly.  grid 256, 256 thr.
+__global__ void __launch_bounds__(256) k_static_tables()
+{
+    const int t = threadIdx.x, r = blockIdx.x;
+    double s, c;
+    sincospi(2.0 * (double)(r * t) / (double)kN, &s, &c);
+    g_static_twN[r * 256 + t] = make_float2((float)c, (float)s);
+    if (r == 0) {
+        sincospi(2.0 * (double)((t >> 4) * (t & 15)) / 256.0, &s, &c);
+        g_static_tw256[t] = make_float2((float)c, (float)s);
+    }
+}
+
+// step B of the forward transform as in k_fwd_cols<true>, but the masked spectrum leaves in NATURAL order
+// (out[m N + k], all 16 row-blocks) so that the caller needs to know nothing of the tile layout.  The 16 columns of a
+// tile are 16 consecutive bins of every row k2: the results go through shared memory once more so that each half-warp
+// stores one full 128-byte line.  grid (16 tiles, n_segments), 256 thr.
+__global__ void __launch_bounds__(256)
+k_fwd_cols_natural(const c2* __restrict__ G, c2* __restrict__ out, const float2* __restrict__ tw256, uint32_t klo, uint32_t khi)
+{
+    __shared__ c2 sm[256 * 17];                    // first the 16 private 256-word exchange regions, then [k2][c] padded to 17
+    const int t = threadIdx.x, b = blockIdx.x;
+    const uint64_t m = blockIdx.y;
+    const int c = t >> 4, g = t & 15;
+    float2 w1[16];
+    load_w1(w1, tw256, g);
+    const c2* in = G + m * (uint64_t)kN + (uint64_t)b * 4096;
+    c2 v[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) v[i] = in[(i * 16 + c) * 16 + g];
+    hw_fft256<-1>(v, w1, sm + c * 256, g);         // lane g now holds X[k1 + 256 k2], k1 = 16 b + c, k2 = g + 16 q, in v[q]
+    __syncthreads();                               // every half-warp is done with its exchange region
+    const uint32_t k1 = 16 * b + c;
+#pragma unroll
+    for (int q = 0; q < 16; ++q) {
+        const uint32_t k = k1 + 256u * (uint32_t)(g + 16 * q);
+        const uint32_t kk = k < (uint32_t)kN / 2 ? k : (uint32_t)kN - k;
+        sm[(g + 16 * q) * 17 + c] = (kk < klo || kk > khi) ? mk(0.f, 0.f) : v[q];
+    }
+    __syncthreads();
+    c2* o = out + m * (uint64_t)kN + 16 * b;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        const int k2 = 16 * i + c;                 // here the half-warp index picks the row and the lane the column
+        o[256 * k2 + g] = sm[k2 * 17 + g];
+    }
+}
+
+namespace {
+struct StaticDev { bool ready = false; c2* G = nullptr; float2 *tw256 = nullptr, *twN = nullptr; };
+constexpr int kStaticMaxDev = 64;
+StaticDev g_static_dev[kStaticMaxDev];
+std::mutex g_static_mu;
+
+int static_fail(char* errbuf, uint64_t errbuf_len, int code, const char* fmt, ...)
+{
+    if (errbuf && errbuf_len) {
+        va_list ap; va_start(ap, fmt); vsnprintf(errbuf, (size_t)errbuf_len, fmt, ap); va_end(ap);
+    }
+    return code;
+}
+
+// One-time set-up of `device` (already current): resolve the device addresses of the static arrays, fill the tables,
+// wait for that to finish.  Returns a cudaError_t and the name of the step that failed.
+cudaError_t static_setup(StaticDev& d, cudaStream_t st, const char** what)
+{
+    cudaError_t e;
+    *what = "cudaGetSymbolAddress(g_static_G)";
+    if ((e = cudaGetSymbolAddress((void**)&d.G, g_static_G)) != cudaSuccess) return e;
+    *what = "cudaGetSymbolAddress(g_static_tw256)";
+    if ((e = cudaGetSymbolAddress((void**)&d.tw256, g_static_tw256)) != cudaSuccess) return e;
+    *what = "cudaGetSymbolAddress(g_static_twN)";
+    if ((e = cudaGetSymbolAddress((void**)&d.twN, g_static_twN)) != cudaSuccess) return e;
+    *what = "k_static_tables";
+    k_static_tables<<<256, 256, 0, st>>>();
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    *what = "cudaStreamSynchronize (set-up)";
+    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return e;   // later calls may come on other streams
+    d.ready = true;
+    return cudaSuccess;
+}
+}  // namespace
+
+extern "C" int bege_segment_spectrum_static(int device, void* cuda_stream, double fs, double lo, double hi, const float* x_dev,
+                                            uint32_t n_segments, float* X_out_dev, char* errbuf, uint64_t errbuf_len)
+{
+    if (errbuf && errbuf_len) errbuf[0] = 0;
+    // argument checks first: none of them needs a device
+    if (!(fs > 0) || !(lo > 0) || !(hi > lo) || !(hi < 0.5 * fs))
+        return static_fail(errbuf, errbuf_len, BEGE_EINVAL, "band must satisfy 0 < band_lo_hz < band_hi_hz < fs/2");
+    if (n_segments == 0) return static_fail(errbuf, errbuf_len, BEGE_EINVAL, "n_segments is 0");
+    if (n_segments > kStaticMaxSeg)
+        return static_fail(errbuf, errbuf_len, BEGE_EINVAL,
+                           "n_segments = %u exceeds BEGE_STATIC_MAX_SEGMENTS = %u: the built-in staging array holds no more; "
+                           "split the call or use a plan (bege_segment_load)", n_segments, kStaticMaxSeg);
+    if (!x_dev || !X_out_dev) return static_fail(errbuf, errbuf_len, BEGE_EINVAL, "x_dev_c64 / X_out_dev_c64 is NULL");
+    if (x_dev == X_out_dev) return static_fail(errbuf, errbuf_len, BEGE_EINVAL, "in-place transform is not supported");
+    if (device < 0 || device >= kStaticMaxDev) return static_fail(errbuf, errbuf_len, BEGE_EINVAL, "device %d outside [0, %d)", device, kStaticMaxDev);
+#define CUS(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { cudaGetLastError(); \
+        return static_fail(errbuf, errbuf_len, BEGE_ECUDA, "%s: %s", #call, cudaGetErrorString(e_)); } } while (0)
+    CUS(cudaSetDevice(device));
+    for (const void* ptr : {(const void*)x_dev, (const void*)X_out_dev}) {
+        cudaPointerAttributes at;
+        if (cudaPointerGetAttributes(&at, ptr) != cudaSuccess || !(at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged)) {
+            cudaGetLastError();
+            return static_fail(errbuf, errbuf_len, BEGE_EINVAL, "%s must be device memory", ptr == (const void*)x_dev ? "x_dev_c64" : "X_out_dev_c64");
+        }
+    }
+    cudaStream_t st = cuda_stream ? (cudaStream_t)cuda_stream : cudaStreamLegacy;
+    StaticDev d;
+    {
+        std::lock_guard<std::mutex> lk(g_static_mu);
+        StaticDev& slot = g_static_dev[device];
+        if (!slot.ready) {
+            int major = 0;
+            CUS(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, device));
+            if (major < 10) return static_fail(errbuf, errbuf_len, BEGE_ECUDA, "device %d is sm_%d0; the library holds sm_100a code only", device, major);
+            const char* what = "";
+            const cudaError_t e = static_setup(slot, st, &what);
+            if (e != cudaSuccess) { cudaGetLastError(); return static_fail(errbuf, errbuf_len, BEGE_ECUDA, "set-up of device %d, %s: %s", device, what, cudaGetErrorString(e)); }
+        }
+        d = slot;
+    }
+    // band in bins exactly as bege_plan_create computes it (inclusive edges)
+    const double df = fs / kN;
+    const uint32_t klo = (uint32_t)ceil(lo / df - 1e-9), khi = (uint32_t)floor(hi / df + 1e-9);
+    // Nothing in G has to start at zero: step A writes all N words of each of the n_segments slots it is given before
+    // step B (same stream) reads them, and slots beyond n_segments are not read.
+    k_fwd_rows_data<<<dim3(16, n_segments), 256, 0, st>>>((const c2*)x_dev, d.tw256, d.twN, d.G);
+    k_fwd_cols_natural<<<dim3(16, n_segments), 256, 0, st>>>(d.G, (c2*)X_out_dev, d.tw256, klo, khi);
+    CUS(cudaGetLastError());
+#undef CUS
     return BEGE_OK;
 }
 
