@@ -51,6 +51,11 @@ NCU_DRAM_BYTES_PER_CORR = (16.914e9 + 0.024e9) / 36864
 NCU_SOURCE = "profiles/r2_search_kernel.md"
 FP32_PEAK = 148 * 128 * 2 * 1.965e9               # SMs x fp32 lanes x 2 flop x max SM clock
 FMA_PIPE_CEILING = 8.6e6                          # what the FMA pipe allows for k_search's instruction mix
+# ncu figures of k_search from the same capture (north_star: "ncu dram throughput and FP32 pipe utilisation shown"):
+# OFFLINE constants like the traffic above, percent of peak sustained over the kernel's duration
+NCU_OFFLINE = {"source": NCU_SOURCE, "pipe_fmaheavy_pct": 55.9, "issue_slots_pct": 58.4, "lsu_wavefronts_pct": 66.7,
+               "dram_throughput_gbs": (16.914e9 + 0.024e9) / 7.614e-3 * 1e-9, "warps_active_pct": 50.0,
+               "note": "measured under ncu (serialised, cold cache) on the build named in source; not re-measured in this run"}
 
 
 # ------------------------------------------------------------------------------------------ clocks
@@ -475,17 +480,19 @@ def run_ours(args, rank, world, local_rank):
     kern_s = pst["fused_kernel_ms"] * 1e-3
     kern_corr = b - a
 
-    times = torch.tensor([acc["search_ms"] * 1e-3, acc["e2e_s"]], dtype=torch.float64, device=dev if dev else "cpu")
+    times = torch.tensor([acc["search_ms"] * 1e-3, acc["e2e_s"], acc["e2e_s"] + acc["gen_s"]], dtype=torch.float64,
+                         device=dev if dev else "cpu")
     gathered = None
     if world > 1:
         dist.all_reduce(times, op=dist.ReduceOp.MAX)
         # the only exchange of the path: the (rare) tail records of every rank's last pass, concatenated on rank 0
         mine = np.concatenate(last_tails) if last_tails else np.zeros(0, dtype=bege.TAIL_DTYPE)
         gathered = shard.gather_tails(mine)
-    t_search, t_e2e = float(times[0]), float(times[1])
+    t_search, t_e2e, t_e2e_gen = float(times[0]), float(times[1]), float(times[2])
     total_corr = T_total * world * args.steps
     value = total_corr / t_search
     e2e = total_corr / t_e2e
+    e2e_gen = total_corr / t_e2e_gen
     plan.close()
     if rank != 0:
         return
@@ -519,7 +526,10 @@ def run_ours(args, rank, world, local_rank):
     if world == 1 and not args.no_cpu_baseline:
         v, used, dt, _ = oracle_rate(f0, fdot, x_np, k_sigma, args.cpu_sample)
         cpu = {"value": v, "unit": UNIT, "cores": used, "kind": "oracle",
-               "sample": f"{args.cpu_sample} templates strided over the 2^20 bank x 1 segment ({dt:.1f} s)"}
+               "sample": f"{args.cpu_sample} templates strided over the 2^20 bank x 1 segment ({dt:.1f} s)",
+               "includes": "template generation + forward transform of every template inside the timed loop: the like-for-"
+                           "like GPU figure is e2e_incl_generation, not value or e2e",
+               "gpu_over_cpu_like_for_like": e2e_gen / v}
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * t_search / args.steps, "higher_is_better": True,
@@ -539,6 +549,9 @@ def run_ours(args, rank, world, local_rank):
         "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": acc["h2d"] // args.steps,
                 "d2h_bytes_per_step": acc["d2h"] // args.steps,
                 "what": "per chunk: bege_segment_load from pinned host memory + bege_search into pinned host memory"},
+        "e2e_incl_generation": {"value": e2e_gen, "unit": UNIT,
+                                "what": "as e2e, plus bege_bank_generate of every chunk (the 2^20-template bank exceeds HBM and "
+                                        "is regenerated on every pass): wall time of generation + segment_load + search"},
         "gpu_launches": int(acc["launches"]),
         "gpu_launches_note": "kernels of libbege.so launched inside the timed calls (per chunk: 3 segment-load kernels + "
                              "the persistent search kernel, up to 8 launches = slices); the untimed bank generation "
@@ -553,6 +566,7 @@ def run_ours(args, rank, world, local_rank):
                                f"{pst['fused_kernel_launches']} launches (slices of one search) over {kern_corr} correlations",
                      "peak_source": "derived: 148 SM x 128 fp32 lanes x 2 x 1.965 GHz (DESIGN.md); "
                                     "flops = 5 N log2 N per correlation (PAPER.md:134)",
+                     "ncu_offline": NCU_OFFLINE,
                      "fma_pipe": {"ceiling_corr_per_s": FMA_PIPE_CEILING, "frac": rate_kernel / FMA_PIPE_CEILING,
                                   "note": "context: ~1,000 FMA-pipe cycles per 32 lags x 16 row pairs of this radix-16 arithmetic "
                                           "(packed f32x2 = 2 cycles; profiles/r2_search_kernel.md); not the roofline denominator"},
