@@ -4,8 +4,12 @@
 // Loads:  cp.async.bulk global -> shared, completion counted in bytes on an mbarrier (SASS UBLKCP).
 // Cross-CTA hand-over: monotone 64-bit counters in global memory.  The PTX memory-model ordering every arrow
 // of the protocol relies on is listed in DESIGN.md section 5 ("hand-over"); in short:
-//   producer:  data stores -> (CTA barrier) -> red.release.gpu by one thread   (release is cumulative)
-//   consumer:  ld.acquire.gpu by one thread sees the count -> (CTA barrier) -> data loads of all threads
+//   producer:  data stores of a warp -> mbarrier.arrive (release, cta scope) on the CTA's per-slot barrier; the thread
+//              that sees the phase complete (mbarrier.test_wait, acquire) -> fence.acq_rel.gpu -> red.relaxed.gpu
+//              (the fence makes the CTA's stores, observed through the barrier, visible at gpu scope: cumulativity)
+//   consumer:  ld.acquire.gpu by one thread sees the count -> fence.proxy.async (the data was written through the
+//              generic proxy, the tensor copy reads it through the async proxy) -> cp.async.bulk.tensor of the rows
+//              -> mbarrier completion -> shared-memory loads of all threads of the team
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -31,8 +35,6 @@ template <int OFF> BEGE_DA void sts64(uint32_t a, unsigned long long v)
 {
     asm volatile("st.shared.b64 [%0+%1], %2;" :: "r"(a), "n"(OFF), "l"(v) : "memory");
 }
-BEGE_DA float lds32(uint32_t a) { float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a)); return v; }
-BEGE_DA void sts32(uint32_t a, float v) { asm volatile("st.shared.f32 [%0], %1;" :: "r"(a), "f"(v) : "memory"); }
 
 // ---- mbarrier
 BEGE_DA void mbar_init(uint32_t bar, uint32_t count)
@@ -159,18 +161,10 @@ BEGE_DA void tmem_wait_ld(unsigned long long (&w)[2])
     asm volatile("tcgen05.wait::ld.sync.aligned;" : "+l"(w[0]), "+l"(w[1]) :: "memory");
 }
 
-// two columns (dual-stream search: two real table entries), and the wait that covers a complex and a real staging array
-BEGE_DA void tmem_ld2f(uint32_t taddr, float (&w)[2])
+// the wait that covers two staging arrays (dual-stream search: stationary values and the streams' powers)
+BEGE_DA void tmem_wait_ld(unsigned long long (&w)[2], unsigned long long (&f)[2])
 {
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];" : "=f"(w[0]), "=f"(w[1]) : "r"(taddr));
-}
-BEGE_DA void tmem_st2(uint32_t taddr, uint32_t r0, uint32_t r1)
-{
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" :: "r"(taddr), "r"(r0), "r"(r1) : "memory");
-}
-BEGE_DA void tmem_wait_ld(unsigned long long (&w)[2], float (&f)[2])
-{
-    asm volatile("tcgen05.wait::ld.sync.aligned;" : "+l"(w[0]), "+l"(w[1]), "+f"(f[0]), "+f"(f[1]) :: "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" : "+l"(w[0]), "+l"(w[1]), "+l"(f[0]), "+l"(f[1]) :: "memory");
 }
 
 // ---- named barrier of `nthreads` threads

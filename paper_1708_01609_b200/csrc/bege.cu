@@ -195,9 +195,11 @@ k_fwd_cols(const c2* __restrict__ G, c2* __restrict__ out, uint64_t out_stride, 
 //                       four-step factor wN^(16 b k1), k1 = a + 16 r, times the inner twiddle w256^(a p); 4 quadrants
 //   columns [32, 96):   pass 1, team 0: the stationary tile, 28 columns per thread, 32 per warp of a lane quadrant
 //   columns [96, 160):  pass 1: theta^p = exp(2 pi i p (256 g + k1) / N), p = 1 .. 15, same arrangement
-//   columns [160, 192): pass 1, dual-stream search only: Re(X[k] X[N-k]) of the segment, 14 columns per thread
+//   columns [160, 192): unused
 //   columns [192, 256): pass 1, team 1: its copy of the stationary tile (batched calls: the teams change template
 //                       at different times)
+//   columns [256, 320): dual-stream search only (that variant allocates all 512 columns): per bin of this thread the
+//                       pair (|H1~[k]|^2, |L1~[k]|^2) of the segment, 28 columns per thread, 32 per warp of a quadrant
 // The CTA-uniform part of the four-step factor, w256^(b r), comes from constant memory (uniform loads, one row per CTA).  All table
 // entries are rounded once from fp64 angles.
 //
@@ -223,14 +225,15 @@ constexpr int kSearchThreads = 32 * 32;
 #define BEGE_STATS 0       // 1: one CTA prints wait statistics of its service threads at the end (experiments only)
 #endif
 constexpr int kTmemCols = 256;
-constexpr uint32_t kTmDelta = 0, kTmStat = 32, kTmTheta = 96, kTmQ = 160, kTmStat1 = 192;   // kTmQ: 16 columns per warp of a quadrant
+constexpr int kTmemColsDual = 512;
+constexpr uint32_t kTmDelta = 0, kTmStat = 32, kTmTheta = 96, kTmStat1 = 192, kTmAB = 256;
 __constant__ float2 c_wb[16][16];          // exp(2 pi i b r / 256): row b = the CTA-uniform part of pass 2's four-step factor;
                                            // rounded from fp64 (host, bege_plan_create)
 constexpr int kSigPart = 128;              // Parseval partial sums per pair: 16 tiles x 8 warps (dual-stream search: two sets)
 
 struct SearchArgs {
     CUtensorMap ring_map;                  // T' of all groups and ring slots as a 2-D fp32 tensor: (512, G * kRing * 256)
-    const c2* bank; const c2* xseg; const float* qseg; c2* ring; float* sigpart; bege_tail* rec; c2* zdbg;
+    const c2* bank; const c2* xseg; const float2* qseg; c2* ring; float* sigpart; bege_tail* rec; c2* zdbg;
     unsigned long long cap; unsigned long long* counter; unsigned long long* done1; unsigned long long* done2;
     int* abort_flag;
     uint64_t j0, nT, sig_pair0;
@@ -294,26 +297,27 @@ template <int I0, bool SINGLE, int IP = 0> BEGE_D void tm_products(uint32_t stre
         tm_products<I0, SINGLE, IP + 1>(stream_a, taddr, v, acc, qa, qb);
     }
 }
-// ... dual-stream search (SINGLE only): besides R = conj(W) X and sum |R|^2 also P = sum_k |W[k]|^2 Re(X[k] X[N-k]), which
-// splits sum |R|^2 into the two detector streams (see k_search); Re(X[k] X[N-k]) comes from tensor memory as well
-template <int I0, int IP = 0> BEGE_D void tm_products_dual(uint32_t stream_a, uint32_t tx, uint32_t tqr, c2 (&v)[16], c2& acc, float& pacc,
-                                                           c2 (&qa)[2], c2 (&qb)[2], float (&ra)[2], float (&rb)[2])
+// ... dual-stream search (SINGLE only): R = conj(W) X as above; instead of sum |R|^2 the two streams' own sums
+// V1 = sum_k |W[k]|^2 |H1~[k]|^2 and V2 = sum_k |W[k]|^2 |L1~[k]|^2 (see k_search), packed in acc = (V1, V2).  Both are
+// sums of non-negative terms: neither stream's variance is a difference of large numbers, however unequal their powers.
+// The pairs (|H1~|^2, |L1~|^2) come from tensor memory like the stationary tile.
+template <int I0, int IP = 0> BEGE_D void tm_products_dual(uint32_t stream_a, uint32_t tx, uint32_t tab, c2 (&v)[16], c2& acc,
+                                                           c2 (&qa)[2], c2 (&qb)[2], c2 (&ra)[2], c2 (&rb)[2])
 {
     if constexpr (IP < 7) {
         c2 (&cur)[2] = (IP & 1) ? qb : qa;
         c2 (&nxt)[2] = (IP & 1) ? qa : qb;
-        float (&rcur)[2] = (IP & 1) ? rb : ra;
-        float (&rnxt)[2] = (IP & 1) ? ra : rb;
+        c2 (&rcur)[2] = (IP & 1) ? rb : ra;
+        c2 (&rnxt)[2] = (IP & 1) ? ra : rb;
         tmem_wait_ld(cur, rcur);
-        if constexpr (IP + 1 < 7) { tmem_ld4(tx + 4 * (IP + 1), nxt); tmem_ld2f(tqr + 2 * (IP + 1), rnxt); }
+        if constexpr (IP + 1 < 7) { tmem_ld4(tx + 4 * (IP + 1), nxt); tmem_ld4(tab + 4 * (IP + 1), rnxt); }
         c2 s0, s1;
         lds128<IP * 512>(stream_a, s0, s1);
         const c2 r0 = cmulc(cur[0], s0), r1 = cmulc(cur[1], s1);
         v[I0 + 2 * IP] = r0; v[(I0 + 2 * IP + 1) & 15] = r1;
-        acc = fma2(r0, r0, acc); acc = fma2(r1, r1, acc);
-        pacc = fmaf(fmaf(im(s0), im(s0), re(s0) * re(s0)), rcur[0], pacc);
-        pacc = fmaf(fmaf(im(s1), im(s1), re(s1) * re(s1)), rcur[1], pacc);
-        tm_products_dual<I0, IP + 1>(stream_a, tx, tqr, v, acc, pacc, qa, qb, ra, rb);
+        acc = fma2(bc(fmaf(im(s0), im(s0), re(s0) * re(s0))), rcur[0], acc);
+        acc = fma2(bc(fmaf(im(s1), im(s1), re(s1) * re(s1))), rcur[1], acc);
+        tm_products_dual<I0, IP + 1>(stream_a, tx, tab, v, acc, qa, qb, ra, rb);
     }
 }
 // ... stationary values from global memory (bands that keep all 16 row-blocks)
@@ -346,9 +350,10 @@ namespace bege {
 
 // DUAL (single-segment calls, 14 row-blocks): the dual-stream search of PAPER.md:155 -- x = H1 + i L1, REAL templates, so
 // Re z and Im z are the two detectors' outputs.  Their variances are the Hermitian split of the product spectrum
-// (eq.7): N^2 sigma_1^2 = (S + P)/2, N^2 sigma_2^2 = (S - P)/2 with S = sum|R|^2 and
-// P = Re sum_k R[k] R[N-k] = sum_k |W[k]|^2 Re(X[k] X[N-k]) (W Hermitian) -- a second per-tile partial sum next to S,
-// no pairing of bins across tiles.  Output: per sample offset and stream the largest |rho|/sigma and its template
+// (eq.7): with H1~[k] = (X[k] + conj X[N-k])/2 and L1~[k] = (X[k] - conj X[N-k])/2i (the transforms of the
+// two real streams) N^2 sigma_1^2 = V1 = sum_k |W[k]|^2 |H1~[k]|^2 and N^2 sigma_2^2 = V2 = sum_k |W[k]|^2 |L1~[k]|^2 --
+// two per-tile partial sums of non-negative terms (k_dual_q tabulates |H1~|^2, |L1~|^2 per bin), no pairing of bins
+// across tiles in the search and no cancellation when one detector is much louder than the other.  Output: per sample offset and stream the largest |rho|/sigma and its template
 // (Table 3), by 64-bit atomicMax as in the max projection.
 template <int I0, int NI, bool SINGLE, bool DBG, bool DUAL>
 __global__ void __launch_bounds__(kSearchThreads, 1)
@@ -389,7 +394,7 @@ k_search(const __grid_constant__ SearchArgs A)
         reinterpret_cast<volatile uint32_t*>(smem_raw + SM::pubit)[1] = 1;
         fence_mbar_init();
     }
-    if (threadIdx.x < 32) tmem_alloc<kTmemCols>(sb + SM::tmem);
+    if (threadIdx.x < 32) tmem_alloc<DUAL ? kTmemColsDual : kTmemCols>(sb + SM::tmem);
     tmem_fence_before_sync();
     __syncthreads();
     tmem_fence_after_sync();
@@ -438,12 +443,13 @@ k_search(const __grid_constant__ SearchArgs A)
                 tmem_st8(tq_a + kTmTheta + 8 * j, r);
             }
         }
-        if (DUAL && n_items > 0) {                           // Re(X[k] X[N-k]) of this thread's 14 bins
-            const float2* src = reinterpret_cast<const float2*>(A.qseg + ((uint64_t)A.m0 * 16 + b) * (uint64_t)(NI * 256)) + tile_word(NI, 0, 0, t);
+        if (DUAL && n_items > 0) {                           // (|H1~|^2, |L1~|^2) of this thread's 14 bins
+            const ulonglong2* src = reinterpret_cast<const ulonglong2*>(A.qseg + ((uint64_t)A.m0 * 16 + b) * (uint64_t)(NI * 256)) + tile_word(NI, 0, 0, t);
 #pragma unroll
             for (int ip = 0; ip < NI / 2; ++ip) {
-                const float2 q = __ldcg(src + ip * 32);
-                tmem_st2(tq + kTmQ + 16u * (uint32_t)(warp >> 2) + 2 * ip, __float_as_uint(q.x), __float_as_uint(q.y));
+                const ulonglong2 q = __ldcg(src + ip * 32);
+                const uint32_t r[4] = {(uint32_t)q.x, (uint32_t)(q.x >> 32), (uint32_t)q.y, (uint32_t)(q.y >> 32)};
+                tmem_st4(tq + kTmAB + 32u * (uint32_t)(warp >> 2) + 4 * ip, r);
             }
         }
         tmem_wait_st();
@@ -497,9 +503,9 @@ k_search(const __grid_constant__ SearchArgs A)
                 tj_prev = tj;
             }
             c2 qa[2], qb[2];                                 // TMEM staging (stationary values, then theta powers)
-            float ra[2], rb[2], pacc = 0.f;                  // dual-stream search: staging of Re(X[k] X[N-k]), P
+            c2 ra[2], rb[2];                                 // dual-stream search: staging of (|H1~|^2, |L1~|^2)
             if (STAT) tmem_ld4(tq_s, qa);
-            if (DUAL) tmem_ld2f(tq + kTmQ + 16u * (uint32_t)(warp >> 2), ra);
+            if (DUAL) tmem_ld4(tq + kTmAB + 32u * (uint32_t)(warp >> 2), ra);
 #if !(BEGE_ABL & 2)
             mbar_wait(bar_w, nload & 1, abort_flag);
 #endif
@@ -508,7 +514,7 @@ k_search(const __grid_constant__ SearchArgs A)
             c2 acc = mk(0.f, 0.f);
 #pragma unroll
             for (int r = 0; r < 16; ++r) if (r < I0 || r >= I0 + NI) v[r] = mk(0.f, 0.f);
-            if constexpr (DUAL) tm_products_dual<I0>(stream_a, tq_s, tq + kTmQ + 16u * (uint32_t)(warp >> 2), v, acc, pacc, qa, qb, ra, rb);
+            if constexpr (DUAL) tm_products_dual<I0>(stream_a, tq_s, tq + kTmAB + 32u * (uint32_t)(warp >> 2), v, acc, qa, qb, ra, rb);
             else if constexpr (STAT) tm_products<I0, SINGLE>(stream_a, tq_s, v, acc, qa, qb);
             else gl_products<I0, NI, SINGLE>(stream_a, statg, v, acc);
             tmem_ld4(tq_a + kTmTheta, qa);
@@ -524,8 +530,8 @@ k_search(const __grid_constant__ SearchArgs A)
             fft16<+1>(v);
             tm_twiddle<1, 8>(tq_a + kTmTheta, v, qa, qb);    // v[p] *= theta^p, p = 1 .. 15
             sts16<8>(xw_a, v);
-            const float sw = warp_sum32(re(acc) + im(acc));  // (includes the __syncwarp the exchange needs)
-            const float pw = DUAL ? warp_sum32(pacc) : 0.f;
+            const float sw = warp_sum32(DUAL ? re(acc) : re(acc) + im(acc));  // (includes the __syncwarp the exchange needs)
+            const float pw = DUAL ? warp_sum32(im(acc)) : 0.f;               // dual-stream search: sw = V1, pw = V2
             __syncwarp();
             lds16<136>(xr_a, v);
             if (lane == 0) {
@@ -712,8 +718,8 @@ k_search(const __grid_constant__ SearchArgs A)
             fft16<+1>(v);
             // lane a holds Z[n1 = a + 16 q]; lag n = 256 n1 + n2
             const float thr = A.k2 * sumR2;
-            // dual-stream search: N^2 sigma_1^2 = (S + P)/2 for Re z (H1), N^2 sigma_2^2 = (S - P)/2 for Im z (L1)
-            const float var1 = 0.5f * (sumR2 + sumP), var2 = 0.5f * (sumR2 - sumP);
+            // dual-stream search: the two sums are N^2 sigma_1^2 = V1 for Re z (H1) and N^2 sigma_2^2 = V2 for Im z (L1)
+            const float var1 = sumR2, var2 = sumP;
             const float thr1 = A.k2 * var1, thr2 = A.k2 * var2;
             bool any = false;
 #pragma unroll
@@ -824,7 +830,7 @@ k_search(const __grid_constant__ SearchArgs A)
     // every warp is done with the tensor memory: give it back
     tmem_fence_before_sync();
     __syncthreads();
-    if (threadIdx.x < 32) tmem_dealloc<kTmemCols>(tq);
+    if (threadIdx.x < 32) tmem_dealloc<DUAL ? kTmemColsDual : kTmemCols>(tq);
 }
 
 // sum of the 8 warp partial sums of a tile, in the order pass 2 uses
@@ -846,31 +852,34 @@ __global__ void k_sigma(const float* __restrict__ sigpart, float* __restrict__ s
     sigma[i] = sqrtf(v[0]) / (float)kN;
 }
 
-// dual-stream search: Q[k] = Re(X[k] X[N-k]) of a stored segment spectrum, same tile layout (one float per bin).
+// dual-stream search: per stored bin k of a segment spectrum X (x = H1 + i L1) the powers of the two real streams,
+// Q[k] = (|H1~[k]|^2, |L1~[k]|^2) = (|X[k] + conj X[N-k]|^2, |X[k] - conj X[N-k]|^2) / 4, same tile layout as X.
 // grid (16 tiles, segments), 256 threads.
 __global__ void __launch_bounds__(256)
-k_dual_q(const c2* __restrict__ xs, float* __restrict__ q, int I0, int NI)
+k_dual_q(const c2* __restrict__ xs, float2* __restrict__ q, int I0, int NI)
 {
     const int t = threadIdx.x, b = blockIdx.x;
     const uint64_t m = blockIdx.y;
     const int c = t >> 4, g = t & 15;
     const c2* X = xs + m * (uint64_t)(16 * NI * 256);
-    float* Q = q + m * (uint64_t)(16 * NI * 256);
+    float2* Q = q + m * (uint64_t)(16 * NI * 256);
     for (int ii = 0; ii < NI; ++ii) {
         const uint32_t k = (uint32_t)(16 * b + c) + 256u * (uint32_t)(g + 16 * (ii + I0));
         const uint32_t km = ((uint32_t)kN - k) & (uint32_t)(kN - 1);
         const int bm = (int)((km & 255u) >> 4), cm = (int)(km & 15u), gm = (int)((km >> 8) & 15u), im_ = (int)(km >> 12) - I0;
         const size_t idx = (size_t)tile_word(NI, b, ii / 2, t) * 2 + (ii & 1);
-        float val = 0.f;
-        if (im_ >= 0 && im_ < NI) {
+        float2 val = make_float2(0.f, 0.f);
+        if (im_ >= 0 && im_ < NI) {                          // (a mirror bin outside the stored row-blocks is out of band, as is k)
             const c2 a = X[idx], d = X[(size_t)tile_word(NI, bm, im_ / 2, 16 * cm + gm) * 2 + (im_ & 1)];
-            val = re(a) * re(d) - im(a) * im(d);
+            const float sr = re(a) + re(d), si = im(a) - im(d);      // X[k] + conj X[N-k]
+            const float dr = re(a) - re(d), di = im(a) + im(d);      // X[k] - conj X[N-k]
+            val = make_float2(0.25f * (sr * sr + si * si), 0.25f * (dr * dr + di * di));
         }
         Q[idx] = val;
     }
 }
 
-// dual-stream search: sigma_1 = sqrt((S + P)/2)/N, sigma_2 = sqrt((S - P)/2)/N from the 2 x 128 partial sums of a pair
+// dual-stream search: sigma_1 = sqrt(V1)/N, sigma_2 = sqrt(V2)/N from the 2 x 128 partial sums of a pair
 __global__ void k_sigma_dual(const float* __restrict__ sigpart, float* __restrict__ s1, float* __restrict__ s2, uint64_t n)
 {
     const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -879,8 +888,8 @@ __global__ void k_sigma_dual(const float* __restrict__ sigpart, float* __restric
     for (int a = 0; a < 16; ++a) { v[a] = tile_sum8(sigpart + i * 2 * kSigPart + 8 * a); w[a] = tile_sum8(sigpart + i * 2 * kSigPart + kSigPart + 8 * a); }
     for (int d = 8; d >= 1; d >>= 1)
         for (int a = 0; a < d; ++a) { v[a] = v[a] + v[a + d]; w[a] = w[a] + w[a + d]; }     // the order of row_sum16
-    s1[i] = sqrtf(fmaxf(0.5f * (v[0] + w[0]), 0.f)) / (float)kN;
-    s2[i] = sqrtf(fmaxf(0.5f * (v[0] - w[0]), 0.f)) / (float)kN;
+    s1[i] = sqrtf(v[0]) / (float)kN;
+    s2[i] = sqrtf(w[0]) / (float)kN;
 }
 
 // dual-stream search: offsets with a hit in both streams, and those whose templates' start frequencies differ by less
@@ -937,13 +946,15 @@ struct bege_plan {
     CUtensorMap ring_map{};          // the ring as a 2-D tensor (pass 2 fetches its row tiles with one tensor copy)
     void* ring_map_for = nullptr;   // ring address the map was encoded for
     void* l2_window = nullptr;      // ring region currently marked persisting in L2 (access policy window of the stream)
-    size_t l2_limit_prev = 0; bool l2_limit_saved = false;   // device limit found before the first search
+    size_t l2_limit_prev = 0; bool l2_limit_raised = false;  // device limit found before this plan raised it (first search)
     uint64_t max_items = ((1ull << 31) - 1) / 2;   // per group and launch (the kernel counts items in 32 bits)
     bege_stats stats{};
     std::string err;
 };
 
-// take the ring's persisting-L2 window off the plan's stream again (the stream may be the caller's)
+// take the ring's persisting-L2 window off the plan's stream again (the stream may be the caller's).  Per search this
+// touches the stream attribute only: no context-wide reset (it would evict other users' persisting lines and
+// synchronise), no change of the device limit.
 static void drop_l2_window(bege_plan* p)
 {
     if (!p->l2_window || !p->stream) return;
@@ -954,10 +965,22 @@ static void drop_l2_window(bege_plan* p)
     av.accessPolicyWindow.hitProp = cudaAccessPropertyNormal;
     av.accessPolicyWindow.missProp = cudaAccessPropertyNormal;
     cudaStreamSetAttribute(p->stream, cudaStreamAttributeAccessPolicyWindow, &av);
-    cudaCtxResetPersistingL2Cache();
-    if (p->l2_limit_saved) cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, p->l2_limit_prev);
     cudaGetLastError();
     p->l2_window = nullptr;
+}
+// every return path of a search, error returns included, leaves the caller's stream without the window
+struct L2WindowGuard { bege_plan* p; ~L2WindowGuard() { drop_l2_window(p); } };
+
+// the ring goes away (plan destroyed / workspace replaced): give its lines back to normal caching and put the device's
+// persisting-L2 limit back to what it was before this plan raised it
+static void release_l2(bege_plan* p)
+{
+    drop_l2_window(p);
+    if (!p->l2_limit_raised) return;
+    cudaCtxResetPersistingL2Cache();
+    cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, p->l2_limit_prev);
+    cudaGetLastError();
+    p->l2_limit_raised = false;
 }
 
 static int fail(bege_plan* p, int code, const char* fmt, ...)
@@ -1001,6 +1024,14 @@ static int slot_get(bege_plan* p, Slot& s, uint64_t need, void** out)
     return BEGE_OK;
 }
 static void slot_free(Slot& s) { if (s.own) cudaFree(s.own); s = Slot(); }
+
+// Parseval partial sums of all pairs: one set of kSigPart per pair, two for the dual-stream search (which needs a bank
+// of real templates).  Inside a caller's workspace the slot cannot grow later, so it takes the larger size at once
+// (bege_plan_workspace_bytes counts that).
+static uint64_t sig_bytes(const bege_plan* p)
+{
+    return p->T * p->S * (uint64_t)((p->bank_real || p->user_ws) ? 2 * kSigPart : kSigPart) * sizeof(float);
+}
 
 static uint64_t tpl_bytes(const bege_plan* p) { return (uint64_t)p->NI * 16 * 256 * sizeof(c2); }
 
@@ -1117,7 +1148,7 @@ extern "C" void bege_plan_destroy(bege_plan* p)
     if (!p) return;
     cudaSetDevice(p->device);
     if (p->stream) cudaStreamSynchronize(p->stream);
-    drop_l2_window(p);
+    release_l2(p);
     if (p->side) { cudaStreamSynchronize(p->side); cudaStreamDestroy(p->side); }
     if (p->own_stream && p->stream) cudaStreamDestroy(p->stream);
     for (Slot* s : {&p->s_bank, &p->s_x, &p->s_q, &p->s_scratch, &p->s_sig, &p->s_rec, &p->s_misc, &p->s_par, &p->s_tmp}) slot_free(*s);
@@ -1147,7 +1178,7 @@ extern "C" int bege_plan_workspace_bytes(const bege_plan* p, uint64_t T, uint32_
     b += al(T * tpl_bytes(p));                         // bank
     b += al(T * 16);                                   // template parameters (f0, fdot)
     b += al((uint64_t)S * tpl_bytes(p));               // segment spectra
-    b += al((uint64_t)S * tpl_bytes(p) / 2);           // Re(X[k] X[N-k]) (dual-stream search)
+    b += al((uint64_t)S * tpl_bytes(p));               // (|H1~|^2, |L1~|^2) per stored bin (dual-stream search)
     b += al(scratch_bytes(p));                          // four-step staging (stays in L2)
     b += al(T * S * 2 * kSigPart * sizeof(float));     // Parseval partial sums (two sets in the dual-stream search)
     b += al(std::max<uint64_t>(cap * sizeof(bege_tail), (uint64_t)S * kN * 16));  // records / max-projection array(s)
@@ -1163,10 +1194,10 @@ extern "C" int bege_plan_set_workspace(bege_plan* p, void* dev_ptr, uint64_t byt
     if (dev_ptr && ((uintptr_t)dev_ptr & 255)) return fail(p, BEGE_EINVAL, "workspace must be 256-byte aligned");
     CU(p, cudaSetDevice(p->device));
     CU(p, cudaStreamSynchronize(p->stream));
-    drop_l2_window(p);
+    release_l2(p);
     for (Slot* s : {&p->s_bank, &p->s_x, &p->s_q, &p->s_scratch, &p->s_sig, &p->s_rec, &p->s_misc, &p->s_par, &p->s_tmp}) slot_free(*s);
     p->ws = (unsigned char*)dev_ptr; p->ws_bytes = dev_ptr ? bytes : 0; p->bump = 0; p->user_ws = dev_ptr != nullptr;
-    p->T = 0; p->S = 0; p->have_sigma = false;
+    p->T = 0; p->S = 0; p->have_sigma = false; p->have_sigma_dual = false; p->bank_real = false;
     return BEGE_OK;
 }
 
@@ -1243,10 +1274,10 @@ extern "C" int bege_segment_load(bege_plan* p, const float* x, uint32_t S)
         k_fwd_cols<true><<<dim3(16, nb), 256, 0, p->stream>>>((const c2*)scr, (c2*)xs + m0 * stride, stride, p->I0, p->NI, p->tw256, p->klo, p->khi);
         count_launch(p, 2);
     }
-    {   // Re(X[k] X[N-k]) for the dual-stream search: one float per stored bin, same layout
+    {   // powers of the two real streams for the dual-stream search: two floats per stored bin, same layout
         void* q;
-        if ((rc = slot_get(p, p->s_q, (uint64_t)S * tpl_bytes(p) / 2, &q))) return rc;
-        k_dual_q<<<dim3(16, S), 256, 0, p->stream>>>((const c2*)xs, (float*)q, p->I0, p->NI);
+        if ((rc = slot_get(p, p->s_q, (uint64_t)S * tpl_bytes(p), &q))) return rc;
+        k_dual_q<<<dim3(16, S), 256, 0, p->stream>>>((const c2*)xs, (float2*)q, p->I0, p->NI);
         count_launch(p);
     }
     CU(p, cudaGetLastError());
@@ -1262,8 +1293,11 @@ static void set_l2_window(bege_plan* p, void* ring)
 {
     if (p->l2_window == ring) return;
     const size_t bytes = (size_t)p->G * kRing * kN * sizeof(c2);
-    if (!p->l2_limit_saved) { cudaDeviceGetLimit(&p->l2_limit_prev, cudaLimitPersistingL2CacheSize); p->l2_limit_saved = true; }
-    cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, bytes);
+    if (!p->l2_limit_raised) {                               // once per plan, and only if the limit has to grow
+        size_t cur = 0;
+        if (cudaDeviceGetLimit(&cur, cudaLimitPersistingL2CacheSize) == cudaSuccess && cur < bytes &&
+            cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, bytes) == cudaSuccess) { p->l2_limit_prev = cur; p->l2_limit_raised = true; }
+    }
     cudaStreamAttrValue av{};
     av.accessPolicyWindow.base_ptr = ring;
     av.accessPolicyWindow.num_bytes = bytes;
@@ -1307,7 +1341,7 @@ static int make_ring_map(bege_plan* p, void* ring)
 // one cooperative launch of the persistent search kernel over templates [j0, j0 + nT) x segments [m0, m0 + nS)
 static int launch_search(bege_plan* p, const c2* bank, const c2* xs, c2* ring, float* sig, uint64_t sig_pair0, float k2, float k2hi,
                          bege_tail* rec, uint64_t cap, unsigned char* misc, c2* zdbg, uint64_t j0, uint64_t nT, uint32_t m0,
-                         uint32_t nS, bool first = true, const float* qseg = nullptr)
+                         uint32_t nS, bool first = true, const float2* qseg = nullptr)
 {
     const bool dual = qseg != nullptr;
     // the first launch of a search also clears the record counter, the abort flag and the hit counters
@@ -1366,9 +1400,10 @@ static int search_impl(bege_plan* p, float k_sigma, float k_hi, bege_tail* tails
         return fail(p, BEGE_EINVAL, "bad search arguments");
     if (!p->T || !p->S) return fail(p, BEGE_ESTATE, "bege_search needs a generated bank and loaded segments");
     CU(p, cudaSetDevice(p->device));
+    L2WindowGuard l2_guard{p};
     void *sig, *rec, *misc, *scr, *bank, *xs;
     int rc;
-    if ((rc = slot_get(p, p->s_sig, p->T * p->S * 2 * kSigPart * sizeof(float), &sig))) return rc;
+    if ((rc = slot_get(p, p->s_sig, sig_bytes(p), &sig))) return rc;
     if ((rc = slot_get(p, p->s_rec, cap * sizeof(bege_tail), &rec))) return rc;
     if ((rc = slot_get(p, p->s_misc, kMiscHdr, &misc))) return rc;
     if ((rc = slot_get(p, p->s_scratch, scratch_bytes(p), &scr))) return rc;
@@ -1387,7 +1422,7 @@ static int search_impl(bege_plan* p, float k_sigma, float k_hi, bege_tail* tails
         const uint64_t jj = i * per;
         if ((rc = launch_search(p, (const c2*)bank, (const c2*)xs, (c2*)scr, (float*)sig, 0, k_sigma * k_sigma, k_hi * k_hi,
                                 (bege_tail*)rec, cap, (unsigned char*)misc, nullptr, jj, std::min(per, p->T - jj), 0, p->S,
-                                i == 0))) { drop_l2_window(p); return rc; }
+                                i == 0))) return rc;
         if (overlap) {
             CU(p, cudaMemcpyAsync(p->h_count + 2 + i, counter, sizeof(unsigned long long), cudaMemcpyDeviceToHost, p->stream));
             CU(p, cudaEventRecord(ev[i], p->stream));
@@ -1459,10 +1494,11 @@ extern "C" int bege_search_maxproj(bege_plan* p, float k_sigma, float* snr_out, 
     if (!snr_out || !id_out || !(k_sigma >= 0.f)) return fail(p, BEGE_EINVAL, "bad search arguments");
     if (!p->T || !p->S) return fail(p, BEGE_ESTATE, "bege_search_maxproj needs a generated bank and loaded segments");
     CU(p, cudaSetDevice(p->device));
+    L2WindowGuard l2_guard{p};
     void *sig, *proj, *misc, *scr, *bank, *xs, *tmp;
     int rc;
     const uint64_t n = (uint64_t)p->S * kN;
-    if ((rc = slot_get(p, p->s_sig, p->T * p->S * 2 * kSigPart * sizeof(float), &sig))) return rc;
+    if ((rc = slot_get(p, p->s_sig, sig_bytes(p), &sig))) return rc;
     if ((rc = slot_get(p, p->s_rec, n * sizeof(unsigned long long), &proj))) return rc;
     if ((rc = slot_get(p, p->s_misc, kMiscHdr, &misc))) return rc;
     if ((rc = slot_get(p, p->s_scratch, scratch_bytes(p), &scr))) return rc;
@@ -1475,7 +1511,7 @@ extern "C" int bege_search_maxproj(bege_plan* p, float k_sigma, float* snr_out, 
         // cap = ~0 switches the kernel's epilogue from appending records to the projection array passed as `rec`
         if ((rc = launch_search(p, (const c2*)bank, (const c2*)xs, (c2*)scr, (float*)sig, 0, k_sigma * k_sigma, INFINITY,
                                 (bege_tail*)proj, ~0ull, (unsigned char*)misc, nullptr, jj, std::min(per, p->T - jj), 0, p->S,
-                                jj == 0))) { drop_l2_window(p); return rc; }
+                                jj == 0))) return rc;
     }
     CU(p, cudaGetLastError());
     float* d_snr = (float*)tmp; uint32_t* d_id = (uint32_t*)(d_snr + n);
@@ -1503,10 +1539,11 @@ extern "C" int bege_search_dual(bege_plan* p, float k_sigma, float* snr1, uint32
     if (!p->bank_real) return fail(p, BEGE_ESTATE, "bege_search_dual needs a bank of real templates (bege_bank_generate_real)");
     if (p->NI != 14) return fail(p, BEGE_EINVAL, "bege_search_dual supports bands inside bins [4096, 61440) only");
     CU(p, cudaSetDevice(p->device));
+    L2WindowGuard l2_guard{p};
     void *sig, *proj, *misc, *scr, *bank, *xs, *q, *tmp, *par;
     int rc;
     const uint64_t n = (uint64_t)p->S * kN;
-    if ((rc = slot_get(p, p->s_sig, p->T * p->S * 2 * kSigPart * sizeof(float), &sig))) return rc;
+    if ((rc = slot_get(p, p->s_sig, sig_bytes(p), &sig))) return rc;
     if ((rc = slot_get(p, p->s_rec, 2 * n * sizeof(unsigned long long), &proj))) return rc;
     if ((rc = slot_get(p, p->s_misc, kMiscHdr, &misc))) return rc;
     if ((rc = slot_get(p, p->s_scratch, scratch_bytes(p), &scr))) return rc;
@@ -1524,7 +1561,7 @@ extern "C" int bege_search_dual(bege_plan* p, float k_sigma, float* snr1, uint32
         for (uint64_t jj = 0; jj < p->T; jj += maxT) {
             if ((rc = launch_search(p, (const c2*)bank, (const c2*)xs, (c2*)scr, (float*)sig, 0, k_sigma * k_sigma, INFINITY,
                                     (bege_tail*)proj, ~0ull, (unsigned char*)misc, nullptr, jj, std::min(maxT, p->T - jj), m, 1,
-                                    first, (const float*)q))) { drop_l2_window(p); return rc; }
+                                    first, (const float2*)q))) return rc;
             first = false;
         }
     CU(p, cudaGetLastError());
@@ -1558,6 +1595,7 @@ extern "C" int bege_get_sigma_dual(bege_plan* p, float* sigma1_out, float* sigma
     if (!p->have_sigma_dual) return fail(p, BEGE_ESTATE, "bege_get_sigma_dual needs a completed bege_search_dual");
     CU(p, cudaSetDevice(p->device));
     const uint64_t n = p->T * p->S;
+    if (n == 0) return fail(p, BEGE_ESTATE, "no bank / segments loaded");
     void *sig, *tmp;
     int rc;
     if ((rc = slot_get(p, p->s_sig, 0, &sig))) return rc;
@@ -1576,6 +1614,7 @@ extern "C" int bege_get_sigma(bege_plan* p, float* sigma_out)
     if (!p->have_sigma) return fail(p, BEGE_ESTATE, "bege_get_sigma needs a completed bege_search");
     CU(p, cudaSetDevice(p->device));
     const uint64_t n = p->T * p->S;
+    if (n == 0) return fail(p, BEGE_ESTATE, "no bank / segments loaded");
     void *sig, *tmp;
     int rc;
     if ((rc = slot_get(p, p->s_sig, 0, &sig))) return rc;
@@ -1593,6 +1632,7 @@ extern "C" int bege_debug_correlate(bege_plan* p, uint64_t j, uint32_t m, float*
     if (!p->T || !p->S) return fail(p, BEGE_ESTATE, "needs a bank and segments");
     if (j >= p->T || m >= p->S) return fail(p, BEGE_EINVAL, "pair (%llu, %u) out of range", (unsigned long long)j, m);
     CU(p, cudaSetDevice(p->device));
+    L2WindowGuard l2_guard{p};
     void *scr, *bank, *xs, *misc, *tmp;
     int rc;
     if ((rc = slot_get(p, p->s_scratch, scratch_bytes(p), &scr))) return rc;

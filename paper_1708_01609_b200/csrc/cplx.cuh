@@ -23,8 +23,6 @@ typedef unsigned long long c2;   // packed (re, im), fp32 each
 BEGE_D c2 mk(float re, float im) { c2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(re), "f"(im)); return r; }
 BEGE_D float re(c2 v) { float a, b; asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); (void)b; return a; }
 BEGE_D float im(c2 v) { float a, b; asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); (void)a; return b; }
-BEGE_D c2 from_f2(float2 v) { return mk(v.x, v.y); }
-BEGE_D float2 to_f2(c2 v) { return make_float2(re(v), im(v)); }
 
 BEGE_D c2 add2(c2 a, c2 b) { c2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
 BEGE_D c2 sub2(c2 a, c2 b) { c2 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
@@ -46,7 +44,6 @@ BEGE_D c2 cmulw(c2 x, float c, float d) {
     return mk(fmaf(-im(x), d, re(t)), fmaf(re(x), d, im(t)));
 }
 BEGE_D c2 cmulw(c2 x, c2 w) { return cmulw(x, re(w), im(w)); }
-BEGE_D c2 cmul(c2 x, float2 w) { return cmulw(x, w.x, w.y); }
 // conj(h) * x = x * conj(h):  (xr hr, xi hr) + (xi hi, -xr hi)
 BEGE_D c2 cmulc(c2 x, c2 h) {
     const c2 t = mul2(x, bc(re(h)));

@@ -613,6 +613,67 @@ def test_dual_stream_search_matches_oracle(bo, bege):
     assert abs(n_sim - os_) <= 0.02 * os_ + 5 and abs(n_coi - oc) <= 0.02 * oc + 5
 
 
+def test_dual_stream_unequal_power(bo, bege):
+    """One detector 30x louder than the other (power ratio 900; a glitchy or uncalibrated stream): the weak stream's
+    sigma must still meet SIGMA_RTOL -- a variance formed as a difference of the two streams' sums would be off by
+    ~3e-7 x 900 -- and its hits must be the oracle's.  The weak stream's rho carries the fp32 error of the whole complex
+    correlation (2e-7 of the loud stream = 6e-6 of its own sigma), hence an absolute bar of the guard width for it."""
+    ratio = 30.0
+    h1 = synth.band_limit(synth.white_noise(70))
+    l1 = synth.band_limit(synth.white_noise(71)) / ratio
+    xs = (h1 + 1j * l1).astype(np.complex64)[None, :]
+    Xs = np.stack([bo.segment_spectrum(x, FS, *BAND) for x in xs])
+    w = synth.config0()
+    f0, fd = w.f0[::5].copy(), w.fdot[::5].copy()             # 52 templates
+    k = 3.0
+    o1, oi1, o2, oi2, sig_o = bo.search_dual(Xs, f0, fd, TAU, FS, k - 1e-3)
+    with bege.Plan(N, FS, BAND) as plan:
+        plan.bank_generate_real(f0, fd, TAU)
+        plan.segment_load(xs)
+        g1, gi1, g2, gi2, _, _ = plan.search_dual(k, 300.0)
+        s1, s2 = plan.get_sigma_dual()
+    assert 25.0 < np.median(sig_o[:, :, 0] / sig_o[:, :, 1]) < 35.0
+    assert np.max(np.abs(s1 - sig_o[:, :, 0]) / sig_o[:, :, 0]) <= SIGMA_RTOL
+    assert np.max(np.abs(s2 - sig_o[:, :, 1]) / sig_o[:, :, 1]) <= SIGMA_RTOL
+    none = np.iinfo(np.uint32).max
+    for g, gi, o, stream in ((g1, gi1, o1, 0), (g2, gi2, o2, 1)):
+        assert np.all((g == 0) == (gi == none))
+        must, may = o > k + GUARD, o > k - GUARD
+        assert not np.any(must & (g == 0)), f"stream {stream}: oracle offsets missing on the GPU"
+        assert not np.any((g > 0) & ~may), f"stream {stream}: GPU offsets the oracle does not have"
+        both = must & (g > 0)
+        assert both.sum() > 5000
+        if stream == 0:
+            assert np.max(np.abs(g[both] - o[both]) / o[both]) < 2e-5
+        else:
+            assert np.max(np.abs(g[both] - o[both])) < GUARD
+
+
+def test_dual_stream_silent_detector(bo, bege):
+    """L1 identically zero (a detector that is off): H1's sigma and hits are untouched, L1's sigma is rounding residue
+    (orders of magnitude below H1's), nothing is NaN or negative."""
+    h1 = synth.band_limit(synth.white_noise(72))
+    xs = (h1 + 0j).astype(np.complex64)[None, :]
+    Xs = np.stack([bo.segment_spectrum(x, FS, *BAND) for x in xs])
+    w = synth.config0()
+    f0, fd = w.f0[::16].copy(), w.fdot[::16].copy()           # 16 templates
+    k = 3.0
+    o1, _, _, _, sig_o = bo.search_dual(Xs, f0, fd, TAU, FS, k - 1e-3)
+    with bege.Plan(N, FS, BAND) as plan:
+        plan.bank_generate_real(f0, fd, TAU)
+        plan.segment_load(xs)
+        g1, gi1, g2, _, _, _ = plan.search_dual(k, 300.0)
+        s1, s2 = plan.get_sigma_dual()
+    assert np.all(np.isfinite(s1)) and np.all(np.isfinite(s2)) and np.all(s2 >= 0)
+    assert np.all(np.isfinite(g1)) and np.all(np.isfinite(g2))
+    assert np.max(np.abs(s1 - sig_o[:, :, 0]) / sig_o[:, :, 0]) <= SIGMA_RTOL
+    assert np.max(s2 / s1) < 1e-5
+    must, may = o1 > k + GUARD, o1 > k - GUARD
+    assert not np.any(must & (g1 == 0)) and not np.any((g1 > 0) & ~may)
+    both = must & (g1 > 0)
+    assert both.sum() > 2000 and np.max(np.abs(g1[both] - o1[both]) / o1[both]) < 2e-5
+
+
 # ----------------------------------------------------------------------------- overlap-save bake-off probe
 def test_overlap_save_probe_matches_oracle(bo, bege):
     """six 16384-point block correlations reproduce the oracle's circular correlation on every lag.
