@@ -95,14 +95,18 @@ class Plan:
     """One plan = one device, one stream (include/bege.h).  Names follow the C ABI."""
 
     def __init__(self, N: int = 1 << 16, fs: float = 4096.0, band=(350.0, 2000.0), device: int = 0,
-                 stream: int | None = None):
+                 stream: int | str | None = None):
+        """stream: a cudaStream_t handle (e.g. torch.cuda.Stream().cuda_stream), None for torch's current stream,
+        or "own" for a private non-blocking stream created and owned by the plan (cuda_stream = NULL in the C ABI)."""
         import torch
 
         if not torch.cuda.is_available():
             raise RuntimeError("bege needs a CUDA device (sm_100a); there is no CPU fallback")
         self._L = load_library()
         self.N, self.fs, self.band, self.device = int(N), float(fs), tuple(band), int(device)
-        if stream is None:
+        if stream == "own":
+            stream = None                 # NULL in the C ABI: the plan creates (and owns) a non-blocking stream
+        elif stream is None:
             stream = torch.cuda.current_stream(self.device).cuda_stream
         if stream == 0:
             # torch's default stream is the legacy default stream; handle 0 would read as "no stream given" and make
