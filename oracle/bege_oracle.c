@@ -383,6 +383,34 @@ int bo_template_real(double f0, double fdot, double tau, double fs, uint32_t N, 
 }
 
 /*
+ * Time-symmetric real template, PAPER.md:70 (Fig.2 caption): "The chirps used in butterfly filtering are symmetric in
+ * time, obtained by superposition of chirp forward and backward in time, suitable in searches for both ascending and
+ * descending chirps."  With u_n = hann_L[n] cos(2 pi c_n) the one-way template of bo_template_real before normalisation
+ * (reading 27):
+ *   w_n = u_n + u_(L-1-n),  n < L;   w <- w / ||w||_2;   zero padded to N.
+ * The Hann window is itself symmetric, so w_n = hann_L[n] (cos 2 pi c_n + cos 2 pi c_(L-1-n)) and w_n = w_(L-1-n).
+ */
+int bo_template_real_sym(double f0, double fdot, double tau, double fs, uint32_t N, double* h)
+{
+    long Ll = lround(tau * fs);
+    if (Ll < 2 || (uint64_t)Ll > N) return 1;
+    uint32_t L = (uint32_t)Ll;
+    memset(h, 0, sizeof(double) * 2 * (size_t)N);
+    double norm2 = 0.0;
+    for (uint32_t n = 0; n < L; ++n) {
+        double wn = 0.5 - 0.5 * cos(2.0 * BO_PI * (double)n / (double)(L - 1));
+        double t = (double)n / fs, tr = (double)(L - 1 - n) / fs;
+        double c = f0 * t + 0.5 * fdot * t * t, cr = f0 * tr + 0.5 * fdot * tr * tr;
+        c -= floor(c); cr -= floor(cr);
+        h[2 * n] = wn * (cos(2.0 * BO_PI * c) + cos(2.0 * BO_PI * cr));
+        norm2 += h[2 * n] * h[2 * n];
+    }
+    double inv = 1.0 / sqrt(norm2);
+    for (uint32_t n = 0; n < L; ++n) h[2 * n] *= inv;
+    return 0;
+}
+
+/*
  * One (real template, packed segment) pair.  z as in bo_correlate_spectra (eq.5); per detector
  * stream the standard deviation of its REAL output by the definition PAPER.md:96 eq.(6):
  *   sigma_1^2 = N^-1 sum_n (Re z[n])^2,   sigma_2^2 = N^-1 sum_n (Im z[n])^2.
@@ -443,16 +471,17 @@ void bo_sigma_dual_parseval(const double* X, const double* Hs, uint32_t N, doubl
  * ("we select data with maximal rho values"); 0 / UINT32_MAX where no template hits; ties go to the
  * smaller template id.  sigma_out (may be NULL): T*S*2 values, [j][m][stream].  Plain serial loops.
  */
-int bo_search_dual(const double* Xs, uint32_t S, const double* f0, const double* fdot, uint64_t T,
-                   double tau, double fs, uint32_t N, double k_sigma,
-                   double* snr1, uint32_t* id1, double* snr2, uint32_t* id2, double* sigma_out)
+static int search_dual_impl(const double* Xs, uint32_t S, const double* f0, const double* fdot, uint64_t T,
+                            double tau, double fs, uint32_t N, double k_sigma,
+                            double* snr1, uint32_t* id1, double* snr2, uint32_t* id2, double* sigma_out, int symmetric)
 {
     double* Hs = (double*)malloc(sizeof(double) * 2 * (size_t)N);
     double* z  = (double*)malloc(sizeof(double) * 2 * (size_t)N);
     if (!Hs || !z) { free(Hs); free(z); return 2; }
     for (size_t i = 0; i < (size_t)S * N; ++i) { snr1[i] = snr2[i] = 0.0; id1[i] = id2[i] = UINT32_MAX; }
     for (uint64_t j = 0; j < T; ++j) {
-        if (bo_template_real(f0[j], fdot[j], tau, fs, N, Hs) || bo_fft(Hs, N, -1)) { free(Hs); free(z); return 1; }
+        if ((symmetric ? bo_template_real_sym(f0[j], fdot[j], tau, fs, N, Hs) : bo_template_real(f0[j], fdot[j], tau, fs, N, Hs))
+            || bo_fft(Hs, N, -1)) { free(Hs); free(z); return 1; }
         for (uint32_t m = 0; m < S; ++m) {
             double s1 = 0.0, s2 = 0.0;
             bo_correlate_dual(Xs + 2 * (size_t)m * N, Hs, N, z, &s1, &s2);
@@ -467,6 +496,21 @@ int bo_search_dual(const double* Xs, uint32_t S, const double* f0, const double*
     }
     free(Hs); free(z);
     return 0;
+}
+
+int bo_search_dual(const double* Xs, uint32_t S, const double* f0, const double* fdot, uint64_t T,
+                   double tau, double fs, uint32_t N, double k_sigma,
+                   double* snr1, uint32_t* id1, double* snr2, uint32_t* id2, double* sigma_out)
+{
+    return search_dual_impl(Xs, S, f0, fdot, T, tau, fs, N, k_sigma, snr1, id1, snr2, id2, sigma_out, 0);
+}
+
+/* The same search with the time-symmetric templates of bo_template_real_sym. */
+int bo_search_dual_sym(const double* Xs, uint32_t S, const double* f0, const double* fdot, uint64_t T,
+                       double tau, double fs, uint32_t N, double k_sigma,
+                       double* snr1, uint32_t* id1, double* snr2, uint32_t* id2, double* sigma_out)
+{
+    return search_dual_impl(Xs, S, f0, fdot, T, tau, fs, N, k_sigma, snr1, id1, snr2, id2, sigma_out, 1);
 }
 
 /*

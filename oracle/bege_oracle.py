@@ -70,6 +70,11 @@ def lib():
         L.bo_search_band.restype = u64
         L.bo_template_real.argtypes = [dbl, dbl, dbl, dbl, u32, dp]
         L.bo_template_real.restype = ctypes.c_int
+        L.bo_template_real_sym.argtypes = [dbl, dbl, dbl, dbl, u32, dp]
+        L.bo_template_real_sym.restype = ctypes.c_int
+        L.bo_search_dual_sym.argtypes = [dp, u32, dp, dp, u64, dbl, dbl, u32, dbl, dp, ctypes.POINTER(u32), dp,
+                                         ctypes.POINTER(u32), dp]
+        L.bo_search_dual_sym.restype = ctypes.c_int
         L.bo_correlate_dual.argtypes = [dp, dp, u32, dp, dp, dp]
         L.bo_correlate_dual.restype = ctypes.c_int
         L.bo_sigma_dual_parseval.argtypes = [dp, dp, u32, dp, dp]
@@ -217,6 +222,14 @@ def template_real(f0: float, fdot: float, tau: float, fs: float, N: int) -> np.n
     return h
 
 
+def template_real_sym(f0: float, fdot: float, tau: float, fs: float, N: int) -> np.ndarray:
+    """Time-symmetric real template (bo_template_real_sym): the chirp plus its time reverse, unit norm."""
+    h = np.zeros(N, dtype=np.complex128)
+    if lib().bo_template_real_sym(float(f0), float(fdot), float(tau), float(fs), N, _dp(h.view(np.float64))):
+        raise ValueError("bo_template_real_sym: bad arguments")
+    return h
+
+
 def correlate_dual(X, h):
     """(z, sigma_1, sigma_2) for a packed segment spectrum X and a real template h (time domain)."""
     X = _c128(X)
@@ -239,8 +252,9 @@ def sigma_dual_parseval(X, h):
     return s1.value, s2.value
 
 
-def search_dual(Xs, f0, fdot, tau: float, fs: float, k_sigma: float):
-    """Dual-stream search (bo_search_dual): (snr1[S, N], id1[S, N], snr2[S, N], id2[S, N], sigma[T, S, 2])."""
+def search_dual(Xs, f0, fdot, tau: float, fs: float, k_sigma: float, symmetric: bool = False):
+    """Dual-stream search (bo_search_dual; symmetric: bo_search_dual_sym, the time-symmetric templates of PAPER.md:70):
+    (snr1[S, N], id1[S, N], snr2[S, N], id2[S, N], sigma[T, S, 2])."""
     Xs = np.atleast_2d(_c128(Xs))
     S, N = Xs.shape
     f0 = np.ascontiguousarray(np.asarray(f0, dtype=np.float64))
@@ -249,7 +263,8 @@ def search_dual(Xs, f0, fdot, tau: float, fs: float, k_sigma: float):
     id1, id2 = np.zeros((S, N), dtype=np.uint32), np.zeros((S, N), dtype=np.uint32)
     sig = np.zeros((f0.size, S, 2))
     u32p = ctypes.POINTER(ctypes.c_uint32)
-    rc = lib().bo_search_dual(_dp(Xs.view(np.float64)), S, _dp(f0), _dp(fdot), f0.size, float(tau), float(fs), N,
+    fn = lib().bo_search_dual_sym if symmetric else lib().bo_search_dual
+    rc = fn(_dp(Xs.view(np.float64)), S, _dp(f0), _dp(fdot), f0.size, float(tau), float(fs), N,
                               float(k_sigma), _dp(snr1), id1.ctypes.data_as(u32p), _dp(snr2), id2.ctypes.data_as(u32p),
                               _dp(sig))
     if rc:

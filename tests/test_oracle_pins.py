@@ -416,6 +416,82 @@ def test_real_template_is_the_normalised_real_part():
     assert np.max(np.abs(w.real - c * h.real)) < 1e-12
 
 
+def test_symmetric_template_is_chirp_plus_time_reverse():
+    """bo_template_real_sym (Fig.2 caption: "symmetric in time, obtained by superposition of chirp forward
+    and backward in time"): w[n] = w[L-1-n]; equal to the normalised sum of the one-way template (pinned above)
+    and its reversal; and equal to the superposition of the ascending chirp (f0, fdot) and the descending chirp that
+    starts where it ends, (f0 + fdot T', -fdot) with a phase offset, T' = (L-1)/fs -- written out with numpy."""
+    L = int(round(TAU * FS))
+    n = np.arange(L)
+    for (f0, fd) in ((777.0, -123.0), (400.0, 390.0), (1500.0, 0.0)):
+        w = bo.template_real_sym(f0, fd, TAU, FS, N)
+        assert np.all(w.imag == 0) and np.all(w[L:] == 0)
+        assert abs(np.linalg.norm(w) - 1) < 1e-14
+        assert np.max(np.abs(w.real[:L] - w.real[:L][::-1])) < 1e-15       # symmetric in time (to the window's rounding)
+        u = bo.template_real(f0, fd, TAU, FS, N).real[:L]                   # one-way template (same norm for both directions)
+        ref = u + u[::-1]
+        ref /= np.linalg.norm(ref)
+        assert np.max(np.abs(w.real[:L] - ref)) < 1e-12
+        Tp = (L - 1) / FS
+        t = n / FS
+        up = np.cos(2 * np.pi * (f0 * t + 0.5 * fd * t ** 2))
+        phi0 = f0 * Tp + 0.5 * fd * Tp ** 2
+        down = np.cos(2 * np.pi * (phi0 - ((f0 + fd * Tp) * t - 0.5 * fd * t ** 2)))   # starts at f0 + fd T', rate -fd
+        ref2 = np.hanning(L) * (up + down)
+        ref2 /= np.linalg.norm(ref2)
+        assert np.max(np.abs(w.real[:L] - ref2)) < 1e-9
+
+
+def test_symmetric_template_finds_ascending_and_descending_chirps():
+    """One time-symmetric template recovers an injection of the ascending chirp AND one of its descending mirror
+    ("suitable in searches for both ascending and descending chirps"), each at the injected offset and
+    with about 1/sqrt 2 of the one-way template's output; the one-way template of the ascending chirp sees the
+    descending one at noise level."""
+    f0, fd = 900.0, 300.0
+    L = int(round(TAU * FS))
+    Tp = (L - 1) / FS
+    w_sym = bo.template_real_sym(f0, fd, TAU, FS, N)
+    w_up = bo.template_real(f0, fd, TAU, FS, N)
+    noise = synth.band_limit(synth.white_noise(31))
+    x_up, n_up = synth.inject_chirp(noise, f0, fd, 4.0, 12.0)
+    x_dn, n_dn = synth.inject_chirp(noise, f0 + fd * Tp, -fd, 11.0, 12.0)
+    for x, n0, one_way_sees_it in ((x_up, n_up, True), (x_dn, n_dn, False)):
+        X = bo.segment_spectrum(x.astype(np.complex128), FS, *BAND)
+        z, s1, _ = bo.correlate_dual(X, w_sym)
+        rho = np.abs(z.real) / s1
+        peak = int(np.argmax(rho))
+        assert abs(peak - n0) <= 8 and rho[peak] > 6.5
+        z1, t1, _ = bo.correlate_dual(X, w_up)
+        rho1 = np.abs(z1.real) / t1
+        if one_way_sees_it:
+            assert abs(int(np.argmax(rho1)) - n0) <= 8
+            assert 0.6 < rho[peak] / rho1.max() < 0.85                      # ~ 1/sqrt 2
+        else:
+            assert rho1[n0 - 64: n0 + 64].max() < 5.5                       # the one-way template misses the mirror chirp
+
+
+def test_symmetric_dual_search_is_the_per_template_maximum():
+    """bo_search_dual_sym is bo_search_dual with the symmetric template: rebuilt offset by offset from
+    bo_correlate_dual on a small bank."""
+    h1, l1, x = _packed_noise(25, 26)
+    X = bo.segment_spectrum(x, FS, *BAND)
+    f0, fd = np.array([500.0, 1200.0, 1700.0]), np.array([150.0, -300.0, 50.0])
+    k = 3.0
+    o1, i1, o2, i2, sig = bo.search_dual(X[None, :], f0, fd, TAU, FS, k, symmetric=True)
+    b1, b2 = np.zeros(N), np.zeros(N)
+    j1, j2 = np.full(N, 0xFFFFFFFF, dtype=np.uint32), np.full(N, 0xFFFFFFFF, dtype=np.uint32)
+    for j in range(3):
+        z, s1, s2 = bo.correlate_dual(X, bo.template_real_sym(f0[j], fd[j], TAU, FS, N))
+        assert abs(sig[j, 0, 0] - s1) < 1e-15 and abs(sig[j, 0, 1] - s2) < 1e-15
+        for b, jj, a, s in ((b1, j1, np.abs(z.real), s1), (b2, j2, np.abs(z.imag), s2)):
+            hit = (a > k * s) & (a / s > b)
+            b[hit] = (a / s)[hit]
+            jj[hit] = j
+    assert np.array_equal(o1[0], b1) and np.array_equal(o2[0], b2)
+    assert np.array_equal(i1[0], j1) and np.array_equal(i2[0], j2)
+    assert (i1[0] != 0xFFFFFFFF).sum() > 100
+
+
 def test_dual_sigma_is_eq6_and_eq7():
     """sigma per detector stream: the definition (eq.6, rms of the real output) against an independent numpy
     evaluation, and against Parseval's half-spectrum form for a real series (eq.7), which is the
