@@ -148,6 +148,15 @@ int bege_search_maxproj(bege_plan*, float k_sigma, float* snr_out, uint32_t* id_
  * bege_get_sigma_dual: sigma_1, sigma_2 of the last bege_search_dual, n_templates*n_segments floats each, template-major.
  */
 int bege_bank_generate_real(bege_plan*, const double* f0_hz, const double* fdot_hz_s, uint64_t n_templates, double tau_s);
+/*
+ * The paper's own template form (Fig.2 caption: "The chirps used in butterfly filtering are symmetric in time,
+ * obtained by superposition of chirp forward and backward in time, suitable in searches for both ascending and descending
+ * chirps"): as bege_bank_generate_real with w_n = u_n + u_(L-1-n), u_n = hann_L[n] cos(2 pi (f0 t_n + fdot t_n^2/2)) the one-way
+ * template, L = round(tau_s fs), unit L2 norm -- the ascending chirp (f0, fdot) plus the descending chirp that starts where it
+ * ends.  One such template answers to both; each at about 1/sqrt 2 of the one-way template's output.  A bank made here counts
+ * as a real bank for bege_search_dual.
+ */
+int bege_bank_generate_real_symmetric(bege_plan*, const double* f0_hz, const double* fdot_hz_s, uint64_t n_templates, double tau_s);
 int bege_search_dual(bege_plan*, float k_sigma, float* snr1_out, uint32_t* id1_out, float* snr2_out, uint32_t* id2_out,
                      double delta_hz, uint64_t* n_simultaneous, uint64_t* n_coincident);
 int bege_get_sigma_dual(bege_plan*, float* sigma1_out, float* sigma2_out);

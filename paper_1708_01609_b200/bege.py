@@ -28,7 +28,7 @@ SYMBOLS = [
     "bege_bank_generate_real", "bege_search_dual", "bege_get_sigma_dual",
     "bege_debug_template_spectrum", "bege_debug_segment_spectrum", "bege_debug_set_max_items", "bege_plan_set_profiling",
     "bege_plan_get_stats", "bege_plan_reset_stats", "bege_last_error", "bege_plan_destroy", "bege_version", "bege_ovs_probe",
-    "bege_segment_spectrum_static",
+    "bege_segment_spectrum_static", "bege_bank_generate_real_symmetric",
 ]
 STATIC_MAX_SEGMENTS = 4           # BEGE_STATIC_MAX_SEGMENTS (include/bege.h)
 
@@ -68,6 +68,7 @@ def load_library() -> ctypes.CDLL:
     L.bege_search_maxproj.argtypes = [vp, ctypes.c_float, vp, vp, ctypes.POINTER(u64)]
     L.bege_get_sigma.argtypes = [vp, vp]
     L.bege_bank_generate_real.argtypes = [vp, vp, vp, u64, dbl]
+    L.bege_bank_generate_real_symmetric.argtypes = [vp, vp, vp, u64, dbl]
     L.bege_search_dual.argtypes = [vp, ctypes.c_float, vp, vp, vp, vp, dbl, ctypes.POINTER(u64), ctypes.POINTER(u64)]
     L.bege_get_sigma_dual.argtypes = [vp, vp, vp]
     L.bege_debug_correlate.argtypes = [vp, u64, u32, vp, ctypes.POINTER(ctypes.c_float)]
@@ -179,12 +180,14 @@ class Plan:
         self._check(self._L.bege_bank_generate(self._h, f0.ctypes.data, fdot.ctypes.data, f0.size, float(tau)))
         self.n_templates = int(f0.size)
 
-    def bank_generate_real(self, f0, fdot, tau: float = 1.0):
-        """Bank of real templates (dual-stream search)."""
+    def bank_generate_real(self, f0, fdot, tau: float = 1.0, symmetric: bool = False):
+        """Bank of real templates (dual-stream search).  symmetric: bege_bank_generate_real_symmetric, the paper's
+        time-symmetric chirps (forward + backward in time)."""
         f0 = np.ascontiguousarray(np.asarray(f0, dtype=np.float64))
         fdot = np.ascontiguousarray(np.asarray(fdot, dtype=np.float64))
         assert f0.ndim == 1 and f0.shape == fdot.shape
-        self._check(self._L.bege_bank_generate_real(self._h, f0.ctypes.data, fdot.ctypes.data, f0.size, float(tau)))
+        fn = self._L.bege_bank_generate_real_symmetric if symmetric else self._L.bege_bank_generate_real
+        self._check(fn(self._h, f0.ctypes.data, fdot.ctypes.data, f0.size, float(tau)))
         self.n_templates = int(f0.size)
 
     def segment_load(self, x):

@@ -68,8 +68,11 @@ BEGE_DD void dfft16f(d2 (&a)[16])
 // hann: L window values times 1 / ||h|| (host, fp64).  tw256d[m] = exp(2 pi i m / 256).
 constexpr int kBankSmem = 3 * 4096 * 16;   // samples + two exchange buffers, fp64 complex
 
-// real_tpl: the real template of the dual-stream search, w_n = hann_n cos(2 pi c_n) / ||.||; its
+// real_tpl = 1: the real template of the dual-stream search, w_n = hann_n cos(2 pi c_n) / ||.||; its
 // norm depends on the template and is formed here (fp64 block sum).
+// real_tpl = 2: the time-symmetric real template ("superposition of chirp forward and backward in time"),
+// w_n = hann_n (cos 2 pi c_n + cos 2 pi c_(L-1-n)) / ||.||.  The reversed phase is itself a quadratic in n,
+// c_(L-1-n) = c(T') - (f0 + fdot T') t_n + fdot t_n^2 / 2 with T' = (L-1)/fs, so it runs on a second recurrence.
 __global__ void __launch_bounds__(256, 1)
 k_bank_gen64(const double* __restrict__ f0, const double* __restrict__ fdot, uint64_t T, double fs, uint32_t L,
              const double* __restrict__ hann, const d2* __restrict__ tw256d, float2* __restrict__ out,
@@ -98,15 +101,21 @@ k_bank_gen64(const double* __restrict__ f0, const double* __restrict__ fdot, uin
             d2 z = expc(f * tt + 0.5 * fd * tt * tt);
             d2 D = expc(f * dt + 0.5 * fd * (2.0 * tt * dt + dt * dt));
             const d2 C = expc(fd * dt * dt);
+            // the time-reversed chirp (real_tpl = 2): start frequency -(f0 + fdot T'), same second difference
+            const double Tp = (double)(L - 1) / fs, fr = -(f + fd * Tp);
+            d2 zr = expc(f * Tp + 0.5 * fd * Tp * Tp + fr * tt + 0.5 * fd * tt * tt);
+            d2 Dr = expc(fr * dt + 0.5 * fd * (2.0 * tt * dt + dt * dt));
             double n2 = 0.0;
 #pragma unroll
             for (int nh = 0; nh < 16; ++nh) {
                 const uint32_t n = (uint32_t)t + 256u * nh;
                 const double w = n < L ? hann[n] : 0.0;
-                base[nh * 256 + t] = dmk(w * z.x, real_tpl ? 0.0 : w * z.y);
-                n2 += (w * z.x) * (w * z.x);
+                const double xr = real_tpl == 2 ? w * (z.x + zr.x) : w * z.x;
+                base[nh * 256 + t] = dmk(xr, real_tpl ? 0.0 : w * z.y);
+                n2 += xr * xr;
                 z = dmul(z, D.x, D.y);
                 D = dmul(D, C.x, C.y);
+                if (real_tpl == 2) { zr = dmul(zr, Dr.x, Dr.y); Dr = dmul(Dr, C.x, C.y); }
             }
             if (real_tpl) {                                  // unit L2 norm of the real template
 #pragma unroll

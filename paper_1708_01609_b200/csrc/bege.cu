@@ -1201,19 +1201,25 @@ extern "C" int bege_plan_set_workspace(bege_plan* p, void* dev_ptr, uint64_t byt
     return BEGE_OK;
 }
 
-static int bank_generate_impl(bege_plan* p, const double* f0, const double* fdot, uint64_t T, double tau, bool real_tpl);
+static int bank_generate_impl(bege_plan* p, const double* f0, const double* fdot, uint64_t T, double tau, int real_tpl);
 
 extern "C" int bege_bank_generate(bege_plan* p, const double* f0, const double* fdot, uint64_t T, double tau)
 {
-    return bank_generate_impl(p, f0, fdot, T, tau, false);
+    return bank_generate_impl(p, f0, fdot, T, tau, 0);
 }
 
 extern "C" int bege_bank_generate_real(bege_plan* p, const double* f0, const double* fdot, uint64_t T, double tau)
 {
-    return bank_generate_impl(p, f0, fdot, T, tau, true);
+    return bank_generate_impl(p, f0, fdot, T, tau, 1);
 }
 
-static int bank_generate_impl(bege_plan* p, const double* f0, const double* fdot, uint64_t T, double tau, bool real_tpl)
+extern "C" int bege_bank_generate_real_symmetric(bege_plan* p, const double* f0, const double* fdot, uint64_t T, double tau)
+{
+    return bank_generate_impl(p, f0, fdot, T, tau, 2);
+}
+
+// real_tpl: 0 complex chirp, 1 its real part, 2 the time-symmetric real template (see k_bank_gen64)
+static int bank_generate_impl(bege_plan* p, const double* f0, const double* fdot, uint64_t T, double tau, int real_tpl)
 {
     if (!p) return BEGE_EINVAL;
     if (!f0 || !fdot || T == 0 || T > 0xffffffffull) return fail(p, BEGE_EINVAL, "bad bank arguments");
@@ -1241,12 +1247,12 @@ static int bank_generate_impl(bege_plan* p, const double* f0, const double* fdot
     CU(p, cudaMemcpyAsync(d_hann, hann.data(), L * sizeof(double), cudaMemcpyHostToDevice, p->stream));
     const uint64_t stride = tpl_bytes(p) / sizeof(c2);
     const unsigned ctas = (unsigned)std::min<uint64_t>(T, (uint64_t)p->n_sm);
-    k_bank_gen64<<<ctas, 256, kBankSmem, p->stream>>>(d_f0, d_fd, T, p->fs, L, d_hann, p->tw256d, (float2*)bank, stride, p->I0, p->NI, real_tpl ? 1 : 0);
+    k_bank_gen64<<<ctas, 256, kBankSmem, p->stream>>>(d_f0, d_fd, T, p->fs, L, d_hann, p->tw256d, (float2*)bank, stride, p->I0, p->NI, real_tpl);
     count_launch(p);
     CU(p, cudaStreamSynchronize(p->stream));                 // `hann` (pageable) must outlive its copy
     CU(p, cudaGetLastError());
     CU(p, cudaStreamSynchronize(p->stream));
-    p->T = T; p->tau = tau; p->L = L; p->bank_real = real_tpl;
+    p->T = T; p->tau = tau; p->L = L; p->bank_real = real_tpl != 0;
     return BEGE_OK;
 }
 

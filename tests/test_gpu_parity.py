@@ -674,6 +674,53 @@ def test_dual_stream_silent_detector(bo, bege):
     assert both.sum() > 2000 and np.max(np.abs(g1[both] - o1[both]) / o1[both]) < 2e-5
 
 
+def test_symmetric_real_bank_matches_oracle(bo, bege):
+    """bege_bank_generate_real_symmetric (chirp forward + backward in time): stored spectra against the
+    oracle's, and a dual-stream search in which ONE template finds an ascending chirp in H1 and its descending mirror
+    in L1."""
+    f0c, fdc = 900.0, 300.0
+    L = int(round(TAU * FS))
+    Tp = (L - 1) / FS
+    h1, n_up = synth.inject_chirp(synth.band_limit(synth.white_noise(80)), f0c, fdc, 4.0, 12.0)
+    l1, n_dn = synth.inject_chirp(synth.band_limit(synth.white_noise(81)), f0c + fdc * Tp, -fdc, 11.0, 12.0)
+    xs = (h1 + 1j * l1).astype(np.complex64)[None, :]
+    Xs = np.stack([bo.segment_spectrum(x, FS, *BAND) for x in xs])
+    w = synth.config0()
+    f0 = np.concatenate([w.f0[::6], [f0c]])                  # 43 + 1 templates, the last one matches the injections
+    fd = np.concatenate([w.fdot[::6], [fdc]])
+    jc = f0.size - 1
+    k = 3.0
+    o1, oi1, o2, oi2, sig_o = bo.search_dual(Xs, f0, fd, TAU, FS, k - 1e-3, symmetric=True)
+    kept = np.zeros(N, dtype=bool)
+    kept[4096:61440] = True
+    with bege.Plan(N, FS, BAND) as plan:
+        plan.bank_generate_real(f0, fd, TAU, symmetric=True)
+        for j in (0, 17, jc):
+            H = bo.fft(bo.template_real_sym(f0[j], fd[j], TAU, FS, N), -1)
+            Hg = plan.debug_template_spectrum(j).astype(np.complex128)
+            assert np.linalg.norm(Hg[kept] - H[kept]) / np.linalg.norm(H) < 1e-6, j
+        plan.segment_load(xs)
+        g1, gi1, g2, gi2, _, _ = plan.search_dual(k, 300.0)
+        s1, s2 = plan.get_sigma_dual()
+        z, _, _ = bo.correlate_dual(Xs[0], bo.template_real_sym(f0[jc], fd[jc], TAU, FS, N))
+        zg, _ = plan.debug_correlate(jc, 0)
+        assert rel_l2(zg.astype(np.complex128), z) <= REL_L2
+    assert np.max(np.abs(s1 - sig_o[:, :, 0]) / sig_o[:, :, 0]) <= SIGMA_RTOL
+    assert np.max(np.abs(s2 - sig_o[:, :, 1]) / sig_o[:, :, 1]) <= SIGMA_RTOL
+    none = np.iinfo(np.uint32).max
+    for g, gi, o, oi in ((g1, gi1, o1, oi1), (g2, gi2, o2, oi2)):
+        assert np.all((g == 0) == (gi == none))
+        must, may = o > k + GUARD, o > k - GUARD
+        assert not np.any(must & (g == 0)) and not np.any((g > 0) & ~may)
+        both = must & (g > 0)
+        assert both.sum() > 3000 and np.max(np.abs(g[both] - o[both]) / o[both]) < 2e-5
+        clear = both & (o > 6.0)                              # well above the noise maxima: the winner is unambiguous
+        assert np.array_equal(gi[clear], oi[clear])
+    p1, p2 = int(np.argmax(g1[0])), int(np.argmax(g2[0]))
+    assert gi1[0, p1] == jc and abs(p1 - n_up) <= 8 and g1[0, p1] > 6.5      # ascending chirp, H1
+    assert gi2[0, p2] == jc and abs(p2 - n_dn) <= 8 and g2[0, p2] > 6.5      # descending chirp, L1, same template
+
+
 # ----------------------------------------------------------------------------- overlap-save bake-off probe
 def test_overlap_save_probe_matches_oracle(bo, bege):
     """six 16384-point block correlations reproduce the oracle's circular correlation on every lag.
