@@ -230,44 +230,6 @@ def run_ovs_probe(args, rank, local_rank):
                       "note": "bake-off probe (SURVEY 8(f)4); correlations/s = templates/s, six blocks each"}), flush=True)
 
 
-# ------------------------------------------------------------------------------------------ launch self-test stand-in
-class _LaunchSelfTestPlan:
-    """NOT a search.  `--selftest-launch` exercises bench.py's own multi-rank plumbing (spawn, rendezvous, barrier,
-    max-over-ranks timing, gather of tail records on rank 0) on a box without GPUs; it stands in for bege.Plan with
-    the same method names, produces a few fixed records per chunk and never runs under any other flag.  The JSON
-    line of such a run carries "selftest_launch": true and value null."""
-
-    def __init__(self, rank):
-        self.rank, self.n, self.launches = rank, 0, 0
-
-    def stats(self):
-        return {"hbm_bytes_per_template": 14 * 32768, "kernel_launches": self.launches, "fused_kernel_ms": 1.0,
-                "fused_kernel_launches": 1}
-
-    def alloc_workspace(self, *a):
-        return 0
-
-    def bank_generate(self, f0, fdot, tau):
-        self.n = len(f0)
-
-    def segment_load(self, x):
-        self.launches += 2
-
-    def search(self, k, cap=0, copy=True):
-        from paper_1708_01609_b200 import bege
-        self.launches += 1
-        t = np.zeros(3, dtype=bege.TAIL_DTYPE)
-        t["template_id"] = [0, self.n // 2, self.n - 1]
-        t["lag"] = 100 + self.rank
-        t["snr"] = 7.0
-        time.sleep(0.01)
-        return t, 3
-
-    def set_profiling(self, on): pass
-    def reset_stats(self): pass
-    def close(self): pass
-
-
 # ------------------------------------------------------------------------------------------ our arm
 def _extra_workloads(args, dev, local_rank):
     """configs[3] (segment-batched) and configs[4] (tail-heavy), measured like the headline: CUDA events around
@@ -374,7 +336,7 @@ def run_ours(args, rank, world, local_rank):
     import torch.distributed as dist
     from paper_1708_01609_b200 import bege, shard
 
-    selftest = args.selftest_launch
+    selftest = bool(args.selftest_launch)
     dev = None
     if not selftest:
         torch.cuda.set_device(local_rank)
@@ -395,7 +357,10 @@ def run_ours(args, rank, world, local_rank):
     k_sigma, cap = 6.0, 1 << 16
 
     if selftest:
-        plan = _LaunchSelfTestPlan(rank)
+        # MODULE:FACTORY of a stand-in plan (tests/launch_selftest_plan.py): nothing in this file fabricates records
+        import importlib
+        mod, _, factory = args.selftest_launch.partition(":")
+        plan = getattr(importlib.import_module(mod), factory)(rank)
         chunk = args.chunk or T_total
     else:
         plan = bege.Plan(synth.N_SEG, synth.FS, synth.BAND, device=local_rank)
@@ -589,7 +554,8 @@ def spawn_ranks(args):
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
            "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
     env = dict(os.environ)
-    env.setdefault("NCCL_DEBUG", "WARN")
+    env.setdefault("NCCL_DEBUG", "INFO")              # communicator / rank lines on stderr (the driver counts ranks from them)
+    env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
     return subprocess.call(cmd, env=env)
 
 
@@ -610,8 +576,9 @@ def main():
     ap.add_argument("--tail-cap", type=int, default=80_000_000)
     ap.add_argument("--cufft-batch", type=int, default=2048, help="templates per step of the --impl cufft reference point")
     ap.add_argument("--ovs-templates", type=int, default=147456, help="templates of the --impl ovs_probe measurement")
-    ap.add_argument("--selftest-launch", action="store_true",
-                    help="exercise the multi-rank plumbing only (gloo, no GPU, no search): see _LaunchSelfTestPlan")
+    ap.add_argument("--selftest-launch", default="", metavar="MODULE:FACTORY",
+                    help="exercise the multi-rank plumbing only (gloo, no GPU, no search) with the stand-in plan that "
+                         "FACTORY(rank) of the importable MODULE returns; used by tests/test_host_logic.py")
     args = ap.parse_args()
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "ours":
         sys.exit(spawn_ranks(args))

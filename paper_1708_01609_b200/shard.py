@@ -1,7 +1,7 @@
 """Multi-GPU host logic: the search shards over the template bank (eq.11-12 partitions the
 bank into sets W_alpha and runs independent GPUs, :211).  One process per GPU, each searches its own slice;
-no collective on the data path.  The only exchange is the concatenation of the (rare) tail records on
-rank 0 after the search, done with torch.distributed (NCCL on GPUs, gloo in the CPU tests).
+no collective on the data path.  The only exchange is the concatenation of the tail records on rank 0 after the
+search: a host-side merge over a gloo group (the records are in pinned host memory already), exact sizes, no padding.
 """
 from __future__ import annotations
 
@@ -31,25 +31,49 @@ def globalize(tails: np.ndarray, offset: int) -> np.ndarray:
     return out
 
 
+_host_groups: dict = {}
+
+
+def _host_group(group):
+    """A gloo group over the ranks of `group` (made once, collectively, on first use).  The records of a search are
+    already in host memory when it returns, so they are merged on the host: no copy back to the device, no NCCL."""
+    import torch.distributed as dist
+
+    if dist.get_backend(group) == "gloo":
+        return group
+    key = id(group) if group is not None else None
+    if key not in _host_groups:
+        ranks = dist.get_process_group_ranks(group) if group is not None else None
+        _host_groups[key] = dist.new_group(ranks=ranks, backend="gloo")
+    return _host_groups[key]
+
+
 def gather_tails(tails: np.ndarray, group=None, dst: int = 0):
-    """Concatenate every rank's records on `dst` (returns None elsewhere).  Records are plain bytes
-    (12 B each); counts go first so that ranks with no tails cost nothing but the count."""
+    """Concatenate every rank's records on `dst` (returns None elsewhere), in rank order -- the host-side merge of the
+    independent GPUs' outputs (PAPER.md:187-191 eq.17, :211).  Records are plain bytes (12 B each).  Sizes go first
+    (one all_gather of an int64); then every rank with records sends exactly its own bytes to `dst` over gloo:
+    nothing is padded to the largest rank and nothing passes through device memory.  Collective: every rank of
+    `group` must call it.  `dst` is a global rank."""
     import torch
     import torch.distributed as dist
 
-    world, rank = dist.get_world_size(group), dist.get_rank(group)
-    backend = dist.get_backend(group)
-    dev = torch.device("cuda", torch.cuda.current_device()) if backend == "nccl" else torch.device("cpu")
-    raw = torch.from_numpy(np.ascontiguousarray(tails).view(np.uint8).copy()).to(dev)
-    counts = [torch.zeros(1, dtype=torch.int64, device=dev) for _ in range(world)]
-    dist.all_gather(counts, torch.tensor([raw.numel()], dtype=torch.int64, device=dev), group=group)
+    pg = _host_group(group)
+    rank = dist.get_rank()
+    ranks = dist.get_process_group_ranks(pg) if pg is not None else list(range(dist.get_world_size()))
+    raw = torch.from_numpy(np.ascontiguousarray(tails).view(np.uint8).reshape(-1).copy())
+    counts = [torch.zeros(1, dtype=torch.int64) for _ in ranks]
+    dist.all_gather(counts, torch.tensor([raw.numel()], dtype=torch.int64), group=pg)
     sizes = [int(c.item()) for c in counts]
-    width = max(max(sizes), 1)
-    padded = torch.zeros(width, dtype=torch.uint8, device=dev)
-    padded[: raw.numel()] = raw
-    bufs = [torch.zeros(width, dtype=torch.uint8, device=dev) for _ in range(world)] if rank == dst else None
-    dist.gather(padded, bufs, dst=dst, group=group)
     if rank != dst:
+        if raw.numel():
+            dist.send(raw, dst=dst, group=pg)
         return None
-    parts = [b[:n].cpu().numpy().view(tails.dtype) for b, n in zip(bufs, sizes)]
-    return np.concatenate(parts) if parts else tails[:0]
+    parts = []
+    for r, n in zip(ranks, sizes):
+        if r == dst:
+            parts.append(raw)
+        elif n:
+            buf = torch.empty(n, dtype=torch.uint8)
+            dist.recv(buf, src=r, group=pg)
+            parts.append(buf)
+    return np.concatenate([b.numpy().view(tails.dtype) for b in parts]) if parts else tails[:0]

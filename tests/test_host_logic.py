@@ -147,6 +147,45 @@ def test_two_rank_bank_sharding_over_gloo():
     assert q.get(timeout=5) is True
 
 
+def _gather_worker(rank, world, port, q):
+    """gather_tails alone: rank 1 holds 10^6 records, rank 0 three, rank 2 none -- exact sizes, rank order, every byte."""
+    import torch.distributed as dist
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        n = (3, 1_000_000, 0)[rank]
+        t = np.zeros(n, dtype=bege.TAIL_DTYPE)
+        t["template_id"] = np.arange(n, dtype=np.uint32) * np.uint32(rank + 1)
+        t["lag"] = np.arange(n, dtype=np.uint32)[::-1]
+        t["snr"] = 5.0 + rank
+        out = shard.gather_tails(t)
+        out2 = shard.gather_tails(t[: n // 2])               # a second call reuses the group
+        if rank == 0:
+            ok = (out.size == 1_000_003 and np.array_equal(out["template_id"][:3], [0, 1, 2])
+                  and np.array_equal(out["template_id"][3:], np.arange(1_000_000, dtype=np.uint32) * np.uint32(2))
+                  and np.array_equal(out["lag"][3:], np.arange(1_000_000, dtype=np.uint32)[::-1])
+                  and np.all(out["snr"][:3] == 5.0) and np.all(out["snr"][3:] == 6.0) and out2.size == 1 + 500_000)
+            q.put(bool(ok))
+        else:
+            assert out is None and out2 is None
+    finally:
+        dist.destroy_process_group()
+
+
+def test_gather_tails_exact_sizes_three_ranks():
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_gather_worker, args=(r, 3, port, q)) for r in range(3)]
+    for p in procs:
+        p.start()
+    for p in procs:
+        p.join(120)
+        assert p.exitcode == 0
+    assert q.get(timeout=5) is True
+
+
 def test_bench_starts_its_own_ranks_and_gathers_tails():
     """`python bench.py --gpus 2` with no torchrun environment must start two ranks by itself, rendezvous on
     127.0.0.1, time with max-over-ranks and gather the tail records on rank 0.  No GPU here: --selftest-launch
@@ -155,8 +194,10 @@ def test_bench_starts_its_own_ranks_and_gathers_tails():
     import json
     import subprocess
     env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    env["PYTHONPATH"] = os.path.join(ROOT, "tests") + os.pathsep + env.get("PYTHONPATH", "")   # the stand-in plan lives here
     out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "1", "--warmup", "0",
-                          "--selftest-launch", "--templates", "1000", "--chunk", "400"],
+                          "--selftest-launch", "launch_selftest_plan:LaunchSelfTestPlan", "--templates", "1000",
+                          "--chunk", "400"],
                          capture_output=True, text=True, timeout=300, env=env)
     assert out.returncode == 0, out.stderr[-2000:]
     lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
