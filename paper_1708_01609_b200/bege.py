@@ -13,6 +13,7 @@ import numpy as np
 
 _HERE = Path(__file__).resolve().parent
 LIB_PATH = _HERE / "libbege.so"
+PROBE_LIB_PATH = _HERE / "libbege_probe.so"      # measurement probes (include/bege_probe.h), not part of the product ABI
 
 TAIL_DTYPE = np.dtype([("template_id", "<u4"), ("lag", "<u4"), ("snr", "<f4")])
 assert TAIL_DTYPE.itemsize == 12
@@ -27,9 +28,10 @@ SYMBOLS = [
     "bege_segment_load", "bege_search", "bege_search_band", "bege_search_maxproj", "bege_get_sigma", "bege_debug_correlate",
     "bege_bank_generate_real", "bege_search_dual", "bege_get_sigma_dual",
     "bege_debug_template_spectrum", "bege_debug_segment_spectrum", "bege_debug_set_max_items", "bege_plan_set_profiling",
-    "bege_plan_get_stats", "bege_plan_reset_stats", "bege_last_error", "bege_plan_destroy", "bege_version", "bege_ovs_probe",
+    "bege_plan_get_stats", "bege_plan_reset_stats", "bege_last_error", "bege_plan_destroy", "bege_version",
     "bege_segment_spectrum_static", "bege_bank_generate_real_symmetric",
 ]
+PROBE_SYMBOLS = ["bege_ovs_probe"]   # include/bege_probe.h
 STATIC_MAX_SEGMENTS = 4           # BEGE_STATIC_MAX_SEGMENTS (include/bege.h)
 
 
@@ -75,7 +77,6 @@ def load_library() -> ctypes.CDLL:
     L.bege_debug_template_spectrum.argtypes = [vp, u64, vp]
     L.bege_debug_segment_spectrum.argtypes = [vp, u32, vp]
     L.bege_debug_set_max_items.argtypes = [vp, u64]
-    L.bege_ovs_probe.argtypes = [i32, u64, u32, u32, ctypes.c_float, vp, vp, vp, u64, ctypes.POINTER(dbl), ctypes.POINTER(u64)]
     L.bege_segment_spectrum_static.argtypes = [i32, vp, dbl, dbl, dbl, vp, u32, vp, ctypes.c_char_p, u64]
     L.bege_plan_set_profiling.argtypes = [vp, i32]
     L.bege_plan_get_stats.argtypes = [vp, ctypes.POINTER(Stats)]
@@ -90,6 +91,23 @@ def load_library() -> ctypes.CDLL:
             getattr(L, name).restype = i32
     _lib = L
     return L
+
+
+_probe_lib = None
+
+
+def load_probe_library() -> ctypes.CDLL:
+    """dlopen the in-tree probe library (experiments that are deliberately not in libbege.so)."""
+    global _probe_lib
+    if _probe_lib is None:
+        if not PROBE_LIB_PATH.exists():
+            raise RuntimeError(f"{PROBE_LIB_PATH} is missing: build it with `python -m paper_1708_01609_b200.build`")
+        L = ctypes.CDLL(str(PROBE_LIB_PATH))
+        vp, u32, u64, dbl, i32 = ctypes.c_void_p, ctypes.c_uint32, ctypes.c_uint64, ctypes.c_double, ctypes.c_int
+        L.bege_ovs_probe.argtypes = [i32, u64, u32, u32, ctypes.c_float, vp, vp, vp, u64, ctypes.POINTER(dbl), ctypes.POINTER(u64)]
+        L.bege_ovs_probe.restype = i32
+        _probe_lib = L
+    return _probe_lib
 
 
 class Plan:
@@ -301,8 +319,9 @@ class Plan:
 
 def ovs_probe(n_templates: int, n_blocks: int = 6, reps: int = 3, thr2: float = 3.0e38, h16=None, x16=None,
               want_z: bool = False, dbg_j: int = 0, device: int = 0):
-    """bege_ovs_probe (include/bege.h): the overlap-save bake-off probe.  Returns (ms per pass, hits, z or None)."""
-    L = load_library()
+    """bege_ovs_probe (include/bege_probe.h, libbege_probe.so): the overlap-save bake-off probe.
+    Returns (ms per pass, hits, z or None)."""
+    L = load_probe_library()
     ms, hits = ctypes.c_double(0.0), ctypes.c_uint64(0)
     z = np.empty((n_blocks, 16384), dtype=np.complex64) if want_z else None
     if h16 is not None:

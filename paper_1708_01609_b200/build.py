@@ -1,4 +1,5 @@
-"""Builds the C-ABI library `libbege.so` in-tree with nvcc for sm_100a (no GPU needed to compile)."""
+"""Builds the C-ABI library `libbege.so` (the product) and `libbege_probe.so` (measurement probes kept out of the
+product) in-tree with nvcc for sm_100a (no GPU needed to compile)."""
 from __future__ import annotations
 
 import os
@@ -9,9 +10,11 @@ from pathlib import Path
 HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 LIB = HERE / "libbege.so"
+PROBE_LIB = HERE / "libbege_probe.so"
 SOURCES = [CSRC / "bege.cu"]
-# everything the library is compiled from: a change to any of these makes the built .so stale
-HEADERS = sorted(CSRC.glob("*.cuh")) + [HERE.parent / "include" / "bege.h"]
+PROBE_SOURCES = [CSRC / "bege_probe.cu"]
+# everything the libraries are compiled from: a change to any of these makes the built .so stale
+HEADERS = sorted(CSRC.glob("*.cuh")) + sorted((HERE.parent / "include").glob("*.h"))
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC", "--use_fast_math=false"]
@@ -24,26 +27,32 @@ def _nvcc() -> str:
     return "nvcc"
 
 
-def stale() -> bool:
-    if not LIB.exists():
+def stale(lib: Path = LIB, sources=None) -> bool:
+    if not lib.exists():
         return True
-    t = LIB.stat().st_mtime
-    return any(f.stat().st_mtime > t for f in SOURCES + HEADERS)
+    t = lib.stat().st_mtime
+    return any(f.stat().st_mtime > t for f in (sources or SOURCES) + HEADERS)
 
 
-def build_library(force: bool = False, verbose: bool = False) -> Path:
-    if not force and not stale():
-        return LIB
-    tmp = LIB.with_suffix(f".so.tmp{os.getpid()}")
+def _build(lib: Path, sources, force: bool, verbose: bool) -> Path:
+    if not force and not stale(lib, sources):
+        return lib
+    tmp = lib.with_suffix(f".so.tmp{os.getpid()}")
     flags = [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")]
-    cmd = [_nvcc(), *flags, *(["-Xptxas", "-v"] if verbose else []), "-o", str(tmp), *map(str, SOURCES)]
+    cmd = [_nvcc(), *flags, *(["-Xptxas", "-v"] if verbose else []), "-o", str(tmp), *map(str, sources)]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if verbose:
         sys.stderr.write(res.stderr)
     if res.returncode != 0:
         raise RuntimeError("nvcc failed:\n" + res.stdout + res.stderr)
-    os.replace(tmp, LIB)
-    return LIB
+    os.replace(tmp, lib)
+    return lib
+
+
+def build_library(force: bool = False, verbose: bool = False) -> Path:
+    """The product library (and, beside it, the probe library: tests and `bench.py --impl ovs_probe` load it)."""
+    _build(PROBE_LIB, PROBE_SOURCES, force, verbose)
+    return _build(LIB, SOURCES, force, verbose)
 
 
 if __name__ == "__main__":

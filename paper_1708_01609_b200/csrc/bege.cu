@@ -30,6 +30,7 @@
 #include "../../include/bege.h"
 #include "cplx.cuh"
 #include "async.cuh"
+#include "regs16.cuh"
 #include "bank64.cuh"
 
 #ifndef BEGE_ABL
@@ -264,15 +265,6 @@ template <int NI> struct SearchSmem {
 template <int NI> __host__ __device__ constexpr bool search_stat() { return NI == 14; }
 template <int NI> constexpr int search_smem() { return (int)SearchSmem<NI>::total + 2048; }
 
-// 16 values to shared memory at a + p * STRIDE bytes
-template <int STRIDE, int P = 0> BEGE_D void sts16(uint32_t a, const c2 (&v)[16])
-{
-    if constexpr (P < 16) { sts64<P * STRIDE>(a, v[P]); sts16<STRIDE, P + 1>(a, v); }
-}
-template <int STRIDE, int P = 0> BEGE_D void lds16(uint32_t a, c2 (&v)[16])
-{
-    if constexpr (P < 16) { v[P] = lds64<P * STRIDE>(a); lds16<STRIDE, P + 1>(a, v); }
-}
 // stage 1 of pass 1: v[I0 + 2 ip], v[I0 + 2 ip + 1] = conj(H) X for the row-block pair ip, acc += |.|^2 (packed);
 // q0, q1: the stationary values.  SINGLE: the template streams, the segment is stationary; batched: the other way round
 template <int I0, bool SINGLE, int IP> BEGE_D void products1(uint32_t stream_a, c2 q0, c2 q1, c2 (&v)[16], c2& acc)
@@ -329,24 +321,6 @@ template <int I0, int NI, bool SINGLE, int IP = 0> BEGE_D void gl_products(uint3
         gl_products<I0, NI, SINGLE, IP + 1>(stream_a, statg, v, acc);
     }
 }
-// v[P0 + 2 j + k] *= table entry (2 j + k), entries streamed from tensor memory two at a time, double buffered;
-// the load of chunk 0 into wa was issued by the caller; chunks [0, NCH)
-template <int P0, int NCH, int J = 0> BEGE_D void tm_twiddle(uint32_t taddr, c2 (&v)[16], c2 (&wa)[2], c2 (&wb)[2])
-{
-    if constexpr (J < NCH) {
-        c2 (&cur)[2] = (J & 1) ? wb : wa;
-        c2 (&nxt)[2] = (J & 1) ? wa : wb;
-        tmem_wait_ld(cur);
-        if constexpr (J + 1 < NCH) tmem_ld4(taddr + 4 * (J + 1), nxt);
-        v[P0 + 2 * J] = cmulw(v[P0 + 2 * J], cur[0]);
-        if constexpr (P0 + 2 * J + 1 < 16) v[P0 + 2 * J + 1] = cmulw(v[P0 + 2 * J + 1], cur[1]);
-        tm_twiddle<P0, NCH, J + 1>(taddr, v, wa, wb);
-    }
-}
-
-}  // namespace bege
-#include "ovs_probe.cuh"
-namespace bege {
 
 // DUAL (single-segment calls, 14 row-blocks): the dual-stream search of PAPER.md:155 -- x = H1 + i L1, REAL templates, so
 // Re z and Im z are the two detectors' outputs.  Their variances are the Hermitian split of the product spectrum
@@ -1878,65 +1852,4 @@ extern "C" int bege_segment_spectrum_static(int device, void* cuda_stream, doubl
     CUS(cudaGetLastError());
 #undef CUS
     return BEGE_OK;
-}
-
-// ------------------------------------------------------------------------------------------------
-// bake-off probe of the overlap-save variant (csrc/ovs_probe.cuh).  Self-contained: own device
-// memory, own stream.  h16: T x 16384 complex template spectra (host; NULL: filled on the device with finite numbers,
-// timing only), x16: n_blocks x 16384 complex block spectra (host; NULL likewise).  z_dbg (host, n_blocks x 16384 complex,
-// may be NULL): the correlation blocks of template dbg_j.  *ms_out: mean time of one pass over all T x n_blocks items.
-__global__ void k_ovs_fill(float2* p, uint64_t n, uint32_t seed)
-{
-    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
-        uint32_t h = (uint32_t)i * 2654435761u ^ seed; h ^= h >> 15; h *= 2246822519u; h ^= h >> 13;
-        p[i] = make_float2((float)(int)(h & 0xffff) * (1.0f / 65536.0f) - 0.5f, (float)(int)(h >> 16) * (1.0f / 65536.0f) - 0.5f);
-    }
-}
-
-extern "C" int bege_ovs_probe(int device, uint64_t T, uint32_t n_blocks, uint32_t reps, float thr2, const float* h16,
-                              const float* x16, float* z_dbg, uint64_t dbg_j, double* ms_out, uint64_t* hits_out)
-{
-    if (T == 0 || n_blocks == 0 || reps == 0 || !ms_out) return BEGE_EINVAL;
-    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return BEGE_ECUDA; }
-    cudaDeviceProp prop;
-    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess || prop.major < 10) return BEGE_ECUDA;
-    c2 *dH = nullptr, *dX = nullptr, *dZ = nullptr; unsigned long long* dcnt = nullptr;
-    const uint64_t nH = T * kOvsP, nX = (uint64_t)n_blocks * kOvsP;
-    int rc = BEGE_OK;
-    cudaStream_t st = nullptr;
-    cudaEvent_t e0 = nullptr, e1 = nullptr;
-    auto done = [&](int code) {
-        if (dH) cudaFree(dH); if (dX) cudaFree(dX); if (dZ) cudaFree(dZ); if (dcnt) cudaFree(dcnt);
-        if (e0) cudaEventDestroy(e0); if (e1) cudaEventDestroy(e1); if (st) cudaStreamDestroy(st);
-        cudaGetLastError();
-        return code;
-    };
-    if (cudaMalloc(&dH, nH * 8) != cudaSuccess || cudaMalloc(&dX, nX * 8) != cudaSuccess || cudaMalloc(&dZ, nX * 8) != cudaSuccess ||
-        cudaMalloc(&dcnt, 256) != cudaSuccess) return done(BEGE_ENOMEM);
-    if (cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) != cudaSuccess || cudaEventCreate(&e0) != cudaSuccess ||
-        cudaEventCreate(&e1) != cudaSuccess) return done(BEGE_ECUDA);
-    if (h16) { if (cudaMemcpyAsync(dH, h16, nH * 8, cudaMemcpyHostToDevice, st) != cudaSuccess) return done(BEGE_ECUDA); }
-    else k_ovs_fill<<<1024, 256, 0, st>>>((float2*)dH, nH, 1u);
-    if (x16) { if (cudaMemcpyAsync(dX, x16, nX * 8, cudaMemcpyHostToDevice, st) != cudaSuccess) return done(BEGE_ECUDA); }
-    else k_ovs_fill<<<64, 256, 0, st>>>((float2*)dX, nX, 2u);
-    if (cudaMemsetAsync(dcnt, 0, 256, st) != cudaSuccess) return done(BEGE_ECUDA);
-    if (cudaFuncSetAttribute(k_ovs_probe, cudaFuncAttributeMaxDynamicSharedMemorySize, kOvsSmem) != cudaSuccess) return done(BEGE_ECUDA);
-    const unsigned ctas = (unsigned)std::min<uint64_t>(T * n_blocks, (uint64_t)prop.multiProcessorCount);
-    int* d_abort = (int*)(dcnt + 16);
-    // warm-up pass (also the one that writes z_dbg), then `reps` timed passes
-    k_ovs_probe<<<ctas, 1024, kOvsSmem, st>>>(dH, dX, T, n_blocks, thr2, dcnt, z_dbg ? dZ : nullptr, dbg_j, d_abort);
-    if (cudaMemsetAsync(dcnt, 0, 8, st) != cudaSuccess) return done(BEGE_ECUDA);
-    cudaEventRecord(e0, st);
-    for (uint32_t r = 0; r < reps; ++r)
-        k_ovs_probe<<<ctas, 1024, kOvsSmem, st>>>(dH, dX, T, n_blocks, thr2, dcnt, nullptr, 0, d_abort);
-    cudaEventRecord(e1, st);
-    if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) return done(BEGE_ECUDA);
-    float ms = 0; cudaEventElapsedTime(&ms, e0, e1);
-    *ms_out = (double)ms / reps;
-    unsigned long long hc[17];
-    if (cudaMemcpy(hc, dcnt, sizeof hc, cudaMemcpyDeviceToHost) != cudaSuccess) return done(BEGE_ECUDA);
-    if (hits_out) *hits_out = hc[0] / reps;
-    if (*(int*)&hc[16]) rc = BEGE_ECUDA;
-    if (z_dbg && cudaMemcpy(z_dbg, dZ, nX * 8, cudaMemcpyDeviceToHost) != cudaSuccess) return done(BEGE_ECUDA);
-    return done(rc);
 }

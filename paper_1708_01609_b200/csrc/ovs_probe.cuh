@@ -20,6 +20,7 @@
 #pragma once
 #include "cplx.cuh"
 #include "async.cuh"
+#include "regs16.cuh"
 
 namespace bege {
 

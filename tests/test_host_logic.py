@@ -29,6 +29,13 @@ def test_library_exports_every_declared_symbol(lib):
     for name in declared:
         assert hasattr(lib, name), name
     assert lib.bege_version().decode().startswith("bege")
+    # the probe library has its own header; nothing of it is in the product ABI
+    probe_header = open(os.path.join(ROOT, "include", "bege_probe.h")).read()
+    probe_declared = set(re.findall(r"\b(bege_[a-z_]+)\s*\(", probe_header))
+    assert probe_declared == set(bege.PROBE_SYMBOLS) and not (probe_declared & declared)
+    probe = bege.load_probe_library()
+    for name in probe_declared:
+        assert hasattr(probe, name) and not hasattr(lib, name), name
 
 
 def test_tail_record_is_12_bytes(lib):
