@@ -45,16 +45,16 @@ UNIT = "correlations/s"
 FFT_FLOP = 5.0 * 65536 * 16                       # PAPER.md:134 eq.(10): 5 N log2 N
 ALG_BYTES_PER_CORR = 52802 * 8                    # two-sided in-band template spectrum, S = 1
 # dram__bytes_read.sum + dram__bytes_write.sum of k_search per correlation: an OFFLINE constant, taken from the
-# `ncu --set full` capture of the kernel as committed (profiles/r2_search_kernel.md: 36,864-template launch,
-# 16.914 GB read + 0.024 GB written); it does not follow later kernel changes by itself.
-NCU_DRAM_BYTES_PER_CORR = (16.914e9 + 0.024e9) / 36864
-NCU_SOURCE = "profiles/r2_search_kernel.md"
+# `ncu --set full` capture of the kernel as committed (profiles/r3_search_kernel.md: 36,864-template launch,
+# 16.913 GB read + 0.0245 GB written); it does not follow later kernel changes by itself.
+NCU_DRAM_BYTES_PER_CORR = (16.913445e9 + 0.02447232e9) / 36864
+NCU_SOURCE = "profiles/r3_search_kernel.md"
 FP32_PEAK = 148 * 128 * 2 * 1.965e9               # SMs x fp32 lanes x 2 flop x max SM clock
 FMA_PIPE_CEILING = 8.6e6                          # what the FMA pipe allows for k_search's instruction mix
 # ncu figures of k_search from the same capture (north_star: "ncu dram throughput and FP32 pipe utilisation shown"):
 # OFFLINE constants like the traffic above, percent of peak sustained over the kernel's duration
-NCU_OFFLINE = {"source": NCU_SOURCE, "pipe_fmaheavy_pct": 55.9, "issue_slots_pct": 58.4, "lsu_wavefronts_pct": 66.7,
-               "dram_throughput_gbs": (16.914e9 + 0.024e9) / 7.614e-3 * 1e-9, "warps_active_pct": 50.0,
+NCU_OFFLINE = {"source": NCU_SOURCE, "pipe_fmaheavy_pct": 53.7, "issue_slots_pct": 57.5, "lsu_wavefronts_pct": 66.9,
+               "dram_throughput_gbs": (16.913445e9 + 0.02447232e9) / 7.605216e-3 * 1e-9, "warps_active_pct": 50.0,
                "note": "measured under ncu (serialised, cold cache) on the build named in source; not re-measured in this run"}
 
 
@@ -534,7 +534,7 @@ def run_ours(args, rank, world, local_rank):
                      "ncu_offline": NCU_OFFLINE,
                      "fma_pipe": {"ceiling_corr_per_s": FMA_PIPE_CEILING, "frac": rate_kernel / FMA_PIPE_CEILING,
                                   "note": "context: ~1,000 FMA-pipe cycles per 32 lags x 16 row pairs of this radix-16 arithmetic "
-                                          "(packed f32x2 = 2 cycles; profiles/r2_search_kernel.md); not the roofline denominator"},
+                                          "(packed f32x2 = 2 cycles; profiles/r2_search_kernel.md, r3_search_kernel.md); not the roofline denominator"},
                      "hbm": {"achieved": hbm_achieved, "peak": hbm_peak, "unit": "GB/s",
                              "frac": hbm_achieved / hbm_peak, "of": "measured" if peaks else "fallback",
                              "stored_bytes_per_template": tpl_bytes}},

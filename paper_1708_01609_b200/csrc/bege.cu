@@ -40,6 +40,14 @@
 #define BEGE_ABL 0
 #endif
 
+#ifndef BEGE_FUSE
+// which passes of k_search use the FMA-fused 16-point DFT (cplx.cuh: 72 instead of 81 packed instructions): bit 0 pass 1,
+// bit 1 pass 2.  Measured on one B200, same box, configs[2]: 0: 4.75 / 4.72, 1: 4.66, 2: 4.76 / 4.74,
+// 3: 4.67 / 4.68 M correlations/s -- pass 1 at its 64-register budget spills 16 bytes with the fused form and loses
+// 1.5 %, pass 2 takes it without spills (18 fewer packed instructions per item, rate unchanged within noise).
+#define BEGE_FUSE 2
+#endif
+
 namespace bege {
 
 constexpr int kN = 65536;
@@ -501,7 +509,7 @@ k_search(const __grid_constant__ SearchArgs A)
                 }
             }
             if (SINGLE) src_run += src_step;
-            fft16<+1>(v);
+            fft16<+1, (BEGE_FUSE & 1) != 0>(v);
             tm_twiddle<1, 8>(tq_a + kTmTheta, v, qa, qb);    // v[p] *= theta^p, p = 1 .. 15
             sts16<8>(xw_a, v);
             const float sw = warp_sum32(DUAL ? re(acc) : re(acc) + im(acc));  // (includes the __syncwarp the exchange needs)
@@ -527,7 +535,7 @@ k_search(const __grid_constant__ SearchArgs A)
                 if (counter_load_acquire(d2 + slot) < need) counter_wait_ge(d2 + slot, need, abort_flag);
             }
             __syncwarp();                                    // exchange region free for the next item; ring slot free
-            fft16<+1>(v);
+            fft16<+1, (BEGE_FUSE & 1) != 0>(v);
             // T'[k1 = 16 b + c][n2 = p + 16 q], p = g: a half-warp stores 128 contiguous bytes per q
             c2* out = myring + (uint64_t)slot * kN + (uint32_t)(16 * b + c) * 256u + g;
 #pragma unroll
@@ -674,7 +682,7 @@ k_search(const __grid_constant__ SearchArgs A)
             for (int r = 1; r < 16; ++r) { const float2 w = c_wb[b][r]; v[r] = cmulw(v[r], w.x, w.y); }
             const float sumR2 = row_sum16(part);
             const float sumP = DUAL ? row_sum16(ppart) : 0.f;
-            fft16<+1>(v);
+            fft16<+1, (BEGE_FUSE & 2) != 0>(v);
             if (t == 0 && ib + 2 < n_items && ld_it == ib + 2)   // first chance to bring in the team's next item
                 try_load(ib + 2, (BEGE_ABL & 1) || (d1v_it == ib + 2 && d1v >= 16ull * ((ib + 2) / kRing + 1)));
             tm_twiddle<0, 8>(tq + kTmDelta, v, wa, wb);      // v[p] *= delta_p = wN^(16 b a) w256^(a p)
@@ -689,7 +697,7 @@ k_search(const __grid_constant__ SearchArgs A)
             if (lane == 0) smem_counter_add_release(sb + SM::bempty + 8 * buf, 1);
             if (t == 0 && ib + 2 < n_items && ld_it == ib + 2)   // bring in the team's next item while this one is finished
                 try_load(ib + 2, (BEGE_ABL & 1) || (d1v_it == ib + 2 && d1v >= 16ull * ((ib + 2) / kRing + 1)));
-            fft16<+1>(v);
+            fft16<+1, (BEGE_FUSE & 2) != 0>(v);
             // lane a holds Z[n1 = a + 16 q]; lag n = 256 n1 + n2
             const float thr = A.k2 * sumR2;
             // dual-stream search: the two sums are N^2 sigma_1^2 = V1 for Re z (H1) and N^2 sigma_2^2 = V2 for Im z (L1)

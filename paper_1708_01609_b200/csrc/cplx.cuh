@@ -9,7 +9,7 @@
 //
 // The packed instructions have no per-half sign, so the cross terms of a multiplication by a RUN-TIME complex
 // number w = (c, d) are two scalar FFMAs (free operand negation, same FMA-pipe time as one FFMA2): 3 issue slots
-// and no sign/pack moves.  Compile-time twiddles keep the 2-slot packed form with an immediate (-d, d) pair.
+// and no sign/pack moves.  Compile-time twiddles (fft16) are folded into the butterflies' FMAs and cost one slot.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -82,7 +82,7 @@ BEGE_D c2 tw16(c2 x) {
 // 16-point DFT in registers: A[k] = sum_i a[i] exp(DIR 2 pi i ik/16); in place, natural order in and out.
 // i = i0 + 4 i1, k = k0 + 4 k1:  radix-4 over i1, twiddle w16^(i0 k0), radix-4 over i0.
 template <int DIR>
-BEGE_D void fft16(c2 (&a)[16]) {
+BEGE_D void fft16_plain(c2 (&a)[16]) {
 #pragma unroll
     for (int i0 = 0; i0 < 4; ++i0) fft4<DIR>(a[i0], a[i0 + 4], a[i0 + 8], a[i0 + 12]);
     // now a[i0 + 4 k0] holds B[i0][k0]
@@ -104,6 +104,62 @@ BEGE_D void fft16(c2 (&a)[16]) {
 #pragma unroll
         for (int k1 = k0 + 1; k1 < 4; ++k1) { const c2 t = a[4 * k0 + k1]; a[4 * k0 + k1] = a[4 * k1 + k0]; a[4 * k1 + k0] = t; }
 }
+
+// y + k * (i x): one packed FMA (the half swap and the (-k, k) pair are operand forms, see the header comment)
+BEGE_D c2 fma_i(c2 x, float k, c2 y) { return fma2(swp(x), mk(-k, k), y); }
+
+// 16-point DFT in registers: A[k] = sum_i a[i] exp(DIR 2 pi i ik/16); in place, natural order in and out.
+// i = i0 + 4 i1, k = k0 + 4 k1:  radix-4 over i1, twiddle w16^(i0 k0), radix-4 over i0.
+//
+// The twiddles of the middle step are never applied as multiplications of their own.  With s = DIR, T = tan(pi/8),
+// C = cos(pi/8), H = cos(pi/4):
+//   w16^1 = C (1 + i s T)      w16^2 = H (1 + i s)        w16^3 = i s C (1 - i s T)
+//   w16^4 = i s                w16^6 = i s H (1 + i s)    w16^9 = -C (1 + i s T)
+// so each twiddled input first becomes u = x + (i s t) x (ONE packed FMA, |t| <= 1), and the real scale C or H and
+// the factor i s that remain ride on the FMAs of the radix-4 butterfly that follows (its sums and differences are
+// formed up to the common scale of the odd pair, which the four output FMAs then carry).  Per quartet 11 (10 for
+// k0 = 2) packed instructions instead of 14 (13): 72 per transform instead of 81, all single-rounded FMAs.
+template <int DIR>
+BEGE_D void fft16_fused(c2 (&a)[16]) {
+    constexpr float s = DIR > 0 ? 1.f : -1.f;
+    constexpr float C = 0.92387953251128675613f, H = 0.70710678118654752440f, T = 0.41421356237309504880f;
+#pragma unroll
+    for (int i0 = 0; i0 < 4; ++i0) fft4<DIR>(a[i0], a[i0 + 4], a[i0 + 8], a[i0 + 12]);
+    // now a[i0 + 4 k0] holds B[i0][k0]; radix-4 over i0 for each k0, outputs k = k0 + 4 k1 left in a[4 k0 + k1]
+    fft4<DIR>(a[0], a[1], a[2], a[3]);                       // k0 = 0: no twiddles
+    {   // k0 = 1: twiddles w16^1, w16^2, w16^3
+        const c2 x0 = a[4];
+        const c2 u1 = fma_i(a[5], s * T, a[5]), u2 = fma_i(a[6], s, a[6]), u3 = fma_i(a[7], -s * T, a[7]);
+        const c2 s02 = fma2(bc(H), u2, x0), d02 = fma2(bc(-H), u2, x0);
+        const c2 s13 = fma_i(u3, s, u1), d13 = fma_i(u3, -s, u1);              // (y1 +- y3) / C
+        a[4] = fma2(bc(C), s13, s02); a[6] = fma2(bc(-C), s13, s02);
+        a[5] = fma_i(d13, s * C, d02); a[7] = fma_i(d13, -s * C, d02);
+    }
+    {   // k0 = 2: twiddles w16^2, w16^4, w16^6
+        const c2 x0 = a[8];
+        const c2 u1 = fma_i(a[9], s, a[9]), u3 = fma_i(a[11], s, a[11]);
+        const c2 s02 = fma_i(a[10], s, x0), d02 = fma_i(a[10], -s, x0);
+        const c2 s13 = fma_i(u3, s, u1), d13 = fma_i(u3, -s, u1);              // (y1 +- y3) / H
+        a[8] = fma2(bc(H), s13, s02); a[10] = fma2(bc(-H), s13, s02);
+        a[9] = fma_i(d13, s * H, d02); a[11] = fma_i(d13, -s * H, d02);
+    }
+    {   // k0 = 3: twiddles w16^3, w16^6, w16^9
+        const c2 x0 = a[12];
+        const c2 u1 = fma_i(a[13], -s * T, a[13]), u2 = fma_i(a[14], s, a[14]), u3 = fma_i(a[15], s * T, a[15]);
+        const c2 s02 = fma_i(u2, s * H, x0), d02 = fma_i(u2, -s * H, x0);
+        const c2 m13 = fma_i(u1, -s, u3), d13 = fma_i(u1, s, u3);              // -(y1 + y3) / C, (y1 - y3) / C
+        a[12] = fma2(bc(-C), m13, s02); a[14] = fma2(bc(C), m13, s02);
+        a[13] = fma_i(d13, s * C, d02); a[15] = fma_i(d13, -s * C, d02);
+    }
+    // a[4 k0 + k1] now holds A[k0 + 4 k1]: transpose the 4x4 index (register renaming, free when unrolled)
+#pragma unroll
+    for (int k0 = 0; k0 < 4; ++k0)
+#pragma unroll
+        for (int k1 = k0 + 1; k1 < 4; ++k1) { const c2 t = a[4 * k0 + k1]; a[4 * k0 + k1] = a[4 * k1 + k0]; a[4 * k1 + k0] = t; }
+}
+
+template <int DIR, bool FUSED = false>
+BEGE_D void fft16(c2 (&a)[16]) { if constexpr (FUSED) fft16_fused<DIR>(a); else fft16_plain<DIR>(a); }
 
 // warp-level sum over the 16 lanes of a half-warp (all lanes get the result), fixed order
 BEGE_D float hw_sum16(float v) {
